@@ -1,0 +1,749 @@
+/*
+ * dock_oracle.c -- CPU ORACLE (double precision, plain C) for the DSDP docking-stage hot path.
+ * TEST INFRASTRUCTURE ONLY: see the header of dock_oracle.h for who may call this, the
+ * passages of PAPER.md each function follows, and which parts are "parity unpinned".
+ *
+ * No blocking, no lookup tables, no cell lists, no fusion: every function is the definition
+ * or the algorithm written out in the paper's order.  OpenMP is used only ACROSS independent
+ * poses / copies / grid nodes (never inside one evaluation), so results do not depend on the
+ * number of threads.
+ */
+#include "dock_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define PI 3.14159265358979323846
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Parameters: readings S1 (weights), S2 (XS radii and flags), S3, S7, S12, S14, S15, S19 of
+ * SURVEY.md 8(c).  The paper prints none of them (PAPER.md:49 only says "same scoring
+ * function" as Vina); they are inputs, so parity does not depend on the values.
+ * ------------------------------------------------------------------------------------- */
+void orc_default_params(orc_params *p)
+{
+    /* id order: C_H C_P N_P N_D N_A N_DA O_P O_D O_A O_DA S_P P_P F_H Cl_H Br_H I_H Met_D */
+    static const double rad[17] = {1.9, 1.9, 1.8, 1.8, 1.8, 1.8, 1.7, 1.7, 1.7, 1.7,
+                                   2.0, 2.1, 1.5, 1.8, 2.0, 2.2, 1.2};
+    static const int hyd[17] = {1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 1, 1, 1, 0};
+    static const int don[17] = {0, 0, 0, 1, 0, 1, 0, 1, 0, 1, 0, 0, 0, 0, 0, 0, 1};
+    static const int acc[17] = {0, 0, 0, 0, 1, 1, 0, 0, 1, 1, 0, 0, 0, 0, 0, 0, 0};
+    memset(p, 0, sizeof(*p));
+    p->n_types = 17;
+    for (int i = 0; i < 17; ++i) {
+        p->radius[i] = rad[i];
+        p->hydrophobic[i] = hyd[i];
+        p->donor[i] = don[i];
+        p->acceptor[i] = acc[i];
+    }
+    p->w[0] = -0.0356;
+    p->w[1] = -0.00516;
+    p->w[2] = 0.840;
+    p->w[3] = -0.0351;
+    p->w[4] = -0.587;
+    p->cutoff = 8.0;
+    p->k_wall = 10.0;
+    p->t_mc = 1.2;
+    p->amp_trans = 2.0;
+    p->amp_rot = 0.3;
+    p->bfgs_c1 = 1e-4;
+    p->bfgs_shrink = 0.5;
+    p->bfgs_max_trials = 12;
+    p->bfgs_gtol = 1e-3;
+    p->bfgs_curv_eps = 1e-8;
+    p->cluster_rmsd = 2.0;
+    p->topk = 10;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O1 pair potential on surface distance d = r - R1 - R2 (terms named in
+ * BASELINE.json:north_star).  Direct evaluation, no radial table.
+ *   f = w1 exp(-(d/0.5)^2) + w2 exp(-((d-3)/2)^2) + w3 (d<0 ? d^2 : 0)
+ *     + w4 [both hydrophobic] H(d) + w5 [donor-acceptor] B(d)
+ *   H = 1 (d<0.5), 1.5-d (0.5<=d<1.5), 0 (d>=1.5);  B = 1 (d<-0.7), -d/0.7 (-0.7<=d<0), 0 (d>=0)
+ * ------------------------------------------------------------------------------------- */
+static int is_hbond_pair(const orc_params *p, int t1, int t2)
+{
+    return (p->donor[t1] && p->acceptor[t2]) || (p->donor[t2] && p->acceptor[t1]);
+}
+
+double orc_pair(const orc_params *p, int t1, int t2, double r, double *dfdr)
+{
+    double e = 0.0, de = 0.0;
+    if (r < p->cutoff) {
+        double d = r - p->radius[t1] - p->radius[t2];
+        double a = d / 0.5;
+        double g1 = exp(-a * a);
+        e += p->w[0] * g1;
+        de += p->w[0] * g1 * (-2.0 * a / 0.5);
+        double b = (d - 3.0) / 2.0;
+        double g2 = exp(-b * b);
+        e += p->w[1] * g2;
+        de += p->w[1] * g2 * (-2.0 * b / 2.0);
+        if (d < 0.0) {
+            e += p->w[2] * d * d;
+            de += p->w[2] * 2.0 * d;
+        }
+        if (p->hydrophobic[t1] && p->hydrophobic[t2]) {
+            if (d < 0.5) {
+                e += p->w[3];
+            } else if (d < 1.5) {
+                e += p->w[3] * (1.5 - d);
+                de += -p->w[3];
+            }
+        }
+        if (is_hbond_pair(p, t1, t2)) {
+            if (d < -0.7) {
+                e += p->w[4];
+            } else if (d < 0.0) {
+                e += p->w[4] * (-d / 0.7);
+                de += -p->w[4] / 0.7;
+            }
+        }
+    }
+    if (dfdr) *dfdr = de;
+    return e;
+}
+
+/* distance of d to the nearest derivative kink of the ACTIVE piecewise-linear terms */
+static double pair_kink_margin(const orc_params *p, int t1, int t2, double r)
+{
+    double m = fabs(r - p->cutoff);
+    double d = r - p->radius[t1] - p->radius[t2];
+    if (p->hydrophobic[t1] && p->hydrophobic[t2]) {
+        m = fmin(m, fabs(d - 0.5));
+        m = fmin(m, fabs(d - 1.5));
+    }
+    if (is_hbond_pair(p, t1, t2)) {
+        m = fmin(m, fabs(d + 0.7));
+        m = fmin(m, fabs(d));
+    }
+    return m;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), R-rules of SURVEY.md 8(c).
+ * ------------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* counter = (copy, step, slot, system); key = (seed lo, seed hi) */
+static void draw(uint64_t seed, uint32_t system, uint32_t copy, uint32_t step, uint32_t slot, uint32_t r[4])
+{
+    uint32_t ctr[4] = {copy, step, slot, system};
+    uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
+    orc_philox4x32_10(ctr, key, r);
+}
+
+/* u = (r >> 8) * 2^-24, exact in fp32 and fp64 */
+static double u24(uint32_t r) { return (double)(r >> 8) * (1.0 / 16777216.0); }
+
+/* ---------------------------------------------------------------------------------------
+ * O2 grid maps (eq. 2's inner sum at 198-199).
+ * ------------------------------------------------------------------------------------- */
+void orc_grid_geometry(const double center[3], const double size[3], double h, int dims[3], double origin[3])
+{
+    for (int c = 0; c < 3; ++c) {
+        dims[c] = (int)floor(size[c] / h + 0.5) + 1;
+        /* DESIGN.md reading D-ORG: the origin is rounded ONCE to fp32 so that both
+         * implementations place node 0 at the same representable coordinate. */
+        origin[c] = (double)(float)(center[c] - 0.5 * size[c]);
+    }
+}
+
+void orc_build_grid(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
+                    const int dims[3], const double origin[3], double h,
+                    int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *G)
+{
+    const int nx = dims[0], ny = dims[1], nz = dims[2];
+    const int64_t nodes = (int64_t)nx * ny * nz;
+    const float hf = (float)h;
+    const float cut2f = (float)p->cutoff * (float)p->cutoff;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t m = 0; m < nodes; ++m) {
+        int ix = (int)(m % nx), iy = (int)((m / nx) % ny), iz = (int)(m / ((int64_t)nx * ny));
+        double mx = origin[0] + h * ix, my = origin[1] + h * iy, mz = origin[2] + h * iz;
+        /* fp32 node coordinate, as the kernel forms it: fmaf(i, h, origin) */
+        float mxf = fmaf((float)ix, hf, (float)origin[0]);
+        float myf = fmaf((float)iy, hf, (float)origin[1]);
+        float mzf = fmaf((float)iz, hf, (float)origin[2]);
+        for (int t = 0; t < n_lig_types; ++t) G[(int64_t)t * nodes + m] = 0.0;
+        for (int j = 0; j < np; ++j) {
+            double dx = mx - pxyz[3 * j], dy = my - pxyz[3 * j + 1], dz = mz - pxyz[3 * j + 2];
+            double r = sqrt(dx * dx + dy * dy + dz * dz);
+            int in_range;
+            if (fp32_cutoff) {
+                float fx = mxf - (float)pxyz[3 * j], fy = myf - (float)pxyz[3 * j + 1], fz = mzf - (float)pxyz[3 * j + 2];
+                float r2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+                in_range = r2f < cut2f;
+                if (in_range && !(r < p->cutoff)) r = nextafter(p->cutoff, 0.0); /* value side of the same decision */
+            } else {
+                in_range = r < p->cutoff;
+            }
+            if (!in_range) continue;
+            for (int t = 0; t < n_lig_types; ++t)
+                G[(int64_t)t * nodes + m] += orc_pair(p, lig_types[t], ptype[j], r, NULL);
+        }
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * small vector / quaternion helpers
+ * ------------------------------------------------------------------------------------- */
+static void cross(const double a[3], const double b[3], double c[3])
+{
+    c[0] = a[1] * b[2] - a[2] * b[1];
+    c[1] = a[2] * b[0] - a[0] * b[2];
+    c[2] = a[0] * b[1] - a[1] * b[0];
+}
+static double dot(const double a[3], const double b[3]) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+static void quat_normalize(double q[4])
+{
+    double n = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+    if (n > 0.0) { q[0] /= n; q[1] /= n; q[2] /= n; q[3] /= n; }
+    else { q[0] = 1.0; q[1] = q[2] = q[3] = 0.0; }
+}
+/* Hamilton product a*b, (w,x,y,z) */
+static void quat_mul(const double a[4], const double b[4], double c[4])
+{
+    c[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
+    c[1] = a[0] * b[1] + a[1] * b[0] + a[2] * b[3] - a[3] * b[2];
+    c[2] = a[0] * b[2] - a[1] * b[3] + a[2] * b[0] + a[3] * b[1];
+    c[3] = a[0] * b[3] + a[1] * b[2] - a[2] * b[1] + a[3] * b[0];
+}
+static void quat_from_rotvec(const double w[3], double q[4])
+{
+    double phi = sqrt(dot(w, w));
+    if (phi < 1e-12) {
+        q[0] = 1.0; q[1] = 0.5 * w[0]; q[2] = 0.5 * w[1]; q[3] = 0.5 * w[2];
+    } else {
+        double s = sin(0.5 * phi) / phi;
+        q[0] = cos(0.5 * phi); q[1] = s * w[0]; q[2] = s * w[1]; q[3] = s * w[2];
+    }
+    quat_normalize(q);
+}
+static void quat_to_matrix(const double qin[4], double R[9])
+{
+    double q[4] = {qin[0], qin[1], qin[2], qin[3]};
+    quat_normalize(q);
+    double w = q[0], x = q[1], y = q[2], z = q[3];
+    R[0] = 1 - 2 * (y * y + z * z); R[1] = 2 * (x * y - w * z);     R[2] = 2 * (x * z + w * y);
+    R[3] = 2 * (x * y + w * z);     R[4] = 1 - 2 * (x * x + z * z); R[5] = 2 * (y * z - w * x);
+    R[6] = 2 * (x * z - w * y);     R[7] = 2 * (y * z + w * x);     R[8] = 1 - 2 * (x * x + y * y);
+}
+/* rotate v about unit axis u by angle th (right-handed), Rodrigues */
+static void rot_axis(const double u[3], double th, const double v[3], double out[3])
+{
+    double c = cos(th), s = sin(th), uxv[3];
+    cross(u, v, uxv);
+    double ud = dot(u, v);
+    for (int k = 0; k < 3; ++k) out[k] = v[k] * c + uxv[k] * s + u[k] * ud * (1.0 - c);
+}
+
+void orc_pose_add(int T, const double *pose, const double *s, double *out)
+{
+    double qw[4], q[4];
+    for (int k = 0; k < 3; ++k) out[k] = pose[k] + s[k];
+    quat_from_rotvec(s + 3, qw);
+    quat_mul(qw, pose + 3, q);
+    quat_normalize(q);
+    for (int k = 0; k < 4; ++k) out[3 + k] = q[k];
+    for (int k = 0; k < T; ++k) out[7 + k] = pose[7 + k] + s[6 + k];
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O3 kinematics (reading S11).  pivot c = mean of the root-fragment reference atoms.
+ * Fragment transforms parents-first: A_0 = id; A_{k+1}(y) = A_parent( Rot(u_k, theta_k)(y - ref[b_k]) + ref[b_k] ),
+ * u_k = unit(ref[b_k] - ref[a_k]).  y_i = A_{frag(i)}(ref_i);  x_i = t + R(q)(y_i - c).
+ * A_f is stored as y -> M_f y + v_f.
+ * ------------------------------------------------------------------------------------- */
+static void root_pivot(const orc_ligand *L, double c[3])
+{
+    int n = 0;
+    c[0] = c[1] = c[2] = 0.0;
+    for (int i = 0; i < L->N; ++i)
+        if (L->frag[i] == 0) { c[0] += L->ref[3 * i]; c[1] += L->ref[3 * i + 1]; c[2] += L->ref[3 * i + 2]; ++n; }
+    c[0] /= n; c[1] /= n; c[2] /= n;
+}
+
+void orc_coords(const orc_ligand *L, const double *pose, double *x)
+{
+    const int T = L->T;
+    double *M = (double *)malloc(sizeof(double) * 9 * (T + 1));
+    double *v = (double *)malloc(sizeof(double) * 3 * (T + 1));
+    for (int k = 0; k < 9; ++k) M[k] = (k % 4 == 0) ? 1.0 : 0.0;
+    v[0] = v[1] = v[2] = 0.0;
+    for (int k = 0; k < T; ++k) {
+        const double *pa = L->ref + 3 * L->tors_a[k], *pb = L->ref + 3 * L->tors_b[k];
+        double u[3] = {pb[0] - pa[0], pb[1] - pa[1], pb[2] - pa[2]};
+        double n = sqrt(dot(u, u));
+        u[0] /= n; u[1] /= n; u[2] /= n;
+        /* local map: y -> Rk (y - pb) + pb  =  Rk y + (pb - Rk pb) */
+        double Rk[9], e[3], col[3];
+        for (int c = 0; c < 3; ++c) {
+            e[0] = e[1] = e[2] = 0.0; e[c] = 1.0;
+            rot_axis(u, pose[7 + k], e, col);
+            Rk[0 + c] = col[0]; Rk[3 + c] = col[1]; Rk[6 + c] = col[2];
+        }
+        double Rpb[3] = {Rk[0] * pb[0] + Rk[1] * pb[1] + Rk[2] * pb[2],
+                         Rk[3] * pb[0] + Rk[4] * pb[1] + Rk[5] * pb[2],
+                         Rk[6] * pb[0] + Rk[7] * pb[1] + Rk[8] * pb[2]};
+        double lk[3] = {pb[0] - Rpb[0], pb[1] - Rpb[1], pb[2] - Rpb[2]};
+        const double *Mp = M + 9 * L->tors_parent[k], *vp = v + 3 * L->tors_parent[k];
+        double *Mc = M + 9 * (k + 1), *vc = v + 3 * (k + 1);
+        for (int r = 0; r < 3; ++r) {
+            for (int c = 0; c < 3; ++c)
+                Mc[3 * r + c] = Mp[3 * r] * Rk[c] + Mp[3 * r + 1] * Rk[3 + c] + Mp[3 * r + 2] * Rk[6 + c];
+            vc[r] = Mp[3 * r] * lk[0] + Mp[3 * r + 1] * lk[1] + Mp[3 * r + 2] * lk[2] + vp[r];
+        }
+    }
+    double R[9], c[3];
+    quat_to_matrix(pose + 3, R);
+    root_pivot(L, c);
+    for (int i = 0; i < L->N; ++i) {
+        const double *Mf = M + 9 * L->frag[i], *vf = v + 3 * L->frag[i], *r0 = L->ref + 3 * i;
+        double y[3];
+        for (int r = 0; r < 3; ++r) y[r] = Mf[3 * r] * r0[0] + Mf[3 * r + 1] * r0[1] + Mf[3 * r + 2] * r0[2] + vf[r] - c[r];
+        for (int r = 0; r < 3; ++r) x[3 * i + r] = pose[r] + R[3 * r] * y[0] + R[3 * r + 1] * y[1] + R[3 * r + 2] * y[2];
+    }
+    free(M);
+    free(v);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O4 inter term for one atom: trilinear energy (eq. 2), its partial
+ * derivatives (eq. 3), clamp + quadratic wall (reading S7),
+ * cell choice i0 = min(floor(u), n-2) (reading S8).
+ * ------------------------------------------------------------------------------------- */
+static void atom_inter(const orc_params *p, const orc_grid *g, int map, const double x[3],
+                       double *e_grid, double *e_wall, double grad[3], double *face_margin, int *outside)
+{
+    int i0[3], clamped[3];
+    double pf[3], over[3];
+    const double h = g->h;
+    *outside = 0;
+    for (int c = 0; c < 3; ++c) {
+        const int n = g->dims[c];
+        double u = (x[c] - g->origin[c]) / h;
+        over[c] = 0.0;
+        clamped[c] = 0;
+        if (u < 0.0) { over[c] = x[c] - g->origin[c]; u = 0.0; clamped[c] = 1; }
+        else if (u > (double)(n - 1)) { over[c] = x[c] - (g->origin[c] + h * (n - 1)); u = (double)(n - 1); clamped[c] = 1; }
+        int fl = (int)floor(u);
+        i0[c] = fl < n - 2 ? fl : n - 2;
+        pf[c] = u - (double)i0[c];
+        if (clamped[c]) *outside = 1;
+        if (face_margin) {
+            double m = clamped[c] ? fabs(over[c]) : fmin(pf[c], 1.0 - pf[c]) * h;
+            if (m < *face_margin) *face_margin = m;
+        }
+    }
+    const int nx = g->dims[0], ny = g->dims[1], nz = g->dims[2];
+    const double *G = g->data + (int64_t)map * nx * ny * nz;
+    double e = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
+    for (int l = 0; l <= 1; ++l)
+        for (int m = 0; m <= 1; ++m)
+            for (int n = 0; n <= 1; ++n) {
+                double wx = l ? pf[0] : 1.0 - pf[0];
+                double wy = m ? pf[1] : 1.0 - pf[1];
+                double wz = n ? pf[2] : 1.0 - pf[2];
+                double val = G[((int64_t)(i0[2] + n) * ny + (i0[1] + m)) * nx + (i0[0] + l)];
+                e += wx * wy * wz * val;                       /* eq. 2 */
+                gx += (2 * l - 1) / h * wy * wz * val;         /* eq. 3, x component */
+                gy += wx * (2 * m - 1) / h * wz * val;         /* eq. 3, y component */
+                gz += wx * wy * (2 * n - 1) / h * val;         /* eq. 3, z component */
+            }
+    double ew = 0.0;
+    double gg[3] = {gx, gy, gz};
+    for (int c = 0; c < 3; ++c) {
+        if (clamped[c]) gg[c] = 0.0;                           /* lookup is constant along a clamped axis */
+        ew += p->k_wall * over[c] * over[c];
+        gg[c] += 2.0 * p->k_wall * over[c];
+        grad[c] = gg[c];
+    }
+    *e_grid = e;
+    *e_wall = ew;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O4-O7: total E = E_grid + E_wall + E_intra and its gradient wrt (t, rotation about t, theta).
+ * ------------------------------------------------------------------------------------- */
+double orc_eval(const orc_params *p, const orc_grid *g, const orc_ligand *L,
+                const double *pose, double terms[3], double *grad, orc_diag *diag)
+{
+    const int N = L->N, T = L->T;
+    double *x = (double *)malloc(sizeof(double) * 3 * N);
+    double *gx = (double *)calloc(3 * N, sizeof(double));
+    double e_grid = 0.0, e_wall = 0.0, e_intra = 0.0;
+    double face_margin = 1e300, kink_margin = 1e300;
+    int n_in = 0, n_out = 0;
+    orc_coords(L, pose, x);
+    for (int i = 0; i < N; ++i) {
+        double eg, ew, ga[3];
+        int outside;
+        int map = g->type_to_map[L->type[i]];
+        atom_inter(p, g, map, x + 3 * i, &eg, &ew, ga, diag ? &face_margin : NULL, &outside);
+        e_grid += eg;
+        e_wall += ew;
+        n_out += outside;
+        for (int c = 0; c < 3; ++c) gx[3 * i + c] += ga[c];
+    }
+    /* O5 intra-ligand pairs */
+    for (int k = 0; k < L->P; ++k) {
+        int i = L->pairs[2 * k], j = L->pairs[2 * k + 1];
+        double d[3] = {x[3 * i] - x[3 * j], x[3 * i + 1] - x[3 * j + 1], x[3 * i + 2] - x[3 * j + 2]};
+        double r = sqrt(dot(d, d)), dfdr;
+        e_intra += orc_pair(p, L->type[i], L->type[j], r, &dfdr);
+        if (r < p->cutoff) ++n_in;
+        if (diag) kink_margin = fmin(kink_margin, pair_kink_margin(p, L->type[i], L->type[j], r));
+        if (r > 1e-12)
+            for (int c = 0; c < 3; ++c) {
+                gx[3 * i + c] += dfdr * d[c] / r;
+                gx[3 * j + c] -= dfdr * d[c] / r;
+            }
+    }
+    if (terms) { terms[0] = e_grid; terms[1] = e_wall; terms[2] = e_intra; }
+    if (grad) {
+        /* O6 chain rule */
+        for (int k = 0; k < 6 + T; ++k) grad[k] = 0.0;
+        for (int i = 0; i < N; ++i) {
+            double lever[3] = {x[3 * i] - pose[0], x[3 * i + 1] - pose[1], x[3 * i + 2] - pose[2]}, tq[3];
+            cross(lever, gx + 3 * i, tq);
+            for (int c = 0; c < 3; ++c) { grad[c] += gx[3 * i + c]; grad[3 + c] += tq[c]; }
+        }
+        for (int k = 0; k < T; ++k) {
+            /* subtree(k) = fragment k+1 and every fragment whose parent chain passes through it */
+            const double *xa = x + 3 * L->tors_a[k], *xb = x + 3 * L->tors_b[k];
+            double u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
+            double n = sqrt(dot(u, u));
+            u[0] /= n; u[1] /= n; u[2] /= n;
+            double acc[3] = {0, 0, 0};
+            for (int i = 0; i < N; ++i) {
+                int f = L->frag[i], in_sub = 0;
+                while (f > 0) {
+                    if (f == k + 1) { in_sub = 1; break; }
+                    f = L->tors_parent[f - 1];
+                }
+                if (!in_sub) continue;
+                double lever[3] = {x[3 * i] - xb[0], x[3 * i + 1] - xb[1], x[3 * i + 2] - xb[2]}, tq[3];
+                cross(lever, gx + 3 * i, tq);
+                acc[0] += tq[0]; acc[1] += tq[1]; acc[2] += tq[2];
+            }
+            grad[6 + k] = dot(u, acc);
+        }
+    }
+    if (diag) {
+        diag->face_margin = face_margin;
+        diag->kink_margin = kink_margin;
+        diag->pairs_in_range = n_in;
+        diag->atoms_outside = n_out;
+    }
+    free(x);
+    free(gx);
+    return e_grid + e_wall + e_intra;   /* O7 */
+}
+
+void orc_score_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n,
+                     const double *poses, double *E, double *grad, double *terms, orc_diag *diag)
+{
+    const int T = L->T;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < n; ++k) {
+        double tr[3];
+        E[k] = orc_eval(p, g, L, poses + k * (7 + T), tr, grad ? grad + k * (6 + T) : NULL, diag ? diag + k : NULL);
+        if (terms) { terms[3 * k] = tr[0]; terms[3 * k + 1] = tr[1]; terms[3 * k + 2] = tr[2]; }
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O8 BFGS with backtracking (Nocedal-Wright inverse update).
+ * Every constant is a reading (S12) and a field of orc_params.
+ *
+ * The optimizer is generic over the objective (`fn` returns f and writes the gradient) and
+ * over the retraction x (+) s (`add`), so that the pin tests can run it on closed-form
+ * quadratics; orc_local_opt instantiates it with the docking objective and orc_pose_add.
+ * `obs` (nullable) is called after every accepted iteration with (it, f, H, s, y, updated).
+ * ------------------------------------------------------------------------------------- */
+double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
+                orc_objective_fn fn, orc_retract_fn add, void *ctx,
+                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx)
+{
+    double *H = (double *)malloc(sizeof(double) * n * n);
+    double *A = (double *)malloc(sizeof(double) * n * n);
+    double *B = (double *)malloc(sizeof(double) * n * n);
+    double *x = (double *)malloc(sizeof(double) * np_), *xt = (double *)malloc(sizeof(double) * np_);
+    double *gr = (double *)malloc(sizeof(double) * n), *gt = (double *)malloc(sizeof(double) * n);
+    double *d = (double *)malloc(sizeof(double) * n), *s = (double *)malloc(sizeof(double) * n), *y = (double *)malloc(sizeof(double) * n);
+    int it = 0, ne = 0, fresh = 1;
+    memcpy(x, x0, sizeof(double) * np_);
+    double f = fn(ctx, x, gr);
+    ++ne;
+    for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? 1.0 : 0.0;
+    for (it = 0; it < cap; ++it) {
+        double gn = 0.0;
+        for (int k = 0; k < n; ++k) gn += gr[k] * gr[k];
+        if (sqrt(gn) < p->bfgs_gtol) break;
+        double gp = 0.0;
+        for (int r = 0; r < n; ++r) {                      /* d = -H g */
+            double a = 0.0;
+            for (int c = 0; c < n; ++c) a += H[r * n + c] * gr[c];
+            d[r] = -a;
+            gp += gr[r] * d[r];
+        }
+        if (gp >= 0.0) {                                   /* not a descent direction: reset H = I */
+            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? 1.0 : 0.0;
+            fresh = 1;
+            gp = 0.0;
+            for (int r = 0; r < n; ++r) { d[r] = -gr[r]; gp += gr[r] * d[r]; }
+        }
+        double alpha = 1.0;
+        if (fresh) {                                       /* alpha0 = min(1, 1/||d||) while H = I */
+            double dn = 0.0;
+            for (int k = 0; k < n; ++k) dn += d[k] * d[k];
+            dn = sqrt(dn);
+            if (dn > 1.0) alpha = 1.0 / dn;
+        }
+        int ok = 0;
+        double ft = f;
+        for (int trial = 0; trial < p->bfgs_max_trials; ++trial) {
+            for (int k = 0; k < n; ++k) s[k] = alpha * d[k];
+            add(ctx, x, s, xt);
+            ft = fn(ctx, xt, gt);
+            ++ne;
+            if (ft - f <= p->bfgs_c1 * alpha * gp) { ok = 1; break; }   /* Armijo */
+            alpha *= p->bfgs_shrink;
+        }
+        if (!ok) break;
+        double ys = 0.0, yy = 0.0, ss = 0.0;
+        for (int k = 0; k < n; ++k) {
+            y[k] = gt[k] - gr[k];
+            ys += y[k] * s[k]; yy += y[k] * y[k]; ss += s[k] * s[k];
+        }
+        memcpy(x, xt, sizeof(double) * np_);
+        memcpy(gr, gt, sizeof(double) * n);
+        f = ft;
+        int updated = 0;
+        if (ys > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) {
+            if (fresh) {                                   /* first update: H = (y.s / y.y) I */
+                double sc = ys / yy;
+                for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? sc : 0.0;
+                fresh = 0;
+            }
+            /* H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T */
+            double rho = 1.0 / ys;
+            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {   /* A = (I - rho s y^T) H */
+                double a = H[r * n + c];
+                for (int k = 0; k < n; ++k) a -= rho * s[r] * y[k] * H[k * n + c];
+                A[r * n + c] = a;
+            }
+            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {   /* B = A (I - rho y s^T) + rho s s^T */
+                double a = A[r * n + c];
+                for (int k = 0; k < n; ++k) a -= A[r * n + k] * rho * y[k] * s[c];
+                B[r * n + c] = a + rho * s[r] * s[c];
+            }
+            memcpy(H, B, sizeof(double) * n * n);
+            updated = 1;
+        }
+        if (obs) obs(obs_ctx, it, f, H, s, y, updated);
+    }
+    memcpy(x_out, x, sizeof(double) * np_);
+    if (iters) *iters = it;
+    if (evals) *evals = ne;
+    free(H); free(A); free(B); free(x); free(xt); free(gr); free(gt); free(d); free(s); free(y);
+    return f;
+}
+
+typedef struct { const orc_params *p; const orc_grid *g; const orc_ligand *L; } dock_ctx;
+static double dock_fn(void *c, const double *x, double *grad)
+{
+    dock_ctx *k = (dock_ctx *)c;
+    return orc_eval(k->p, k->g, k->L, x, NULL, grad, NULL);
+}
+static void dock_add(void *c, const double *x, const double *s, double *out)
+{
+    orc_pose_add(((dock_ctx *)c)->L->T, x, s, out);
+}
+
+double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap,
+                     const double *pose_in, double *pose_out, int *iters, int *evals)
+{
+    const int T = L->T;
+    dock_ctx ctx = {p, g, L};
+    double *x0 = (double *)malloc(sizeof(double) * (7 + T));
+    memcpy(x0, pose_in, sizeof(double) * (7 + T));
+    quat_normalize(x0 + 3);
+    double f = orc_bfgs(p, 6 + T, 7 + T, cap, x0, dock_fn, dock_add, &ctx, pose_out, iters, evals, NULL, NULL);
+    free(x0);
+    return f;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O9 Monte Carlo (readings S14-S16; R-rules).
+ * ------------------------------------------------------------------------------------- */
+void orc_init_pose(const double box_center[3], const double box_size[3], int T,
+                   uint64_t seed, uint32_t system, uint32_t copy, double *pose)
+{
+    uint32_t r[4];
+    draw(seed, system, copy, 0xFFFFFFFFu, 0, r);
+    for (int c = 0; c < 3; ++c) pose[c] = box_center[c] - 0.5 * box_size[c] + u24(r[c]) * box_size[c];
+    draw(seed, system, copy, 0xFFFFFFFFu, 1, r);
+    double u1 = u24(r[0]), u2 = u24(r[1]), u3 = u24(r[2]);
+    pose[3] = sqrt(u1) * cos(2.0 * PI * u3);
+    pose[4] = sqrt(1.0 - u1) * sin(2.0 * PI * u2);
+    pose[5] = sqrt(1.0 - u1) * cos(2.0 * PI * u2);
+    pose[6] = sqrt(u1) * sin(2.0 * PI * u3);
+    for (int k = 0; k < T; ++k) {
+        if (k % 4 == 0) draw(seed, system, copy, 0xFFFFFFFFu, 2 + (uint32_t)(k / 4), r);
+        pose[7 + k] = PI * (2.0 * u24(r[k % 4]) - 1.0);
+    }
+    for (int k = 0; k < 7 + T; ++k) pose[k] = (double)(float)pose[k];   /* stored fp32 once (S16) */
+}
+
+int orc_mc_perturb(const orc_params *p, int T, uint64_t seed, uint32_t system, uint32_t copy,
+                   uint32_t step, const double *pose, double *cand)
+{
+    uint32_t r[4];
+    draw(seed, system, copy, step, 0, r);
+    const uint32_t K = T > 0 ? 3u : 2u;
+    int kind = (int)(((uint64_t)r[0] * K) >> 32);
+    memcpy(cand, pose, sizeof(double) * (7 + T));
+    if (kind == 0) {
+        for (int c = 0; c < 3; ++c) cand[c] = pose[c] + p->amp_trans * (2.0 * u24(r[1 + c]) - 1.0);
+    } else if (kind == 1) {
+        double w[3], qw[4], q[4];
+        for (int c = 0; c < 3; ++c) w[c] = p->amp_rot * (2.0 * u24(r[1 + c]) - 1.0);
+        quat_from_rotvec(w, qw);
+        quat_mul(qw, pose + 3, q);
+        quat_normalize(q);
+        for (int c = 0; c < 4; ++c) cand[3 + c] = q[c];
+    } else {
+        int k = (int)(((uint64_t)r[1] * (uint32_t)T) >> 32);
+        cand[7 + k] = PI * (2.0 * u24(r[2]) - 1.0);
+    }
+    return kind;
+}
+
+double orc_mc_uniform(uint64_t seed, uint32_t system, uint32_t copy, uint32_t step)
+{
+    uint32_t r[4];
+    draw(seed, system, copy, step, 1, r);
+    return u24(r[0]);
+}
+
+double orc_search_copy(const orc_params *p, const orc_grid *g, const orc_ligand *L,
+                       int steps, int cap, uint64_t seed, uint32_t system, uint32_t copy,
+                       const double *init_pose, double *best_pose,
+                       double *trace_pose, orc_step_rec *trace, orc_step_rec *init_rec)
+{
+    const int np_ = 7 + L->T;
+    double *cur = (double *)malloc(sizeof(double) * np_);
+    double *c0 = (double *)malloc(sizeof(double) * np_);
+    double *c1 = (double *)malloc(sizeof(double) * np_);
+    int it, ne;
+    double e_cur = orc_local_opt(p, g, L, cap, init_pose, cur, &it, &ne);
+    if (init_rec) { init_rec->e_cur = 0; init_rec->e_cand = e_cur; init_rec->u = 0; init_rec->accept = 1; init_rec->iters = it; init_rec->evals = ne; }
+    double e_best = e_cur;
+    memcpy(best_pose, cur, sizeof(double) * np_);
+    for (int s = 0; s < steps; ++s) {
+        if (trace_pose) memcpy(trace_pose + (int64_t)s * np_, cur, sizeof(double) * np_);
+        orc_mc_perturb(p, L->T, seed, system, copy, (uint32_t)s, cur, c0);
+        double e_c = orc_local_opt(p, g, L, cap, c0, c1, &it, &ne);
+        double u = orc_mc_uniform(seed, system, copy, (uint32_t)s);
+        int accept = (e_c < e_cur) || (u < exp((e_cur - e_c) / p->t_mc));
+        if (trace) { trace[s].e_cur = e_cur; trace[s].e_cand = e_c; trace[s].u = u; trace[s].accept = accept; trace[s].iters = it; trace[s].evals = ne; }
+        if (accept) { memcpy(cur, c1, sizeof(double) * np_); e_cur = e_c; }
+        if (e_cur < e_best) { e_best = e_cur; memcpy(best_pose, cur, sizeof(double) * np_); }
+    }
+    free(cur); free(c0); free(c1);
+    return e_best;
+}
+
+int64_t orc_search(const orc_params *p, const orc_grid *g, const orc_ligand *L,
+                   int copies, int steps, int cap, uint64_t seed, uint32_t system,
+                   const double *init_poses, double *best_pose, double *best_e,
+                   double *trace_pose, orc_step_rec *trace, orc_step_rec *init_rec)
+{
+    const int np_ = 7 + L->T;
+    int64_t total = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : total)
+    for (int c = 0; c < copies; ++c) {
+        orc_step_rec *tr = trace ? trace + (int64_t)c * steps : NULL;
+        orc_step_rec ir;
+        best_e[c] = orc_search_copy(p, g, L, steps, cap, seed, system, (uint32_t)c,
+                                    init_poses + (int64_t)c * np_, best_pose + (int64_t)c * np_,
+                                    trace_pose ? trace_pose + (int64_t)c * steps * np_ : NULL, tr, &ir);
+        if (init_rec) init_rec[c] = ir;
+        total += ir.evals;
+        if (tr) for (int s = 0; s < steps; ++s) total += tr[s].evals;
+    }
+    return total;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O10 ranking and greedy RMSD clustering (reading S19).
+ * ------------------------------------------------------------------------------------- */
+double orc_rmsd(const orc_ligand *L, const double *pose_a, const double *pose_b)
+{
+    double *xa = (double *)malloc(sizeof(double) * 3 * L->N), *xb = (double *)malloc(sizeof(double) * 3 * L->N);
+    orc_coords(L, pose_a, xa);
+    orc_coords(L, pose_b, xb);
+    double s = 0.0;
+    for (int i = 0; i < 3 * L->N; ++i) s += (xa[i] - xb[i]) * (xa[i] - xb[i]);
+    free(xa); free(xb);
+    return sqrt(s / L->N);
+}
+
+int orc_topk(const orc_params *p, const orc_ligand *L, int copies, const double *poses,
+             const double *e, int k, double rmsd_min, int32_t *out_idx)
+{
+    (void)p;
+    const int np_ = 7 + L->T;
+    int *order = (int *)malloc(sizeof(int) * copies);
+    for (int i = 0; i < copies; ++i) order[i] = i;
+    /* insertion sort: ascending E, ties -> lower copy index (stable) */
+    for (int i = 1; i < copies; ++i) {
+        int v = order[i], j = i - 1;
+        while (j >= 0 && e[order[j]] > e[v]) { order[j + 1] = order[j]; --j; }
+        order[j + 1] = v;
+    }
+    int kept = 0;
+    for (int i = 0; i < copies && kept < k; ++i) {
+        int c = order[i], ok = 1;
+        for (int m = 0; m < kept; ++m)
+            if (orc_rmsd(L, poses + (int64_t)c * np_, poses + (int64_t)out_idx[m] * np_) < rmsd_min) { ok = 0; break; }
+        if (ok) out_idx[kept++] = c;
+    }
+    free(order);
+    return kept;
+}

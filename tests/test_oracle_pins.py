@@ -1,0 +1,567 @@
+"""Pins for the CPU oracle (oracle/dock_oracle.c) against things OTHER than itself:
+hand-computed values (tests/golden/), closed forms, invariants, finite differences,
+brute force on tiny inputs (SURVEY.md 8(c) "What pins each part").  CPU only."""
+import math
+import os
+from types import SimpleNamespace
+
+import numpy as np
+import pytest
+
+from dock_synth import XS, make_system
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ----------------------------------------------------------------------------- helpers
+def _single_atom_ligand(O, typ):
+    lig = SimpleNamespace(ref_xyz=np.zeros((1, 3)), type=np.array([typ], np.int32), frag=np.zeros(1, np.int32),
+                          tors_parent=np.zeros(0, np.int32), tors_a=np.zeros(0, np.int32),
+                          tors_b=np.zeros(0, np.int32), pairs=np.zeros((0, 2), np.int32))
+    return O.Ligand(lig)
+
+
+def _affine_grid(O, n=9, h=0.375, origin=(1.0, -2.0, 3.0), a=0.7, b=(0.3, -1.1, 2.5), typ=0):
+    ax = [origin[c] + h * np.arange(n) for c in range(3)]
+    Z, Y, X = np.meshgrid(ax[2], ax[1], ax[0], indexing="ij")
+    data = a + b[0] * X + b[1] * Y + b[2] * Z
+    return O.Grid((n, n, n), origin, h, [typ], data[None])
+
+
+def _random_pose(rng, T, center, spread=2.0):
+    q = rng.normal(size=4)
+    q /= np.linalg.norm(q)
+    return np.concatenate([np.asarray(center) + spread * (rng.random(3) - 0.5), q, rng.uniform(-np.pi, np.pi, T)])
+
+
+@pytest.fixture(scope="module")
+def tiny(orc):
+    s = make_system(0, seed=0)
+    p = orc.default_params()
+    g = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
+    return s, p, g, orc.Ligand(s.ligand)
+
+
+# ----------------------------------------------------------------------------- O1 pair potential
+def test_pair_golden_values(orc):
+    p = orc.default_params()
+    rows = [l.split() for l in open(os.path.join(GOLD, "pair_pins.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 15
+    for t1, t2, r, f in rows:
+        e, _ = orc.pair(p, XS[t1], XS[t2], float(r))
+        assert abs(e - float(f)) < 5e-10, (t1, t2, r, e, f)
+
+
+def test_pair_closed_forms(orc):
+    p = orc.default_params()
+    w = [-0.0356, -0.00516, 0.840, -0.0351, -0.587]
+    # d = 0 for two hydrophobic carbons: gauss1 = 1, gauss2 = e^-2.25, H = 1, no repulsion
+    e, _ = orc.pair(p, XS["C_H"], XS["C_H"], 3.8)
+    assert abs(e - (w[0] + w[1] * math.exp(-2.25) + w[3])) < 1e-15
+    # d = 3 (r = 6.8): gauss2 = 1, gauss1 = e^-36, hydrophobic 0
+    e, _ = orc.pair(p, XS["C_H"], XS["C_H"], 6.8)
+    assert abs(e - (w[0] * math.exp(-36.0) + w[1])) < 1e-15
+    # donor-acceptor at d = -0.7: full hbond weight, repulsion 0.49 w3
+    e, _ = orc.pair(p, XS["N_D"], XS["O_A"], 2.8)
+    assert abs(e - (w[0] * math.exp(-1.96) + w[1] * math.exp(-(3.7 / 2) ** 2) + w[2] * 0.49 + w[4])) < 1e-14
+    # cutoff is strict and hard
+    assert orc.pair(p, 0, 0, 8.0) == (0.0, 0.0)
+    assert orc.pair(p, 0, 0, 9.5) == (0.0, 0.0)
+    assert orc.pair(p, 0, 0, 7.9999999)[0] != 0.0
+
+
+def test_pair_symmetry_and_flags(orc):
+    p = orc.default_params()
+    for t1 in range(17):
+        for t2 in range(17):
+            for r in (2.013, 3.307, 4.111, 5.457, 7.219):  # away from the derivative kinks
+                a, b = orc.pair(p, t1, t2, r), orc.pair(p, t2, t1, r)  # equal up to the rounding of r-R1-R2
+                assert abs(a[0] - b[0]) < 1e-14 and abs(a[1] - b[1]) < 1e-13
+    # donor-donor and acceptor-acceptor get no hbond term; polar carbon gets no hydrophobic term
+    e_dd, _ = orc.pair(p, XS["N_D"], XS["N_D"], 3.0)
+    e_pp, _ = orc.pair(p, XS["N_P"], XS["N_P"], 3.0)
+    assert e_dd == e_pp
+    assert orc.pair(p, XS["C_P"], XS["C_H"], 4.0)[0] == orc.pair(p, XS["C_P"], XS["C_P"], 4.0)[0]
+    assert orc.pair(p, XS["C_H"], XS["C_H"], 4.0)[0] < orc.pair(p, XS["C_P"], XS["C_H"], 4.0)[0]
+
+
+def test_pair_derivative_vs_central_difference(orc):
+    p = orc.default_params()
+    rng = np.random.default_rng(1)
+    n = 0
+    for _ in range(4000):
+        t1, t2 = int(rng.integers(17)), int(rng.integers(17))
+        r = float(rng.uniform(0.5, 7.9))
+        d = r - p.radius[t1] - p.radius[t2]
+        if min(abs(d - k) for k in (0.5, 1.5, -0.7, 0.0)) < 1e-3:
+            continue  # derivative kinks of the piecewise terms
+        hh = 1e-6
+        fd = (orc.pair(p, t1, t2, r + hh)[0] - orc.pair(p, t1, t2, r - hh)[0]) / (2 * hh)
+        _, de = orc.pair(p, t1, t2, r)
+        assert abs(fd - de) < 1e-7 * max(1.0, abs(de)), (t1, t2, r, fd, de)
+        n += 1
+    assert n > 3000
+
+
+# ----------------------------------------------------------------------------- Philox
+def test_philox_known_answers(orc):
+    rows = [l.split() for l in open(os.path.join(GOLD, "philox_kat.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for row in rows:
+        v = [int(x, 16) for x in row]
+        assert orc.philox(v[0:4], v[4:6]) == v[6:10]
+
+
+def test_counter_layout_and_uniform_mapping(orc):
+    # counter = (copy, step, slot, system), key = (seed lo, seed hi); u = (r >> 8) * 2^-24
+    seed = 0x0123456789ABCDEF
+    r = orc.philox([7, 3, 1, 5], [seed & 0xFFFFFFFF, seed >> 32])
+    assert orc.mc_uniform(seed, 5, 7, 3) == (r[0] >> 8) / 16777216.0
+    u = orc.mc_uniform(seed, 5, 7, 3)
+    assert float(np.float32(u)) == u and 0.0 <= u < 1.0  # exact in fp32
+
+
+# ----------------------------------------------------------------------------- O2 grid
+def test_single_atom_grid_equals_pair_values(orc):
+    p = orc.default_params()
+    atom = np.array([[0.3, -0.2, 0.1]])
+    lig_types = [XS["C_H"], XS["N_D"], XS["O_A"]]
+    for fp32 in (False, True):
+        g = orc.build_grid(p, atom, [XS["O_A"]], [0, 0, 0], [6, 6, 6], 0.375, lig_types, fp32_cutoff=fp32)
+        assert g.dims == (17, 17, 17)
+        assert np.allclose(g.origin, [-3, -3, -3])
+        rng = np.random.default_rng(0)
+        for _ in range(300):
+            ix, iy, iz = rng.integers(17, size=3)
+            m = g.origin + 0.375 * np.array([ix, iy, iz])
+            r = float(np.linalg.norm(m - atom[0]))
+            for k, t in enumerate(lig_types):
+                assert abs(g.maps[k, iz, iy, ix] - orc.pair(p, t, XS["O_A"], r)[0]) < 1e-14
+
+
+def test_grid_is_plain_sum_over_atoms_within_cutoff(orc, tiny):
+    s, p, g, L = tiny
+    rng = np.random.default_rng(3)
+    nx, ny, nz = g.dims
+    for _ in range(40):
+        ix, iy, iz = int(rng.integers(nx)), int(rng.integers(ny)), int(rng.integers(nz))
+        m = g.origin + g.h * np.array([ix, iy, iz])
+        r = np.linalg.norm(s.protein_xyz.astype(np.float64) - m, axis=1)
+        for k, t in enumerate(s.lig_types):
+            ref = sum(orc.pair(p, t, int(s.protein_type[j]), float(r[j]))[0] for j in range(len(r)) if abs(r[j] - 8.0) > 1e-5)
+            near = any(abs(r[j] - 8.0) <= 1e-5 for j in range(len(r)))
+            if not near:
+                assert abs(g.maps[k, iz, iy, ix] - ref) < 1e-12
+
+
+def test_fp32_cutoff_rule_only_matters_at_the_cutoff(orc):
+    s = make_system(0, seed=0)
+    p = orc.default_params()
+    a = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, 0.375, s.lig_types, fp32_cutoff=True)
+    b = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, 0.375, s.lig_types, fp32_cutoff=False)
+    diff = np.abs(a.maps - b.maps)
+    # a flipped pair changes a node by |f(cutoff^-)| <= ~0.006; everything else is identical
+    assert diff.max() < 0.01
+    assert (diff > 0).mean() < 1e-3
+
+
+def test_grid_geometry(orc):
+    dims, org = orc.grid_geometry([1.0, 2.0, 3.0], [15.0, 30.0, 60.0], 0.375)
+    assert dims == [41, 81, 161]
+    assert org == [1.0 - 7.5, 2.0 - 15.0, 3.0 - 30.0]
+
+
+# ----------------------------------------------------------------------------- O4 interpolation + wall
+def test_trilinear_reproduces_affine_function_and_gradient(orc):
+    p = orc.default_params()
+    a, b = 0.7, (0.3, -1.1, 2.5)
+    g = _affine_grid(orc, a=a, b=b)
+    L = _single_atom_ligand(orc, 0)
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        x = g.origin + rng.random(3) * g.h * 8
+        pose = np.concatenate([x, [1, 0, 0, 0]])
+        e, terms, grad, _ = orc.evaluate(p, g, L, pose)
+        assert abs(e - (a + np.dot(b, x))) < 1e-12
+        assert np.allclose(grad[:3], b, atol=1e-11)
+        assert np.allclose(grad[3:6], 0.0, atol=1e-12)  # atom sits on the pivot
+        assert terms[1] == 0.0 and terms[2] == 0.0
+
+
+def test_trilinear_node_values_and_eq2_eq3_closed_form(orc):
+    p = orc.default_params()
+    rng = np.random.default_rng(6)
+    n, h, origin = 6, 0.375, np.array([0.5, 0.25, -1.0])
+    data = rng.normal(size=(1, n, n, n))
+    g = orc.Grid((n, n, n), origin, h, [0], data)
+    L = _single_atom_ligand(orc, 0)
+    for iz in range(n):
+        for iy in range(n):
+            for ix in range(n):
+                x = origin + h * np.array([ix, iy, iz])
+                e, _, _, _ = orc.evaluate(p, g, L, np.concatenate([x, [1, 0, 0, 0]]))
+                assert abs(e - data[0, iz, iy, ix]) < 1e-13
+    # eq. 2 / eq. 3 written out independently with numpy on one cell
+    for _ in range(100):
+        i0 = rng.integers(n - 1, size=3)
+        pf = rng.random(3)
+        x = origin + h * (i0 + pf)
+        e, _, grad, _ = orc.evaluate(p, g, L, np.concatenate([x, [1, 0, 0, 0]]))
+        c = data[0, i0[2]:i0[2] + 2, i0[1]:i0[1] + 2, i0[0]:i0[0] + 2]  # [n][m][l]
+        wx, wy, wz = np.array([1 - pf[0], pf[0]]), np.array([1 - pf[1], pf[1]]), np.array([1 - pf[2], pf[2]])
+        dx = np.array([-1.0, 1.0]) / h
+        assert abs(e - np.einsum("nml,n,m,l->", c, wz, wy, wx)) < 1e-12
+        assert abs(grad[0] - np.einsum("nml,n,m,l->", c, wz, wy, dx)) < 1e-11
+        assert abs(grad[1] - np.einsum("nml,n,m,l->", c, wz, dx, wx)) < 1e-11
+        assert abs(grad[2] - np.einsum("nml,n,m,l->", c, dx, wy, wx)) < 1e-11
+
+
+def test_wall_is_quadratic_and_lookup_is_clamped(orc):
+    p = orc.default_params()
+    g = _affine_grid(orc, n=9, a=0.0, b=(1.0, 2.0, 3.0))
+    L = _single_atom_ligand(orc, 0)
+    hi = g.origin + g.h * 8
+    inside = g.origin + g.h * np.array([3.3, 4.4, 5.5])
+    # 1 A outside on +x: wall adds exactly k_wall = 10 and gradient 20 along x; grid gradient on x is 0
+    x = np.array([hi[0] + 1.0, inside[1], inside[2]])
+    e, terms, grad, d = orc.evaluate(p, g, L, np.concatenate([x, [1, 0, 0, 0]]))
+    assert abs(terms[1] - 10.0) < 1e-12
+    assert abs(grad[0] - 20.0) < 1e-12
+    assert abs(grad[1] - 2.0) < 1e-11 and abs(grad[2] - 3.0) < 1e-11
+    assert abs(terms[0] - (1.0 * hi[0] + 2.0 * x[1] + 3.0 * x[2])) < 1e-11
+    assert d.atoms_outside == 1
+    # 0.5 A outside on -y and 2 A outside on +z
+    x = np.array([inside[0], g.origin[1] - 0.5, hi[2] + 2.0])
+    e, terms, grad, _ = orc.evaluate(p, g, L, np.concatenate([x, [1, 0, 0, 0]]))
+    assert abs(terms[1] - (10 * 0.25 + 10 * 4.0)) < 1e-12
+    assert abs(grad[1] + 10.0) < 1e-12 and abs(grad[2] - 40.0) < 1e-12 and abs(grad[0] - 1.0) < 1e-11
+    assert abs(terms[0] - (x[0] + 2.0 * g.origin[1] + 3.0 * hi[2])) < 1e-11
+
+
+# ----------------------------------------------------------------------------- O3 kinematics
+def test_identity_pose_reproduces_reference(orc, tiny):
+    s, p, g, L = tiny
+    root = s.ligand.ref_xyz[s.ligand.frag == 0].mean(axis=0)
+    pose = np.concatenate([root, [1, 0, 0, 0], np.zeros(L.T)])
+    assert np.allclose(orc.coords(L, pose), s.ligand.ref_xyz, atol=1e-13)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 4])
+def test_pose_preserves_bonds_and_rigid_fragments(orc, cfg):
+    s = make_system(cfg, seed=2)
+    L = orc.Ligand(s.ligand)
+    rng = np.random.default_rng(7)
+    ref = s.ligand.ref_xyz
+    for _ in range(10):
+        x = orc.coords(L, _random_pose(rng, L.T, [3, -4, 5]))
+        for (i, j) in s.ligand.bonds:
+            assert abs(np.linalg.norm(x[i] - x[j]) - 1.5) < 1e-10
+        for f in range(L.T + 1):
+            idx = np.where(s.ligand.frag == f)[0]
+            if len(idx) > 1:
+                d0 = np.linalg.norm(ref[idx][:, None] - ref[idx][None], axis=-1)
+                d1 = np.linalg.norm(x[idx][:, None] - x[idx][None], axis=-1)
+                assert np.allclose(d0, d1, atol=1e-10)
+
+
+def test_single_torsion_moves_only_its_subtree_by_a_rotation_about_the_axis(orc):
+    s = make_system(1, seed=4)
+    L = orc.Ligand(s.ligand)
+    lig = s.ligand
+    root = lig.ref_xyz[lig.frag == 0].mean(axis=0)
+    for k in range(L.T):
+        th = np.zeros(L.T)
+        th[k] = 0.7
+        x = orc.coords(L, np.concatenate([root, [1, 0, 0, 0], th]))
+        sub = set()
+        for f in range(1, L.T + 1):
+            ff = f
+            while ff > 0:
+                if ff == k + 1:
+                    sub.add(f)
+                    break
+                ff = int(lig.tors_parent[ff - 1])
+        a, b = lig.ref_xyz[lig.tors_a[k]], lig.ref_xyz[lig.tors_b[k]]
+        u = (b - a) / np.linalg.norm(b - a)
+        for i in range(L.N):
+            if int(lig.frag[i]) in sub:
+                v = lig.ref_xyz[i] - b
+                want = b + v * math.cos(0.7) + np.cross(u, v) * math.sin(0.7) + u * np.dot(u, v) * (1 - math.cos(0.7))
+                assert np.allclose(x[i], want, atol=1e-12)
+            else:
+                assert np.allclose(x[i], lig.ref_xyz[i], atol=1e-12)
+
+
+def test_rigid_body_part_is_t_plus_R_of_centered_coordinates(orc, tiny):
+    s, p, g, L = tiny
+    lig = s.ligand
+    root = lig.ref_xyz[lig.frag == 0].mean(axis=0)
+    # 90 degrees about z: (w,x,y,z) = (c,0,0,s)
+    q = [math.cos(math.pi / 4), 0, 0, math.sin(math.pi / 4)]
+    t = np.array([1.0, 2.0, 3.0])
+    x = orc.coords(L, np.concatenate([t, q, np.zeros(L.T)]))
+    y = lig.ref_xyz - root
+    want = t + np.stack([-y[:, 1], y[:, 0], y[:, 2]], axis=1)
+    assert np.allclose(x, want, atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- O5/O6 gradients
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_total_gradient_vs_central_differences(orc, cfg):
+    s = make_system(cfg, seed=0)
+    p = orc.default_params()
+    if cfg == 0:
+        g = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
+    else:  # a smooth random grid is enough to exercise the chain rule on the 6-torsion ligand
+        rng0 = np.random.default_rng(0)
+        n = 33
+        g = orc.Grid((n, n, n), np.array(s.box_center, float) - 6.0, 0.375, s.lig_types,
+                     rng0.normal(size=(len(s.lig_types), n, n, n)))
+    L = orc.Ligand(s.ligand)
+    rng = np.random.default_rng(11)
+    checked = 0
+    while checked < 12:
+        pose = _random_pose(rng, L.T, s.box_center, spread=3.0)
+        e, terms, grad, d = orc.evaluate(p, g, L, pose)
+        if d.face_margin < 1e-4 or d.kink_margin < 1e-4:
+            continue
+        hh = 1e-6
+        for k in range(6 + L.T):
+            sv = np.zeros(6 + L.T)
+            sv[k] = hh
+            ep = orc.evaluate(p, g, L, orc.pose_add(L.T, pose, sv))[0]
+            em = orc.evaluate(p, g, L, orc.pose_add(L.T, pose, -sv))[0]
+            fd = (ep - em) / (2 * hh)
+            assert abs(fd - grad[k]) < 2e-6 * max(1.0, abs(grad[k])), (cfg, k, fd, grad[k])
+        checked += 1
+
+
+def test_intra_term_is_rigid_motion_invariant_with_zero_net_force_and_torque(orc):
+    s = make_system(1, seed=0)
+    p = orc.default_params()
+    n = 9
+    zero = orc.Grid((n, n, n), [-500.0, -500.0, -500.0], 125.0, s.lig_types, np.zeros((len(s.lig_types), n, n, n)))
+    L = orc.Ligand(s.ligand)
+    rng = np.random.default_rng(13)
+    for _ in range(10):
+        th = rng.uniform(-np.pi, np.pi, L.T)
+        ref_e = None
+        for _ in range(4):
+            pose = _random_pose(rng, L.T, [0, 0, 0], spread=50.0)
+            pose[7:] = th
+            e, terms, grad, d = orc.evaluate(p, zero, L, pose)
+            assert terms[0] == 0.0 and terms[1] == 0.0
+            assert np.allclose(grad[:6], 0.0, atol=1e-9)  # sum g_i = 0 and sum (x_i - t) x g_i = 0
+            ref_e = e if ref_e is None else ref_e
+            assert abs(e - ref_e) < 1e-10 * max(1.0, abs(ref_e))
+
+
+def test_intra_energy_is_the_plain_pair_sum(orc):
+    s = make_system(2, seed=1)
+    p = orc.default_params()
+    n = 5
+    zero = orc.Grid((n, n, n), [-500.0] * 3, 250.0, s.lig_types, np.zeros((len(s.lig_types), n, n, n)))
+    L = orc.Ligand(s.ligand)
+    rng = np.random.default_rng(17)
+    pose = _random_pose(rng, L.T, [0, 0, 0])
+    e, terms, _, d = orc.evaluate(p, zero, L, pose)
+    x = orc.coords(L, pose)
+    want, n_in = 0.0, 0
+    for (i, j) in s.ligand.pairs:
+        r = float(np.linalg.norm(x[i] - x[j]))
+        want += orc.pair(p, int(s.ligand.type[i]), int(s.ligand.type[j]), r)[0]
+        n_in += r < 8.0
+    assert abs(terms[2] - want) < 1e-12 and d.pairs_in_range == n_in
+
+
+# ----------------------------------------------------------------------------- O8 BFGS (generic core)
+def test_bfgs_reaches_closed_form_minimiser_of_convex_quadratic(orc):
+    p = orc.default_params()
+    rng = np.random.default_rng(19)
+    for n in (2, 5, 13, 21):
+        M = rng.normal(size=(n, n))
+        A = M @ M.T + n * np.eye(n)
+        b = rng.normal(size=n)
+        xstar = np.linalg.solve(A, b)
+        fs, Hs, secant_ok = [], [], []
+
+        def obs(it, f, H, s, y, updated):
+            fs.append(f)
+            Hs.append(H)
+            if updated:
+                secant_ok.append(np.allclose(H @ y, s, rtol=1e-9, atol=1e-12))
+
+        f, x, it, ne = orc.bfgs_generic(p, rng.normal(size=n) * 3, lambda x: (0.5 * x @ A @ x - b @ x, A @ x - b), 500, obs)
+        assert np.linalg.norm(A @ x - b) < p.bfgs_gtol
+        assert np.allclose(x, xstar, atol=1e-3)
+        assert abs(f - (0.5 * xstar @ A @ xstar - b @ xstar)) < 1e-6
+        assert all(f1 <= f0 + 1e-15 for f0, f1 in zip(fs, fs[1:]))      # monotone
+        assert secant_ok and all(secant_ok)                              # H_{k+1} y = s
+        for H in Hs:
+            assert np.allclose(H, H.T, atol=1e-10)
+            assert np.linalg.eigvalsh(0.5 * (H + H.T)).min() > 0.0        # stays SPD
+        assert it <= 4 * n + 10 and ne >= it + 1
+
+
+def test_bfgs_first_step_length_and_armijo_rule(orc):
+    p = orc.default_params()
+    calls = []
+
+    def fn(x):
+        calls.append(x.copy())
+        return 0.5 * 100.0 * float(x @ x), 100.0 * x
+
+    x0 = np.array([3.0, 4.0])
+    orc.bfgs_generic(p, x0, fn, 1)
+    # iteration 0: d = -g = -(300, 400), |d| = 500 > 1 -> alpha0 = 1/500; trial point = x0 + d/500
+    assert np.allclose(calls[1], x0 - np.array([300.0, 400.0]) / 500.0)
+    # f(x0)=1250, trial f = 0.5*100*(2.4^2+3.2^2) = 800 <= 1250 - 1e-4*(1/500)*250000 -> accepted at the first trial
+    assert len(calls) == 2
+
+
+def test_bfgs_stops_when_line_search_fails_and_respects_cap(orc):
+    p = orc.default_params()
+    # gradient reported with the wrong sign: no trial can satisfy Armijo -> 12 trials, then stop
+    f, x, it, ne = orc.bfgs_generic(p, np.array([1.0, 1.0]), lambda x: (float(x @ x), -2.0 * x), 50)
+    assert it == 0 and ne == 1 + p.bfgs_max_trials and np.allclose(x, [1.0, 1.0])
+    f, x, it, ne = orc.bfgs_generic(p, np.array([5.0, -3.0, 2.0]), lambda x: (float(np.sum(x ** 4)), 4 * x ** 3), 3)
+    assert it == 3
+
+
+def test_local_opt_pulls_atom_back_to_the_box(orc):
+    p = orc.default_params()
+    n = 9
+    g = orc.Grid((n, n, n), [0.0, 0.0, 0.0], 0.375, [0], np.zeros((1, n, n, n)))
+    L = _single_atom_ligand(orc, 0)
+    e0 = orc.evaluate(p, g, L, [5.0, -1.0, 4.5, 1, 0, 0, 0])[0]
+    assert abs(e0 - 10.0 * (4.0 + 1.0 + 2.25)) < 1e-12
+    e, pose, it, ne = orc.local_opt(p, g, L, [5.0, -1.0, 4.5, 1, 0, 0, 0], 100)
+    assert e < 1e-6 and it < 100
+
+
+def test_local_opt_never_increases_energy(orc, tiny):
+    s, p, g, L = tiny
+    rng = np.random.default_rng(23)
+    for _ in range(10):
+        pose = _random_pose(rng, L.T, s.box_center, spread=6.0)
+        e0 = orc.evaluate(p, g, L, pose)[0]
+        e1, out, it, ne = orc.local_opt(p, g, L, pose, 50)
+        assert e1 <= e0 and abs(orc.evaluate(p, g, L, out)[0] - e1) < 1e-12
+        assert abs(np.linalg.norm(out[3:7]) - 1.0) < 1e-12
+        assert ne >= it + 1
+
+
+# ----------------------------------------------------------------------------- O9 Monte Carlo
+def test_initial_poses_are_fp32_inside_the_box_with_unit_quaternions(orc):
+    c, sz = [1.0, -2.0, 3.0], [30.0, 30.0, 30.0]
+    P = orc.init_poses(c, sz, 7, 42, 3, 200)
+    assert np.array_equal(P, P.astype(np.float32).astype(np.float64))
+    assert np.all(np.abs(P[:, :3] - np.array(c)) <= 15.0)
+    assert np.allclose(np.linalg.norm(P[:, 3:7], axis=1), 1.0, atol=1e-6)
+    assert np.all(np.abs(P[:, 7:]) <= np.pi + 1e-6)
+    # different copies / systems / seeds give different poses; same arguments reproduce
+    assert not np.allclose(P[0], P[1])
+    assert np.array_equal(orc.init_pose(c, sz, 7, 42, 3, 5), P[5])
+    assert not np.allclose(orc.init_pose(c, sz, 7, 42, 4, 5), P[5])
+    # uniformity of t (coarse): mean near centre, std near size/sqrt(12)
+    assert np.all(np.abs(P[:, :3].mean(axis=0) - np.array(c)) < 3.0)
+    assert np.all(np.abs(P[:, :3].std(axis=0) - 30 / math.sqrt(12)) < 2.0)
+
+
+def test_perturbation_kinds_and_amplitudes(orc, tiny):
+    s, p, g, L = tiny
+    rng = np.random.default_rng(29)
+    pose = _random_pose(rng, L.T, s.box_center)
+    kinds = np.zeros(3, int)
+    for step in range(300):
+        kind, cand = orc.mc_perturb(p, L.T, 9, 0, 1, step, pose)
+        kinds[kind] += 1
+        changed_t = not np.array_equal(cand[:3], pose[:3])
+        changed_q = not np.array_equal(cand[3:7], pose[3:7])
+        changed_th = np.sum(cand[7:] != pose[7:])
+        if kind == 0:
+            assert changed_t and not changed_q and changed_th == 0
+            assert np.all(np.abs(cand[:3] - pose[:3]) <= 2.0)
+        elif kind == 1:
+            assert changed_q and not changed_t and changed_th == 0
+            dq = abs(float(np.dot(cand[3:7], pose[3:7])))
+            assert 2 * math.acos(min(1.0, dq)) <= 0.3 * math.sqrt(3) + 1e-9
+            assert abs(np.linalg.norm(cand[3:7]) - 1) < 1e-12
+        else:
+            assert changed_th == 1 and not changed_t and not changed_q
+            assert np.all(np.abs(cand[7:]) <= np.pi)
+    assert kinds.min() > 60  # uniform over the three kinds
+
+
+def test_search_invariants(orc, tiny):
+    s, p, g, L = tiny
+    init = orc.init_poses(s.box_center, s.box_size, L.T, 0, 0, 6)
+    # steps = 0 -> local_opt(init)
+    r0 = orc.search(p, g, L, init, 0, 50, 0)
+    for c in range(6):
+        e, out, _, _ = orc.local_opt(p, g, L, init[c], 50)
+        assert r0["best_e"][c] == e and np.array_equal(r0["best_pose"][c], out)
+    r = orc.search(p, g, L, init, 20, 50, 0)
+    tr = r["trace"]
+    for c in range(6):
+        acc_e = [r["init_rec"]["e_cand"][c]] + [tr["e_cand"][c, k] for k in range(20) if tr["accept"][c, k]]
+        assert abs(r["best_e"][c] - min(acc_e)) < 1e-15          # best <= every accepted E
+        assert abs(orc.evaluate(p, g, L, r["best_pose"][c])[0] - r["best_e"][c]) < 1e-12
+        # downhill always accepted; uphill accepted iff u < exp(-dE/T)
+        for k in range(20):
+            de = tr["e_cand"][c, k] - tr["e_cur"][c, k]
+            want = de < 0 or tr["u"][c, k] < math.exp(-de / p.t_mc)
+            assert bool(tr["accept"][c, k]) == want
+    # a copy's result does not depend on how many copies run
+    r3 = orc.search(p, g, L, init[:3], 20, 50, 0)
+    assert np.array_equal(r3["best_e"], r["best_e"][:3]) and np.array_equal(r3["best_pose"], r["best_pose"][:3])
+    assert r["evals"] == int(r["init_rec"]["evals"].sum() + tr["evals"].sum())
+
+
+def test_zero_temperature_search_is_monotone(orc, tiny):
+    s, p, g, L = tiny
+    import ctypes
+    q = orc.Params()
+    ctypes.memmove(ctypes.byref(q), ctypes.byref(p), ctypes.sizeof(q))
+    q.t_mc = 1e-12
+    init = orc.init_poses(s.box_center, s.box_size, L.T, 1, 0, 4)
+    r = orc.search(q, g, L, init, 20, 50, 1)
+    tr = r["trace"]
+    for c in range(4):
+        assert np.all(np.diff(tr["e_cur"][c]) <= 0.0)
+        assert np.all(tr["accept"][c] == (tr["e_cand"][c] < tr["e_cur"][c]))
+
+
+# ----------------------------------------------------------------------------- O10 top-k / clustering
+def test_rmsd_definition(orc, tiny):
+    s, p, g, L = tiny
+    rng = np.random.default_rng(31)
+    a, b = _random_pose(rng, L.T, [0, 0, 0]), _random_pose(rng, L.T, [0, 0, 0])
+    xa, xb = orc.coords(L, a), orc.coords(L, b)
+    assert abs(orc.rmsd(L, a, b) - math.sqrt(np.mean(np.sum((xa - xb) ** 2, axis=1)))) < 1e-12
+    a2 = a.copy()
+    a2[0] += 3.0
+    assert abs(orc.rmsd(L, a, a2) - 3.0) < 1e-12
+
+
+def test_topk_against_brute_force_and_properties(orc, tiny):
+    s, p, g, L = tiny
+    rng = np.random.default_rng(37)
+    for trial in range(5):
+        n = 40
+        centers = rng.normal(size=(6, 3)) * 4
+        poses = np.stack([_random_pose(rng, L.T, centers[rng.integers(6)], spread=1.0) for _ in range(n)])
+        e = rng.normal(size=n).round(1)  # ties on purpose
+        k = 5
+        cnt, idx = orc.topk(p, L, poses, e, k, 2.0)
+        # brute force with numpy
+        X = np.stack([orc.coords(L, q) for q in poses])
+        order = sorted(range(n), key=lambda i: (e[i], i))
+        kept = []
+        for i in order:
+            if len(kept) == k:
+                break
+            if all(math.sqrt(np.mean(np.sum((X[i] - X[j]) ** 2, axis=1))) >= 2.0 for j in kept):
+                kept.append(i)
+        assert cnt == len(kept) and list(idx[:cnt]) == kept
+        assert all(e[idx[a]] <= e[idx[a + 1]] for a in range(cnt - 1))
