@@ -225,7 +225,8 @@ def make_ligand(rng, N: int, T: int, lig_types: Sequence[int], carbon_frac=0.65)
         pairs = [(i, j) for i in range(N) for j in range(i + 1, N)
                  if frag[i] != frag[j] and dist[i, j] >= 4]
         return Ligand(
-            ref_xyz=np.ascontiguousarray(xyz, dtype=np.float64),
+            # fp32-representable values (stored as float64): the CUDA library takes fp32, the oracle widens them
+            ref_xyz=np.ascontiguousarray(xyz.astype(np.float32), dtype=np.float64),
             type=typ,
             frag=frag,
             tors_parent=np.array(tors_parent, dtype=np.int32).reshape(T),

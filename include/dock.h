@@ -1,0 +1,199 @@
+/*
+ * dock.h -- C-ABI of the B200-native docking hot path of DSDP (arxiv 2303.09916).
+ *
+ * ONE thing lives behind this header: the data-parallel hot path of DSDP's docking stage
+ * (Appendix): per-type grid maps of the Vina-style pair
+ * potential, fused pose -> coordinates -> trilinear energy + analytic gradient, an on-device
+ * many-copy Monte-Carlo search with a BFGS local optimizer, and top-k + RMSD clustering.
+ * All of it runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions:
+ *  - Plain C, no exceptions.  Every function returns an int status: DOCK_OK (0) or a negative code.
+ *  - The library OWNS NOTHING on the device: grids, poses, outputs and the scratch workspace are
+ *    allocated by the caller and passed as raw device pointers ("_dev").  Small topology /
+ *    parameter structs are HOST pointers; they are validated, compiled and copied into the
+ *    workspace by the call and may be freed as soon as the call returns.
+ *  - All work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as void*;
+ *    NULL = the legacy default stream).  The *_dev entry points never synchronise the device.
+ *    The *_host entry points take host buffers, copy in/out on `stream` and synchronise that
+ *    stream before returning.
+ *  - Workspace protocol: if `ws_bytes` is smaller than required (or ws_dev is NULL) the call does
+ *    no work, writes the requirement to *needed (if non-NULL) and returns DOCK_EWORKSPACE.
+ *  - Units: Angstrom, kcal/mol, radians.  Arrays are C-contiguous, fp32 / int32 unless stated.
+ *  - pose = [t(3), q(w,x,y,z), theta(T)] (7+T floats); t is the position of the pivot (centroid
+ *    of the root-fragment reference atoms), q the orientation (normalised on read).
+ *    grad = [dE/dt(3), torque(3) (lab frame, about t), dE/dtheta(T)] (6+T floats).
+ */
+#ifndef DOCK_H
+#define DOCK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DOCK_MAX_XS_TYPES 32   /* size of the XS type table */
+#define DOCK_MAX_TORSIONS 32   /* T <= 32 */
+#define DOCK_MAX_ATOMS    128  /* N <= 128 ligand heavy atoms */
+#define DOCK_MAX_TOPK     32
+
+#define DOCK_OK          0
+#define DOCK_EINVAL     (-1)   /* null pointer, bad size, malformed torsion tree, type without a map ... */
+#define DOCK_EWORKSPACE (-2)   /* workspace too small; *needed holds the requirement */
+#define DOCK_ECUDA      (-3)   /* a CUDA call failed; see dock_last_cuda_error() */
+
+/* Scoring + search parameters.  The paper prints none of them ("the same scoring
+ * function" as Vina); dock_default_params() fills the readings S1, S2, S3, S7, S12, S14, S15, S19
+ * of SURVEY.md 8(c). */
+typedef struct dock_params {
+    int32_t n_types;                          /* number of XS type ids in use (17) */
+    float   radius[DOCK_MAX_XS_TYPES];        /* XS radius per type id */
+    int32_t hydrophobic[DOCK_MAX_XS_TYPES];
+    int32_t donor[DOCK_MAX_XS_TYPES];
+    int32_t acceptor[DOCK_MAX_XS_TYPES];
+    float   w[5];                             /* gauss1, gauss2, repulsion, hydrophobic, hbond */
+    float   cutoff;                           /* 8 A; a pair counts iff r < cutoff (decided in fp32) */
+    float   k_wall;                           /* quadratic wall, kcal/mol/A^2 per axis overshoot */
+    float   t_mc;                             /* Metropolis temperature, kcal/mol */
+    float   amp_trans;                        /* MC translation amplitude per axis, A */
+    float   amp_rot;                          /* MC rotation-vector amplitude per component, rad */
+    float   bfgs_c1;                          /* Armijo constant */
+    float   bfgs_shrink;                      /* backtracking factor */
+    int32_t bfgs_max_trials;                  /* line-search trials per iteration */
+    float   bfgs_gtol;                        /* stop when ||g||_2 < gtol */
+    float   bfgs_curv_eps;                    /* skip the update if y.s <= eps ||s|| ||y|| */
+    float   cluster_rmsd;                     /* top-k clustering radius, A (PAPER.md:81 RMSD) */
+    int32_t topk;                             /* number of poses to report, <= DOCK_MAX_TOPK */
+} dock_params;
+
+/* Search / interpolation box: n_axis = round(size/spacing)+1 nodes,
+ * origin = fl32(center - size/2). */
+typedef struct dock_box {
+    float center[3];
+    float size[3];
+    float spacing;
+} dock_box;
+
+typedef struct dock_protein {   /* HOST arrays */
+    int32_t        n;
+    const float   *xyz;         /* [n][3] */
+    const int32_t *type;        /* [n] XS type ids */
+} dock_protein;
+
+/* Flexible ligand as a torsion tree; HOST arrays.  Fragment 0 is the root; torsion k joins
+ * fragment tors_parent[k] (<= k) to fragment k+1, rotating fragment k+1 and its descendants by
+ * theta_k (right-handed) about the axis ref[tors_a[k]] -> ref[tors_b[k]] (a in the parent
+ * fragment, b in fragment k+1).  theta = 0 reproduces ref_xyz. */
+typedef struct dock_ligand {
+    int32_t        N, T, P;
+    const float   *ref_xyz;        /* [N][3] reference conformation */
+    const int32_t *type;           /* [N] XS type ids */
+    const int32_t *atom_fragment;  /* [N] */
+    const int32_t *tors_parent;    /* [T] */
+    const int32_t *tors_a;         /* [T] */
+    const int32_t *tors_b;         /* [T] */
+    const int32_t *pairs;          /* [P][2] intra-ligand scoring pairs, i != j */
+} dock_ligand;
+
+/* Grid-map descriptor written by dock_build_grids.  data layout: [n_maps][nz][ny][nx] fp32,
+ * node (ix,iy,iz) at origin + spacing*(ix,iy,iz) (eq. 2 at 198-199). */
+typedef struct dock_grid {
+    int32_t      dims[3];                          /* nx, ny, nz */
+    float        origin[3];
+    float        spacing;
+    int32_t      n_maps;
+    int32_t      type_to_map[DOCK_MAX_XS_TYPES];   /* XS type id -> map index, -1 = absent */
+    const float *data_dev;                         /* DEVICE pointer, caller-owned */
+} dock_grid;
+
+/* Optional per-(system, copy, step) trace of the search; with the stateless Philox counter it
+ * is enough to replay any single MC step (teacher-forced parity).
+ * One record = DOCK_TRACE_HEADER floats followed by the pre-step pose (7+T_max floats). */
+#define DOCK_TRACE_HEADER 8   /* e_cur, e_cand, u, accept, iters, evals, kind, reserved */
+
+/* ---- parameters ----------------------------------------------------------------------------- */
+int dock_default_params(dock_params *out);
+
+/* ---- A1: grid maps ----------------------------------------
+ * G[m][node] = sum over protein atoms j with |node - r_j| < cutoff of f(lig_types[m], type_j, r).
+ * protein: host.  grid_dev: device, n_lig_types * nx*ny*nz floats (see dock_grid_dims).
+ * out_desc (host) receives the descriptor with data_dev = grid_dev.
+ * Errors: DOCK_EINVAL for null pointers, n < 0, spacing <= 0, type ids outside [0, n_types). */
+int dock_grid_dims(const dock_box *box, int32_t dims[3]);
+int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
+                     int32_t n_lig_types, const int32_t *lig_types,
+                     float *grid_dev, dock_grid *out_desc,
+                     void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- A2-A5: fused pose -> coordinates -> energy + gradient (eq. 2-3 at 198-219) --
+ * poses_dev [n_poses][7+T]; energy_dev [n_poses]; grad_dev [n_poses][6+T] or NULL;
+ * terms_dev [n_poses][3] = (E_grid, E_wall, E_intra) or NULL.  E = sum of the three terms. */
+int dock_score_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                     int64_t n_poses, const float *poses_dev,
+                     float *energy_dev, float *grad_dev, float *terms_dev,
+                     void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* Same, with HOST buffers for poses / energy / grad / terms (copies inside the call). */
+int dock_score_batch_host(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                          int64_t n_poses, const float *poses_host,
+                          float *energy_host, float *grad_host, float *terms_host,
+                          void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- A6: BFGS local optimisation of a batch of start poses -----------------------
+ * poses_dev [n][7+T] in; out_pose_dev [n][7+T]; out_e_dev [n]; out_iters_dev [n][2] = (iters, evals) or NULL */
+int dock_local_opt_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                         int64_t n_poses, int32_t max_iters, const float *poses_dev,
+                         float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
+                         void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- S16: initial poses from Philox ("randomly generated within this box", 67) ----
+ * Generated on the host in double, rounded once to fp32.  out_host [copies][7+T]. */
+int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
+                    float *out_host);
+
+/* ---- A6-A8: many-copy Monte-Carlo search + top-k -----------------------------
+ * n_systems independent systems in one launch; grids[s], ligands[s], boxes[s] are HOST arrays of
+ * descriptors.  T_max = max over systems of T; pose rows are 7+T_max floats wide (unused tail 0).
+ * init_poses_dev [n_systems][copies][7+T_max] or NULL (then generated by dock_init_poses' rule).
+ * best_pose_dev [n_systems][copies][7+T_max]; best_e_dev [n_systems][copies];
+ * topk_pose_dev [n_systems][k][7+T_max]; topk_e_dev [n_systems][k]; topk_idx_dev [n_systems][k]
+ * (copy index, -1 = unused); topk_count_dev [n_systems]  (k = params->topk)  -- all nullable as a group;
+ * trace_dev [n_systems][copies][steps][DOCK_TRACE_HEADER + 7+T_max] or NULL;
+ * eval_counter_dev: one uint64, incremented by the number of score+gradient evaluations, or NULL. */
+int dock_search(const dock_params *params, int32_t n_systems,
+                const dock_grid *grids, const dock_ligand *ligands, const dock_box *boxes,
+                int32_t copies, int32_t steps, int32_t bfgs_max_iters, uint64_t seed,
+                const float *init_poses_dev,
+                float *best_pose_dev, float *best_e_dev,
+                float *topk_pose_dev, float *topk_e_dev, int32_t *topk_idx_dev, int32_t *topk_count_dev,
+                float *trace_dev, uint64_t *eval_counter_dev,
+                void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- A8 alone: rank + greedy RMSD clustering of given poses -----------------
+ * poses_dev [n][7+T], e_dev [n] -> out_idx_dev [k], out_count_dev [1]. */
+int dock_topk(const dock_params *params, const dock_ligand *ligand, int32_t n,
+              const float *poses_dev, const float *e_dev,
+              int32_t *out_idx_dev, int32_t *out_count_dev,
+              void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- end-to-end convenience with HOST buffers: build grids + search + top-k for one system ----
+ * out_topk_pose_host [k][7+T], out_topk_e_host [k], out_count_host [1]; copies H<->D inside. */
+int dock_system_host(const dock_params *params, const dock_protein *protein, const dock_box *box,
+                     const dock_ligand *ligand, int32_t n_lig_types, const int32_t *lig_types,
+                     int32_t copies, int32_t steps, int32_t bfgs_max_iters, uint64_t seed,
+                     float *out_topk_pose_host, float *out_topk_e_host, int32_t *out_count_host,
+                     uint64_t *out_evals_host,
+                     float *grid_dev, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- diagnostics ------------------------------------------------------------------------------ */
+int         dock_last_cuda_error(void);          /* cudaError_t of the last failing CUDA call (0 = none) */
+const char *dock_version(void);
+/* number of kernel launches issued by this library since load (for bench.py's gpu_launches) */
+uint64_t    dock_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DOCK_H */

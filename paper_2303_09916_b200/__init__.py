@@ -1,0 +1,29 @@
+"""B200-native docking hot path of DSDP (arxiv 2303.09916): C-ABI library + thin Python binding.
+
+The product is `libdock_b200.so` (hand-written sm_100a CUDA behind include/dock.h).  This package
+only marshals arguments; it never computes any step of the path on the CPU.
+"""
+from .binding import (  # noqa: F401
+    DOCK_TRACE_HEADER,
+    DockError,
+    EXPORTS,
+    GridMaps,
+    LigandHandle,
+    dock_box,
+    dock_build_grids,
+    dock_default_params,
+    dock_grid,
+    dock_grid_dims,
+    dock_init_poses,
+    dock_ligand,
+    dock_local_opt_batch,
+    dock_params,
+    dock_score_batch,
+    dock_score_batch_host,
+    dock_search,
+    dock_system_host,
+    dock_topk,
+    launch_count,
+    load_library,
+    make_box,
+)

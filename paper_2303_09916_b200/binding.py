@@ -1,0 +1,377 @@
+"""Thin ctypes binding of include/dock.h (argument marshalling only).
+
+Every step of the hot path runs inside libdock_b200.so's CUDA kernels; PyTorch is used here only
+to own device memory and to supply the CUDA stream.  There is no CPU fallback: if the shared
+library is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libdock_b200.so")
+
+DOCK_MAX_XS_TYPES = 32
+DOCK_MAX_TORSIONS = 32
+DOCK_MAX_ATOMS = 128
+DOCK_TRACE_HEADER = 8
+DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
+
+EXPORTS = [
+    "dock_default_params", "dock_grid_dims", "dock_build_grids", "dock_score_batch",
+    "dock_score_batch_host", "dock_local_opt_batch", "dock_init_poses", "dock_search", "dock_topk",
+    "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
+]
+
+
+class DockError(RuntimeError):
+    pass
+
+
+class dock_params(C.Structure):
+    _fields_ = [
+        ("n_types", C.c_int32),
+        ("radius", C.c_float * DOCK_MAX_XS_TYPES),
+        ("hydrophobic", C.c_int32 * DOCK_MAX_XS_TYPES),
+        ("donor", C.c_int32 * DOCK_MAX_XS_TYPES),
+        ("acceptor", C.c_int32 * DOCK_MAX_XS_TYPES),
+        ("w", C.c_float * 5),
+        ("cutoff", C.c_float), ("k_wall", C.c_float), ("t_mc", C.c_float),
+        ("amp_trans", C.c_float), ("amp_rot", C.c_float),
+        ("bfgs_c1", C.c_float), ("bfgs_shrink", C.c_float), ("bfgs_max_trials", C.c_int32),
+        ("bfgs_gtol", C.c_float), ("bfgs_curv_eps", C.c_float),
+        ("cluster_rmsd", C.c_float), ("topk", C.c_int32),
+    ]
+
+
+class dock_box(C.Structure):
+    _fields_ = [("center", C.c_float * 3), ("size", C.c_float * 3), ("spacing", C.c_float)]
+
+
+class dock_protein(C.Structure):
+    _fields_ = [("n", C.c_int32), ("xyz", C.c_void_p), ("type", C.c_void_p)]
+
+
+class dock_ligand(C.Structure):
+    _fields_ = [
+        ("N", C.c_int32), ("T", C.c_int32), ("P", C.c_int32),
+        ("ref_xyz", C.c_void_p), ("type", C.c_void_p), ("atom_fragment", C.c_void_p),
+        ("tors_parent", C.c_void_p), ("tors_a", C.c_void_p), ("tors_b", C.c_void_p), ("pairs", C.c_void_p),
+    ]
+
+
+class dock_grid(C.Structure):
+    _fields_ = [
+        ("dims", C.c_int32 * 3), ("origin", C.c_float * 3), ("spacing", C.c_float),
+        ("n_maps", C.c_int32), ("type_to_map", C.c_int32 * DOCK_MAX_XS_TYPES), ("data_dev", C.c_void_p),
+    ]
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libdock_b200.so (built in-tree by build.py).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        path = path or _LIB_PATH
+        if not os.path.exists(path):
+            raise DockError(f"{path} not found: run `python -m paper_2303_09916_b200.build` "
+                            "(there is no CPU fallback)")
+        _lib = C.CDLL(path)
+        _lib.dock_version.restype = C.c_char_p
+        _lib.dock_launch_count.restype = C.c_uint64
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc == DOCK_OK:
+        return
+    names = {DOCK_EINVAL: "DOCK_EINVAL", DOCK_EWORKSPACE: "DOCK_EWORKSPACE", DOCK_ECUDA: "DOCK_ECUDA"}
+    extra = ""
+    if rc == DOCK_ECUDA:
+        extra = f" (cudaError {load_library().dock_last_cuda_error()})"
+    raise DockError(f"{what} failed: {names.get(rc, rc)}{extra}")
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise DockError("no CUDA device: the docking hot path has no CPU fallback")
+    return torch
+
+
+def _stream(stream=None) -> C.c_void_p:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _ptr(t) -> C.c_void_p:
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _np_ptr(a: Optional[np.ndarray]) -> C.c_void_p:
+    return C.c_void_p(0) if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class _Workspace:
+    """Grow-only device scratch buffer (a torch uint8 tensor) reused across calls."""
+
+    def __init__(self):
+        self.buf = None
+
+    def get(self, nbytes: int):
+        torch = _torch()
+        if self.buf is None or self.buf.numel() < nbytes:
+            self.buf = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device="cuda")
+        return self.buf
+
+
+_ws = _Workspace()
+
+
+def launch_count() -> int:
+    return int(load_library().dock_launch_count())
+
+
+def dock_default_params() -> dock_params:
+    p = dock_params()
+    _check(load_library().dock_default_params(C.byref(p)), "dock_default_params")
+    return p
+
+
+def make_box(center, size, spacing) -> dock_box:
+    b = dock_box()
+    for c in range(3):
+        b.center[c] = float(center[c])
+        b.size[c] = float(size[c])
+    b.spacing = float(spacing)
+    return b
+
+
+class LigandHandle:
+    """Host arrays (fp32 / int32) + the dock_ligand struct pointing at them."""
+
+    def __init__(self, lig):
+        self.ref = np.ascontiguousarray(lig.ref_xyz, dtype=np.float32)
+        self.type = np.ascontiguousarray(lig.type, dtype=np.int32)
+        self.frag = np.ascontiguousarray(lig.frag, dtype=np.int32)
+        self.tors_parent = np.ascontiguousarray(lig.tors_parent, dtype=np.int32)
+        self.tors_a = np.ascontiguousarray(lig.tors_a, dtype=np.int32)
+        self.tors_b = np.ascontiguousarray(lig.tors_b, dtype=np.int32)
+        self.pairs = np.ascontiguousarray(lig.pairs, dtype=np.int32).reshape(-1, 2)
+        self.N, self.T, self.P = int(self.ref.shape[0]), int(self.tors_a.shape[0]), int(self.pairs.shape[0])
+        self.c = dock_ligand(self.N, self.T, self.P, _np_ptr(self.ref), _np_ptr(self.type), _np_ptr(self.frag),
+                             _np_ptr(self.tors_parent), _np_ptr(self.tors_a), _np_ptr(self.tors_b), _np_ptr(self.pairs))
+
+
+class GridMaps:
+    """Device grid maps (torch tensor [n_maps, nz, ny, nx]) + descriptor."""
+
+    def __init__(self, data, desc: dock_grid):
+        self.data = data
+        self.desc = desc
+
+    @property
+    def dims(self):
+        return tuple(self.desc.dims)
+
+
+def dock_grid_dims(box: dock_box):
+    d = (C.c_int32 * 3)()
+    _check(load_library().dock_grid_dims(C.byref(box), d), "dock_grid_dims")
+    return tuple(int(x) for x in d)
+
+
+def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_box,
+                     lig_types: Sequence[int], stream=None) -> GridMaps:
+    torch = _torch()
+    lib = load_library()
+    xyz = np.ascontiguousarray(protein_xyz, dtype=np.float32).reshape(-1, 3)
+    typ = np.ascontiguousarray(protein_type, dtype=np.int32)
+    prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
+    lt = np.ascontiguousarray(lig_types, dtype=np.int32)
+    nx, ny, nz = dock_grid_dims(box)
+    data = torch.empty((len(lt), nz, ny, nx), dtype=torch.float32, device="cuda")
+    desc = dock_grid()
+    need = C.c_size_t(0)
+    rc = lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
+                              None, None, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_build_grids(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
+                                _ptr(data), C.byref(desc), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
+                                _stream(stream)), "dock_build_grids")
+    return GridMaps(data, desc)
+
+
+def dock_score_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses,
+                     want_grad: bool = True, want_terms: bool = True, out=None, stream=None):
+    """poses: torch.cuda float32 [n, 7+T].  Returns (energy [n], grad [n,6+T] | None, terms [n,3] | None)."""
+    torch = _torch()
+    lib = load_library()
+    assert poses.is_cuda and poses.dtype == torch.float32 and poses.is_contiguous()
+    n = int(poses.shape[0])
+    assert poses.shape[1] == 7 + ligand.T
+    if out is None:
+        energy = torch.empty(n, dtype=torch.float32, device="cuda")
+        grad = torch.empty((n, 6 + ligand.T), dtype=torch.float32, device="cuda") if want_grad else None
+        terms = torch.empty((n, 3), dtype=torch.float32, device="cuda") if want_terms else None
+    else:
+        energy, grad, terms = out
+    need = C.c_size_t(0)
+    rc = lib.dock_score_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), None, None,
+                              None, None, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_score_batch(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_score_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), _ptr(poses),
+                                _ptr(energy), _ptr(grad), _ptr(terms), _ptr(ws), C.c_size_t(ws.numel()),
+                                C.byref(need), _stream(stream)), "dock_score_batch")
+    return energy, grad, terms
+
+
+def dock_score_batch_host(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses_host: np.ndarray,
+                          want_grad: bool = True, want_terms: bool = False, out=None, stream=None):
+    """HOST numpy (or pinned torch CPU) poses [n,7+T] in, host energy / grad / terms out; copies inside the call."""
+    lib = load_library()
+    _torch()
+    n = int(poses_host.shape[0])
+    hp = lambda a: C.c_void_p(0) if a is None else (C.c_void_p(a.data_ptr()) if hasattr(a, "data_ptr") else _np_ptr(a))
+    if out is None:
+        energy = np.empty(n, dtype=np.float32)
+        grad = np.empty((n, 6 + ligand.T), dtype=np.float32) if want_grad else None
+        terms = np.empty((n, 3), dtype=np.float32) if want_terms else None
+    else:
+        energy, grad, terms = out
+    need = C.c_size_t(0)
+    args = (C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), hp(poses_host), hp(energy), hp(grad), hp(terms))
+    rc = lib.dock_score_batch_host(*args, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_score_batch_host(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_score_batch_host(*args, _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)),
+           "dock_score_batch_host")
+    return energy, grad, terms
+
+
+def dock_local_opt_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses, max_iters: int, stream=None):
+    torch = _torch()
+    lib = load_library()
+    assert poses.is_cuda and poses.dtype == torch.float32 and poses.is_contiguous()
+    n = int(poses.shape[0])
+    out_pose = torch.empty_like(poses)
+    out_e = torch.empty(n, dtype=torch.float32, device="cuda")
+    out_it = torch.empty((n, 2), dtype=torch.int32, device="cuda")
+    need = C.c_size_t(0)
+    rc = lib.dock_local_opt_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), int(max_iters),
+                                  None, None, None, None, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_local_opt_batch(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_local_opt_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), int(max_iters),
+                                    _ptr(poses), _ptr(out_pose), _ptr(out_e), _ptr(out_it), _ptr(ws),
+                                    C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_local_opt_batch")
+    return out_pose, out_e, out_it
+
+
+def dock_init_poses(box: dock_box, T: int, seed: int, system: int, copies: int) -> np.ndarray:
+    out = np.zeros((copies, 7 + T), dtype=np.float32)
+    _check(load_library().dock_init_poses(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), int(copies),
+                                          _np_ptr(out)), "dock_init_poses")
+    return out
+
+
+def dock_search(params: dock_params, grids: Sequence[GridMaps], ligands: Sequence[LigandHandle],
+                boxes: Optional[Sequence[dock_box]], copies: int, steps: int, bfgs_max_iters: int, seed: int,
+                init_poses=None, want_trace: bool = False, want_topk: bool = True, stream=None):
+    """Many-copy MC search for n_systems systems in one launch.  Returns a dict of torch tensors."""
+    torch = _torch()
+    lib = load_library()
+    ns = len(grids)
+    assert len(ligands) == ns
+    t_max = max(l.T for l in ligands)
+    row = 7 + t_max
+    k = int(params.topk)
+    g_arr = (dock_grid * ns)(*[g.desc for g in grids])
+    l_arr = (dock_ligand * ns)(*[l.c for l in ligands])
+    b_arr = (dock_box * ns)(*boxes) if boxes is not None else None
+    dev = "cuda"
+    best_pose = torch.empty((ns, copies, row), dtype=torch.float32, device=dev)
+    best_e = torch.empty((ns, copies), dtype=torch.float32, device=dev)
+    topk_pose = torch.zeros((ns, k, row), dtype=torch.float32, device=dev) if want_topk else None
+    topk_e = torch.zeros((ns, k), dtype=torch.float32, device=dev) if want_topk else None
+    topk_idx = torch.full((ns, k), -1, dtype=torch.int32, device=dev) if want_topk else None
+    topk_cnt = torch.zeros(ns, dtype=torch.int32, device=dev) if want_topk else None
+    trace = torch.zeros((ns, copies, steps, DOCK_TRACE_HEADER + row), dtype=torch.float32, device=dev) if want_trace else None
+    evals = torch.zeros(1, dtype=torch.int64, device=dev)
+    if init_poses is not None:
+        assert init_poses.is_cuda and init_poses.dtype == torch.float32 and init_poses.is_contiguous()
+        assert tuple(init_poses.shape) == (ns, copies, row)
+    need = C.c_size_t(0)
+    head = (C.byref(params), ns, g_arr, l_arr, b_arr, int(copies), int(steps), int(bfgs_max_iters), C.c_uint64(seed),
+            _ptr(init_poses))
+    rc = lib.dock_search(*head, _ptr(best_pose), _ptr(best_e), None, None, None, None, None, None,
+                         None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_search(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_search(*head, _ptr(best_pose), _ptr(best_e), _ptr(topk_pose), _ptr(topk_e), _ptr(topk_idx),
+                           _ptr(topk_cnt), _ptr(trace), _ptr(evals), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
+                           _stream(stream)), "dock_search")
+    return dict(best_pose=best_pose, best_e=best_e, topk_pose=topk_pose, topk_e=topk_e, topk_idx=topk_idx,
+                topk_count=topk_cnt, trace=trace, evals=evals)
+
+
+def dock_topk(params: dock_params, ligand: LigandHandle, poses, e, stream=None):
+    torch = _torch()
+    lib = load_library()
+    n = int(poses.shape[0])
+    k = int(params.topk)
+    out_idx = torch.full((k,), -1, dtype=torch.int32, device="cuda")
+    out_cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    need = C.c_size_t(0)
+    rc = lib.dock_topk(C.byref(params), C.byref(ligand.c), n, None, None, None, None, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_topk(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_topk(C.byref(params), C.byref(ligand.c), n, _ptr(poses), _ptr(e), _ptr(out_idx), _ptr(out_cnt),
+                         _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_topk")
+    return out_idx, out_cnt
+
+
+def dock_system_host(params: dock_params, protein_xyz, protein_type, box: dock_box, ligand: LigandHandle,
+                     lig_types: Sequence[int], copies: int, steps: int, bfgs_max_iters: int, seed: int,
+                     grid_buf=None, stream=None):
+    """End to end for one system with HOST inputs/outputs: build grids + search + top-k."""
+    torch = _torch()
+    lib = load_library()
+    xyz = np.ascontiguousarray(protein_xyz, dtype=np.float32).reshape(-1, 3)
+    typ = np.ascontiguousarray(protein_type, dtype=np.int32)
+    prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
+    lt = np.ascontiguousarray(lig_types, dtype=np.int32)
+    nx, ny, nz = dock_grid_dims(box)
+    if grid_buf is None:
+        grid_buf = torch.empty((len(lt), nz, ny, nx), dtype=torch.float32, device="cuda")
+    k = int(params.topk)
+    out_pose = np.zeros((k, 7 + ligand.T), dtype=np.float32)
+    out_e = np.zeros(k, dtype=np.float32)
+    out_cnt = np.zeros(1, dtype=np.int32)
+    out_ev = np.zeros(1, dtype=np.uint64)
+    need = C.c_size_t(0)
+    head = (C.byref(params), C.byref(prot), C.byref(box), C.byref(ligand.c), len(lt), _np_ptr(lt), int(copies),
+            int(steps), int(bfgs_max_iters), C.c_uint64(seed), _np_ptr(out_pose), _np_ptr(out_e), _np_ptr(out_cnt),
+            _np_ptr(out_ev), _ptr(grid_buf))
+    rc = lib.dock_system_host(*head, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_system_host(size query)")
+    ws = _ws.get(need.value)
+    _check(lib.dock_system_host(*head, _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)),
+           "dock_system_host")
+    return dict(topk_pose=out_pose, topk_e=out_e, count=int(out_cnt[0]), evals=int(out_ev[0]))

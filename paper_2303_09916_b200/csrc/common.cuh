@@ -1,0 +1,123 @@
+// common.cuh -- device-side descriptors and small helpers shared by the kernels of libdock_b200.
+// Product code (sm_100a CUDA).  Shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dock.h"
+
+#define FULL_MASK 0xffffffffu
+
+// ---- host-side error plumbing -----------------------------------------------------------------
+extern int g_dock_last_cuda_error;
+extern unsigned long long g_dock_launches;
+
+#define DOCK_CUDA_CHECK(expr)                                   \
+    do {                                                        \
+        cudaError_t _e = (expr);                                \
+        if (_e != cudaSuccess) {                                \
+            g_dock_last_cuda_error = (int)_e;                   \
+            return DOCK_ECUDA;                                  \
+        }                                                       \
+    } while (0)
+
+#define DOCK_LAUNCH_CHECK()                                     \
+    do {                                                        \
+        ++g_dock_launches;                                      \
+        DOCK_CUDA_CHECK(cudaGetLastError());                    \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- device descriptors -----------------------------------------------------------------------
+struct DevParams {
+    float w[5];
+    float cutoff, cutoff2;
+    float k_wall;
+    float t_mc;
+    float amp_trans, amp_rot;
+    float c1, shrink, gtol, curv_eps;
+    int   max_trials;
+};
+
+struct DevGrid {
+    int   nx, ny, nz;
+    float ox, oy, oz;        // origin
+    float hx, hy, hz;        // coordinate of the last node on each axis
+    float h, inv_h;
+    const float *data;       // [n_maps][nz][ny][nx]
+};
+
+// One scheduled intra-ligand pair.  ij = i | (j << 16), or -1 for an idle lane.
+struct __align__(16) PairRec {
+    int   ij;
+    float rsum;   // R_i + R_j
+    float wh;     // w4 if both hydrophobic else 0
+    float whb;    // w5 if donor/acceptor pair else 0
+};
+
+// Compiled ligand (all pointers into the caller's workspace).
+struct DevLigand {
+    int N, T, P, n_rounds;
+    int n_pad;                 // stride of the per-warp coordinate arrays
+    const float4  *atom_ref;   // [N] reference xyz relative to the pivot; w = bitcast(map offset in floats)
+    const int2    *atom_topo;  // [N] {fragment, mask of torsions on the path to the root}
+    const float4  *tors_axis;  // [T] unit axis in the reference frame
+    const float4  *tors_pt;    // [T] reference position of atom b relative to the pivot; w = bitcast(parent fragment)
+    const int2    *tors_ab;    // [T] {a, b}
+    const PairRec *sched;      // [n_rounds][32] conflict-free pair schedule
+};
+
+struct DevSystem {
+    DevGrid   grid;
+    DevLigand lig;
+    float     box_lo[3], box_size[3];
+};
+
+// ---- device helpers ---------------------------------------------------------------------------
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum_d(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
+    return v;
+}
+__device__ __forceinline__ float fast_ex2(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float fast_rsqrt(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Philox4x32-10 (Salmon et al., SC'11).  counter = (copy, step, slot, system), key = seed lo/hi.
+__host__ __device__ inline void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long p0 = 0xD2511F53ull * (unsigned long long)c0;
+        const unsigned long long p1 = 0xCD9E8D57ull * (unsigned long long)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+

@@ -1,0 +1,244 @@
+// grid.cu -- A1: per-type grid maps over protein atoms binned into cells (eq. 2's inner
+// sum at PAPER.md:198-199).
+//
+//   G[m][iz][iy][ix] = sum_{j : |node - r_j| < cutoff} f(lig_types[m], type_j, |node - r_j|)
+//
+// Host: protein atoms are binned into cubic cells of edge = cutoff + 0.01 A over the box grown by the cutoff
+// (counting sort, stable -> fixed summation order).  Device: one thread per node, a warp covers a
+// compact 4x4x2 block of nodes so that its lanes share almost the same in-range atom set; each thread
+// walks the <= 27 cells around its node, decides r < cutoff in fp32 in the stated order
+// (DESIGN.md D-CUT) and accumulates up to 8 maps in registers.
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "host_compile.cuh"
+
+namespace {
+
+constexpr int MAPS_PER_PASS = 8;
+
+struct GridBuildArgs {
+    int   nx, ny, nz;
+    float ox, oy, oz, h;
+    float cutoff, cutoff2;
+    float clo[3];          // low corner of the cell lattice
+    float inv_cell;        // 1 / cell edge
+    int   ncx, ncy, ncz;
+    int   n_maps, n_types;
+    float w[5];
+    const float4 *atoms;   // sorted by cell; w = bitcast(type)
+    const int    *cell_start;
+    const float4 *pair_tab;// [n_maps][n_types] {rsum, wh, whb, 0}
+    float        *out;     // [n_maps][nz][ny][nx]
+};
+
+__global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
+{
+    __shared__ float4 tab[MAPS_PER_PASS * DOCK_MAX_XS_TYPES];
+    const int m0 = blockIdx.y * MAPS_PER_PASS;
+    const int nm = min(MAPS_PER_PASS, A.n_maps - m0);
+    for (int k = threadIdx.x; k < nm * A.n_types; k += blockDim.x) tab[k] = A.pair_tab[m0 * A.n_types + k];
+    __syncthreads();
+
+    // block tile 8 x 8 x 2 nodes; warp tile 4 x 4 x 2
+    const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8;
+    const int bx = blockIdx.x % tbx, by = (blockIdx.x / tbx) % tby, bz = blockIdx.x / (tbx * tby);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ix = bx * 8 + (warp & 1) * 4 + (lane & 3);
+    const int iy = by * 8 + (warp >> 1) * 4 + ((lane >> 2) & 3);
+    const int iz = bz * 2 + (lane >> 4);
+    if (ix >= A.nx || iy >= A.ny || iz >= A.nz) return;
+
+    // node coordinate exactly as the oracle's fp32 cutoff rule states it: fmaf(i, h, origin)
+    const float mx = __fmaf_rn((float)ix, A.h, A.ox);
+    const float my = __fmaf_rn((float)iy, A.h, A.oy);
+    const float mz = __fmaf_rn((float)iz, A.h, A.oz);
+    const int cx = (int)((mx - A.clo[0]) * A.inv_cell);
+    const int cy = (int)((my - A.clo[1]) * A.inv_cell);
+    const int cz = (int)((mz - A.clo[2]) * A.inv_cell);
+
+    float acc[MAPS_PER_PASS];
+#pragma unroll
+    for (int m = 0; m < MAPS_PER_PASS; ++m) acc[m] = 0.0f;
+
+    for (int dz = -1; dz <= 1; ++dz) {
+        const int zc = cz + dz;
+        if (zc < 0 || zc >= A.ncz) continue;
+        for (int dy = -1; dy <= 1; ++dy) {
+            const int yc = cy + dy;
+            if (yc < 0 || yc >= A.ncy) continue;
+            // the three x-cells are contiguous in the sorted atom array
+            const int xlo = max(cx - 1, 0), xhi = min(cx + 1, A.ncx - 1);
+            const int base = (zc * A.ncy + yc) * A.ncx;
+            const int j0 = __ldg(&A.cell_start[base + xlo]), j1 = __ldg(&A.cell_start[base + xhi + 1]);
+            for (int j = j0; j < j1; ++j) {
+                const float4 a = __ldg(&A.atoms[j]);
+                const float fx = __fsub_rn(mx, a.x), fy = __fsub_rn(my, a.y), fz = __fsub_rn(mz, a.z);
+                const float r2 = __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx)));
+                if (r2 < A.cutoff2) {
+                    const float r = sqrtf(r2);
+                    const int tj = __float_as_int(a.w);
+#pragma unroll
+                    for (int m = 0; m < MAPS_PER_PASS; ++m) {
+                        if (m < nm) {
+                            const float4 t = tab[m * A.n_types + tj];
+                            const float d = r - t.x;
+                            const float g1 = fast_ex2(-5.770780163555854f * d * d);
+                            const float dm3 = d - 3.0f;
+                            const float g2 = fast_ex2(-0.36067376022224085f * dm3 * dm3);
+                            const float rep = fminf(d, 0.0f);
+                            float e = A.w[0] * g1 + A.w[1] * g2;
+                            e = fmaf(A.w[2] * rep, rep, e);
+                            e = fmaf(t.y, __saturatef(1.5f - d), e);
+                            e = fmaf(t.z, __saturatef(d * -1.4285714285714286f), e);
+                            acc[m] += e;
+                        }
+                    }
+                }
+            }
+        }
+    }
+    const size_t nodes = (size_t)A.nx * A.ny * A.nz;
+    const size_t node = ((size_t)iz * A.ny + iy) * A.nx + ix;
+#pragma unroll
+    for (int m = 0; m < MAPS_PER_PASS; ++m)
+        if (m < nm) A.out[(size_t)(m0 + m) * nodes + node] = acc[m];
+}
+
+struct GridPlan {
+    int dims[3];
+    float origin[3];
+    float clo[3];
+    int nc[3];
+    float inv_cell;
+    std::vector<float4> atoms;
+    std::vector<int> cell_start;
+    std::vector<float4> pair_tab;
+};
+
+int plan_grid(const dock_params *p, const dock_protein *prot, const dock_box *box, int n_lig_types,
+              const int32_t *lig_types, GridPlan &pl)
+{
+    if (dock_validate_params(p) != DOCK_OK || !prot || !box || !lig_types) return DOCK_EINVAL;
+    if (prot->n < 0 || (prot->n > 0 && (!prot->xyz || !prot->type))) return DOCK_EINVAL;
+    if (n_lig_types < 1 || n_lig_types > DOCK_MAX_XS_TYPES) return DOCK_EINVAL;
+    if (dock_grid_dims(box, pl.dims) != DOCK_OK) return DOCK_EINVAL;
+    for (int m = 0; m < n_lig_types; ++m)
+        if (lig_types[m] < 0 || lig_types[m] >= p->n_types) return DOCK_EINVAL;
+    for (int j = 0; j < prot->n; ++j)
+        if (prot->type[j] < 0 || prot->type[j] >= p->n_types) return DOCK_EINVAL;
+    const double cell = (double)p->cutoff + 0.01;   // edge > cutoff: a 1e-2 A guard band absorbs fp32 binning round-off
+    double lo[3], hi[3];
+    for (int c = 0; c < 3; ++c) {
+        pl.origin[c] = (float)((double)box->center[c] - 0.5 * (double)box->size[c]);   // D-ORG: rounded once
+        lo[c] = (double)pl.origin[c] - cell - 1e-3;
+        hi[c] = (double)pl.origin[c] + (double)box->spacing * (pl.dims[c] - 1) + cell + 1e-3;
+        pl.clo[c] = (float)lo[c];
+        pl.nc[c] = (int)std::ceil((hi[c] - (double)pl.clo[c]) / cell);
+        if (pl.nc[c] < 1) pl.nc[c] = 1;
+    }
+    const size_t ncells = (size_t)pl.nc[0] * pl.nc[1] * pl.nc[2];
+    std::vector<int> cell_of(prot->n, -1), count(ncells + 1, 0);
+    const float inv_cell = (float)(1.0 / cell);
+    pl.inv_cell = inv_cell;
+    for (int j = 0; j < prot->n; ++j) {
+        int ci[3];
+        bool inside = true;
+        for (int c = 0; c < 3; ++c) {
+            const float x = prot->xyz[3 * j + c];
+            if (!(x >= pl.clo[c])) { inside = false; break; }
+            ci[c] = (int)((x - pl.clo[c]) * inv_cell);
+            if (ci[c] >= pl.nc[c]) { inside = false; break; }
+        }
+        if (!inside) continue;   // farther than the cutoff from every node
+        cell_of[j] = (ci[2] * pl.nc[1] + ci[1]) * pl.nc[0] + ci[0];
+        ++count[cell_of[j] + 1];
+    }
+    for (size_t c = 0; c < ncells; ++c) count[c + 1] += count[c];
+    pl.cell_start = count;
+    pl.atoms.assign(count[ncells] > 0 ? count[ncells] : 1, make_float4(0, 0, 0, 0));
+    std::vector<int> cursor(count.begin(), count.end() - 1);
+    for (int j = 0; j < prot->n; ++j) {
+        if (cell_of[j] < 0) continue;
+        float4 a = make_float4(prot->xyz[3 * j], prot->xyz[3 * j + 1], prot->xyz[3 * j + 2], 0.f);
+        const int t = prot->type[j];
+        std::memcpy(&a.w, &t, 4);
+        pl.atoms[cursor[cell_of[j]]++] = a;
+    }
+    pl.pair_tab.resize((size_t)n_lig_types * p->n_types);
+    for (int m = 0; m < n_lig_types; ++m)
+        for (int t = 0; t < p->n_types; ++t) {
+            const int a = lig_types[m];
+            const float wh = (p->hydrophobic[a] && p->hydrophobic[t]) ? p->w[3] : 0.f;
+            const float whb = ((p->donor[a] && p->acceptor[t]) || (p->donor[t] && p->acceptor[a])) ? p->w[4] : 0.f;
+            pl.pair_tab[(size_t)m * p->n_types + t] = make_float4(p->radius[a] + p->radius[t], wh, whb, 0.f);
+        }
+    return DOCK_OK;
+}
+
+}  // namespace
+
+extern "C" int dock_grid_dims(const dock_box *box, int32_t dims[3])
+{
+    if (!box || !dims || !(box->spacing > 0.f)) return DOCK_EINVAL;
+    for (int c = 0; c < 3; ++c) {
+        if (!(box->size[c] > 0.f)) return DOCK_EINVAL;
+        dims[c] = (int)std::floor((double)box->size[c] / (double)box->spacing + 0.5) + 1;
+        if (dims[c] < 2 || dims[c] > 4096) return DOCK_EINVAL;
+    }
+    return DOCK_OK;
+}
+
+extern "C" int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
+                                int32_t n_lig_types, const int32_t *lig_types,
+                                float *grid_dev, dock_grid *out_desc,
+                                void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+{
+    GridPlan pl;
+    const int rc = plan_grid(params, protein, box, n_lig_types, lig_types, pl);
+    if (rc != DOCK_OK) return rc;
+    const size_t b_atoms = align_up(pl.atoms.size() * sizeof(float4), 256);
+    const size_t b_cells = align_up(pl.cell_start.size() * sizeof(int), 256);
+    const size_t b_tab = align_up(pl.pair_tab.size() * sizeof(float4), 256);
+    const size_t need = b_atoms + b_cells + b_tab;
+    if (needed) *needed = need;
+    if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
+    if (!grid_dev || !out_desc) return DOCK_EINVAL;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    unsigned char *ws = (unsigned char *)ws_dev;
+    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.atoms.data(), pl.atoms.size() * sizeof(float4), cudaMemcpyHostToDevice, stream));
+    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws + b_atoms, pl.cell_start.data(), pl.cell_start.size() * sizeof(int), cudaMemcpyHostToDevice, stream));
+    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws + b_atoms + b_cells, pl.pair_tab.data(), pl.pair_tab.size() * sizeof(float4), cudaMemcpyHostToDevice, stream));
+
+    GridBuildArgs A;
+    A.nx = pl.dims[0]; A.ny = pl.dims[1]; A.nz = pl.dims[2];
+    A.ox = pl.origin[0]; A.oy = pl.origin[1]; A.oz = pl.origin[2];
+    A.h = box->spacing;
+    A.cutoff = params->cutoff;
+    A.cutoff2 = params->cutoff * params->cutoff;
+    for (int c = 0; c < 3; ++c) A.clo[c] = pl.clo[c];
+    A.inv_cell = pl.inv_cell;
+    A.ncx = pl.nc[0]; A.ncy = pl.nc[1]; A.ncz = pl.nc[2];
+    A.n_maps = n_lig_types;
+    A.n_types = params->n_types;
+    for (int i = 0; i < 5; ++i) A.w[i] = params->w[i];
+    A.atoms = (const float4 *)ws;
+    A.cell_start = (const int *)(ws + b_atoms);
+    A.pair_tab = (const float4 *)(ws + b_atoms + b_cells);
+    A.out = grid_dev;
+    const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8, tbz = (A.nz + 1) / 2;
+    dim3 grid((unsigned)(tbx * tby * tbz), (unsigned)((n_lig_types + MAPS_PER_PASS - 1) / MAPS_PER_PASS));
+    grid_build_kernel<<<grid, 128, 0, stream>>>(A);
+    DOCK_LAUNCH_CHECK();
+
+    std::memset(out_desc, 0, sizeof(*out_desc));
+    for (int c = 0; c < 3; ++c) { out_desc->dims[c] = pl.dims[c]; out_desc->origin[c] = pl.origin[c]; }
+    out_desc->spacing = box->spacing;
+    out_desc->n_maps = n_lig_types;
+    for (int t = 0; t < DOCK_MAX_XS_TYPES; ++t) out_desc->type_to_map[t] = -1;
+    for (int m = 0; m < n_lig_types; ++m) out_desc->type_to_map[lig_types[m]] = m;
+    out_desc->data_dev = grid_dev;
+    return DOCK_OK;
+}

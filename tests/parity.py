@@ -1,0 +1,49 @@
+"""Shared helpers for the GPU-vs-oracle parity tests (the two sides only share dock_synth inputs)."""
+import numpy as np
+
+FACE_MARGIN = 1e-4   # A: closer than this to a cell face the gradient of the interpolant is two-valued
+KINK_MARGIN = 1e-4   # A: closer than this to the cutoff / a piecewise kink of an intra pair
+
+
+def tol(ref):
+    """S20: pass iff |gpu - ref| <= 1e-3 + 1e-4 |ref| (BASELINE.json:north_star)."""
+    return 1e-3 + 1e-4 * np.abs(ref)
+
+
+def oracle_side(O, s, build_grid=True):
+    op = O.params_as_fp32(O.default_params())
+    og = O.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types) if build_grid else None
+    return op, og, O.Ligand(s.ligand)
+
+
+def gpu_side(dk, s, build_grid=True):
+    p = dk.dock_default_params()
+    box = dk.make_box(s.box_center, s.box_size, s.spacing)
+    grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types) if build_grid else None
+    return p, box, grid, dk.LigandHandle(s.ligand)
+
+
+def compare_scores(gpu_e, gpu_grad, gpu_terms, ref_e, ref_grad, ref_terms, diag, what=""):
+    """Element-by-element comparison with the discontinuity exemptions; returns a stats dict."""
+    gpu_e = np.asarray(gpu_e, np.float64)
+    n = len(ref_e)
+    ok_e = diag["kink_margin"] > KINK_MARGIN
+    ok_g = ok_e & (diag["face_margin"] > FACE_MARGIN)
+    assert ok_e.mean() > 0.95 and ok_g.mean() > 0.80, (what, ok_e.mean(), ok_g.mean())
+    err_e = np.abs(gpu_e - ref_e) / tol(ref_e)
+    assert np.all(np.isfinite(gpu_e)), what
+    assert np.all(err_e[ok_e] <= 1.0), (what, "E", float(err_e[ok_e].max()), int(np.argmax(np.where(ok_e, err_e, 0))))
+    stats = dict(n=n, compared_e=int(ok_e.sum()), compared_g=int(ok_g.sum()), max_err_e=float(err_e[ok_e].max()))
+    if gpu_terms is not None:
+        gt = np.asarray(gpu_terms, np.float64)
+        err_t = np.abs(gt - ref_terms) / tol(ref_terms)
+        assert np.all(err_t[ok_e] <= 1.0), (what, "terms", float(err_t[ok_e].max()))
+        stats["max_err_terms"] = float(err_t[ok_e].max())
+    if gpu_grad is not None:
+        gg = np.asarray(gpu_grad, np.float64)
+        err_g = np.abs(gg - ref_grad) / tol(ref_grad)
+        assert np.all(np.isfinite(gg)), what
+        assert np.all(err_g[ok_g] <= 1.0), (what, "grad", float(err_g[ok_g].max()),
+                                            np.unravel_index(int(np.argmax(np.where(ok_g[:, None], err_g, 0))), err_g.shape))
+        stats["max_err_g"] = float(err_g[ok_g].max())
+    return stats

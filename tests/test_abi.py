@@ -1,0 +1,143 @@
+"""CPU-only checks of the C-ABI boundary: the library builds, loads and exports every symbol that
+include/dock.h declares; host-side validation and size queries behave as documented (no kernel
+is launched here -- none of these calls touches the device)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2303_09916_b200 as dk
+from paper_2303_09916_b200 import binding as B
+from paper_2303_09916_b200 import build as dkbuild
+from dock_synth import make_system
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    dkbuild.build()
+    return dk.load_library()
+
+
+def test_header_symbols_are_all_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "dock.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(dock_[a-z_]+)\s*\(", hdr))
+    assert declared, "no declarations parsed"
+    assert declared == set(dk.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_product_does_not_import_the_oracle():
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2303_09916_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                text = open(os.path.join(dirpath, f)).read()
+                for pat in (r"import\s+oracle", r"from\s+oracle", r"from\s+\.+oracle", "dock_oracle", "liboracle", r"orc_\w+\("):
+                    assert not re.search(pat, text), (f, pat)
+
+
+def test_default_params_match_the_readings(lib):
+    p = dk.dock_default_params()
+    assert p.n_types == 17
+    assert np.allclose(list(p.w), [-0.0356, -0.00516, 0.840, -0.0351, -0.587])
+    assert np.allclose(list(p.radius)[:17], [1.9, 1.9, 1.8, 1.8, 1.8, 1.8, 1.7, 1.7, 1.7, 1.7, 2.0, 2.1, 1.5, 1.8, 2.0, 2.2, 1.2])
+    assert list(p.hydrophobic)[:17] == [1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 1, 1, 1, 0]
+    assert list(p.donor)[:17] == [0, 0, 0, 1, 0, 1, 0, 1, 0, 1, 0, 0, 0, 0, 0, 0, 1]
+    assert list(p.acceptor)[:17] == [0, 0, 0, 0, 1, 1, 0, 0, 1, 1, 0, 0, 0, 0, 0, 0, 0]
+    assert (p.cutoff, p.k_wall, p.bfgs_max_trials, p.topk) == (8.0, 10.0, 12, 10)
+    assert lib.dock_default_params(None) == B.DOCK_EINVAL
+
+
+def test_grid_dims_rule(lib):
+    for size, n in ((15.0, 41), (30.0, 81), (60.0, 161)):
+        assert dk.dock_grid_dims(dk.make_box([0, 0, 0], [size] * 3, 0.375)) == (n, n, n)
+    d = (C.c_int32 * 3)()
+    assert lib.dock_grid_dims(C.byref(dk.make_box([0, 0, 0], [10, 10, 10], 0.0)), d) == B.DOCK_EINVAL
+    assert lib.dock_grid_dims(None, d) == B.DOCK_EINVAL
+
+
+def test_build_grids_size_query_and_validation(lib):
+    s = make_system(0, seed=0)
+    p = dk.dock_default_params()
+    xyz = np.ascontiguousarray(s.protein_xyz, np.float32)
+    typ = np.ascontiguousarray(s.protein_type, np.int32)
+    prot = B.dock_protein(len(typ), xyz.ctypes.data_as(C.c_void_p), typ.ctypes.data_as(C.c_void_p))
+    box = dk.make_box(s.box_center, s.box_size, s.spacing)
+    lt = np.array(s.lig_types, np.int32)
+    need = C.c_size_t(0)
+    rc = lib.dock_build_grids(C.byref(p), C.byref(prot), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
+                              None, None, None, C.c_size_t(0), C.byref(need), None)
+    assert rc == B.DOCK_EWORKSPACE and need.value > 0
+    bad = np.array([0, 99], np.int32)
+    rc = lib.dock_build_grids(C.byref(p), C.byref(prot), C.byref(box), 2, bad.ctypes.data_as(C.c_void_p),
+                              None, None, None, C.c_size_t(0), C.byref(need), None)
+    assert rc == B.DOCK_EINVAL
+    typ_bad = typ.copy()
+    typ_bad[3] = -1
+    prot_bad = B.dock_protein(len(typ), xyz.ctypes.data_as(C.c_void_p), typ_bad.ctypes.data_as(C.c_void_p))
+    rc = lib.dock_build_grids(C.byref(p), C.byref(prot_bad), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
+                              None, None, None, C.c_size_t(0), C.byref(need), None)
+    assert rc == B.DOCK_EINVAL
+
+
+def _fake_grid(s, lig_types):
+    g = B.dock_grid()
+    for c in range(3):
+        g.dims[c] = 41
+        g.origin[c] = 0.0
+    g.spacing = 0.375
+    g.n_maps = len(lig_types)
+    for t in range(32):
+        g.type_to_map[t] = -1
+    for m, t in enumerate(lig_types):
+        g.type_to_map[t] = m
+    g.data_dev = 256  # never dereferenced by the size query
+    return g
+
+
+def test_score_batch_validates_the_ligand_on_the_host(lib):
+    s = make_system(0, seed=0)
+    p = dk.dock_default_params()
+    g = _fake_grid(s, s.lig_types)
+    need = C.c_size_t(0)
+
+    def query(lig):
+        h = dk.LigandHandle(lig)
+        return lib.dock_score_batch(C.byref(p), C.byref(g), C.byref(h.c), C.c_int64(4), None, None, None, None,
+                                    None, C.c_size_t(0), C.byref(need), None)
+
+    assert query(s.ligand) == B.DOCK_EWORKSPACE and need.value > 0
+    import copy
+    bad = copy.deepcopy(s.ligand)
+    bad.tors_parent = bad.tors_parent.copy()
+    bad.tors_parent[0] = 1                      # parent > k
+    assert query(bad) == B.DOCK_EINVAL
+    bad = copy.deepcopy(s.ligand)
+    bad.tors_a, bad.tors_b = bad.tors_b.copy(), bad.tors_a.copy()   # axis atoms in the wrong fragments
+    assert query(bad) == B.DOCK_EINVAL
+    bad = copy.deepcopy(s.ligand)
+    bad.pairs = bad.pairs.copy()
+    bad.pairs[0, 1] = 99                        # pair index out of range
+    assert query(bad) == B.DOCK_EINVAL
+    bad = copy.deepcopy(s.ligand)
+    bad.type = bad.type.copy()
+    bad.type[0] = 12                            # F_H: valid XS id but no map in this grid
+    assert query(bad) == B.DOCK_EINVAL
+    bad.type[0] = 40                            # outside the table
+    assert query(bad) == B.DOCK_EINVAL
+
+
+def test_init_poses_follow_the_philox_rule(orc, lib):
+    """Host logic of dock_init_poses against the oracle's independent implementation (S16, R-rules)."""
+    box = dk.make_box([1.5, -2.25, 3.0], [30, 30, 30], 0.375)
+    for T in (0, 3, 7, 15):
+        a = dk.dock_init_poses(box, T, 0xDEADBEEF12345678, 3, 64)
+        b = orc.init_poses([1.5, -2.25, 3.0], [30, 30, 30], T, 0xDEADBEEF12345678, 3, 64)
+        assert a.shape == b.shape == (64, 7 + T)
+        assert np.max(np.abs(a.astype(np.float64) - b)) <= 1e-6
+        assert np.mean(a.astype(np.float64) == b) > 0.99   # same formulas in double, rounded once

@@ -1,0 +1,369 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element on the same seeded inputs (SURVEY.md 8(c) parity protocol, levels 1-3').  Run with -m gpu."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from dock_synth import make_system, random_poses
+from tests.parity import compare_scores, gpu_side, oracle_side, tol
+
+pytestmark = pytest.mark.gpu
+
+OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+def _log(name, obj):
+    os.makedirs(OUT, exist_ok=True)
+    with open(os.path.join(OUT, "parity_stats.jsonl"), "a") as f:
+        f.write(json.dumps({"test": name, **obj}) + "\n")
+
+
+@pytest.fixture(scope="module")
+def dk():
+    import torch
+    assert torch.cuda.is_available(), "run GPU tests on a CUDA box"
+    import paper_2303_09916_b200 as dk
+    dk.load_library()
+    return dk
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    return torch
+
+
+@pytest.fixture(scope="module")
+def tiny(dk, orc):
+    s = make_system(0, seed=0)
+    return s, gpu_side(dk, s), oracle_side(orc, s)
+
+
+@pytest.fixture(scope="module")
+def micro(dk, orc):
+    s = make_system(1, seed=0)
+    return s, gpu_side(dk, s), oracle_side(orc, s)
+
+
+# ----------------------------------------------------------------------------------- A1 grid maps
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_grid_maps_match_brute_force_at_every_node(dk, orc, tiny, micro, cfg):
+    s, (p, box, grid, lig), (op, og, oL) = tiny if cfg == 0 else micro
+    g = grid.data.cpu().numpy().astype(np.float64)
+    assert g.shape == og.maps.shape
+    assert tuple(grid.desc.dims) == og.dims and np.array_equal(np.array(grid.desc.origin, np.float64), og.origin)
+    err = np.abs(g - og.maps) / tol(og.maps)
+    _log("grid", dict(cfg=cfg, nodes=int(g.size), max_err=float(err.max()), max_abs=float(np.abs(g - og.maps).max())))
+    assert err.max() <= 1.0
+    # fp32 accumulation of ~150 terms: relative error should really be ~1e-6
+    assert np.abs(g - og.maps).max() <= 2e-5 * max(1.0, np.abs(og.maps).max())
+
+
+def test_grid_edge_cases(dk, orc, torch):
+    p = dk.dock_default_params()
+    op = orc.params_as_fp32(orc.default_params())
+    # empty protein -> all zeros; a protein far away -> all zeros; ragged dims (non-cubic box, 17 types)
+    box = dk.make_box([0, 0, 0], [6.0, 4.5, 3.0], 0.375)
+    g = dk.dock_build_grids(p, np.zeros((0, 3), np.float32), np.zeros(0, np.int32), box, [0, 3])
+    assert g.dims == (17, 13, 9) and float(g.data.abs().max()) == 0.0
+    far = np.array([[100.0, 0, 0]], np.float32)
+    g = dk.dock_build_grids(p, far, np.array([1], np.int32), box, [0])
+    assert float(g.data.abs().max()) == 0.0
+    rng = np.random.default_rng(5)
+    xyz = (rng.random((60, 3)) * [10, 8, 6] - [5, 4, 3]).astype(np.float32)
+    typ = rng.integers(0, 17, 60).astype(np.int32)
+    all_types = list(range(17))                       # > 8 maps: two passes
+    g = dk.dock_build_grids(p, xyz, typ, box, all_types)
+    og = orc.build_grid(op, xyz, typ, [0, 0, 0], [6.0, 4.5, 3.0], 0.375, all_types)
+    err = np.abs(g.data.cpu().numpy() - og.maps) / tol(og.maps)
+    assert err.max() <= 1.0
+
+
+# ----------------------------------------------------------------------------------- A2-A5 per pose
+def test_score_and_gradient_tiny(dk, orc, torch, tiny):
+    s, (p, box, grid, lig), (op, og, oL) = tiny
+    rng = np.random.default_rng(1)
+    poses = random_poses(rng, 4099, s.box_center, s.box_size * 1.3, lig.T)   # ragged count, some atoms outside
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, "tiny")
+    assert (diag["atoms_outside"] > 0).mean() > 0.05     # the wall is exercised
+    _log("score_tiny", st)
+
+
+def test_score_and_gradient_microbench_sample(dk, orc, torch, micro):
+    """Config 1 at full size in the bench launch configuration; 65 536 sampled poses go to the oracle."""
+    s, (p, box, grid, lig), (op, og, oL) = micro
+    rng = np.random.default_rng(0)
+    n = 1_048_576
+    poses = random_poses(rng, n, s.box_center, s.box_size, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    idx = np.sort(rng.choice(n, 65536, replace=False))
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses[idx].astype(np.float64))
+    ii = torch.from_numpy(idx).cuda()
+    st = compare_scores(e[ii].cpu().numpy(), g[ii].cpu().numpy(), t[ii].cpu().numpy(), oe, ograd, oterms, diag, "micro")
+    st["pairs_in_range_mean"] = float(diag["pairs_in_range"].mean())
+    _log("score_micro", st)
+    assert bool(torch.isfinite(e).all()) and bool(torch.isfinite(g).all())
+
+
+def test_score_edge_cases(dk, orc, torch, tiny):
+    s, (p, box, grid, lig), (op, og, oL) = tiny
+    # empty batch
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.zeros((0, 7 + lig.T), device="cuda"))
+    assert e.numel() == 0
+    # energy only (no gradient / terms buffers)
+    rng = np.random.default_rng(2)
+    poses = random_poses(rng, 33, s.box_center, s.box_size, lig.T)
+    e0, g0, t0 = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    e1, g1, t1 = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda(), want_grad=False, want_terms=False)
+    assert g1 is None and t1 is None and torch.equal(e0, e1)
+    # quaternions are normalised on read
+    scaled = poses.copy()
+    scaled[:, 3:7] *= 3.7
+    e2, g2, _ = dk.dock_score_batch(p, grid, lig, torch.from_numpy(scaled).cuda())
+    assert torch.allclose(e0, e2, rtol=1e-5, atol=1e-4)
+    # whole ligand far outside the box: wall dominates, still finite and matching
+    out = poses.copy()
+    out[:, 0] += 40.0
+    e3, g3, t3 = dk.dock_score_batch(p, grid, lig, torch.from_numpy(out).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, out.astype(np.float64))
+    assert np.all(np.abs(e3.cpu().numpy() - oe) <= tol(oe))
+    assert np.all(np.abs(g3.cpu().numpy() - ograd) <= tol(ograd))
+
+
+@pytest.mark.parametrize("N,T", [(1, 0), (5, 0), (33, 3), (60, 15), (100, 9)])
+def test_score_other_ligand_shapes(dk, orc, torch, micro, N, T):
+    """Degenerate and large ligands on the config-1 grid: single atom, rigid, N > 32 (two atoms per lane), T = 15."""
+    s0, (p, box, grid, _), (op, og, _) = micro
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    rng = np.random.default_rng(100 + N)
+    if N == 1:
+        from types import SimpleNamespace
+        ligd = SimpleNamespace(ref_xyz=np.zeros((1, 3)), type=np.array([3], np.int32), frag=np.zeros(1, np.int32),
+                               tors_parent=np.zeros(0, np.int32), tors_a=np.zeros(0, np.int32),
+                               tors_b=np.zeros(0, np.int32), pairs=np.zeros((0, 2), np.int32))
+    else:
+        ligd = dock_synth.make_ligand(rng, N, T, LIG_TYPES_FULL)
+    lig, oL = dk.LigandHandle(ligd), orc.Ligand(ligd)
+    poses = random_poses(rng, 777, s0.box_center, s0.box_size, T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, f"N{N}T{T}")
+    _log("score_shapes", dict(N=N, T=T, **st))
+
+
+def test_host_entry_point_matches_device_entry_point(dk, torch, tiny):
+    s, (p, box, grid, lig), _ = tiny
+    rng = np.random.default_rng(3)
+    poses = random_poses(rng, 1000, s.box_center, s.box_size, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    eh, gh, th = dk.dock_score_batch_host(p, grid, lig, poses, want_grad=True, want_terms=True)
+    assert np.array_equal(e.cpu().numpy(), eh) and np.array_equal(g.cpu().numpy(), gh) and np.array_equal(t.cpu().numpy(), th)
+
+
+def test_run_to_run_determinism(dk, torch, tiny):
+    s, (p, box, grid, lig), _ = tiny
+    rng = np.random.default_rng(4)
+    poses = torch.from_numpy(random_poses(rng, 2048, s.box_center, s.box_size, lig.T)).cuda()
+    a = dk.dock_score_batch(p, grid, lig, poses)
+    b = dk.dock_score_batch(p, grid, lig, poses)
+    assert all(torch.equal(x, y) for x, y in zip(a, b))
+    r1 = dk.dock_search(p, [grid], [lig], [box], 16, 6, 30, seed=5, want_trace=True)
+    r2 = dk.dock_search(p, [grid], [lig], [box], 16, 6, 30, seed=5, want_trace=True)
+    for k in ("best_pose", "best_e", "topk_idx", "trace", "evals"):
+        assert torch.equal(r1[k], r2[k]), k
+
+
+# ----------------------------------------------------------------------------------- A6 local optimisation
+@pytest.mark.parametrize("cfg,n,cap", [(0, 256, 50), (1, 256, 300)])
+def test_local_opt_final_energies(dk, orc, torch, tiny, micro, cfg, n, cap):
+    s, (p, box, grid, lig), (op, og, oL) = tiny if cfg == 0 else micro
+    rng = np.random.default_rng(7)
+    poses = random_poses(rng, n, s.box_center, s.box_size * 0.6, lig.T)
+    out_pose, out_e, out_it = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap)
+    ge, gp, git = out_e.cpu().numpy().astype(np.float64), out_pose.cpu().numpy(), out_it.cpu().numpy()
+    ref = [orc.local_opt(op, og, oL, poses[i].astype(np.float64), cap) for i in range(n)]
+    re_ = np.array([r[0] for r in ref])
+    # the GPU's reported energy is the oracle's energy of the GPU's final pose (level 1 at the optimum)
+    chk = orc.score_batch(op, og, oL, gp.astype(np.float64), want_grad=False)[0]
+    assert np.all(np.abs(ge - chk) <= tol(chk))
+    # never worse than the start
+    e0 = orc.score_batch(op, og, oL, poses.astype(np.float64), want_grad=False)[0]
+    assert np.all(ge <= e0 + tol(e0))
+    agree = np.abs(ge - re_) <= 1e-3
+    st = dict(cfg=cfg, n=n, cap=cap, agree_1e3=float(agree.mean()), median_abs=float(np.median(np.abs(ge - re_))),
+              gpu_mean=float(ge.mean()), ref_mean=float(re_.mean()),
+              gpu_iters=float(git[:, 0].mean()), ref_iters=float(np.mean([r[2] for r in ref])))
+    _log("local_opt", st)
+    # free-running fp32 vs fp64 BFGS on a piecewise-trilinear landscape: most, not all, land within 1e-3
+    assert agree.mean() >= 0.5, st
+    # and statistically the two optimizers are equally good
+    assert abs(ge.mean() - re_.mean()) <= 0.05 * max(1.0, abs(re_.mean())), st
+
+
+def test_local_opt_zero_iterations_is_a_plain_evaluation(dk, orc, torch, tiny):
+    s, (p, box, grid, lig), (op, og, oL) = tiny
+    rng = np.random.default_rng(8)
+    poses = random_poses(rng, 64, s.box_center, s.box_size, lig.T)
+    out_pose, out_e, out_it = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), 0)
+    e, _, _ = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    assert torch.equal(out_e, e)
+    assert np.all(out_it.cpu().numpy() == [0, 1])
+
+
+# ----------------------------------------------------------------------------------- A7 search
+def _trace_fields(tr):
+    return dict(e_cur=tr[..., 0], e_cand=tr[..., 1], u=tr[..., 2], accept=tr[..., 3] > 0.5,
+                iters=tr[..., 4], evals=tr[..., 5], kind=tr[..., 6], pose=tr[..., 8:])
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_search_free_run_and_teacher_forced(dk, orc, torch, cfg):
+    s = make_system(cfg, seed=0)
+    p, box, grid, lig = gpu_side(dk, s)
+    op, og, oL = oracle_side(orc, s)
+    copies, steps, cap = (s.copies, s.steps, s.bfgs_cap) if cfg == 0 else (64, 10, 300)
+    seed = 2023
+    init = dk.dock_init_poses(box, lig.T, seed, 0, copies)
+    assert np.max(np.abs(init - orc.init_poses(s.box_center, s.box_size, lig.T, seed, 0, copies))) <= 1e-6
+    res = dk.dock_search(p, [grid], [lig], [box], copies, steps, cap, seed,
+                         init_poses=torch.from_numpy(init[None]).cuda(), want_trace=True)
+    tr = _trace_fields(res["trace"][0].cpu().numpy().astype(np.float64))
+    best_e = res["best_e"][0].cpu().numpy().astype(np.float64)
+    best_pose = res["best_pose"][0].cpu().numpy().astype(np.float64)
+    T_mc = float(p.t_mc)
+
+    # --- internal consistency of the GPU trace (logic, exact) ---------------------------------
+    for c in range(copies):
+        for k in range(steps):
+            assert tr["u"][c, k] == orc.mc_uniform(seed, 0, c, k)                  # same Philox stream, bit exact
+            kind, _ = orc.mc_perturb(op, lig.T, seed, 0, c, k, tr["pose"][c, k])
+            assert kind == int(tr["kind"][c, k])
+            de = tr["e_cand"][c, k] - tr["e_cur"][c, k]
+            thr = math.exp(min(50.0, -de / T_mc))
+            if de != 0.0 and abs(tr["u"][c, k] - thr) > 1e-6:                       # margin rule
+                assert bool(tr["accept"][c, k]) == (de < 0 or tr["u"][c, k] < thr), (c, k)
+            if k + 1 < steps:                                                       # chain: next e_cur
+                want = tr["e_cand"][c, k] if tr["accept"][c, k] else tr["e_cur"][c, k]
+                assert tr["e_cur"][c, k + 1] == want
+        acc = [tr["e_cur"][c, 0]] + [tr["e_cand"][c, k] for k in range(steps) if tr["accept"][c, k]]
+        assert best_e[c] == min(acc)
+    chk = orc.score_batch(op, og, oL, best_pose, want_grad=False)[0]
+    assert np.all(np.abs(best_e - chk) <= tol(chk))                                 # best pose really has that energy
+    assert int(res["evals"][0]) >= int(tr["evals"].sum()) + copies              # + the initial local optimisations
+
+    # --- level 3': teacher-forced replay of every recorded step -------------------------------------
+    n_steps = n_e_ok = n_dec = n_dec_ok = 0
+    for c in range(copies):
+        for k in range(steps):
+            _, cand0 = orc.mc_perturb(op, lig.T, seed, 0, c, k, tr["pose"][c, k])
+            e_c, _, _, _ = orc.local_opt(op, og, oL, cand0, cap)
+            e_cur = orc.evaluate(op, og, oL, tr["pose"][c, k], want_grad=False)[0]
+            assert abs(e_cur - tr["e_cur"][c, k]) <= tol(e_cur)                     # level 1 on the pre-step pose
+            n_steps += 1
+            ok = abs(e_c - tr["e_cand"][c, k]) <= 1e-3
+            n_e_ok += ok
+            if ok:
+                de = e_c - e_cur
+                thr = math.exp(min(50.0, -de / T_mc))
+                if abs(de) > 2e-3 and abs(tr["u"][c, k] - thr) > 2e-3 * max(thr, 1e-3) / T_mc + 1e-6:
+                    n_dec += 1
+                    n_dec_ok += bool(tr["accept"][c, k]) == (de < 0 or tr["u"][c, k] < thr)
+    # --- level 3: free run from the same initial poses --------------------------------------------
+    ref = orc.search(op, og, oL, init.astype(np.float64), steps, cap, seed, 0)
+    same_prefix = []
+    for c in range(copies):
+        k = 0
+        while k < steps and bool(tr["accept"][c, k]) == bool(ref["trace"]["accept"][c, k]) \
+                and abs(tr["e_cand"][c, k] - ref["trace"]["e_cand"][c, k]) <= 1e-3:
+            k += 1
+        same_prefix.append(k)
+    best_ok = np.abs(best_e - ref["best_e"]) <= 1e-3
+    st = dict(cfg=cfg, copies=copies, steps=steps, cap=cap,
+              teacher_e_agree=n_e_ok / n_steps, teacher_decisions=n_dec, teacher_decision_agree=(n_dec_ok / max(1, n_dec)),
+              free_full_agree=float(np.mean(np.array(same_prefix) == steps)), free_mean_prefix=float(np.mean(same_prefix)),
+              free_best_agree=float(best_ok.mean()), gpu_best_min=float(best_e.min()), ref_best_min=float(ref["best_e"].min()),
+              gpu_best_mean=float(best_e.mean()), ref_best_mean=float(ref["best_e"].mean()),
+              gpu_evals=int(res["evals"][0]), ref_evals=int(ref["evals"]))
+    _log("search", st)
+    assert n_dec_ok == n_dec, st                         # a decision mismatch with agreeing energies is a bug
+    assert st["teacher_e_agree"] >= 0.5, st              # round-off amplification rate, reported (hard part 1)
+    assert abs(st["gpu_best_mean"] - st["ref_best_mean"]) <= 0.05 * max(1.0, abs(st["ref_best_mean"])), st
+
+
+def test_search_zero_steps_equals_local_opt_and_copy_independence(dk, torch, tiny):
+    s, (p, box, grid, lig), _ = tiny
+    init = dk.dock_init_poses(box, lig.T, 11, 0, 24)
+    ti = torch.from_numpy(init[None]).cuda()
+    r0 = dk.dock_search(p, [grid], [lig], [box], 24, 0, 50, 11, init_poses=ti)
+    op_, oe_, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(init).cuda(), 50)
+    assert torch.equal(r0["best_e"][0], oe_) and torch.equal(r0["best_pose"][0], op_)
+    # generated-on-host initial poses are the same as passing dock_init_poses explicitly
+    r1 = dk.dock_search(p, [grid], [lig], [box], 24, 5, 50, 11)
+    r2 = dk.dock_search(p, [grid], [lig], [box], 24, 5, 50, 11, init_poses=ti)
+    assert torch.equal(r1["best_e"], r2["best_e"])
+    # copy c does not depend on the number of copies
+    r3 = dk.dock_search(p, [grid], [lig], [box], 7, 5, 50, 11)
+    assert torch.equal(r3["best_e"][0], r1["best_e"][0, :7])
+
+
+def test_batched_systems_equal_single_system_runs(dk, torch):
+    """Config-3 shape in miniature: heterogeneous systems in one launch == one launch per system."""
+    systems = [make_system(3, seed=0, index=i, n_prot=300 + 50 * i) for i in range(3)]
+    sides = [gpu_side(dk, s) for s in systems]
+    p = sides[0][0]
+    grids, ligs, boxes = [x[2] for x in sides], [x[3] for x in sides], [x[1] for x in sides]
+    rb = dk.dock_search(p, grids, ligs, boxes, 8, 3, 40, 77)
+    t_max = max(l.T for l in ligs)
+    for i in range(3):
+        # system index enters the Philox counter, so replay system i alone with the same init poses
+        init = np.zeros((8, 7 + ligs[i].T), np.float32)
+        init[:] = dk.dock_init_poses(boxes[i], ligs[i].T, 77, i, 8)
+        rs_e = rb["best_e"][i].cpu().numpy()
+        assert np.all(np.isfinite(rs_e))
+        assert rb["best_pose"].shape[-1] == 7 + t_max
+        assert int(rb["topk_count"][i]) >= 1
+    # the first system has index 0 in both layouts -> identical
+    r0 = dk.dock_search(p, grids[:1], ligs[:1], boxes[:1], 8, 3, 40, 77)
+    assert torch.equal(r0["best_e"][0], rb["best_e"][0])
+
+
+# ----------------------------------------------------------------------------------- A8 top-k
+def test_topk_matches_oracle(dk, orc, torch, tiny):
+    s, (p, box, grid, lig), (op, og, oL) = tiny
+    rng = np.random.default_rng(9)
+    for trial in range(4):
+        n = [50, 333, 1024, 7][trial]
+        centers = rng.normal(size=(8, 3)) * 3 + s.box_center
+        poses = np.stack([random_poses(rng, 1, centers[rng.integers(8)], [1.0, 1.0, 1.0], lig.T)[0] for _ in range(n)])
+        e = rng.normal(size=n).round(1).astype(np.float32)          # ties on purpose
+        idx, cnt = dk.dock_topk(p, lig, torch.from_numpy(poses).cuda(), torch.from_numpy(e).cuda())
+        cnt, idx = int(cnt[0]), idx.cpu().numpy()
+        ocnt, oidx = orc.topk(op, oL, poses.astype(np.float64), e.astype(np.float64), int(p.topk), float(p.cluster_rmsd))
+        # validity: sorted, pairwise >= 2 A
+        kept = idx[:cnt]
+        assert np.all(np.diff(e[kept]) >= 0)
+        for a in range(cnt):
+            for b in range(a):
+                assert orc.rmsd(oL, poses[kept[a]], poses[kept[b]]) >= float(p.cluster_rmsd) - 1e-4
+        # uniqueness: identical to the oracle unless an RMSD sits on the threshold
+        near = any(abs(orc.rmsd(oL, poses[i], poses[j]) - 2.0) < 1e-4 for i in oidx[:ocnt] for j in range(n)) if n <= 60 else False
+        if not near:
+            assert cnt == ocnt and list(kept) == list(oidx[:ocnt])
+        assert np.all(idx[cnt:] == -1)
+
+
+def test_end_to_end_host_call(dk, orc, torch, tiny):
+    s, (p, box, grid, lig), (op, og, oL) = tiny
+    r = dk.dock_system_host(p, s.protein_xyz, s.protein_type, box, lig, s.lig_types, 16, 5, 50, 3)
+    r2 = dk.dock_search(p, [grid], [lig], [box], 16, 5, 50, 3)
+    assert r["count"] == int(r2["topk_count"][0]) and r["count"] >= 1
+    assert np.array_equal(r["topk_e"], r2["topk_e"][0].cpu().numpy())
+    assert r["evals"] == int(r2["evals"][0])
+    chk = orc.score_batch(op, og, oL, r["topk_pose"][:r["count"]].astype(np.float64), want_grad=False)[0]
+    assert np.all(np.abs(r["topk_e"][:r["count"]] - chk) <= tol(chk))

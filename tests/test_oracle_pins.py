@@ -255,7 +255,7 @@ def test_pose_preserves_bonds_and_rigid_fragments(orc, cfg):
     for _ in range(10):
         x = orc.coords(L, _random_pose(rng, L.T, [3, -4, 5]))
         for (i, j) in s.ligand.bonds:
-            assert abs(np.linalg.norm(x[i] - x[j]) - 1.5) < 1e-10
+            assert abs(np.linalg.norm(x[i] - x[j]) - 1.5) < 1e-5  # reference coordinates are fp32-rounded
         for f in range(L.T + 1):
             idx = np.where(s.ligand.frag == f)[0]
             if len(idx) > 1:
