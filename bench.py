@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the docking hot path on B200 (driver contract).
+
+Default arm: the CUDA library through its C-ABI binding.
+    python bench.py [--gpus N] [--steps K] [--warmup W]
+  N=1 workload = BASELINE.json:configs[1], the scoring microbench: 1,048,576 random poses of a
+  30-atom / 6-torsion ligand scored (energy + gradient + terms) against 81^3 x 8 grid maps of a
+  3000-atom synthetic protein.  One "step" = one dock_score_batch call over the whole batch
+  (A2-A5).  The grid build (A1) and a config-2 site-docking search (A6-A8) are timed next to it
+  and reported under "extra" so that one line covers every row of the hot path.
+  N>1 (torchrun): every rank scores its own seeded batch of the same size (weak scaling, no
+  data-path collective: poses are independent); value = all ranks' evals / max time.
+
+Reference arm: `--impl reference` times the CPU oracle (oracle/), as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "score+gradient pose evals/sec"
+UNIT = "evals/s"
+# FP32 ALU roof derived from the guide's unit counts and clocks:
+# 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (clocks.max.sm)
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+def algorithmic_flops(N: int, T: int, p_in: float, p_out: float) -> float:
+    """Algorithmic fp operations of one score+gradient evaluation (counted on
+    the oracle's statements, one per add/mul/div/sqrt/exp/compare/min/max, fused nothing)."""
+    return 93.0 * N + 130.0 * T + 62.0 * p_in + 8.0 * p_out + 50.0
+
+
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "50", "-f", self.path], stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.12)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        try:
+            rows = [r.split(",") for r in open(self.path).read().strip().splitlines() if r.strip()]
+            os.unlink(self.path)
+        except OSError:
+            return out
+        sm, reasons, smax, pw = [], set(), None, []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                smax = float(r[1])
+                pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].strip().lower().startswith("active"):
+                    reasons.add(nm)
+        if sm:
+            # "under load" = the upper half of the samples (the sampler also sees the idle edges)
+            hi = sorted(sm)[len(sm) // 2:]
+            out.update(sm_mhz=float(np.median(hi)), sm_max_mhz=smax, reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw) if pw else None)
+        return out
+
+
+def _dist_setup(n_gpus: int):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    import torch
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        torch.cuda.set_device(0)
+    assert world == n_gpus or world == 1, f"--gpus {n_gpus} but WORLD_SIZE={world}"
+    return rank, world, local
+
+
+def _max_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def _barrier(world: int):
+    import torch
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------------
+def _workload(rank: int):
+    """Config 1 inputs (seeded): system, poses.  Rank r draws its own pose batch."""
+    from dock_synth import CONFIGS, make_system, random_poses
+    s = make_system(1, seed=0)
+    n = CONFIGS[1]["n_poses"]
+    rng = np.random.default_rng(np.random.PCG64([0, 1, 1000 + rank]))
+    poses = random_poses(rng, n, s.box_center, s.box_size, s.ligand.T)
+    return s, poses
+
+
+def run_reference(args) -> dict:
+    """The CPU oracle, as it stands, on the host cores; each step scores a bounded sample."""
+    from oracle import oracle as O
+    O.build()
+    s, poses = _workload(0)
+    op = O.params_as_fp32(O.default_params())
+    og = O.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
+    oL = O.Ligand(s.ligand)
+    n = min(args.ref_sample, poses.shape[0])
+    p64 = poses[:n].astype(np.float64)
+    for _ in range(args.warmup):
+        O.score_batch(op, og, oL, p64)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        O.score_batch(op, og, oL, p64)
+    dt = (time.perf_counter() - t0) / max(1, args.steps)
+    v = n / dt
+    cores = O.num_threads()
+    sample = f"first {n} poses of the config-1 batch per step, fp64, OpenMP over poses"
+    return {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[1] scoring microbench (bounded sample)", "n_poses": n, "N": oL.N, "T": oL.T,
+                   "P": oL.P, "grid": "81^3 x 8 fp64"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+def _time_events(torch, fn, reps: int, flush=None):
+    """Per-call CUDA-event times (ms) on the current stream; `flush` runs untimed before each call."""
+    out = []
+    for _ in range(reps):
+        if flush is not None:
+            flush()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        b.synchronize()
+        out.append(a.elapsed_time(b))
+    return out
+
+
+def run_ours(args) -> dict:
+    import torch
+    rank, world, local = _dist_setup(args.gpus)
+    import paper_2303_09916_b200 as dk
+    dk.load_library()
+    from dock_synth import make_system
+
+    s, poses_h = _workload(rank)
+    p = dk.dock_default_params()
+    box = dk.make_box(s.box_center, s.box_size, s.spacing)
+    lig = dk.LigandHandle(s.ligand)
+    n = poses_h.shape[0]
+    np_, ng = 7 + lig.T, 6 + lig.T
+
+    # A1: grid maps (timed as an extra; the maps then stay resident for the scoring steps)
+    grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types)
+    torch.cuda.synchronize()
+    t_grid = _time_events(torch, lambda: dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types), 3)
+
+    poses = torch.from_numpy(poses_h).cuda()
+    out = (torch.empty(n, dtype=torch.float32, device="cuda"),
+           torch.empty((n, ng), dtype=torch.float32, device="cuda"),
+           torch.empty((n, 3), dtype=torch.float32, device="cuda"))
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def flush():
+        flush_buf.fill_(1)
+
+    def step():
+        dk.dock_score_batch(p, grid, lig, poses, out=out)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    _barrier(world)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = dk.launch_count()
+    wall0 = time.perf_counter()
+    ts = _time_events(torch, step, args.steps, flush if not args.no_flush else None)
+    _barrier(world)
+    wall = time.perf_counter() - wall0
+    launches = dk.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else {}
+    t_step = _max_over_ranks(float(np.sum(ts)) / 1e3, world) / args.steps          # seconds per step, max over ranks
+    value = world * n / t_step
+
+    # e2e: the same call with HOST (pinned) buffers, copies inside the timed region
+    ph = torch.from_numpy(poses_h).pin_memory()
+    eh = (torch.empty(n, dtype=torch.float32).pin_memory(), torch.empty((n, ng), dtype=torch.float32).pin_memory(),
+          torch.empty((n, 3), dtype=torch.float32).pin_memory())
+
+    def step_host():
+        dk.dock_score_batch_host(p, grid, lig, ph, want_grad=True, want_terms=True, out=eh)
+
+    for _ in range(2):
+        step_host()
+    _barrier(world)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_host()
+    torch.cuda.synchronize()
+    t_e2e = _max_over_ranks((time.perf_counter() - t0) / args.steps, world)
+    h2d = n * np_ * 4
+    d2h = n * (1 + ng + 3) * 4
+    assert np.array_equal(eh[0].numpy(), out[0].cpu().numpy()), "host and device entry points disagree"
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": t_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "configs[1] scoring microbench", "n_poses_per_gpu": n, "N": lig.N, "T": lig.T, "P": lig.P,
+                   "grid": "81^3 x 8 fp32", "outputs": "energy+gradient+terms",
+                   "l2": "flushed between timed steps (256 MiB write)" if not args.no_flush else "not flushed",
+                   "parallelism": f"pose-sharded x{world}, no collective"},
+        "e2e": {"value": world * n / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": t_e2e * 1e3},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "wall_s_timed_region": wall,
+    }
+    if rank != 0:
+        return {}
+
+    # roofline of the dominant kernel (score kernel = the whole step)
+    from oracle import oracle as O          # cpu_baseline leg + in-range pair statistics for the flop count
+    O.build()
+    op = O.params_as_fp32(O.default_params())
+    og = O.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
+    oL = O.Ligand(s.ligand)
+    ns = min(args.ref_sample, n)
+    p64 = poses_h[:ns].astype(np.float64)
+    O.score_batch(op, og, oL, p64[:4096])
+    t0 = time.perf_counter()
+    oe, ograd, oterms, diag = O.score_batch(op, og, oL, p64)
+    t_cpu = time.perf_counter() - t0
+    p_in = float(diag["pairs_in_range"].mean())
+    flops = algorithmic_flops(lig.N, lig.T, p_in, lig.P - p_in)
+    achieved = flops * n / (float(np.mean(ts)) / 1e3) / 1e12
+    line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                        "frac": achieved / ALU_PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                        "kernel": "score_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
+                        "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+    line["cpu_baseline"] = {"value": ns / t_cpu, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+                            "sample": f"first {ns} poses of the same batch, fp64, OpenMP over poses"}
+    # spot parity inside the bench run: what is timed is what is correct
+    ge = out[0][:ns].cpu().numpy().astype(np.float64)
+    safe = diag["kink_margin"] > 1e-4
+    err = np.abs(ge - oe) / (1e-3 + 1e-4 * np.abs(oe))
+    line["parity_in_bench"] = {"poses": int(safe.sum()), "max_err_tol_units": float(err[safe].max())}
+
+    # extras: A1 and A6-A8 next to the headline
+    extra = {"grid_build_ms": float(np.median(t_grid)), "grid_nodes": int(np.prod(grid.dims)) * len(s.lig_types)}
+    if not args.no_search:
+        s2 = make_system(2, seed=0)
+        box2 = dk.make_box(s2.box_center, s2.box_size, s2.spacing)
+        lig2 = dk.LigandHandle(s2.ligand)
+        grid2 = dk.dock_build_grids(p, s2.protein_xyz, s2.protein_type, box2, s2.lig_types)
+        run = lambda: dk.dock_search(p, [grid2], [lig2], [box2], s2.copies, s2.steps, s2.bfgs_cap, 2023)
+        run()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        res = run()
+        torch.cuda.synchronize()
+        t_s = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        r_h = dk.dock_system_host(p, s2.protein_xyz, s2.protein_type, box2, lig2, s2.lig_types, s2.copies, s2.steps,
+                                  s2.bfgs_cap, 2023)
+        t_h = time.perf_counter() - t0
+        extra["site_docking"] = {"workload": "configs[2]: 384 copies x 40 steps, BFGS<=300", "search_s": t_s,
+                                 "evals": int(res["evals"][0]), "evals_per_s": int(res["evals"][0]) / t_s,
+                                 "systems_per_s_search_only": 1.0 / t_s, "end_to_end_host_s": t_h,
+                                 "systems_per_s_end_to_end": 1.0 / t_h, "best_e": float(res["topk_e"][0, 0]),
+                                 "paper_context": "DSDP 384x40 redocking 0.55 s/system on RTX 2080 SUPER (PAPER.md:108)"}
+    line["extra"] = extra
+    return line
+
+
+# per-launch DRAM traffic of the score kernel from the committed `ncu --set full` capture
+# (profiles/); None until a capture exists for the current kernel.
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-sample", type=int, default=1048576, help="poses the CPU oracle scores per step")
+    ap.add_argument("--no-flush", action="store_true")
+    ap.add_argument("--no-search", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        print(json.dumps(run_reference(args)))
+        return
+    line = run_ours(args)
+    if line:
+        print(json.dumps(line))
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -97,8 +97,14 @@ typedef struct dock_ligand {
     const int32_t *pairs;          /* [P][2] intra-ligand scoring pairs, i != j */
 } dock_ligand;
 
-/* Grid-map descriptor written by dock_build_grids.  data layout: [n_maps][nz][ny][nx] fp32,
- * node (ix,iy,iz) at origin + spacing*(ix,iy,iz) (eq. 2 at 198-199). */
+/* Grid-map descriptor written by dock_build_grids.  Two DEVICE images of the same maps live in the
+ * caller's buffer (dock_grid_bytes() bytes, 256-byte aligned):
+ *   data_dev   [n_maps][nz][ny][nx] fp32 -- the maps themselves: node (ix,iy,iz) at
+ *              origin + spacing*(ix,iy,iz) holds eq. 2's vertex score;
+ *   packed_dev [n_maps][nz][ny][nx][4] fp32 -- the gather layout read by every evaluator: entry
+ *              (ix,iy,iz) = {G(ix,iy), G(ix+1,iy), G(ix,iy+1), G(ix+1,iy+1)} at plane iz (indices
+ *              clamped to the last node), so the 8 corners of a cell are two 16-byte loads
+ *              (DESIGN.md "Data layout").  Values are bit-identical copies of data_dev. */
 typedef struct dock_grid {
     int32_t      dims[3];                          /* nx, ny, nz */
     float        origin[3];
@@ -106,6 +112,7 @@ typedef struct dock_grid {
     int32_t      n_maps;
     int32_t      type_to_map[DOCK_MAX_XS_TYPES];   /* XS type id -> map index, -1 = absent */
     const float *data_dev;                         /* DEVICE pointer, caller-owned */
+    const float *packed_dev;                       /* DEVICE pointer into the same buffer */
 } dock_grid;
 
 /* Optional per-(system, copy, step) trace of the search; with the stateless Philox counter it
@@ -118,10 +125,12 @@ int dock_default_params(dock_params *out);
 
 /* ---- A1: grid maps ----------------------------------------
  * G[m][node] = sum over protein atoms j with |node - r_j| < cutoff of f(lig_types[m], type_j, r).
- * protein: host.  grid_dev: device, n_lig_types * nx*ny*nz floats (see dock_grid_dims).
- * out_desc (host) receives the descriptor with data_dev = grid_dev.
+ * protein: host.  grid_dev: device, dock_grid_bytes(box, n_lig_types) bytes, 256-byte aligned.
+ * out_desc (host) receives the descriptor with data_dev = grid_dev and packed_dev behind it.
  * Errors: DOCK_EINVAL for null pointers, n < 0, spacing <= 0, type ids outside [0, n_types). */
 int dock_grid_dims(const dock_box *box, int32_t dims[3]);
+/* bytes of the caller's grid buffer for n_lig_types maps over `box` (both images); 0 on bad input */
+size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types);
 int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
                      int32_t n_lig_types, const int32_t *lig_types,
                      float *grid_dev, dock_grid *out_desc,

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     dock_build_grids,
     dock_default_params,
     dock_grid,
+    dock_grid_bytes,
     dock_grid_dims,
     dock_init_poses,
     dock_ligand,

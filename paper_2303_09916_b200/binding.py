@@ -22,7 +22,7 @@ DOCK_TRACE_HEADER = 8
 DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
 
 EXPORTS = [
-    "dock_default_params", "dock_grid_dims", "dock_build_grids", "dock_score_batch",
+    "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_score_batch",
     "dock_score_batch_host", "dock_local_opt_batch", "dock_init_poses", "dock_search", "dock_topk",
     "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
 ]
@@ -68,6 +68,7 @@ class dock_grid(C.Structure):
     _fields_ = [
         ("dims", C.c_int32 * 3), ("origin", C.c_float * 3), ("spacing", C.c_float),
         ("n_maps", C.c_int32), ("type_to_map", C.c_int32 * DOCK_MAX_XS_TYPES), ("data_dev", C.c_void_p),
+        ("packed_dev", C.c_void_p),
     ]
 
 
@@ -85,6 +86,7 @@ def load_library(path: Optional[str] = None):
         _lib = C.CDLL(path)
         _lib.dock_version.restype = C.c_char_p
         _lib.dock_launch_count.restype = C.c_uint64
+        _lib.dock_grid_bytes.restype = C.c_size_t
     return _lib
 
 
@@ -171,9 +173,11 @@ class LigandHandle:
 
 
 class GridMaps:
-    """Device grid maps (torch tensor [n_maps, nz, ny, nx]) + descriptor."""
+    """Device grid maps + descriptor.  `buf` owns the memory (both images, see dock.h);
+    `data` is the [n_maps, nz, ny, nx] view of the maps themselves."""
 
-    def __init__(self, data, desc: dock_grid):
+    def __init__(self, buf, data, desc: dock_grid):
+        self.buf = buf
         self.data = data
         self.desc = desc
 
@@ -188,6 +192,13 @@ def dock_grid_dims(box: dock_box):
     return tuple(int(x) for x in d)
 
 
+def dock_grid_bytes(box: dock_box, n_lig_types: int) -> int:
+    n = int(load_library().dock_grid_bytes(C.byref(box), int(n_lig_types)))
+    if n == 0:
+        raise DockError("dock_grid_bytes: bad box or type count")
+    return n
+
+
 def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_box,
                      lig_types: Sequence[int], stream=None) -> GridMaps:
     torch = _torch()
@@ -197,7 +208,8 @@ def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_b
     prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
     lt = np.ascontiguousarray(lig_types, dtype=np.int32)
     nx, ny, nz = dock_grid_dims(box)
-    data = torch.empty((len(lt), nz, ny, nx), dtype=torch.float32, device="cuda")
+    buf = torch.empty(dock_grid_bytes(box, len(lt)), dtype=torch.uint8, device="cuda")
+    data = buf[: len(lt) * nz * ny * nx * 4].view(torch.float32).view(len(lt), nz, ny, nx)
     desc = dock_grid()
     need = C.c_size_t(0)
     rc = lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
@@ -206,9 +218,9 @@ def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_b
         _check(rc, "dock_build_grids(size query)")
     ws = _ws.get(need.value)
     _check(lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
-                                _ptr(data), C.byref(desc), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
+                                _ptr(buf), C.byref(desc), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
                                 _stream(stream)), "dock_build_grids")
-    return GridMaps(data, desc)
+    return GridMaps(buf, data, desc)
 
 
 def dock_score_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses,
@@ -356,9 +368,8 @@ def dock_system_host(params: dock_params, protein_xyz, protein_type, box: dock_b
     typ = np.ascontiguousarray(protein_type, dtype=np.int32)
     prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
     lt = np.ascontiguousarray(lig_types, dtype=np.int32)
-    nx, ny, nz = dock_grid_dims(box)
     if grid_buf is None:
-        grid_buf = torch.empty((len(lt), nz, ny, nx), dtype=torch.float32, device="cuda")
+        grid_buf = torch.empty(dock_grid_bytes(box, len(lt)), dtype=torch.uint8, device="cuda")
     k = int(params.topk)
     out_pose = np.zeros((k, 7 + ligand.T), dtype=np.float32)
     out_e = np.zeros(k, dtype=np.float32)

@@ -41,14 +41,23 @@ struct DevParams {
     int   max_trials;
 };
 
+// Grid maps as the evaluators see them.  Positions are handled relative to a reference node of the
+// lattice near its centre (node index ic* on each axis): coordinates stay small, so fp32 keeps
+// ~1e-6 A where lab-frame coordinates of 30-50 A would keep ~4e-6 A.
 struct DevGrid {
     int   nx, ny, nz;
-    float ox, oy, oz;        // origin
-    float hx, hy, hz;        // coordinate of the last node on each axis
-    float h, inv_h;
-    const float *data;       // [n_maps][nz][ny][nx]
+    int   icx, icy, icz;            // index of the reference node
+    float rx, ry, rz;               // fp32 position of the reference node ...
+    float rdx, rdy, rdz;            // ... and the remainder (true - fp32) of that position
+    float lo_x, lo_y, lo_z;         // -ic*            (cell units, relative to the reference node)
+    float hi_x, hi_y, hi_z;         // n-1-ic*
+    float h, inv_h, inv_h_lo;       // spacing; fl(1/h) and 1/h - fl(1/h)
+    float kw_g, kw_e;               // wall: 2 k h (gradient per cell of overshoot), k h^2
+    const float4 *packed;           // [n_maps][nz][ny][nx] gather layout (see dock.h)
+    const float  *data;             // [n_maps][nz][ny][nx]
 };
 
+// ---- warp-per-pose evaluator (search kernels): compiled ligand in the caller's workspace --------
 // One scheduled intra-ligand pair.  ij = i | (j << 16), or -1 for an idle lane.
 struct __align__(16) PairRec {
     int   ij;
@@ -57,11 +66,10 @@ struct __align__(16) PairRec {
     float whb;    // w5 if donor/acceptor pair else 0
 };
 
-// Compiled ligand (all pointers into the caller's workspace).
 struct DevLigand {
     int N, T, P, n_rounds;
     int n_pad;                 // stride of the per-warp coordinate arrays
-    const float4  *atom_ref;   // [N] reference xyz relative to the pivot; w = bitcast(map offset in floats)
+    const float4  *atom_ref;   // [N] reference xyz relative to the pivot; w = bitcast(map offset in packed entries)
     const int2    *atom_topo;  // [N] {fragment, mask of torsions on the path to the root}
     const float4  *tors_axis;  // [T] unit axis in the reference frame
     const float4  *tors_pt;    // [T] reference position of atom b relative to the pivot; w = bitcast(parent fragment)
@@ -73,6 +81,27 @@ struct DevSystem {
     DevGrid   grid;
     DevLigand lig;
     float     box_lo[3], box_size[3];
+};
+
+// ---- thread-per-pose evaluator (batch scoring): ligand tables in the kernel-parameter constant
+// bank, so that every table read is a uniform constant load and costs no L1 wavefront ------------
+#define TPP_TILE 4                      // atoms of the i-tile held in registers in the pair phase
+#define TPP_REC_WORDS (1 + TPP_TILE)    // word0 + one R_i+R_j per tile atom
+#define TPP_SCHED_WORDS 6400            // capacity of the in-parameter schedule (25.6 KB)
+
+struct TppLigand {
+    int N, T, n_groups, sched_in_param;
+    float4 atom_ref[DOCK_MAX_ATOMS];        // slot order (sorted by fragment): xyz rel. pivot, w = bitcast(map offset in entries)
+    float4 tors_axis[DOCK_MAX_TORSIONS];    // reference-frame unit axis; w = bitcast(parent fragment)
+    float4 tors_pt[DOCK_MAX_TORSIONS];      // reference position of atom b rel. pivot; w = 1 / |ref_b - ref_a|
+    unsigned char  atom_frag[DOCK_MAX_ATOMS];
+    unsigned char  tors_a[DOCK_MAX_TORSIONS], tors_b[DOCK_MAX_TORSIONS];   // slots of the axis atoms
+    unsigned char  frag_end[DOCK_MAX_TORSIONS + 4];                        // one past the last slot of fragment f
+    // Pair schedule: groups of <= TPP_TILE i-slots; per group a header
+    //   {i-slots (4 bytes), number of records}, then records of TPP_REC_WORDS words:
+    //   word0 = j | mask << 8 | hyd << 12 | hb << 16  (bit t of each field = tile atom t),  then R_i+R_j for t = 0..3.
+    const uint32_t *sched_global;           // the same stream in global memory (used when it does not fit below)
+    uint32_t sched[TPP_SCHED_WORDS];
 };
 
 // ---- device helpers ---------------------------------------------------------------------------

@@ -1,0 +1,166 @@
+// eval_warp.cuh -- fused pose -> coordinates -> energy + gradient, ONE WARP PER POSE (SURVEY.md 8(a)
+// A2-A5).  The latency evaluator behind the search kernels, where a few hundred copies must fill the
+// GPU and each copy's evaluations are sequential (the throughput evaluator is eval_thread.cuh).
+//
+//   A2 kinematics : every lane owns atoms i = lane, lane+32, ... and walks the torsions on the path
+//                   from the atom's fragment to the root (deepest first), one Rodrigues rotation
+//                   about the reference-frame axis each, then x = t + R(q) y (box-relative).
+//   A3 inter term : two 16-byte gathers from the packed map of the atom's type, trilinear energy
+//                   (eq. 2, 198-207) and the partial derivatives of the interpolant (eq. 3,
+//                   213-219); clamp + quadratic wall outside the box.
+//   A4 intra term : host-built conflict-free schedule, 32 pairs per round; forces go to the per-warp
+//                   shared-memory gradient array with plain read-modify-writes in two phases
+//                   (all sources, then all destinations) -> deterministic, no float atomics.
+//   A5 chain rule : force = sum g_i, torque = sum (x_i - t) x g_i, dE/dtheta_k = u_k . sum_{subtree} (x_i - x_b) x g_i.
+//
+// All lanes of the warp return the same energy.  `pose` (7+T floats) and `grad` (6+T floats) live
+// in shared memory owned by the warp; `scratch` is eval_scratch_floats() floats of the same.
+#pragma once
+
+#include "common.cuh"
+#include "eval_thread.cuh"   // EvalTerms
+#include "mathx.cuh"
+
+// A2 for atom i: box-relative position.  `sn`, `cs` hold sin/cos(theta_k).
+__device__ __forceinline__ void atom_coords(const DevLigand &L, const Rot3 &R, float tx, float ty, float tz,
+                                            const float *sn, const float *cs, int i,
+                                            float &x0, float &x1, float &x2, int &map_off)
+{
+    const float4 a = __ldg(&L.atom_ref[i]);
+    float y0 = a.x, y1 = a.y, y2 = a.z;
+    map_off = __float_as_int(a.w);
+    int f = __ldg(&L.atom_topo[i]).x;
+    while (f > 0) {
+        const int k = f - 1;
+        const float4 u = __ldg(&L.tors_axis[k]);
+        const float4 b = __ldg(&L.tors_pt[k]);
+        const float c = cs[k];
+        rodrigues(u.x, u.y, u.z, b.x, b.y, b.z, sn[k], c, 1.0f - c, y0, y1, y2);
+        f = __float_as_int(b.w);
+    }
+    x0 = fmaf(R.m00, y0, fmaf(R.m01, y1, fmaf(R.m02, y2, tx)));
+    x1 = fmaf(R.m10, y0, fmaf(R.m11, y1, fmaf(R.m12, y2, ty)));
+    x2 = fmaf(R.m20, y0, fmaf(R.m21, y1, fmaf(R.m22, y2, tz)));
+}
+
+// Coordinates only (used by the top-k kernel): xs[c*np + i].
+__device__ __forceinline__ void pose_coords_warp(const DevLigand &L, const float *pose, float *xs, float *sc)
+{
+    const int lane = threadIdx.x & 31, T = L.T, np = L.n_pad;
+    float *sn = sc, *cs = sc + ((T + 3) & ~3);
+    if (lane < T) {
+        float s, c;
+        sincos_cw(pose[7 + lane], s, c);
+        sn[lane] = s; cs[lane] = c;
+    }
+    const Rot3 R = quat_to_rot(pose[3], pose[4], pose[5], pose[6]);
+    __syncwarp();
+    for (int i = lane; i < L.N; i += 32) {
+        float x0, x1, x2;
+        int mo;
+        atom_coords(L, R, pose[0], pose[1], pose[2], sn, cs, i, x0, x1, x2, mo);
+        xs[i] = x0; xs[np + i] = x1; xs[2 * np + i] = x2;
+    }
+    __syncwarp();
+}
+
+template <bool WANT_GRAD>
+__device__ __noinline__ float eval_pose_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
+                                             const float *pose, float *grad, float *scratch, EvalTerms *terms)
+{
+    const int lane = threadIdx.x & 31;
+    const int N = L.N, T = L.T, np = L.n_pad;
+    float *xs = scratch, *gs = scratch + 3 * np;
+    float *sn = gs + 3 * np, *cs = sn + ((T + 3) & ~3);
+
+    if (lane < T) {
+        float s, c;
+        sincos_cw(pose[7 + lane], s, c);
+        sn[lane] = s; cs[lane] = c;
+    }
+    const float tx = (pose[0] - G.rx) - G.rdx, ty = (pose[1] - G.ry) - G.rdy, tz = (pose[2] - G.rz) - G.rdz;
+    const Rot3 R = quat_to_rot(pose[3], pose[4], pose[5], pose[6]);
+    __syncwarp();
+
+    // ---- A2 + A3 -------------------------------------------------------------------------------
+    float e_grid = 0.0f, e_wall = 0.0f;
+    for (int i = lane; i < N; i += 32) {
+        float x0, x1, x2, gx, gy, gz;
+        int map_off;
+        atom_coords(L, R, tx, ty, tz, sn, cs, i, x0, x1, x2, map_off);
+        xs[i] = x0; xs[np + i] = x1; xs[2 * np + i] = x2;
+        const CellRef cr = locate_cell(G, x0, x1, x2);
+        const float4 *e0 = G.packed + (size_t)map_off + cr.idx;
+        const float4 q0 = __ldg(e0), q1 = __ldg(e0 + G.nx * G.ny);
+        e_grid += trilinear(G, cr, q0, q1, e_wall, gx, gy, gz);
+        if (WANT_GRAD) { gs[i] = gx; gs[np + i] = gy; gs[2 * np + i] = gz; }
+    }
+    __syncwarp();
+
+    // ---- A4 ------------------------------------------------------------------------------------
+    float e_intra = 0.0f;
+    for (int r = 0; r < L.n_rounds; ++r) {
+        const float4 raw = __ldg(reinterpret_cast<const float4 *>(L.sched + r * 32 + lane));
+        const int ij = __float_as_int(raw.x);
+        int i = 0, j = 0;
+        float fx = 0.0f, fy = 0.0f, fz = 0.0f;
+        bool hit = false;
+        if (ij >= 0) {
+            i = ij & 0xffff; j = ij >> 16;
+            const float dx = xs[i] - xs[j], dy = xs[np + i] - xs[np + j], dz = xs[2 * np + i] - xs[2 * np + j];
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (r2 < P.cutoff2) {
+                float k;
+                e_intra += pair_term_rt(P, r2, raw.y, raw.z, raw.w, k);
+                fx = k * dx; fy = k * dy; fz = k * dz;
+                hit = true;
+            }
+        }
+        if (WANT_GRAD) {
+            if (hit) { gs[i] += fx; gs[np + i] += fy; gs[2 * np + i] += fz; }
+            __syncwarp();
+            if (hit) { gs[j] -= fx; gs[np + j] -= fy; gs[2 * np + j] -= fz; }
+            __syncwarp();
+        }
+    }
+
+    e_grid = warp_sum(e_grid);
+    e_wall = warp_sum(e_wall);
+    e_intra = warp_sum(e_intra);
+    if (terms) { terms->e_grid = e_grid; terms->e_wall = e_wall; terms->e_intra = e_intra; }
+
+    // ---- A5 ------------------------------------------------------------------------------------
+    if (WANT_GRAD) {
+        float fx = 0.f, fy = 0.f, fz = 0.f, qx = 0.f, qy = 0.f, qz = 0.f;
+        for (int i = lane; i < N; i += 32) {
+            const float gx = gs[i], gy = gs[np + i], gz = gs[2 * np + i];
+            const float lx = xs[i] - tx, ly = xs[np + i] - ty, lz = xs[2 * np + i] - tz;
+            fx += gx; fy += gy; fz += gz;
+            qx += ly * gz - lz * gy;
+            qy += lz * gx - lx * gz;
+            qz += lx * gy - ly * gx;
+        }
+        fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
+        qx = warp_sum(qx); qy = warp_sum(qy); qz = warp_sum(qz);
+        if (lane == 0) { grad[0] = fx; grad[1] = fy; grad[2] = fz; grad[3] = qx; grad[4] = qy; grad[5] = qz; }
+        for (int k = 0; k < T; ++k) {
+            const int2 ab = __ldg(&L.tors_ab[k]);
+            const float bx = xs[ab.y], by = xs[np + ab.y], bz = xs[2 * np + ab.y];
+            float ux = bx - xs[ab.x], uy = by - xs[np + ab.x], uz = bz - xs[2 * np + ab.x];
+            const float inv = 1.0f / sqrtf(ux * ux + uy * uy + uz * uz);
+            ux *= inv; uy *= inv; uz *= inv;
+            float c = 0.0f;
+            for (int i = lane; i < N; i += 32) {
+                if ((__ldg(&L.atom_topo[i]).y >> k) & 1) {
+                    const float gx = gs[i], gy = gs[np + i], gz = gs[2 * np + i];
+                    const float lx = xs[i] - bx, ly = xs[np + i] - by, lz = xs[2 * np + i] - bz;
+                    c += ux * (ly * gz - lz * gy) + uy * (lz * gx - lx * gz) + uz * (lx * gy - ly * gx);
+                }
+            }
+            c = warp_sum(c);
+            if (lane == 0) grad[6 + k] = c;
+        }
+        __syncwarp();
+    }
+    return e_grid + e_wall + e_intra;
+}

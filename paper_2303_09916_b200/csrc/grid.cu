@@ -8,6 +8,7 @@
 // compact 4x4x2 block of nodes so that its lanes share almost the same in-range atom set; each thread
 // walks the <= 27 cells around its node, decides r < cutoff in fp32 in the stated order
 // (DESIGN.md D-CUT) and accumulates up to 8 maps in registers.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <vector>
@@ -107,6 +108,24 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
         if (m < nm) A.out[(size_t)(m0 + m) * nodes + node] = acc[m];
 }
 
+// Gather layout: entry (ix,iy,iz) of map m = {G(ix,iy), G(ix+1,iy), G(ix,iy+1), G(ix+1,iy+1)} at plane iz
+// (indices clamped to the last node).  Pure data movement: values are bit-identical copies.
+__global__ void __launch_bounds__(256) grid_pack_kernel(const float *__restrict__ plain, float4 *__restrict__ packed,
+                                                        int nx, int ny, long long rows)
+{
+    // one thread per (map, iz, iy) row segment element; consecutive threads walk x -> coalesced
+    const long long total = rows * nx;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+        const int ix = (int)(e % nx);
+        const long long row = e / nx;                 // (m * nz + iz) * ny + iy
+        const int iy = (int)(row % ny);
+        const long long up = (iy + 1 < ny) ? nx : 0;
+        const int rt = (ix + 1 < nx) ? 1 : 0;
+        const float *q = plain + e;
+        packed[e] = make_float4(__ldg(q), __ldg(q + rt), __ldg(q + up), __ldg(q + up + rt));
+    }
+}
+
 struct GridPlan {
     int dims[3];
     float origin[3];
@@ -191,6 +210,14 @@ extern "C" int dock_grid_dims(const dock_box *box, int32_t dims[3])
     return DOCK_OK;
 }
 
+extern "C" size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types)
+{
+    int32_t dims[3];
+    if (n_lig_types < 1 || n_lig_types > DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
+    const size_t nodes = (size_t)dims[0] * dims[1] * dims[2] * (size_t)n_lig_types;
+    return align_up(nodes * sizeof(float), 256) + nodes * sizeof(float4);
+}
+
 extern "C" int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
                                 int32_t n_lig_types, const int32_t *lig_types,
                                 float *grid_dev, dock_grid *out_desc,
@@ -205,7 +232,7 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     const size_t need = b_atoms + b_cells + b_tab;
     if (needed) *needed = need;
     if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
-    if (!grid_dev || !out_desc) return DOCK_EINVAL;
+    if (!grid_dev || !out_desc || ((uintptr_t)grid_dev & 255)) return DOCK_EINVAL;
     cudaStream_t stream = (cudaStream_t)stream_;
     unsigned char *ws = (unsigned char *)ws_dev;
     DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.atoms.data(), pl.atoms.size() * sizeof(float4), cudaMemcpyHostToDevice, stream));
@@ -232,6 +259,12 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     dim3 grid((unsigned)(tbx * tby * tbz), (unsigned)((n_lig_types + MAPS_PER_PASS - 1) / MAPS_PER_PASS));
     grid_build_kernel<<<grid, 128, 0, stream>>>(A);
     DOCK_LAUNCH_CHECK();
+    const size_t nodes = (size_t)A.nx * A.ny * A.nz * (size_t)n_lig_types;
+    float4 *packed = reinterpret_cast<float4 *>(reinterpret_cast<unsigned char *>(grid_dev) + align_up(nodes * sizeof(float), 256));
+    const long long rows = (long long)n_lig_types * A.nz * A.ny;
+    const unsigned pack_blocks = (unsigned)std::min<long long>((rows * A.nx + 255) / 256, 148LL * 16);
+    grid_pack_kernel<<<pack_blocks, 256, 0, stream>>>(grid_dev, packed, A.nx, A.ny, rows);
+    DOCK_LAUNCH_CHECK();
 
     std::memset(out_desc, 0, sizeof(*out_desc));
     for (int c = 0; c < 3; ++c) { out_desc->dims[c] = pl.dims[c]; out_desc->origin[c] = pl.origin[c]; }
@@ -240,5 +273,6 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     for (int t = 0; t < DOCK_MAX_XS_TYPES; ++t) out_desc->type_to_map[t] = -1;
     for (int m = 0; m < n_lig_types; ++m) out_desc->type_to_map[lig_types[m]] = m;
     out_desc->data_dev = grid_dev;
+    out_desc->packed_dev = reinterpret_cast<const float *>(packed);
     return DOCK_OK;
 }

@@ -80,18 +80,32 @@ int dock_make_dev_params(const dock_params *p, DevParams *o)
     return DOCK_OK;
 }
 
-int dock_make_dev_grid(const dock_grid *g, DevGrid *o)
+int dock_make_dev_grid(const dock_params *p, const dock_grid *g, DevGrid *o)
 {
-    if (!g || !g->data_dev) return DOCK_EINVAL;
+    if (!p || !g || !g->data_dev || !g->packed_dev) return DOCK_EINVAL;
     if (g->dims[0] < 2 || g->dims[1] < 2 || g->dims[2] < 2 || !(g->spacing > 0.f)) return DOCK_EINVAL;
     if (g->n_maps < 1 || g->n_maps > DOCK_MAX_XS_TYPES) return DOCK_EINVAL;
     o->nx = g->dims[0]; o->ny = g->dims[1]; o->nz = g->dims[2];
-    o->ox = g->origin[0]; o->oy = g->origin[1]; o->oz = g->origin[2];
+    const double h = (double)g->spacing;
+    int ic[3];
+    float r32[3], rd[3];
+    for (int c = 0; c < 3; ++c) {
+        ic[c] = (g->dims[c] - 1) / 2;                                   // reference node near the centre
+        const double r = (double)g->origin[c] + h * ic[c];              // its exact position
+        r32[c] = (float)r;
+        rd[c] = (float)(r - (double)r32[c]);
+    }
+    o->icx = ic[0]; o->icy = ic[1]; o->icz = ic[2];
+    o->rx = r32[0]; o->ry = r32[1]; o->rz = r32[2];
+    o->rdx = rd[0]; o->rdy = rd[1]; o->rdz = rd[2];
+    o->lo_x = -(float)ic[0]; o->lo_y = -(float)ic[1]; o->lo_z = -(float)ic[2];
+    o->hi_x = (float)(g->dims[0] - 1 - ic[0]); o->hi_y = (float)(g->dims[1] - 1 - ic[1]); o->hi_z = (float)(g->dims[2] - 1 - ic[2]);
     o->h = g->spacing;
-    o->inv_h = 1.0f / g->spacing;
-    o->hx = fmaf((float)(g->dims[0] - 1), g->spacing, g->origin[0]);
-    o->hy = fmaf((float)(g->dims[1] - 1), g->spacing, g->origin[1]);
-    o->hz = fmaf((float)(g->dims[2] - 1), g->spacing, g->origin[2]);
+    o->inv_h = (float)(1.0 / h);
+    o->inv_h_lo = (float)(1.0 / h - (double)o->inv_h);
+    o->kw_g = (float)(2.0 * (double)p->k_wall * h);
+    o->kw_e = (float)((double)p->k_wall * h * h);
+    o->packed = reinterpret_cast<const float4 *>(g->packed_dev);
     o->data = g->data_dev;
     return DOCK_OK;
 }
@@ -250,4 +264,127 @@ DevLigand dock_relocate_ligand(const LigandBlob &b, const unsigned char *base)
     d.tors_ab = (const int2 *)(base + (size_t)b.rel.tors_ab);
     d.sched = (const PairRec *)(base + (size_t)b.rel.sched);
     return d;
+}
+
+// ---- thread-per-pose tables ------------------------------------------------------------------------
+int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand *L, TppLigand &out,
+                     std::vector<uint32_t> &overflow)
+{
+    LigandBlob chk;                                   // reuse the validation of the warp-per-pose compiler
+    if (!g || dock_compile_ligand(p, g, L, chk) != DOCK_OK) return DOCK_EINVAL;
+    const int N = L->N, T = L->T, P = L->P;
+    std::memset(&out, 0, sizeof(out));
+    overflow.clear();
+    out.N = N; out.T = T;
+
+    double c[3] = {0, 0, 0};
+    int nroot = 0;
+    for (int i = 0; i < N; ++i)
+        if (L->atom_fragment[i] == 0) {
+            for (int d = 0; d < 3; ++d) c[d] += (double)L->ref_xyz[3 * i + d];
+            ++nroot;
+        }
+    for (int d = 0; d < 3; ++d) c[d] /= nroot;
+
+    // slots = atoms sorted by fragment (stable), so that a fragment's atoms are contiguous
+    std::vector<int> atom_of(N), slot_of(N);
+    for (int i = 0; i < N; ++i) atom_of[i] = i;
+    std::stable_sort(atom_of.begin(), atom_of.end(),
+                     [&](int a, int b) { return L->atom_fragment[a] < L->atom_fragment[b]; });
+    for (int s = 0; s < N; ++s) slot_of[atom_of[s]] = s;
+    const long long map_stride = (long long)g->dims[0] * g->dims[1] * g->dims[2];
+    int f_cur = 0;
+    for (int s = 0; s < N; ++s) {
+        const int i = atom_of[s];
+        const long long off = (long long)g->type_to_map[L->type[i]] * map_stride;
+        if (off > 0x7fffffffLL) return DOCK_EINVAL;
+        const int ioff = (int)off;
+        out.atom_ref[s] = make_float4((float)((double)L->ref_xyz[3 * i] - c[0]), (float)((double)L->ref_xyz[3 * i + 1] - c[1]),
+                                      (float)((double)L->ref_xyz[3 * i + 2] - c[2]), 0.f);
+        std::memcpy(&out.atom_ref[s].w, &ioff, 4);
+        out.atom_frag[s] = (unsigned char)L->atom_fragment[i];
+        while (f_cur < L->atom_fragment[i]) out.frag_end[f_cur++] = (unsigned char)s;
+    }
+    while (f_cur <= T) out.frag_end[f_cur++] = (unsigned char)N;
+    for (int k = 0; k < T; ++k) {
+        const int a = L->tors_a[k], b = L->tors_b[k];
+        double u[3], n = 0;
+        for (int d = 0; d < 3; ++d) { u[d] = (double)L->ref_xyz[3 * b + d] - (double)L->ref_xyz[3 * a + d]; n += u[d] * u[d]; }
+        n = std::sqrt(n);
+        const int par = L->tors_parent[k];
+        out.tors_axis[k] = make_float4((float)(u[0] / n), (float)(u[1] / n), (float)(u[2] / n), 0.f);
+        std::memcpy(&out.tors_axis[k].w, &par, 4);
+        out.tors_pt[k] = make_float4((float)((double)L->ref_xyz[3 * b] - c[0]), (float)((double)L->ref_xyz[3 * b + 1] - c[1]),
+                                     (float)((double)L->ref_xyz[3 * b + 2] - c[2]), (float)(1.0 / n));
+        out.tors_a[k] = (unsigned char)slot_of[a];
+        out.tors_b[k] = (unsigned char)slot_of[b];
+    }
+
+    // pair schedule: tiles of TPP_TILE consecutive slots.  The pairs between two tiles A < B form a
+    // small bit matrix; they all go either to A's group (one record per partner j in B) or to B's
+    // group (one record per partner j in A), whichever needs fewer records.
+    const int n_tiles = (N + TPP_TILE - 1) / TPP_TILE;
+    struct Rec { int j; uint32_t mask, hyd, hb; float rsum[TPP_TILE]; };
+    std::vector<std::vector<Rec>> groups(n_tiles);
+    std::vector<std::vector<std::pair<int, int>>> between((size_t)n_tiles * n_tiles);   // (slot in A, slot in B)
+    for (int k = 0; k < P; ++k) {
+        int sa = slot_of[L->pairs[2 * k]], sb = slot_of[L->pairs[2 * k + 1]];
+        if (sa > sb) std::swap(sa, sb);
+        between[(size_t)(sa / TPP_TILE) * n_tiles + sb / TPP_TILE].push_back({sa, sb});
+    }
+    auto add = [&](int tile, int i_slot, int j_slot) {
+        std::vector<Rec> &grp = groups[tile];
+        Rec *r = nullptr;
+        for (Rec &q : grp) if (q.j == j_slot) { r = &q; break; }
+        if (!r) { grp.push_back(Rec{j_slot, 0u, 0u, 0u, {0.f, 0.f, 0.f, 0.f}}); r = &grp.back(); }
+        const int t = i_slot - tile * TPP_TILE;
+        const int ti = L->type[atom_of[i_slot]], tj = L->type[atom_of[j_slot]];
+        r->mask |= 1u << t;
+        if (p->hydrophobic[ti] && p->hydrophobic[tj]) r->hyd |= 1u << t;
+        if ((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) r->hb |= 1u << t;
+        r->rsum[t] = p->radius[ti] + p->radius[tj];
+    };
+    for (int A = 0; A < n_tiles; ++A)
+        for (int B = A; B < n_tiles; ++B) {
+            const auto &pl = between[(size_t)A * n_tiles + B];
+            if (pl.empty()) continue;
+            uint32_t rows = 0, cols = 0;
+            for (auto &e : pl) { rows |= 1u << (e.first - A * TPP_TILE); cols |= 1u << (e.second - B * TPP_TILE); }
+            const bool to_a = (A == B) || __builtin_popcount(cols) <= __builtin_popcount(rows);
+            for (auto &e : pl) {
+                if (to_a) add(A, e.first, e.second);
+                else add(B, e.second, e.first);
+            }
+        }
+    std::vector<uint32_t> words;
+    int n_groups = 0;
+    for (int A = 0; A < n_tiles; ++A) {
+        std::vector<Rec> &grp = groups[A];
+        if (grp.empty()) continue;
+        std::stable_sort(grp.begin(), grp.end(), [](const Rec &a, const Rec &b) { return a.j < b.j; });
+        const int n_i = std::min(TPP_TILE, N - A * TPP_TILE);
+        uint32_t h0 = 0;
+        for (int t = 0; t < TPP_TILE; ++t) h0 |= (uint32_t)(A * TPP_TILE + (t < n_i ? t : 0)) << (8 * t);
+        if (grp.size() > 0xffffu) return DOCK_EINVAL;
+        words.push_back(h0);
+        words.push_back((uint32_t)grp.size() | ((uint32_t)n_i << 16));
+        for (const Rec &r : grp) {
+            words.push_back((uint32_t)r.j | (r.mask << 8) | (r.hyd << 12) | (r.hb << 16));
+            for (int t = 0; t < TPP_TILE; ++t) {
+                uint32_t w;
+                std::memcpy(&w, &r.rsum[t], 4);
+                words.push_back(w);
+            }
+        }
+        ++n_groups;
+    }
+    out.n_groups = n_groups;
+    if (words.size() <= (size_t)TPP_SCHED_WORDS) {
+        out.sched_in_param = 1;
+        std::memcpy(out.sched, words.data(), words.size() * sizeof(uint32_t));
+    } else {
+        out.sched_in_param = 0;
+        overflow.swap(words);
+    }
+    return DOCK_OK;
 }

@@ -20,7 +20,13 @@ DevLigand dock_relocate_ligand(const LigandBlob &b, const unsigned char *dev_bas
 
 int dock_validate_params(const dock_params *p);
 int dock_make_dev_params(const dock_params *p, DevParams *out);
-int dock_make_dev_grid(const dock_grid *g, DevGrid *out);
+int dock_make_dev_grid(const dock_params *p, const dock_grid *g, DevGrid *out);
 
-// number of floats of per-warp shared memory the evaluator needs for this ligand
+// Thread-per-pose tables (eval_thread.cuh).  DOCK_OK or DOCK_EINVAL.  If the pair schedule does not
+// fit TppLigand::sched, out.sched_in_param = 0 and `overflow` holds the stream for the caller to
+// upload (then point out.sched_global at it); otherwise `overflow` is empty.
+int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand *lig, TppLigand &out,
+                     std::vector<uint32_t> &overflow);
+
+// number of floats of per-warp shared memory the warp-per-pose evaluator needs for this ligand
 static inline int eval_scratch_floats(int n_pad, int T) { return 6 * n_pad + 2 * ((T + 3) & ~3); }

@@ -11,7 +11,7 @@
 #include <vector>
 
 #include "common.cuh"
-#include "eval.cuh"
+#include "eval_warp.cuh"
 #include "host_compile.cuh"
 
 namespace {
@@ -434,7 +434,7 @@ extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *
     DevParams P;
     DevGrid G;
     LigandBlob blob;
-    if (dock_make_dev_params(params, &P) != DOCK_OK || dock_make_dev_grid(grid, &G) != DOCK_OK) return DOCK_EINVAL;
+    if (dock_make_dev_params(params, &P) != DOCK_OK || dock_make_dev_grid(params, grid, &G) != DOCK_OK) return DOCK_EINVAL;
     if (dock_compile_ligand(params, grid, ligand, blob) != DOCK_OK) return DOCK_EINVAL;
     if (n_poses < 0 || max_iters < 0) return DOCK_EINVAL;
     if (needed) *needed = blob.bytes.size();
@@ -474,7 +474,7 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
     int t_max = 0, wf_max = 0;
     size_t blob_bytes = 0;
     for (int s = 0; s < n_systems; ++s) {
-        if (dock_make_dev_grid(&grids[s], &sys[s].grid) != DOCK_OK) return DOCK_EINVAL;
+        if (dock_make_dev_grid(params, &grids[s], &sys[s].grid) != DOCK_OK) return DOCK_EINVAL;
         if (dock_compile_ligand(params, &grids[s], &ligands[s], blobs[s]) != DOCK_OK) return DOCK_EINVAL;
         blob_bytes += blobs[s].bytes.size();
         t_max = ligands[s].T > t_max ? ligands[s].T : t_max;
@@ -594,7 +594,8 @@ extern "C" int dock_system_host(const dock_params *params, const dock_protein *p
     for (int t = 0; t < DOCK_MAX_XS_TYPES; ++t) desc.type_to_map[t] = -1;
     for (int m = 0; m < n_lig_types; ++m)
         if (lig_types[m] >= 0 && lig_types[m] < DOCK_MAX_XS_TYPES) desc.type_to_map[lig_types[m]] = m;
-    desc.data_dev = grid_dev ? grid_dev : (const float *)16;
+    desc.data_dev = grid_dev ? grid_dev : (const float *)256;
+    desc.packed_dev = desc.data_dev;
     float dummy;
     rc = dock_search(params, 1, &desc, ligand, box, copies, steps, bfgs_max_iters, seed, nullptr, &dummy, &dummy,
                      nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, &need_search, nullptr);

@@ -97,6 +97,7 @@ def _fake_grid(s, lig_types):
     for m, t in enumerate(lig_types):
         g.type_to_map[t] = m
     g.data_dev = 256  # never dereferenced by the size query
+    g.packed_dev = 512
     return g
 
 
