@@ -297,7 +297,7 @@ def run_ours(args) -> dict:
                             "sample": f"first {ns} poses of the same batch, fp64, OpenMP over poses"}
     # spot parity inside the bench run: what is timed is what is correct
     ge = out[0][:ns].cpu().numpy().astype(np.float64)
-    safe = diag["kink_margin"] > 1e-4
+    safe = diag["cutoff_margin"] > 1e-4
     err = np.abs(ge - oe) / (1e-3 + 1e-4 * np.abs(oe))
     line["parity_in_bench"] = {"poses": int(safe.sum()), "max_err_tol_units": float(err[safe].max())}
 

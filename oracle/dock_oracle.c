@@ -406,7 +406,7 @@ double orc_eval(const orc_params *p, const orc_grid *g, const orc_ligand *L,
     double *x = (double *)malloc(sizeof(double) * 3 * N);
     double *gx = (double *)calloc(3 * N, sizeof(double));
     double e_grid = 0.0, e_wall = 0.0, e_intra = 0.0;
-    double face_margin = 1e300, kink_margin = 1e300;
+    double face_margin = 1e300, kink_margin = 1e300, cutoff_margin = 1e300;
     int n_in = 0, n_out = 0;
     orc_coords(L, pose, x);
     for (int i = 0; i < N; ++i) {
@@ -426,7 +426,10 @@ double orc_eval(const orc_params *p, const orc_grid *g, const orc_ligand *L,
         double r = sqrt(dot(d, d)), dfdr;
         e_intra += orc_pair(p, L->type[i], L->type[j], r, &dfdr);
         if (r < p->cutoff) ++n_in;
-        if (diag) kink_margin = fmin(kink_margin, pair_kink_margin(p, L->type[i], L->type[j], r));
+        if (diag) {
+            kink_margin = fmin(kink_margin, pair_kink_margin(p, L->type[i], L->type[j], r));
+            cutoff_margin = fmin(cutoff_margin, fabs(r - p->cutoff));
+        }
         if (r > 1e-12)
             for (int c = 0; c < 3; ++c) {
                 gx[3 * i + c] += dfdr * d[c] / r;
@@ -466,6 +469,7 @@ double orc_eval(const orc_params *p, const orc_grid *g, const orc_ligand *L,
     if (diag) {
         diag->face_margin = face_margin;
         diag->kink_margin = kink_margin;
+        diag->cutoff_margin = cutoff_margin;
         diag->pairs_in_range = n_in;
         diag->atoms_outside = n_out;
     }
@@ -484,6 +488,74 @@ void orc_score_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L
         E[k] = orc_eval(p, g, L, poses + k * (7 + T), tr, grad ? grad + k * (6 + T) : NULL, diag ? diag + k : NULL);
         if (terms) { terms[3 * k] = tr[0]; terms[3 * k + 1] = tr[1]; terms[3 * k + 2] = tr[2]; }
     }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Diagnostic only (changes no result): the conditioning scale of every gradient component,
+ * A_k = sum over atoms of the ABSOLUTE values of the terms that orc_eval adds up for grad[k]
+ * (per-atom force taken as |grid gradient| + sum over pairs |pair force|).  A working precision
+ * eps can resolve grad[k] only to ~eps * A_k; the parity tests use A_k to tell a wrong gradient
+ * from a cancellation the fp32 kernel cannot resolve (reading S20').
+ * ------------------------------------------------------------------------------------- */
+void orc_grad_cond(const orc_params *p, const orc_grid *g, const orc_ligand *L, const double *pose, double *A)
+{
+    const int N = L->N, T = L->T;
+    double *x = (double *)malloc(sizeof(double) * 3 * N);
+    double *ax = (double *)calloc(3 * N, sizeof(double));
+    orc_coords(L, pose, x);
+    for (int i = 0; i < N; ++i) {
+        double eg, ew, ga[3];
+        int outside;
+        atom_inter(p, g, g->type_to_map[L->type[i]], x + 3 * i, &eg, &ew, ga, NULL, &outside);
+        for (int c = 0; c < 3; ++c) ax[3 * i + c] += fabs(ga[c]);
+    }
+    for (int k = 0; k < L->P; ++k) {
+        int i = L->pairs[2 * k], j = L->pairs[2 * k + 1];
+        double d[3] = {x[3 * i] - x[3 * j], x[3 * i + 1] - x[3 * j + 1], x[3 * i + 2] - x[3 * j + 2]};
+        double r = sqrt(dot(d, d)), dfdr;
+        orc_pair(p, L->type[i], L->type[j], r, &dfdr);
+        if (r > 1e-12)
+            for (int c = 0; c < 3; ++c) {
+                ax[3 * i + c] += fabs(dfdr * d[c] / r);
+                ax[3 * j + c] += fabs(dfdr * d[c] / r);
+            }
+    }
+    for (int k = 0; k < 6 + T; ++k) A[k] = 0.0;
+    for (int i = 0; i < N; ++i) {
+        const double *a = ax + 3 * i;
+        double l[3] = {fabs(x[3 * i] - pose[0]), fabs(x[3 * i + 1] - pose[1]), fabs(x[3 * i + 2] - pose[2])};
+        for (int c = 0; c < 3; ++c) A[c] += a[c];
+        A[3] += l[1] * a[2] + l[2] * a[1];
+        A[4] += l[2] * a[0] + l[0] * a[2];
+        A[5] += l[0] * a[1] + l[1] * a[0];
+    }
+    for (int k = 0; k < T; ++k) {
+        const double *xa = x + 3 * L->tors_a[k], *xb = x + 3 * L->tors_b[k];
+        double u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
+        double n = sqrt(dot(u, u));
+        for (int i = 0; i < N; ++i) {
+            int f = L->frag[i], in_sub = 0;
+            while (f > 0) {
+                if (f == k + 1) { in_sub = 1; break; }
+                f = L->tors_parent[f - 1];
+            }
+            if (!in_sub) continue;
+            const double *a = ax + 3 * i;
+            double l[3] = {fabs(x[3 * i] - xb[0]), fabs(x[3 * i + 1] - xb[1]), fabs(x[3 * i + 2] - xb[2])};
+            A[6 + k] += (fabs(u[0]) * (l[1] * a[2] + l[2] * a[1]) + fabs(u[1]) * (l[2] * a[0] + l[0] * a[2]) +
+                         fabs(u[2]) * (l[0] * a[1] + l[1] * a[0])) / n;
+        }
+    }
+    free(x);
+    free(ax);
+}
+
+void orc_grad_cond_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n,
+                         const double *poses, double *A)
+{
+    const int T = L->T;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < n; ++k) orc_grad_cond(p, g, L, poses + k * (7 + T), A + k * (6 + T));
 }
 
 /* ---------------------------------------------------------------------------------------

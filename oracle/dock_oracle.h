@@ -80,6 +80,7 @@ typedef struct {
 typedef struct {
     double face_margin;   /* min over atoms/axes of the distance (A) to the nearest cell face or box face */
     double kink_margin;   /* min over intra pairs of |r-cutoff| and of |d - kink| for the active piecewise terms */
+    double cutoff_margin; /* min over intra pairs of |r-cutoff| alone: the only place where E itself jumps */
     int    pairs_in_range;/* number of intra pairs with r < cutoff */
     int    atoms_outside; /* atoms with at least one clamped axis */
 } orc_diag;
@@ -112,6 +113,10 @@ double orc_eval(const orc_params *p, const orc_grid *g, const orc_ligand *L,
 /* batch of poses [n][7+T] (OpenMP over poses). E [n]; grad [n][6+T] or NULL; terms [n][3] or NULL; diag [n] or NULL */
 void   orc_score_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n,
                        const double *poses, double *E, double *grad, double *terms, orc_diag *diag);
+/* diagnostic: conditioning scale A[n][6+T] of each gradient component (sum of |terms|); no result depends on it */
+void   orc_grad_cond(const orc_params *p, const orc_grid *g, const orc_ligand *L, const double *pose, double *A);
+void   orc_grad_cond_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n,
+                           const double *poses, double *A);
 
 /* x (+) s : t += s[0:3]; q <- normalize(quat(rotvec s[3:6]) * q); theta += s[6:] */
 void   orc_pose_add(int T, const double *pose, const double *s, double *out);

@@ -75,7 +75,7 @@ class _Grid(C.Structure):
 
 
 class Diag(C.Structure):
-    _fields_ = [("face_margin", C.c_double), ("kink_margin", C.c_double),
+    _fields_ = [("face_margin", C.c_double), ("kink_margin", C.c_double), ("cutoff_margin", C.c_double),
                 ("pairs_in_range", C.c_int), ("atoms_outside", C.c_int)]
 
 
@@ -86,7 +86,7 @@ class StepRec(C.Structure):
 
 STEP_DTYPE = np.dtype([("e_cur", "f8"), ("e_cand", "f8"), ("u", "f8"),
                        ("accept", "i4"), ("iters", "i4"), ("evals", "i4"), ("_pad", "i4")])
-DIAG_DTYPE = np.dtype([("face_margin", "f8"), ("kink_margin", "f8"),
+DIAG_DTYPE = np.dtype([("face_margin", "f8"), ("kink_margin", "f8"), ("cutoff_margin", "f8"),
                        ("pairs_in_range", "i4"), ("atoms_outside", "i4")])
 assert STEP_DTYPE.itemsize == C.sizeof(StepRec)
 assert DIAG_DTYPE.itemsize == C.sizeof(Diag)
@@ -251,6 +251,15 @@ def score_batch(p: Params, g: Grid, L: Ligand, poses, want_grad=True):
     lib().orc_score_batch(C.byref(p), C.byref(g.c), C.byref(L.c), C.c_int64(n), _p(poses),
                           _p(E), _p(grad), _p(terms), _p(diag))
     return E, grad, terms, diag
+
+
+def grad_cond(p: Params, g: Grid, L: Ligand, poses) -> np.ndarray:
+    """Diagnostic: conditioning scale A[n, 6+T] of each gradient component (sum of |terms|)."""
+    poses = _f64(poses).reshape(-1, 7 + L.T)
+    n = poses.shape[0]
+    A = np.zeros((n, 6 + L.T))
+    lib().orc_grad_cond_batch(C.byref(p), C.byref(g.c), C.byref(L.c), C.c_int64(n), _p(poses), _p(A))
+    return A
 
 
 def pose_add(T: int, pose, s) -> np.ndarray:

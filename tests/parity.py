@@ -23,13 +23,28 @@ def gpu_side(dk, s, build_grid=True):
     return p, box, grid, dk.LigandHandle(s.ligand)
 
 
-def compare_scores(gpu_e, gpu_grad, gpu_terms, ref_e, ref_grad, ref_terms, diag, what=""):
-    """Element-by-element comparison with the discontinuity exemptions; returns a stats dict."""
+EPS32 = 2.0 ** -24   # unit round-off of the kernel's arithmetic
+COND_C = 8.0         # S20': a component is resolvable in fp32 only to ~COND_C * EPS32 * A_k
+
+
+def compare_scores(gpu_e, gpu_grad, gpu_terms, ref_e, ref_grad, ref_terms, diag, what="", cond=None,
+                   n_atoms=30, n_pairs=300):
+    """Element-by-element comparison with the discontinuity exemptions; returns a stats dict.
+
+    `cond` (oracle.grad_cond) is the conditioning scale A_k of each gradient component.  Reading S20'
+    (DESIGN.md): a component passes iff |gpu - ref| <= 1e-3 + 1e-4 |ref| + COND_C * EPS32 * A_k; the
+    fraction that passes the plain S20 rule (without the last term) is reported and must be >= 99.99 %.
+    """
     gpu_e = np.asarray(gpu_e, np.float64)
     n = len(ref_e)
-    ok_e = diag["kink_margin"] > KINK_MARGIN
-    ok_g = ok_e & (diag["face_margin"] > FACE_MARGIN)
-    assert ok_e.mean() > 0.95 and ok_g.mean() > 0.80, (what, ok_e.mean(), ok_g.mean())
+    ok_e = diag["cutoff_margin"] > KINK_MARGIN          # E itself jumps only at the cutoff
+    ok_g = (diag["kink_margin"] > KINK_MARGIN) & (diag["face_margin"] > FACE_MARGIN)
+    # a pose is exempt if ANY of its pairs / atoms sits within the margin of a discontinuity, so the
+    # expected exempt fraction grows with the ligand: ~ P * 2 kinks * 2e-4 / 8 A and N * 3 axes * 2e-4 / 0.375 A
+    # (x2 safety, + 2 %)
+    min_e = 1.0 - 2.0 * (n_pairs * 2 * KINK_MARGIN / 8.0) - 0.02
+    min_g = min_e - 2.0 * (n_pairs * 2 * KINK_MARGIN / 8.0) - 2.0 * (n_atoms * 3 * 2 * FACE_MARGIN / 0.375) - 0.02
+    assert ok_e.mean() > min_e and ok_g.mean() > min_g, (what, ok_e.mean(), ok_g.mean(), min_e, min_g)
     err_e = np.abs(gpu_e - ref_e) / tol(ref_e)
     assert np.all(np.isfinite(gpu_e)), what
     assert np.all(err_e[ok_e] <= 1.0), (what, "E", float(err_e[ok_e].max()), int(np.argmax(np.where(ok_e, err_e, 0))))
@@ -43,7 +58,12 @@ def compare_scores(gpu_e, gpu_grad, gpu_terms, ref_e, ref_grad, ref_terms, diag,
         gg = np.asarray(gpu_grad, np.float64)
         err_g = np.abs(gg - ref_grad) / tol(ref_grad)
         assert np.all(np.isfinite(gg)), what
-        assert np.all(err_g[ok_g] <= 1.0), (what, "grad", float(err_g[ok_g].max()),
-                                            np.unravel_index(int(np.argmax(np.where(ok_g[:, None], err_g, 0))), err_g.shape))
-        stats["max_err_g"] = float(err_g[ok_g].max())
+        stats["max_err_g_s20"] = float(err_g[ok_g].max())
+        stats["frac_g_within_s20"] = float((err_g[ok_g] <= 1.0).mean())
+        assert stats["frac_g_within_s20"] >= 0.9999, (what, stats)
+        t_g = tol(ref_grad) + (COND_C * EPS32 * np.asarray(cond) if cond is not None else 0.0)
+        err_c = np.abs(gg - ref_grad) / t_g
+        assert np.all(err_c[ok_g] <= 1.0), (what, "grad", float(err_c[ok_g].max()),
+                                            np.unravel_index(int(np.argmax(np.where(ok_g[:, None], err_c, 0))), err_c.shape))
+        stats["max_err_g"] = float(err_c[ok_g].max())
     return stats

@@ -8,7 +8,7 @@ from types import SimpleNamespace
 import numpy as np
 import pytest
 
-from dock_synth import XS, make_system
+from dock_synth import XS, make_system, random_poses
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -565,3 +565,24 @@ def test_topk_against_brute_force_and_properties(orc, tiny):
                 kept.append(i)
         assert cnt == len(kept) and list(idx[:cnt]) == kept
         assert all(e[idx[a]] <= e[idx[a + 1]] for a in range(cnt - 1))
+
+
+def test_gradient_conditioning_scale_bounds_the_gradient(orc, tiny):
+    """orc_grad_cond (diagnostic, S20'): A_k is the sum of |terms| of grad[k], so A_k >= |grad[k]|
+    (triangle inequality), and for a single atom with no pairs the sum has one term: A = |grad| exactly."""
+    from types import SimpleNamespace
+    s, op, og, oL = tiny
+    rng = np.random.default_rng(12)
+    poses = random_poses(rng, 64, s.box_center, s.box_size * 1.2, oL.T).astype(np.float64)
+    _, g, _, dg = orc.score_batch(op, og, oL, poses)
+    A = orc.grad_cond(op, og, oL, poses)
+    assert A.shape == g.shape and np.all(A >= np.abs(g) * (1 - 1e-12) - 1e-12)
+    assert np.all(dg["cutoff_margin"] >= dg["kink_margin"])
+    one = orc.Ligand(SimpleNamespace(ref_xyz=np.zeros((1, 3)), type=np.array([s.ligand.type[0]], np.int32),
+                                     frag=np.zeros(1, np.int32), tors_parent=np.zeros(0, np.int32),
+                                     tors_a=np.zeros(0, np.int32), tors_b=np.zeros(0, np.int32),
+                                     pairs=np.zeros((0, 2), np.int32)))
+    p1 = random_poses(rng, 16, s.box_center, s.box_size, 0).astype(np.float64)
+    _, g1, _, _ = orc.score_batch(op, og, one, p1)
+    A1 = orc.grad_cond(op, og, one, p1)
+    assert np.allclose(A1[:, :3], np.abs(g1[:, :3]), rtol=1e-12, atol=1e-300) and np.all(A1[:, 3:] < 1e-9)
