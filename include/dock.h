@@ -94,7 +94,7 @@ typedef struct dock_ligand {
     const int32_t *tors_parent;    /* [T] */
     const int32_t *tors_a;         /* [T] */
     const int32_t *tors_b;         /* [T] */
-    const int32_t *pairs;          /* [P][2] intra-ligand scoring pairs, i != j */
+    const int32_t *pairs;          /* [P][2] intra-ligand scoring pairs, i != j, each unordered pair at most once */
 } dock_ligand;
 
 /* Grid-map descriptor written by dock_build_grids.  Two DEVICE images of the same maps live in the

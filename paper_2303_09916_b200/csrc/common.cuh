@@ -39,6 +39,12 @@ struct DevParams {
     float amp_trans, amp_rot;
     float c1, shrink, gtol, curv_eps;
     int   max_trials;
+    // pair term with the weights folded into the exponent arguments (eval_thread.cuh):
+    //   |w1| exp(-(d/0.5)^2) = ex2(cA d^2 + lw1),  |w2| exp(-((d-3)/2)^2) = ex2(cB (d-3)^2 + lw2)
+    float lw1, lw2;            // log2|w1|, log2|w2|  (-inf for a zero weight)
+    float s1, s2;              // sign(w1), sign(w2)
+    float k1, k2;              // -8 s1, -0.5 s2: d/dd of the two Gaussians = k * (d or d-3) * value
+    float w3x2;                // 2 w3
 };
 
 // Grid maps as the evaluators see them.  Positions are handled relative to a reference node of the
@@ -86,22 +92,32 @@ struct DevSystem {
 // ---- thread-per-pose evaluator (batch scoring): ligand tables in the kernel-parameter constant
 // bank, so that every table read is a uniform constant load and costs no L1 wavefront ------------
 #define TPP_TILE 4                      // atoms of the i-tile held in registers in the pair phase
-#define TPP_REC_WORDS (1 + TPP_TILE)    // word0 + one R_i+R_j per tile atom
-#define TPP_SCHED_WORDS 6400            // capacity of the in-parameter schedule (25.6 KB)
+#define TPP_SCHED_QUADS 1600            // capacity of the in-parameter schedule (25.6 KB of 16-byte quads)
+
+// Pair schedule = a stream of 16-byte quads (one uniform 128-bit constant load each):
+//   group   : header {i-slots (4 bytes, byte t = slot of tile atom t), n2_plain | n1_plain << 16,
+//                      n2_special | n1_special << 16, 0}
+//             then n2_plain double records, n1_plain (0/1) single records,
+//             then n2_special double records, n1_special (0/1) single records.
+//   record  : one partner slot j against the 4 tile atoms.  A pair that is not listed gets
+//             R_i+R_j = TPP_MASKED_RSUM: its surface distance is then +1e18 and every term and
+//             derivative evaluates to exactly 0 -- no mask test in the instruction stream.
+//     single plain   : {j, 0, 0, 0} {rsum[4]}
+//     double plain   : {jA, jB, 0, 0} {rsumA[4]} {rsumB[4]}
+//     single special : {j, 0, 0, 0} {rsum[4]} {wh[4]} {whb[4]}         (wh = w4 or 0, whb = w5 or 0 per pair)
+//     double special : {jA, jB, 0, 0} {rsumA[4]} {whA[4]} {whbA[4]} {rsumB[4]} {whB[4]} {whbB[4]}
+//   j is stored as the byte offset of the slot's z column (j * 128); the (x,y) column is at twice that.
+#define TPP_MASKED_RSUM (-1.0e18f)
 
 struct TppLigand {
     int N, T, n_groups, sched_in_param;
     float4 atom_ref[DOCK_MAX_ATOMS];        // slot order (sorted by fragment): xyz rel. pivot, w = bitcast(map offset in entries)
     float4 tors_axis[DOCK_MAX_TORSIONS];    // reference-frame unit axis; w = bitcast(parent fragment)
     float4 tors_pt[DOCK_MAX_TORSIONS];      // reference position of atom b rel. pivot; w = 1 / |ref_b - ref_a|
-    unsigned char  atom_frag[DOCK_MAX_ATOMS];
     unsigned char  tors_a[DOCK_MAX_TORSIONS], tors_b[DOCK_MAX_TORSIONS];   // slots of the axis atoms
     unsigned char  frag_end[DOCK_MAX_TORSIONS + 4];                        // one past the last slot of fragment f
-    // Pair schedule: groups of <= TPP_TILE i-slots; per group a header
-    //   {i-slots (4 bytes), number of records}, then records of TPP_REC_WORDS words:
-    //   word0 = j | mask << 8 | hyd << 12 | hb << 16  (bit t of each field = tile atom t),  then R_i+R_j for t = 0..3.
-    const uint32_t *sched_global;           // the same stream in global memory (used when it does not fit below)
-    uint32_t sched[TPP_SCHED_WORDS];
+    const uint4 *sched_global;              // the same stream in global memory (used when it does not fit below)
+    uint4 sched[TPP_SCHED_QUADS];
 };
 
 // ---- device helpers ---------------------------------------------------------------------------

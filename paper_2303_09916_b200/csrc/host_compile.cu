@@ -77,6 +77,13 @@ int dock_make_dev_params(const dock_params *p, DevParams *o)
     o->gtol = p->bfgs_gtol;
     o->curv_eps = p->bfgs_curv_eps;
     o->max_trials = p->bfgs_max_trials;
+    o->lw1 = p->w[0] != 0.f ? (float)std::log2(std::fabs((double)p->w[0])) : -INFINITY;
+    o->lw2 = p->w[1] != 0.f ? (float)std::log2(std::fabs((double)p->w[1])) : -INFINITY;
+    o->s1 = p->w[0] < 0.f ? -1.f : 1.f;
+    o->s2 = p->w[1] < 0.f ? -1.f : 1.f;
+    o->k1 = -8.f * o->s1;
+    o->k2 = -0.5f * o->s2;
+    o->w3x2 = 2.f * p->w[2];
     return DOCK_OK;
 }
 
@@ -192,9 +199,15 @@ int dock_compile_ligand(const dock_params *p, const dock_grid *g, const dock_lig
         if (L->atom_fragment[a] != L->tors_parent[k]) return DOCK_EINVAL;            // axis atom in the wrong fragment
         if (L->atom_fragment[b] != k + 1) return DOCK_EINVAL;
     }
-    for (int k = 0; k < P; ++k) {
-        const int i = L->pairs[2 * k], j = L->pairs[2 * k + 1];
-        if (i < 0 || i >= N || j < 0 || j >= N || i == j) return DOCK_EINVAL;
+    {
+        std::vector<unsigned char> seen((size_t)N * N, 0);
+        for (int k = 0; k < P; ++k) {
+            const int i = L->pairs[2 * k], j = L->pairs[2 * k + 1];
+            if (i < 0 || i >= N || j < 0 || j >= N || i == j) return DOCK_EINVAL;
+            const size_t key = (size_t)std::min(i, j) * N + std::max(i, j);
+            if (seen[key]) return DOCK_EINVAL;                                       // a pair may be listed once
+            seen[key] = 1;
+        }
     }
     // pivot = centroid of the root-fragment reference atoms (reading S11), in double
     double c[3] = {0, 0, 0};
@@ -268,7 +281,7 @@ DevLigand dock_relocate_ligand(const LigandBlob &b, const unsigned char *base)
 
 // ---- thread-per-pose tables ------------------------------------------------------------------------
 int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand *L, TppLigand &out,
-                     std::vector<uint32_t> &overflow)
+                     std::vector<uint4> &overflow)
 {
     LigandBlob chk;                                   // reuse the validation of the warp-per-pose compiler
     if (!g || dock_compile_ligand(p, g, L, chk) != DOCK_OK) return DOCK_EINVAL;
@@ -302,7 +315,6 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
         out.atom_ref[s] = make_float4((float)((double)L->ref_xyz[3 * i] - c[0]), (float)((double)L->ref_xyz[3 * i + 1] - c[1]),
                                       (float)((double)L->ref_xyz[3 * i + 2] - c[2]), 0.f);
         std::memcpy(&out.atom_ref[s].w, &ioff, 4);
-        out.atom_frag[s] = (unsigned char)L->atom_fragment[i];
         while (f_cur < L->atom_fragment[i]) out.frag_end[f_cur++] = (unsigned char)s;
     }
     while (f_cur <= T) out.frag_end[f_cur++] = (unsigned char)N;
@@ -322,9 +334,9 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
 
     // pair schedule: tiles of TPP_TILE consecutive slots.  The pairs between two tiles A < B form a
     // small bit matrix; they all go either to A's group (one record per partner j in B) or to B's
-    // group (one record per partner j in A), whichever needs fewer records.
+    // group (one record per partner j in A), whichever needs fewer records.  Format: common.cuh.
     const int n_tiles = (N + TPP_TILE - 1) / TPP_TILE;
-    struct Rec { int j; uint32_t mask, hyd, hb; float rsum[TPP_TILE]; };
+    struct Rec { int j; bool special; float rsum[TPP_TILE], wh[TPP_TILE], whb[TPP_TILE]; };
     std::vector<std::vector<Rec>> groups(n_tiles);
     std::vector<std::vector<std::pair<int, int>>> between((size_t)n_tiles * n_tiles);   // (slot in A, slot in B)
     for (int k = 0; k < P; ++k) {
@@ -336,13 +348,19 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
         std::vector<Rec> &grp = groups[tile];
         Rec *r = nullptr;
         for (Rec &q : grp) if (q.j == j_slot) { r = &q; break; }
-        if (!r) { grp.push_back(Rec{j_slot, 0u, 0u, 0u, {0.f, 0.f, 0.f, 0.f}}); r = &grp.back(); }
+        if (!r) {
+            Rec fresh;
+            fresh.j = j_slot;
+            fresh.special = false;
+            for (int t = 0; t < TPP_TILE; ++t) { fresh.rsum[t] = TPP_MASKED_RSUM; fresh.wh[t] = 0.f; fresh.whb[t] = 0.f; }
+            grp.push_back(fresh);
+            r = &grp.back();
+        }
         const int t = i_slot - tile * TPP_TILE;
         const int ti = L->type[atom_of[i_slot]], tj = L->type[atom_of[j_slot]];
-        r->mask |= 1u << t;
-        if (p->hydrophobic[ti] && p->hydrophobic[tj]) r->hyd |= 1u << t;
-        if ((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) r->hb |= 1u << t;
         r->rsum[t] = p->radius[ti] + p->radius[tj];
+        if (p->hydrophobic[ti] && p->hydrophobic[tj]) { r->wh[t] = p->w[3]; r->special = true; }
+        if ((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) { r->whb[t] = p->w[4]; r->special = true; }
     };
     for (int A = 0; A < n_tiles; ++A)
         for (int B = A; B < n_tiles; ++B) {
@@ -356,35 +374,51 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
                 else add(B, e.second, e.first);
             }
         }
-    std::vector<uint32_t> words;
+    std::vector<uint4> quads;
+    auto fq = [](const float *v) {
+        uint4 q;
+        std::memcpy(&q, v, 16);
+        return q;
+    };
     int n_groups = 0;
     for (int A = 0; A < n_tiles; ++A) {
         std::vector<Rec> &grp = groups[A];
         if (grp.empty()) continue;
         std::stable_sort(grp.begin(), grp.end(), [](const Rec &a, const Rec &b) { return a.j < b.j; });
+        std::vector<const Rec *> cls[2];
+        for (const Rec &r : grp) cls[r.special ? 1 : 0].push_back(&r);
+        if (cls[0].size() > 0x1fffeu || cls[1].size() > 0x1fffeu) return DOCK_EINVAL;
         const int n_i = std::min(TPP_TILE, N - A * TPP_TILE);
-        uint32_t h0 = 0;
-        for (int t = 0; t < TPP_TILE; ++t) h0 |= (uint32_t)(A * TPP_TILE + (t < n_i ? t : 0)) << (8 * t);
-        if (grp.size() > 0xffffu) return DOCK_EINVAL;
-        words.push_back(h0);
-        words.push_back((uint32_t)grp.size() | ((uint32_t)n_i << 16));
-        for (const Rec &r : grp) {
-            words.push_back((uint32_t)r.j | (r.mask << 8) | (r.hyd << 12) | (r.hb << 16));
-            for (int t = 0; t < TPP_TILE; ++t) {
-                uint32_t w;
-                std::memcpy(&w, &r.rsum[t], 4);
-                words.push_back(w);
+        uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
+        for (int t = 0; t < TPP_TILE; ++t) hdr.x |= (uint32_t)(A * TPP_TILE + (t < n_i ? t : 0)) << (8 * t);
+        hdr.y = (uint32_t)(cls[0].size() / 2) | ((uint32_t)(cls[0].size() & 1) << 16);
+        hdr.z = (uint32_t)(cls[1].size() / 2) | ((uint32_t)(cls[1].size() & 1) << 16);
+        quads.push_back(hdr);
+        for (int c = 0; c < 2; ++c) {
+            const std::vector<const Rec *> &v = cls[c];
+            size_t k = 0;
+            for (; k + 1 < v.size(); k += 2) {
+                quads.push_back(make_uint4((uint32_t)v[k]->j * 128u, (uint32_t)v[k + 1]->j * 128u, 0u, 0u));
+                for (int h = 0; h < 2; ++h) {
+                    quads.push_back(fq(v[k + h]->rsum));
+                    if (c) { quads.push_back(fq(v[k + h]->wh)); quads.push_back(fq(v[k + h]->whb)); }
+                }
+            }
+            if (k < v.size()) {
+                quads.push_back(make_uint4((uint32_t)v[k]->j * 128u, 0u, 0u, 0u));
+                quads.push_back(fq(v[k]->rsum));
+                if (c) { quads.push_back(fq(v[k]->wh)); quads.push_back(fq(v[k]->whb)); }
             }
         }
         ++n_groups;
     }
     out.n_groups = n_groups;
-    if (words.size() <= (size_t)TPP_SCHED_WORDS) {
+    if (quads.size() <= (size_t)TPP_SCHED_QUADS) {
         out.sched_in_param = 1;
-        std::memcpy(out.sched, words.data(), words.size() * sizeof(uint32_t));
+        if (!quads.empty()) std::memcpy(out.sched, quads.data(), quads.size() * sizeof(uint4));
     } else {
         out.sched_in_param = 0;
-        overflow.swap(words);
+        overflow.swap(quads);
     }
     return DOCK_OK;
 }

@@ -26,7 +26,7 @@ int dock_make_dev_grid(const dock_params *p, const dock_grid *g, DevGrid *out);
 // fit TppLigand::sched, out.sched_in_param = 0 and `overflow` holds the stream for the caller to
 // upload (then point out.sched_global at it); otherwise `overflow` is empty.
 int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand *lig, TppLigand &out,
-                     std::vector<uint32_t> &overflow);
+                     std::vector<uint4> &overflow);
 
 // number of floats of per-warp shared memory the warp-per-pose evaluator needs for this ligand
 static inline int eval_scratch_floats(int n_pad, int T) { return 6 * n_pad + 2 * ((T + 3) & ~3); }

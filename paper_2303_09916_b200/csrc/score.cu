@@ -30,7 +30,7 @@ struct ScorePlan {
     DevParams P;
     DevGrid G;
     TppLigand L;
-    std::vector<uint32_t> overflow;
+    std::vector<uint4> overflow;
     size_t need;
 };
 
@@ -39,7 +39,7 @@ int plan_score(const dock_params *params, const dock_grid *grid, const dock_liga
     if (dock_make_dev_params(params, &pl.P) != DOCK_OK) return DOCK_EINVAL;
     if (dock_make_dev_grid(params, grid, &pl.G) != DOCK_OK) return DOCK_EINVAL;
     if (dock_compile_tpp(params, grid, lig, pl.L, pl.overflow) != DOCK_OK) return DOCK_EINVAL;
-    pl.need = align_up(pl.overflow.size() * sizeof(uint32_t) + 16, 256);
+    pl.need = align_up(pl.overflow.size() * sizeof(uint4) + 16, 256);
     return DOCK_OK;
 }
 
@@ -65,9 +65,9 @@ int score_launch(ScorePlan &pl, long long n_poses, const float *poses_dev, float
 {
     if (n_poses < 1) return DOCK_OK;
     if (!pl.L.sched_in_param) {
-        DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.overflow.data(), pl.overflow.size() * sizeof(uint32_t),
+        DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.overflow.data(), pl.overflow.size() * sizeof(uint4),
                                         cudaMemcpyHostToDevice, stream));
-        pl.L.sched_global = (const uint32_t *)ws;
+        pl.L.sched_global = (const uint4 *)ws;
         return grad_dev ? launch<true, false>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream)
                         : launch<false, false>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
     }
