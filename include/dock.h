@@ -101,9 +101,10 @@ typedef struct dock_ligand {
  * caller's buffer (dock_grid_bytes() bytes, 256-byte aligned):
  *   data_dev   [n_maps][nz][ny][nx] fp32 -- the maps themselves: node (ix,iy,iz) at
  *              origin + spacing*(ix,iy,iz) holds eq. 2's vertex score;
- *   packed_dev [n_maps][nz][ny][nx][4] fp32 -- the gather layout read by every evaluator: entry
- *              (ix,iy,iz) = {G(ix,iy), G(ix+1,iy), G(ix,iy+1), G(ix+1,iy+1)} at plane iz (indices
- *              clamped to the last node), so the 8 corners of a cell are two 16-byte loads
+ *   packed_dev [n_maps][nz][ny][nx][8] fp32 -- the gather layout read by every evaluator: entry
+ *              (ix,iy,iz) = the 8 corners of the cell whose low corner is that node, in the order
+ *              {G(ix,iy,iz), G(ix+1,iy,iz), G(ix,iy+1,iz), G(ix+1,iy+1,iz)} then the same four at
+ *              iz+1 (indices clamped to the last node), so a cell is ONE aligned 32-byte load
  *              (DESIGN.md "Data layout").  Values are bit-identical copies of data_dev. */
 typedef struct dock_grid {
     int32_t      dims[3];                          /* nx, ny, nz */

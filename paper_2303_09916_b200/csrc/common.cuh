@@ -31,6 +31,15 @@ extern unsigned long long g_dock_launches;
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // ---- device descriptors -----------------------------------------------------------------------
+// One entry of the gather layout: the 8 corners of the cell whose low corner is node (ix,iy,iz).
+//   lo = {G(ix,iy,iz), G(ix+1,iy,iz), G(ix,iy+1,iz), G(ix+1,iy+1,iz)},  hi = the same at iz+1.
+// 32 bytes = one L2 sector = one 256-bit load (LDG.E.ENL2.256 on sm_100a): a fully divergent warp
+// load costs the L1TEX pipe ~1.8 cycles per lane whatever its width, so one 32-byte load per atom
+// halves the gather cost of two 16-byte loads (profiles/r1f.md).
+struct __align__(32) Cell8 {
+    float4 lo, hi;
+};
+
 struct DevParams {
     float w[5];
     float cutoff, cutoff2;
@@ -39,12 +48,17 @@ struct DevParams {
     float amp_trans, amp_rot;
     float c1, shrink, gtol, curv_eps;
     int   max_trials;
-    // pair term with the weights folded into the exponent arguments (eval_thread.cuh):
-    //   |w1| exp(-(d/0.5)^2) = ex2(cA d^2 + lw1),  |w2| exp(-((d-3)/2)^2) = ex2(cB (d-3)^2 + lw2)
-    float lw1, lw2;            // log2|w1|, log2|w2|  (-inf for a zero weight)
-    float s1, s2;              // sign(w1), sign(w2)
-    float k1, k2;              // -8 s1, -0.5 s2: d/dd of the two Gaussians = k * (d or d-3) * value
-    float w3x2;                // 2 w3
+    // pair term of the thread-per-pose evaluator (eval_thread.cuh), weights folded into the exponents:
+    //   A = 8|w1| exp(-(d/0.5)^2) = ex2(cA d^2 + lw1),   B = |w2|/2 exp(-((d-3)/2)^2) = ex2(cB (d-3)^2 + lw2)
+    // with sigma = -sign(w1):  sigma dE/dd = d (A + q B) - 3 q B + c4 min(d,0) + wh' [hyd ramp] + whb' [hb ramp]
+    // and E = eA sum A + eB sum B + (sigma/2) sum c4 min(d,0)^2 - sigma sum wh' H - 0.7 sigma sum whb' B_hb,
+    // where the schedule stores wh' = -sigma w4 and whb' = -sigma w5 / 0.7.  Forces are carried
+    // sigma-scaled and multiplied by sigma (exactly, it is +-1) on output.
+    float lw1, lw2;            // log2(8|w1|), log2(|w2|/2)  (-inf for a zero weight)
+    float sigma;               // -sign(w1)
+    float q, m3q;              // sign(w1) sign(w2), -3 q
+    float c4;                  // sigma 2 w3
+    float eA, eB;              // sign(w1)/8, 2 sign(w2)
 };
 
 // Grid maps as the evaluators see them.  Positions are handled relative to a reference node of the
@@ -59,7 +73,7 @@ struct DevGrid {
     float hi_x, hi_y, hi_z;         // n-1-ic*
     float h, inv_h, inv_h_lo;       // spacing; fl(1/h) and 1/h - fl(1/h)
     float kw_g, kw_e;               // wall: 2 k h (gradient per cell of overshoot), k h^2
-    const float4 *packed;           // [n_maps][nz][ny][nx] gather layout (see dock.h)
+    const Cell8  *packed;           // [n_maps][nz][ny][nx] gather layout: the 8 corners of a cell in one 32-byte entry (see dock.h)
     const float  *data;             // [n_maps][nz][ny][nx]
 };
 
@@ -94,19 +108,22 @@ struct DevSystem {
 #define TPP_TILE 4                      // atoms of the i-tile held in registers in the pair phase
 #define TPP_SCHED_QUADS 1600            // capacity of the in-parameter schedule (25.6 KB of 16-byte quads)
 
-// Pair schedule = a stream of 16-byte quads (one uniform 128-bit constant load each):
-//   group   : header {i-slots (4 bytes, byte t = slot of tile atom t), n2_plain | n1_plain << 16,
-//                      n2_special | n1_special << 16, 0}
-//             then n2_plain double records, n1_plain (0/1) single records,
-//             then n2_special double records, n1_special (0/1) single records.
+// Pair schedule = a stream of 16-byte quads (one uniform 128-bit constant load each).  There is one
+// group per tile of TPP_TILE consecutive slots, in slot order, so every atom belongs to exactly one
+// group (the evaluator also does the atom's grid lookup there):
+//   group   : header {i-slots (4 bytes, byte t = slot of tile atom t; padding repeats slot 0 of the tile),
+//                      n2_plain | n1_plain << 8 | n2_hyd << 16 | n1_hyd << 24,
+//                      n2_hb | n1_hb << 8 | n_live << 16, 0}
+//             then per class (plain, hyd, hb) n2 double records and n1 (0/1) single records.
 //   record  : one partner slot j against the 4 tile atoms.  A pair that is not listed gets
 //             R_i+R_j = TPP_MASKED_RSUM: its surface distance is then +1e18 and every term and
 //             derivative evaluates to exactly 0 -- no mask test in the instruction stream.
-//     single plain   : {j, 0, 0, 0} {rsum[4]}
-//     double plain   : {jA, jB, 0, 0} {rsumA[4]} {rsumB[4]}
-//     single special : {j, 0, 0, 0} {rsum[4]} {wh[4]} {whb[4]}         (wh = w4 or 0, whb = w5 or 0 per pair)
-//     double special : {jA, jB, 0, 0} {rsumA[4]} {whA[4]} {whbA[4]} {rsumB[4]} {whB[4]} {whbB[4]}
+//             class plain: no pair of the record has a hydrophobic or H-bond term; hyd: some pair has
+//             the hydrophobic term, none the H-bond term; hb: some pair has the H-bond term.
+//     single : {j, 0, 0, 0} {rsum[4]} [{wh'[4]}  (hyd, hb)] [{whb'[4]}  (hb)]
+//     double : {jA, jB, 0, 0} then the single-record payload of A, then that of B
 //   j is stored as the byte offset of the slot's z column (j * 128); the (x,y) column is at twice that.
+//   wh' = -sigma w4 or 0, whb' = -sigma w5 / 0.7 or 0 per pair (see DevParams).
 #define TPP_MASKED_RSUM (-1.0e18f)
 
 struct TppLigand {
@@ -132,6 +149,15 @@ __device__ __forceinline__ double warp_sum_d(double v)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
     return v;
+}
+__device__ __forceinline__ void ldg_cell(const Cell8 *p, float4 &lo, float4 &hi)
+{
+    unsigned long long a, b, c, d;
+    asm("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p));
+    lo.x = __uint_as_float((unsigned)a); lo.y = __uint_as_float((unsigned)(a >> 32));
+    lo.z = __uint_as_float((unsigned)b); lo.w = __uint_as_float((unsigned)(b >> 32));
+    hi.x = __uint_as_float((unsigned)c); hi.y = __uint_as_float((unsigned)(c >> 32));
+    hi.z = __uint_as_float((unsigned)d); hi.w = __uint_as_float((unsigned)(d >> 32));
 }
 __device__ __forceinline__ float fast_ex2(float x)
 {

@@ -5,7 +5,7 @@
 //   A2 kinematics : every lane owns atoms i = lane, lane+32, ... and walks the torsions on the path
 //                   from the atom's fragment to the root (deepest first), one Rodrigues rotation
 //                   about the reference-frame axis each, then x = t + R(q) y (box-relative).
-//   A3 inter term : two 16-byte gathers from the packed map of the atom's type, trilinear energy
+//   A3 inter term : one 32-byte gather (the cell's 8 corners) from the packed map of the atom's type, trilinear energy
 //                   (eq. 2, 198-207) and the partial derivatives of the interpolant (eq. 3,
 //                   213-219); clamp + quadratic wall outside the box.
 //   A4 intra term : host-built conflict-free schedule, 32 pairs per round; forces go to the per-warp
@@ -90,8 +90,8 @@ __device__ __noinline__ float eval_pose_warp(const DevParams &P, const DevGrid &
         atom_coords(L, R, tx, ty, tz, sn, cs, i, x0, x1, x2, map_off);
         xs[i] = x0; xs[np + i] = x1; xs[2 * np + i] = x2;
         const CellRef cr = locate_cell(G, x0, x1, x2);
-        const float4 *e0 = G.packed + (size_t)map_off + cr.idx;
-        const float4 q0 = __ldg(e0), q1 = __ldg(e0 + G.nx * G.ny);
+        float4 q0, q1;
+        ldg_cell(G.packed + (size_t)map_off + cr.idx, q0, q1);
         e_grid += trilinear(G, cr, q0, q1, e_wall, gx, gy, gz);
         if (WANT_GRAD) { gs[i] = gx; gs[np + i] = gy; gs[2 * np + i] = gz; }
     }

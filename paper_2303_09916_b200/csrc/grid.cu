@@ -108,21 +108,26 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
         if (m < nm) A.out[(size_t)(m0 + m) * nodes + node] = acc[m];
 }
 
-// Gather layout: entry (ix,iy,iz) of map m = {G(ix,iy), G(ix+1,iy), G(ix,iy+1), G(ix+1,iy+1)} at plane iz
-// (indices clamped to the last node).  Pure data movement: values are bit-identical copies.
-__global__ void __launch_bounds__(256) grid_pack_kernel(const float *__restrict__ plain, float4 *__restrict__ packed,
-                                                        int nx, int ny, long long rows)
+// Gather layout (Cell8, common.cuh): entry (ix,iy,iz) of map m = the 8 corners of the cell whose low corner is that
+// node (indices clamped to the last node).  Pure data movement: values are bit-identical copies.
+__global__ void __launch_bounds__(256) grid_pack_kernel(const float *__restrict__ plain, Cell8 *__restrict__ packed,
+                                                        int nx, int ny, int nz, long long rows)
 {
-    // one thread per (map, iz, iy) row segment element; consecutive threads walk x -> coalesced
+    // one thread per entry; consecutive threads walk x -> coalesced reads, 32-byte stores
     const long long total = rows * nx;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
         const int ix = (int)(e % nx);
         const long long row = e / nx;                 // (m * nz + iz) * ny + iy
         const int iy = (int)(row % ny);
+        const int iz = (int)((row / ny) % nz);
         const long long up = (iy + 1 < ny) ? nx : 0;
+        const long long fw = (iz + 1 < nz) ? (long long)nx * ny : 0;
         const int rt = (ix + 1 < nx) ? 1 : 0;
         const float *q = plain + e;
-        packed[e] = make_float4(__ldg(q), __ldg(q + rt), __ldg(q + up), __ldg(q + up + rt));
+        Cell8 c;
+        c.lo = make_float4(__ldg(q), __ldg(q + rt), __ldg(q + up), __ldg(q + up + rt));
+        c.hi = make_float4(__ldg(q + fw), __ldg(q + fw + rt), __ldg(q + fw + up), __ldg(q + fw + up + rt));
+        packed[e] = c;
     }
 }
 
@@ -215,7 +220,7 @@ extern "C" size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types)
     int32_t dims[3];
     if (n_lig_types < 1 || n_lig_types > DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
     const size_t nodes = (size_t)dims[0] * dims[1] * dims[2] * (size_t)n_lig_types;
-    return align_up(nodes * sizeof(float), 256) + nodes * sizeof(float4);
+    return align_up(nodes * sizeof(float), 256) + nodes * sizeof(Cell8);
 }
 
 extern "C" int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
@@ -260,10 +265,10 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     grid_build_kernel<<<grid, 128, 0, stream>>>(A);
     DOCK_LAUNCH_CHECK();
     const size_t nodes = (size_t)A.nx * A.ny * A.nz * (size_t)n_lig_types;
-    float4 *packed = reinterpret_cast<float4 *>(reinterpret_cast<unsigned char *>(grid_dev) + align_up(nodes * sizeof(float), 256));
+    Cell8 *packed = reinterpret_cast<Cell8 *>(reinterpret_cast<unsigned char *>(grid_dev) + align_up(nodes * sizeof(float), 256));
     const long long rows = (long long)n_lig_types * A.nz * A.ny;
     const unsigned pack_blocks = (unsigned)std::min<long long>((rows * A.nx + 255) / 256, 148LL * 16);
-    grid_pack_kernel<<<pack_blocks, 256, 0, stream>>>(grid_dev, packed, A.nx, A.ny, rows);
+    grid_pack_kernel<<<pack_blocks, 256, 0, stream>>>(grid_dev, packed, A.nx, A.ny, A.nz, rows);
     DOCK_LAUNCH_CHECK();
 
     std::memset(out_desc, 0, sizeof(*out_desc));

@@ -77,13 +77,15 @@ int dock_make_dev_params(const dock_params *p, DevParams *o)
     o->gtol = p->bfgs_gtol;
     o->curv_eps = p->bfgs_curv_eps;
     o->max_trials = p->bfgs_max_trials;
-    o->lw1 = p->w[0] != 0.f ? (float)std::log2(std::fabs((double)p->w[0])) : -INFINITY;
-    o->lw2 = p->w[1] != 0.f ? (float)std::log2(std::fabs((double)p->w[1])) : -INFINITY;
-    o->s1 = p->w[0] < 0.f ? -1.f : 1.f;
-    o->s2 = p->w[1] < 0.f ? -1.f : 1.f;
-    o->k1 = -8.f * o->s1;
-    o->k2 = -0.5f * o->s2;
-    o->w3x2 = 2.f * p->w[2];
+    const double s1 = p->w[0] < 0.f ? -1.0 : 1.0, s2 = p->w[1] < 0.f ? -1.0 : 1.0;
+    o->lw1 = p->w[0] != 0.f ? (float)std::log2(8.0 * std::fabs((double)p->w[0])) : -INFINITY;
+    o->lw2 = p->w[1] != 0.f ? (float)std::log2(0.5 * std::fabs((double)p->w[1])) : -INFINITY;
+    o->sigma = (float)-s1;
+    o->q = (float)(s1 * s2);
+    o->m3q = -3.f * o->q;
+    o->c4 = o->sigma * 2.f * p->w[2];
+    o->eA = (float)(s1 / 8.0);
+    o->eB = (float)(2.0 * s2);
     return DOCK_OK;
 }
 
@@ -112,7 +114,7 @@ int dock_make_dev_grid(const dock_params *p, const dock_grid *g, DevGrid *o)
     o->inv_h_lo = (float)(1.0 / h - (double)o->inv_h);
     o->kw_g = (float)(2.0 * (double)p->k_wall * h);
     o->kw_e = (float)((double)p->k_wall * h * h);
-    o->packed = reinterpret_cast<const float4 *>(g->packed_dev);
+    o->packed = reinterpret_cast<const Cell8 *>(g->packed_dev);
     o->data = g->data_dev;
     return DOCK_OK;
 }
@@ -336,7 +338,10 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
     // small bit matrix; they all go either to A's group (one record per partner j in B) or to B's
     // group (one record per partner j in A), whichever needs fewer records.  Format: common.cuh.
     const int n_tiles = (N + TPP_TILE - 1) / TPP_TILE;
-    struct Rec { int j; bool special; float rsum[TPP_TILE], wh[TPP_TILE], whb[TPP_TILE]; };
+    const float sigma = p->w[0] < 0.f ? 1.f : -1.f;                 // DevParams::sigma
+    const float whp = -sigma * p->w[3];                             // wh'
+    const float whbp = (float)(-(double)sigma * (double)p->w[4] / 0.7);   // whb'
+    struct Rec { int j; int cls; float rsum[TPP_TILE], wh[TPP_TILE], whb[TPP_TILE]; };
     std::vector<std::vector<Rec>> groups(n_tiles);
     std::vector<std::vector<std::pair<int, int>>> between((size_t)n_tiles * n_tiles);   // (slot in A, slot in B)
     for (int k = 0; k < P; ++k) {
@@ -351,7 +356,7 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
         if (!r) {
             Rec fresh;
             fresh.j = j_slot;
-            fresh.special = false;
+            fresh.cls = 0;
             for (int t = 0; t < TPP_TILE; ++t) { fresh.rsum[t] = TPP_MASKED_RSUM; fresh.wh[t] = 0.f; fresh.whb[t] = 0.f; }
             grp.push_back(fresh);
             r = &grp.back();
@@ -359,8 +364,8 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
         const int t = i_slot - tile * TPP_TILE;
         const int ti = L->type[atom_of[i_slot]], tj = L->type[atom_of[j_slot]];
         r->rsum[t] = p->radius[ti] + p->radius[tj];
-        if (p->hydrophobic[ti] && p->hydrophobic[tj]) { r->wh[t] = p->w[3]; r->special = true; }
-        if ((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) { r->whb[t] = p->w[4]; r->special = true; }
+        if (p->hydrophobic[ti] && p->hydrophobic[tj] && p->w[3] != 0.f) { r->wh[t] = whp; r->cls = std::max(r->cls, 1); }
+        if (((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) && p->w[4] != 0.f) { r->whb[t] = whbp; r->cls = 2; }
     };
     for (int A = 0; A < n_tiles; ++A)
         for (int B = A; B < n_tiles; ++B) {
@@ -380,38 +385,38 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
         std::memcpy(&q, v, 16);
         return q;
     };
-    int n_groups = 0;
     for (int A = 0; A < n_tiles; ++A) {
         std::vector<Rec> &grp = groups[A];
-        if (grp.empty()) continue;
         std::stable_sort(grp.begin(), grp.end(), [](const Rec &a, const Rec &b) { return a.j < b.j; });
-        std::vector<const Rec *> cls[2];
-        for (const Rec &r : grp) cls[r.special ? 1 : 0].push_back(&r);
-        if (cls[0].size() > 0x1fffeu || cls[1].size() > 0x1fffeu) return DOCK_EINVAL;
+        std::vector<const Rec *> cls[3];
+        for (const Rec &r : grp) cls[r.cls].push_back(&r);
         const int n_i = std::min(TPP_TILE, N - A * TPP_TILE);
         uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
         for (int t = 0; t < TPP_TILE; ++t) hdr.x |= (uint32_t)(A * TPP_TILE + (t < n_i ? t : 0)) << (8 * t);
-        hdr.y = (uint32_t)(cls[0].size() / 2) | ((uint32_t)(cls[0].size() & 1) << 16);
-        hdr.z = (uint32_t)(cls[1].size() / 2) | ((uint32_t)(cls[1].size() & 1) << 16);
+        hdr.y = (uint32_t)(cls[0].size() / 2) | ((uint32_t)(cls[0].size() & 1) << 8) |
+                ((uint32_t)(cls[1].size() / 2) << 16) | ((uint32_t)(cls[1].size() & 1) << 24);
+        hdr.z = (uint32_t)(cls[2].size() / 2) | ((uint32_t)(cls[2].size() & 1) << 8) | ((uint32_t)n_i << 16);
         quads.push_back(hdr);
-        for (int c = 0; c < 2; ++c) {
+        for (int c = 0; c < 3; ++c) {
             const std::vector<const Rec *> &v = cls[c];
+            auto payload = [&](const Rec *r) {
+                quads.push_back(fq(r->rsum));
+                if (c >= 1) quads.push_back(fq(r->wh));
+                if (c >= 2) quads.push_back(fq(r->whb));
+            };
             size_t k = 0;
             for (; k + 1 < v.size(); k += 2) {
                 quads.push_back(make_uint4((uint32_t)v[k]->j * 128u, (uint32_t)v[k + 1]->j * 128u, 0u, 0u));
-                for (int h = 0; h < 2; ++h) {
-                    quads.push_back(fq(v[k + h]->rsum));
-                    if (c) { quads.push_back(fq(v[k + h]->wh)); quads.push_back(fq(v[k + h]->whb)); }
-                }
+                payload(v[k]);
+                payload(v[k + 1]);
             }
             if (k < v.size()) {
                 quads.push_back(make_uint4((uint32_t)v[k]->j * 128u, 0u, 0u, 0u));
-                quads.push_back(fq(v[k]->rsum));
-                if (c) { quads.push_back(fq(v[k]->wh)); quads.push_back(fq(v[k]->whb)); }
+                payload(v[k]);
             }
         }
-        ++n_groups;
     }
+    const int n_groups = n_tiles;
     out.n_groups = n_groups;
     if (quads.size() <= (size_t)TPP_SCHED_QUADS) {
         out.sched_in_param = 1;
