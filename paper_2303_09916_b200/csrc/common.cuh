@@ -128,6 +128,7 @@ struct DevSystem {
 
 struct TppLigand {
     int N, T, n_groups, sched_in_param;
+    int fm_alias, pad_[3];                  // fragment sums alias consumed force slots (eval_thread.cuh)
     float4 atom_ref[DOCK_MAX_ATOMS];        // slot order (sorted by fragment): xyz rel. pivot, w = bitcast(map offset in entries)
     float4 tors_axis[DOCK_MAX_TORSIONS];    // reference-frame unit axis; w = bitcast(parent fragment)
     float4 tors_pt[DOCK_MAX_TORSIONS];      // reference position of atom b rel. pivot; w = 1 / |ref_b - ref_a|

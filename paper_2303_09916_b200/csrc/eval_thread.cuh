@@ -37,16 +37,18 @@ struct EvalTerms {
 };
 
 // floats of shared memory one THREAD of the evaluator needs:
-//   [xy: 2N][z: N][R: max(3N, 12 T)  per-atom forces, aliased by the fragment frames in phase 1][fm: 6 T]
-__host__ __device__ inline int tpp_thread_floats(int N, int T, bool want_grad)
+//   [xy: 2N][z: N][R: max(3N, 12 T)  per-atom forces, aliased by the fragment frames in phase 1][fm: 6 T unless aliased]
+// fm (force / torque sums of fragments 1..T) aliases the force slots of atoms 2(f-1), 2(f-1)+1 when the host
+// found that those atoms are consumed before fragment f's sums are written (TppLigand::fm_alias).
+__host__ __device__ inline int tpp_thread_floats(int N, int T, bool want_grad, bool fm_alias)
 {
     const int frames = 12 * T;
     if (!want_grad) return 3 * N + frames;
-    return 3 * N + (3 * N > frames ? 3 * N : frames) + 6 * T;
+    return 3 * N + (3 * N > frames ? 3 * N : frames) + (fm_alias ? 0 : 6 * T);
 }
-__host__ __device__ inline int tpp_warp_floats(int N, int T, bool want_grad)
+__host__ __device__ inline int tpp_warp_floats(int N, int T, bool want_grad, bool fm_alias)
 {
-    return 32 * tpp_thread_floats(N, T, want_grad);
+    return 32 * tpp_thread_floats(N, T, want_grad, fm_alias);
 }
 
 template <bool SCHED_PARAM>
@@ -190,7 +192,9 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
     float2 *const fr = reinterpret_cast<float2 *>(rbase) + lane;                   // [T][6] frames of fragments 0..T-1 (phase 1 only)
     float2 *const gxy = reinterpret_cast<float2 *>(rbase) + lane;                  // [N]
     float *const gz = rbase + 64 * N + lane;                                       // [N]
-    float2 *const fm = reinterpret_cast<float2 *>(rbase + 32 * rg) + lane;         // [T][3]: (Fx,Fy) (Fz,Mx) (My,Mz) of fragments 1..T
+    // force / torque sums of fragments 1..T: fragment f -> (Fx,Fy) (Fz,Mx) in fmA[2(f-1)], fmA[2(f-1)+1], My, Mz in fmB[..]
+    float2 *const fmA = L.fm_alias ? gxy : reinterpret_cast<float2 *>(rbase + 32 * rg) + lane;   // [2T] stride 32
+    float *const fmB = L.fm_alias ? gz : rbase + 32 * rg + 128 * T + lane;                       // [2T] stride 32
 
     const float tx = (pose[0] - G.rx) - G.rdx;
     const float ty = (pose[ps] - G.ry) - G.rdy;
@@ -333,14 +337,15 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
             }
             if (f == 0) { rFx = Fx; rFy = Fy; rFz = Fz; rMx = Mx; rMy = My; rMz = Mz; }
             else {
-                fm[(3 * (f - 1)) * 32] = make_float2(Fx, Fy);
-                fm[(3 * (f - 1) + 1) * 32] = make_float2(Fz, Mx);
-                fm[(3 * (f - 1) + 2) * 32] = make_float2(My, Mz);
+                fmA[(2 * (f - 1)) * 32] = make_float2(Fx, Fy);
+                fmA[(2 * (f - 1) + 1) * 32] = make_float2(Fz, Mx);
+                fmB[(2 * (f - 1)) * 32] = My;
+                fmB[(2 * (f - 1) + 1) * 32] = Mz;
             }
         }
         for (int f = T; f >= 1; --f) {
-            const float2 a0 = fm[(3 * (f - 1)) * 32], a1 = fm[(3 * (f - 1) + 1) * 32], a2 = fm[(3 * (f - 1) + 2) * 32];
-            const float Fx = a0.x, Fy = a0.y, Fz = a1.x, Mx = a1.y, My = a2.x, Mz = a2.y;
+            const float2 a0 = fmA[(2 * (f - 1)) * 32], a1 = fmA[(2 * (f - 1) + 1) * 32];
+            const float Fx = a0.x, Fy = a0.y, Fz = a1.x, Mx = a1.y, My = fmB[(2 * (f - 1)) * 32], Mz = fmB[(2 * (f - 1) + 1) * 32];
             const int as = L.tors_a[f - 1], bs = L.tors_b[f - 1];
             const float4 tp = L.tors_pt[f - 1];
             const float2 xb = xy[bs * 32], xa = xy[as * 32];
@@ -353,12 +358,12 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
                 const int pb = L.tors_b[p - 1];
                 const float2 o = xy[pb * 32];
                 const float lx = xb.x - o.x, ly = xb.y - o.y, lz = zb - zz[pb * 32];
-                float2 b0 = fm[(3 * (p - 1)) * 32], b1 = fm[(3 * (p - 1) + 1) * 32], b2 = fm[(3 * (p - 1) + 2) * 32];
+                float2 b0 = fmA[(2 * (p - 1)) * 32], b1 = fmA[(2 * (p - 1) + 1) * 32];
                 b0.x += Fx; b0.y += Fy; b1.x += Fz;
                 b1.y += Mx + fmaf(ly, Fz, -lz * Fy);
-                b2.x += My + fmaf(lz, Fx, -lx * Fz);
-                b2.y += Mz + fmaf(lx, Fy, -ly * Fx);
-                fm[(3 * (p - 1)) * 32] = b0; fm[(3 * (p - 1) + 1) * 32] = b1; fm[(3 * (p - 1) + 2) * 32] = b2;
+                fmA[(2 * (p - 1)) * 32] = b0; fmA[(2 * (p - 1) + 1) * 32] = b1;
+                fmB[(2 * (p - 1)) * 32] += My + fmaf(lz, Fx, -lx * Fz);
+                fmB[(2 * (p - 1) + 1) * 32] += Mz + fmaf(lx, Fy, -ly * Fx);
             } else {
                 rFx += Fx; rFy += Fy; rFz += Fz;
                 rMx += Mx + fmaf(xb.y, Fz, -zb * Fy);

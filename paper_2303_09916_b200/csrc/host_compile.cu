@@ -320,6 +320,10 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
         while (f_cur < L->atom_fragment[i]) out.frag_end[f_cur++] = (unsigned char)s;
     }
     while (f_cur <= T) out.frag_end[f_cur++] = (unsigned char)N;
+    // fragment f's sums may overwrite the force slots 2(f-1), 2(f-1)+1 iff those atoms were consumed before: frag_end[f] >= 2f
+    out.fm_alias = 1;
+    for (int f = 1; f <= T; ++f)
+        if ((int)out.frag_end[f] < 2 * f) out.fm_alias = 0;
     for (int k = 0; k < T; ++k) {
         const int a = L->tors_a[k], b = L->tors_b[k];
         double u[3], n = 0;

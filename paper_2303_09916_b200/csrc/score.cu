@@ -1,7 +1,8 @@
 // score.cu -- dock_score_batch: fused pose -> coordinates -> interpolated energy + gradient for a
 // batch of poses (eq. 2-3 at 198-219).  One THREAD per pose
-// (eval_thread.cuh); a CTA is a single warp, because the threads never cooperate and a 1-warp CTA
-// packs the shared memory of an SM most tightly.
+// (eval_thread.cuh).  The threads never cooperate; the CTA size (1..8 warps) is chosen on the host as
+// the one that packs most warps into an SM's shared memory (each CTA also costs 1 KB of reserved smem).
+#include <algorithm>
 #include <vector>
 
 #include "common.cuh"
@@ -11,15 +12,16 @@
 namespace {
 
 template <bool WANT_GRAD, bool SCHED_PARAM>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(256)
 score_thread_kernel(const DevParams P, const DevGrid G, const __grid_constant__ TppLigand L, long long n_poses,
                     const float *__restrict__ poses, float *__restrict__ energy,
-                    float *__restrict__ grad, float *__restrict__ terms)
+                    float *__restrict__ grad, float *__restrict__ terms, int warp_floats)
 {
-    extern __shared__ float smem[];
+    extern __shared__ float smem_all[];
+    float *const smem = smem_all + (size_t)(threadIdx.x >> 5) * warp_floats;
     const int np_ = 7 + L.T, ng = 6 + L.T;
     // idle lanes of the last warp redo the last pose: same inputs, same bits, same stores (benign)
-    const long long p = min((long long)blockIdx.x * 32 + threadIdx.x, n_poses - 1);
+    const long long p = min((long long)blockIdx.x * blockDim.x + threadIdx.x, n_poses - 1);
     EvalTerms t;
     const float e = eval_pose_thread<WANT_GRAD, SCHED_PARAM>(P, G, L, poses + p * np_, 1, grad + p * ng, 1, smem, t);
     energy[p] = e;
@@ -48,13 +50,26 @@ int launch(const ScorePlan &pl, long long n_poses, const float *poses_dev, float
            float *terms_dev, cudaStream_t stream)
 {
     auto kern = score_thread_kernel<WANT_GRAD, SCHED_PARAM>;
-    const size_t smem = (size_t)tpp_warp_floats(pl.L.N, pl.L.T, WANT_GRAD) * sizeof(float);
-    if (smem > 227 * 1024) return DOCK_EINVAL;
-    if (smem > 48 * 1024)
-        DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const long long blocks = (n_poses + 31) / 32;
+    const int warp_floats = tpp_warp_floats(pl.L.N, pl.L.T, WANT_GRAD, pl.L.fm_alias != 0);
+    const size_t warp_bytes = (size_t)warp_floats * sizeof(float);
+    if (warp_bytes > 227 * 1024) return DOCK_EINVAL;
+    // CTA size: most resident warps per SM (shared memory + 1 KB reserved per CTA, registers), ties -> fewer warps per CTA
+    if (warp_bytes > 48 * 1024 / 8)
+        DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)std::min<size_t>(8 * warp_bytes, 227 * 1024)));
+    int best_w = 1, best_res = 0;
+    for (int w = 1; w <= 8; ++w) {
+        if (w * warp_bytes > 227 * 1024) break;
+        int ctas = 0;
+        DOCK_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, kern, 32 * w, w * warp_bytes));
+        if (ctas * w > best_res) { best_res = ctas * w; best_w = w; }
+    }
+    if (best_res == 0) return DOCK_EINVAL;
+    const size_t smem = best_w * warp_bytes;
+    const long long per_cta = 32LL * best_w;
+    const long long blocks = (n_poses + per_cta - 1) / per_cta;
     if (blocks > 0x7fffffffLL) return DOCK_EINVAL;
-    kern<<<(unsigned)blocks, 32, smem, stream>>>(pl.P, pl.G, pl.L, n_poses, poses_dev, energy_dev, grad_dev, terms_dev);
+    kern<<<(unsigned)blocks, (unsigned)per_cta, smem, stream>>>(pl.P, pl.G, pl.L, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, warp_floats);
     DOCK_LAUNCH_CHECK();
     return DOCK_OK;
 }
