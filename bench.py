@@ -116,13 +116,8 @@ def _dist_setup(n_gpus: int):
 
 
 def _max_over_ranks(x: float, world: int) -> float:
-    if world == 1:
-        return x
-    import torch
-    import torch.distributed as dist
-    t = torch.tensor([x], dtype=torch.float64, device="cuda")
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    return float(t.item())
+    from paper_2303_09916_b200.shard import max_over_ranks
+    return max_over_ranks(x, device="cuda") if world > 1 else x
 
 
 def _barrier(world: int):
