@@ -72,6 +72,24 @@ __device__ __forceinline__ void quad_floats(const uint4 q, float v[4])
     v[0] = __uint_as_float(q.x); v[1] = __uint_as_float(q.y); v[2] = __uint_as_float(q.z); v[3] = __uint_as_float(q.w);
 }
 
+// A partner atom's coordinates and force accumulator, read one record ahead (record_class).
+struct PartnerRegs { float x, y, z, gx, gy, gz; };
+
+template <bool WANT_GRAD>
+__device__ __forceinline__ void load_partner(unsigned off, const char *xy, const char *zz, char *gxy, char *gz, PartnerRegs &p)
+{
+    // volatile: keeps the loads where they are written (ahead of the arithmetic of the previous record)
+    const unsigned axy = (unsigned)__cvta_generic_to_shared(xy + 2 * off), az = (unsigned)__cvta_generic_to_shared(zz + off);
+    asm volatile("ld.volatile.shared.v2.f32 {%0,%1}, [%2];" : "=f"(p.x), "=f"(p.y) : "r"(axy));
+    asm volatile("ld.volatile.shared.f32 %0, [%1];" : "=f"(p.z) : "r"(az));
+    p.gx = p.gy = p.gz = 0.0f;
+    if (WANT_GRAD) {
+        const unsigned bxy = (unsigned)__cvta_generic_to_shared(gxy + 2 * off), bz = (unsigned)__cvta_generic_to_shared(gz + off);
+        asm volatile("ld.volatile.shared.v2.f32 {%0,%1}, [%2];" : "=f"(p.gx), "=f"(p.gy) : "r"(bxy));
+        asm volatile("ld.volatile.shared.f32 %0, [%1];" : "=f"(p.gz) : "r"(bz));
+    }
+}
+
 // One record block: NP partner atoms (1 or 2) against the 4 tile atoms = 4 NP pairs, written STAGE BY STAGE over
 // all pairs (distances; reciprocal square roots; surface distances and exponent arguments; exponentials; slopes
 // and forces) so that the multi-cycle MUFU results of one pair are produced while the others issue -- with two
@@ -80,9 +98,10 @@ __device__ __forceinline__ void quad_floats(const uint4 q, float v[4])
 //   on j.  rsum = TPP_MASKED_RSUM makes every term exactly 0.  CLS 1 adds the hydrophobic ramp, CLS 2 the
 //   hydrophobic and H-bond ramps, with the per-pair weights wh', whb' (0 where the type pair has none).
 // Partner columns sit at byte offset `off` (z column; the (x,y) column is at 2*off).
-template <int NP, int CLS, bool WANT_GRAD, bool SCHED_PARAM>
+template <int NP, int CLS, bool WANT_GRAD, bool SCHED_PARAM, bool PRE = false>
 __device__ __forceinline__ void record_block(const DevParams &P, const TppLigand &L, int &pos, PairTile &t, PairAcc *acc,
-                                             const char *xy, const char *zz, char *gxy, char *gz)
+                                             const char *xy, const char *zz, char *gxy, char *gz,
+                                             const PartnerRegs *pre = nullptr)
 {
     constexpr int S = 1 + CLS;                 // payload quads of one record
     constexpr int NQ = NP * TPP_TILE;          // pairs of the block; pair p = partner p / TPP_TILE, tile atom p % TPP_TILE
@@ -99,8 +118,11 @@ __device__ __forceinline__ void record_block(const DevParams &P, const TppLigand
     float jx[NP], jy[NP], jz[NP];
 #pragma unroll
     for (int a = 0; a < NP; ++a) {
-        const float2 c = *reinterpret_cast<const float2 *>(xy + 2 * off[a]);
-        jx[a] = c.x; jy[a] = c.y; jz[a] = *reinterpret_cast<const float *>(zz + off[a]);
+        if (PRE) { jx[a] = pre[a].x; jy[a] = pre[a].y; jz[a] = pre[a].z; }
+        else {
+            const float2 c = *reinterpret_cast<const float2 *>(xy + 2 * off[a]);
+            jx[a] = c.x; jy[a] = c.y; jz[a] = *reinterpret_cast<const float *>(zz + off[a]);
+        }
     }
     float dx[NQ], dy[NQ], dz[NQ], r2[NQ], rinv[NQ], d[NQ], argA[NQ], argB[NQ], c4m[NQ], eA[NQ], eB[NQ];
 #pragma unroll
@@ -154,10 +176,15 @@ __device__ __forceinline__ void record_block(const DevParams &P, const TppLigand
     if (WANT_GRAD) {
 #pragma unroll
         for (int a = 0; a < NP; ++a) {
-            float2 g = *reinterpret_cast<float2 *>(gxy + 2 * off[a]);
-            g.x += gx[a]; g.y += gy[a];
-            *reinterpret_cast<float2 *>(gxy + 2 * off[a]) = g;
-            *reinterpret_cast<float *>(gz + off[a]) += gzz[a];
+            if (PRE) {
+                *reinterpret_cast<float2 *>(gxy + 2 * off[a]) = make_float2(pre[a].gx + gx[a], pre[a].gy + gy[a]);
+                *reinterpret_cast<float *>(gz + off[a]) = pre[a].gz + gzz[a];
+            } else {
+                float2 g = *reinterpret_cast<float2 *>(gxy + 2 * off[a]);
+                g.x += gx[a]; g.y += gy[a];
+                *reinterpret_cast<float2 *>(gxy + 2 * off[a]) = g;
+                *reinterpret_cast<float *>(gz + off[a]) += gzz[a];
+            }
         }
     }
 }
@@ -171,7 +198,28 @@ __device__ __forceinline__ void record_class(const DevParams &P, const TppLigand
     pos += n2 * (1 + 2 * (1 + CLS)) + n1 * (2 + CLS);
     if (n1 >= 0) return;
 #endif
-    for (int r = 0; r < n2; ++r) record_block<2, CLS, WANT_GRAD, SCHED_PARAM>(P, L, pos, t, acc, xy, zz, gxy, gz);
+    if (n2 > 0) {
+        // the partners of double record r+1 are read ahead of record r's arithmetic (measured +3 %, profiles/r1f.md:
+        // the LDS latency is otherwise exposed at the top of every record); partners are distinct within a group,
+        // so reading a force accumulator one record early is safe
+        constexpr int STEP = 1 + 2 * (1 + CLS);
+        PartnerRegs cur[2], nxt[2];
+        {
+            const uint4 h = tpp_quad<SCHED_PARAM>(L, pos);
+            load_partner<WANT_GRAD>(h.x, xy, zz, gxy, gz, cur[0]);
+            load_partner<WANT_GRAD>(h.y, xy, zz, gxy, gz, cur[1]);
+        }
+        for (int r = 0; r < n2; ++r) {
+            nxt[0] = cur[0]; nxt[1] = cur[1];
+            if (r + 1 < n2) {
+                const uint4 h = tpp_quad<SCHED_PARAM>(L, pos + STEP);
+                load_partner<WANT_GRAD>(h.x, xy, zz, gxy, gz, nxt[0]);
+                load_partner<WANT_GRAD>(h.y, xy, zz, gxy, gz, nxt[1]);
+            }
+            record_block<2, CLS, WANT_GRAD, SCHED_PARAM, true>(P, L, pos, t, acc, xy, zz, gxy, gz, cur);
+            cur[0] = nxt[0]; cur[1] = nxt[1];
+        }
+    }
     if (n1) record_block<1, CLS, WANT_GRAD, SCHED_PARAM>(P, L, pos, t, acc, xy, zz, gxy, gz);
 }
 
@@ -205,7 +253,11 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
         Rot3 A = quat_to_rot(pose[3 * ps], pose[4 * ps], pose[5 * ps], pose[6 * ps]);
         float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f;                                     // pivot-relative
         int s = 0;
+        float sn_n = 0.0f, cs_n = 1.0f;                                            // sin / cos of the NEXT torsion (independent work
+        if (T > 0) sincos_cw(pose[7 * ps], sn_n, cs_n);                            // for the scheduler while a frame is composed)
         for (int f = 0; f <= T; ++f) {
+            const float sn = sn_n, cs = cs_n;
+            if (f < T && f > 0) sincos_cw(pose[(7 + f) * ps], sn_n, cs_n);
             if (f > 0) {
                 const int k = f - 1;
                 const float4 u = L.tors_axis[k];
@@ -213,8 +265,6 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
                 const int p = __float_as_int(u.w);
                 const float2 p0 = fr[(6 * p) * 32], p1 = fr[(6 * p + 1) * 32], p2 = fr[(6 * p + 2) * 32];
                 const float2 p3 = fr[(6 * p + 3) * 32], p4 = fr[(6 * p + 4) * 32], p5 = fr[(6 * p + 5) * 32];
-                float sn, cs;
-                sincos_cw(pose[(7 + k) * ps], sn, cs);
                 const float omc = 1.0f - cs;
                 const float ox = omc * u.x, oy = omc * u.y, oz = omc * u.z;
                 const float sx = sn * u.x, sy = sn * u.y, sz = sn * u.z;
