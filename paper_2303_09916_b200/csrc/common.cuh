@@ -78,12 +78,12 @@ struct DevGrid {
 };
 
 // ---- warp-per-pose evaluator (search kernels): compiled ligand in the caller's workspace --------
-// One scheduled intra-ligand pair.  ij = i | (j << 16), or -1 for an idle lane.
+// One scheduled intra-ligand pair.  ij = i | (j << 16), or -1 for an idle lane (rsum = TPP_MASKED_RSUM).
 struct __align__(16) PairRec {
     int   ij;
     float rsum;   // R_i + R_j
-    float wh;     // w4 if both hydrophobic else 0
-    float whb;    // w5 if donor/acceptor pair else 0
+    float wh;     // wh'  = -sigma w4 if both hydrophobic else 0        (DevParams)
+    float whb;    // whb' = -sigma w5 / 0.7 if donor/acceptor pair else 0
 };
 
 struct DevLigand {

@@ -98,31 +98,48 @@ __device__ __noinline__ float eval_pose_warp(const DevParams &P, const DevGrid &
     __syncwarp();
 
     // ---- A4 ------------------------------------------------------------------------------------
-    float e_intra = 0.0f;
-    for (int r = 0; r < L.n_rounds; ++r) {
-        const float4 raw = __ldg(reinterpret_cast<const float4 *>(L.sched + r * 32 + lane));
-        const int ij = __float_as_int(raw.x);
-        int i = 0, j = 0;
-        float fx = 0.0f, fy = 0.0f, fz = 0.0f;
-        bool hit = false;
-        if (ij >= 0) {
-            i = ij & 0xffff; j = ij >> 16;
+    // Branch-free rounds: an idle lane or an out-of-range pair gets the surface distance 1e18, for which every
+    // term and derivative is exactly 0 (weights folded into the exponents as in eval_thread.cuh, see DevParams);
+    // the next round's record is fetched while this one computes.
+    float aA = 0.0f, aB = 0.0f, aRep = 0.0f, aHyd = 0.0f, aHb = 0.0f;
+    {
+        const float4 *sched = reinterpret_cast<const float4 *>(L.sched) + lane;
+        const int n_rounds = L.n_rounds;
+        float4 raw = n_rounds > 0 ? __ldg(sched) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int r = 0; r < n_rounds; ++r) {
+            const float4 cur = raw;
+            if (r + 1 < n_rounds) raw = __ldg(sched + (r + 1) * 32);
+            const int ij = __float_as_int(cur.x);
+            const bool valid = ij >= 0;
+            const int i = valid ? (ij & 0xffff) : 0, j = valid ? (ij >> 16) : 0;
             const float dx = xs[i] - xs[j], dy = xs[np + i] - xs[np + j], dz = xs[2 * np + i] - xs[2 * np + j];
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (r2 < P.cutoff2) {
-                float k;
-                e_intra += pair_term_rt(P, r2, raw.y, raw.z, raw.w, k);
-                fx = k * dx; fy = k * dy; fz = k * dz;
-                hit = true;
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, 1e-12f)));
+            const float rinv = fast_rsqrt(r2);
+            const float d = (valid && r2 < P.cutoff2) ? fmaf(r2, rinv, -cur.y) : 1.0e18f;
+            const float A = fast_ex2(fmaf(d * -5.770780163555854f, d, P.lw1));
+            const float B = fast_ex2(fmaf(d, fmaf(d, -0.36067376022224085f, 2.1640425613334453f), P.lw2 - 3.2460638420001677f));
+            const float m = fminf(d, 0.0f);
+            const float c4m = P.c4 * m;
+            aA += A; aB += B;
+            aRep = fmaf(c4m, m, aRep);
+            float de = fmaf(d, fmaf(P.q, B, A), fmaf(P.m3q, B, c4m));            // sigma dE/dd
+            const float th = 1.5f - d, hh = __saturatef(th);
+            aHyd = fmaf(cur.z, hh, aHyd);
+            de = fmaf(cur.z, (hh == th) ? 1.0f : 0.0f, de);
+            const float tb = d * -1.4285714285714286f, hb = __saturatef(tb);
+            aHb = fmaf(cur.w, hb, aHb);
+            de = fmaf(cur.w, (hb == tb) ? 1.0f : 0.0f, de);
+            if (WANT_GRAD) {
+                const float k = P.sigma * de * rinv;
+                const float fx = k * dx, fy = k * dy, fz = k * dz;
+                if (valid) { gs[i] += fx; gs[np + i] += fy; gs[2 * np + i] += fz; }
+                __syncwarp();
+                if (valid) { gs[j] -= fx; gs[np + j] -= fy; gs[2 * np + j] -= fz; }
+                __syncwarp();
             }
         }
-        if (WANT_GRAD) {
-            if (hit) { gs[i] += fx; gs[np + i] += fy; gs[2 * np + i] += fz; }
-            __syncwarp();
-            if (hit) { gs[j] -= fx; gs[np + j] -= fy; gs[2 * np + j] -= fz; }
-            __syncwarp();
-        }
     }
+    float e_intra = fmaf(P.eA, aA, fmaf(P.eB, aB, P.sigma * fmaf(0.5f, aRep, fmaf(-0.7f, aHb, -aHyd))));
 
     e_grid = warp_sum(e_grid);
     e_wall = warp_sum(e_wall);
@@ -130,35 +147,56 @@ __device__ __noinline__ float eval_pose_warp(const DevParams &P, const DevGrid &
     if (terms) { terms->e_grid = e_grid; terms->e_wall = e_wall; terms->e_intra = e_intra; }
 
     // ---- A5 ------------------------------------------------------------------------------------
+    // With p_i = x_i - t (lever arm about the pivot) and m_i = p_i x g_i:
+    //   torque = sum m_i;   dE/dtheta_k = u_k . sum_{i in subtree k} m_i - (u_k x p_b) . sum_{i in subtree k} g_i.
+    // Lane k prepares (u_k, u_k x p_b); every lane then forms its atoms' share of all T torsion sums in its own
+    // column tsum[k][lane], and lane k adds row k -- no per-torsion shuffle reductions.
     if (WANT_GRAD) {
-        float fx = 0.f, fy = 0.f, fz = 0.f, qx = 0.f, qy = 0.f, qz = 0.f;
-        for (int i = lane; i < N; i += 32) {
-            const float gx = gs[i], gy = gs[np + i], gz = gs[2 * np + i];
-            const float lx = xs[i] - tx, ly = xs[np + i] - ty, lz = xs[2 * np + i] - tz;
-            fx += gx; fy += gy; fz += gz;
-            qx += ly * gz - lz * gy;
-            qy += lz * gx - lx * gz;
-            qz += lx * gy - ly * gx;
-        }
-        fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
-        qx = warp_sum(qx); qy = warp_sum(qy); qz = warp_sum(qz);
-        if (lane == 0) { grad[0] = fx; grad[1] = fy; grad[2] = fz; grad[3] = qx; grad[4] = qy; grad[5] = qz; }
-        for (int k = 0; k < T; ++k) {
+        float *tsum = cs + ((T + 3) & ~3);                                       // [T][32]
+        float4 *uw = reinterpret_cast<float4 *>(tsum + 32 * T);                  // [T][2]
+        for (int k = lane; k < T; k += 32) {
             const int2 ab = __ldg(&L.tors_ab[k]);
             const float bx = xs[ab.y], by = xs[np + ab.y], bz = xs[2 * np + ab.y];
             float ux = bx - xs[ab.x], uy = by - xs[np + ab.x], uz = bz - xs[2 * np + ab.x];
             const float inv = 1.0f / sqrtf(ux * ux + uy * uy + uz * uz);
             ux *= inv; uy *= inv; uz *= inv;
-            float c = 0.0f;
-            for (int i = lane; i < N; i += 32) {
-                if ((__ldg(&L.atom_topo[i]).y >> k) & 1) {
-                    const float gx = gs[i], gy = gs[np + i], gz = gs[2 * np + i];
-                    const float lx = xs[i] - bx, ly = xs[np + i] - by, lz = xs[2 * np + i] - bz;
-                    c += ux * (ly * gz - lz * gy) + uy * (lz * gx - lx * gz) + uz * (lx * gy - ly * gx);
-                }
+            const float lx = bx - tx, ly = by - ty, lz = bz - tz;
+            uw[2 * k] = make_float4(ux, uy, uz, 0.0f);
+            uw[2 * k + 1] = make_float4(uy * lz - uz * ly, uz * lx - ux * lz, ux * ly - uy * lx, 0.0f);
+        }
+        for (int k = 0; k < T; ++k) tsum[k * 32 + lane] = 0.0f;
+        __syncwarp();
+        float fx = 0.f, fy = 0.f, fz = 0.f, qx = 0.f, qy = 0.f, qz = 0.f;
+        for (int i = lane; i < N; i += 32) {
+            const float gx = gs[i], gy = gs[np + i], gz = gs[2 * np + i];
+            const float px = xs[i] - tx, py = xs[np + i] - ty, pz = xs[2 * np + i] - tz;
+            const float mx = py * gz - pz * gy, my = pz * gx - px * gz, mz = px * gy - py * gx;
+            fx += gx; fy += gy; fz += gz;
+            qx += mx; qy += my; qz += mz;
+            unsigned mask = (unsigned)__ldg(&L.atom_topo[i]).y;
+            while (mask) {                                                        // torsions on the path to the root
+                const int k = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const float4 u = uw[2 * k], w = uw[2 * k + 1];
+                tsum[k * 32 + lane] += fmaf(u.x, mx, fmaf(u.y, my, u.z * mz)) - fmaf(w.x, gx, fmaf(w.y, gy, w.z * gz));
             }
-            c = warp_sum(c);
-            if (lane == 0) grad[6 + k] = c;
+        }
+        __syncwarp();
+        fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
+        qx = warp_sum(qx); qy = warp_sum(qy); qz = warp_sum(qz);
+        if (lane == 0) {
+            grad[0] = fx; grad[1] = fy; grad[2] = fz;
+            grad[3] = qx; grad[4] = qy; grad[5] = qz;
+        }
+        for (int k = lane; k < T; k += 32) {
+            float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;
+#pragma unroll
+            for (int l = 0; l < 32; l += 4) {
+                const int a = (l + lane) & 31;                                    // skewed: conflict-free
+                c0 += tsum[k * 32 + a]; c1 += tsum[k * 32 + ((a + 1) & 31)];
+                c2 += tsum[k * 32 + ((a + 2) & 31)]; c3 += tsum[k * 32 + ((a + 3) & 31)];
+            }
+            grad[6 + k] = (c0 + c1) + (c2 + c3);
         }
         __syncwarp();
     }

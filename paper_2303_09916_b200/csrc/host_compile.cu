@@ -165,10 +165,13 @@ void build_schedule(const dock_params *p, const dock_ligand *L, std::vector<Pair
                 const int ti = L->type[rnd[l].i], tj = L->type[rnd[l].j];
                 r.ij = rnd[l].i | (rnd[l].j << 16);
                 r.rsum = p->radius[ti] + p->radius[tj];
-                r.wh = (p->hydrophobic[ti] && p->hydrophobic[tj]) ? p->w[3] : 0.f;
-                r.whb = ((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) ? p->w[4] : 0.f;
+                // wh' = -sigma w4, whb' = -sigma w5 / 0.7 (DevParams)
+                const float sigma = p->w[0] < 0.f ? 1.f : -1.f;
+                r.wh = (p->hydrophobic[ti] && p->hydrophobic[tj]) ? -sigma * p->w[3] : 0.f;
+                r.whb = ((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti]))
+                            ? (float)(-(double)sigma * (double)p->w[4] / 0.7) : 0.f;
             } else {
-                r.ij = -1; r.rsum = 0.f; r.wh = 0.f; r.whb = 0.f;
+                r.ij = -1; r.rsum = TPP_MASKED_RSUM; r.wh = 0.f; r.whb = 0.f;
             }
             sched.push_back(r);
         }
