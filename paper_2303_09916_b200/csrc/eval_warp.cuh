@@ -65,7 +65,7 @@ __device__ __forceinline__ void pose_coords_warp(const DevLigand &L, const float
 }
 
 template <bool WANT_GRAD>
-__device__ __noinline__ float eval_pose_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
+__device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
                                              const float *pose, float *grad, float *scratch, EvalTerms *terms)
 {
     const int lane = threadIdx.x & 31;

@@ -94,8 +94,11 @@ __device__ __forceinline__ void set_identity(float *H, int n, float diag)
 }
 
 // O8: BFGS with backtracking.  b.x holds the start pose (quaternion normalised here) and the result.
-__device__ __noinline__ float local_opt_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
-                                             const OptBuf &b, int cap, int &iters, int &evals)
+// Written as one loop around a SINGLE evaluation site (the start pose is "trial" INIT), so that the evaluator and
+// this routine inline into the kernels once: the compiler then sees that every buffer is shared memory and keeps
+// P, G, L in registers / the constant bank instead of local memory (profiles/r1g.md).
+__device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
+                                                const OptBuf &b, int cap, int &iters, int &evals)
 {
     const int lane = threadIdx.x & 31;
     const int T = L.T, n = 6 + T, np_ = 7 + T;
@@ -106,12 +109,66 @@ __device__ __noinline__ float local_opt_warp(const DevParams &P, const DevGrid &
         else { b.x[3] = 1.f; b.x[4] = b.x[5] = b.x[6] = 0.f; }
     }
     __syncwarp();
-    float f = eval_pose_warp<true>(P, G, L, b.x, b.g, b.scratch, nullptr);
-    evals = 1;
-    set_identity(b.H, n, 1.0f);
-    bool fresh = true;
-    int it = 0;
-    for (it = 0; it < cap; ++it) {
+    for (int k = lane; k < np_; k += 32) b.xt[k] = b.x[k];
+    __syncwarp();
+    float f = 0.0f, alpha = 1.0f;
+    double gp = 0.0;
+    bool init = true, fresh = true;
+    int it = 0, trial = 0;
+    evals = 0;
+    for (;;) {
+        const float ft = eval_pose_warp<true>(P, G, L, b.xt, b.gt, b.scratch, nullptr);
+        ++evals;
+        if (init) {
+            init = false;
+            f = ft;
+            for (int r = lane; r < n; r += 32) b.g[r] = b.gt[r];
+            set_identity(b.H, n, 1.0f);
+        } else if ((double)ft - (double)f <= (double)P.c1 * (double)alpha * gp) {   // Armijo: accept the step
+            double ys = 0.0, yy = 0.0, ss = 0.0;
+            for (int r = lane; r < n; r += 32) {
+                const float s = alpha * b.d[r], yv = b.gt[r] - b.g[r];
+                b.d[r] = s;                        // d now holds s
+                b.y[r] = yv;
+                ys += (double)yv * (double)s; yy += (double)yv * (double)yv; ss += (double)s * (double)s;
+            }
+            ys = warp_sum_d(ys); yy = warp_sum_d(yy); ss = warp_sum_d(ss);
+            for (int k = lane; k < np_; k += 32) b.x[k] = b.xt[k];
+            for (int r = lane; r < n; r += 32) b.g[r] = b.gt[r];
+            f = ft;
+            __syncwarp();
+            if (ys > (double)P.curv_eps * sqrt(ss) * sqrt(yy)) {
+                if (fresh) { set_identity(b.H, n, (float)(ys / yy)); fresh = false; }
+                for (int r = lane; r < n; r += 32) {
+                    float a = 0.0f;
+                    for (int c = 0; c < n; ++c) a = fmaf(b.H[r * n + c], b.y[c], a);
+                    b.hy[r] = a;
+                }
+                __syncwarp();
+                double acc = 0.0;
+                for (int r = lane; r < n; r += 32) acc += (double)b.y[r] * (double)b.hy[r];
+                const double yhy = warp_sum_d(acc);
+                const double rho_d = 1.0 / ys;
+                const float rho = (float)rho_d, coef = (float)(rho_d * rho_d * yhy + rho_d);
+                // H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T, expanded for symmetric H
+                for (int r = lane; r < n; r += 32) {
+                    const float sr = b.d[r], hr = b.hy[r];
+                    for (int c = 0; c < n; ++c) {
+                        const float sc = b.d[c], hc = b.hy[c];
+                        b.H[r * n + c] += fmaf(coef * sr, sc, -rho * fmaf(sr, hc, hr * sc));
+                    }
+                }
+                __syncwarp();
+            }
+            ++it;
+        } else {                                   // backtrack
+            alpha *= P.shrink;
+            if (++trial >= P.max_trials) break;    // no acceptable trial: stop
+            pose_add_warp(T, b.x, b.d, alpha, b.xt);
+            continue;
+        }
+        // ---- start iteration `it` ----
+        if (it >= cap) break;
         double acc = 0.0;
         for (int r = lane; r < n; r += 32) acc += (double)b.g[r] * (double)b.g[r];
         const double gn2 = warp_sum_d(acc);
@@ -124,66 +181,23 @@ __device__ __noinline__ float local_opt_warp(const DevParams &P, const DevGrid &
         __syncwarp();
         acc = 0.0;
         for (int r = lane; r < n; r += 32) acc += (double)b.g[r] * (double)b.d[r];
-        double gp = warp_sum_d(acc);
-        if (gp >= 0.0) {                       // not a descent direction: reset H = I
+        gp = warp_sum_d(acc);
+        if (gp >= 0.0) {                           // not a descent direction: reset H = I
             set_identity(b.H, n, 1.0f);
             fresh = true;
             for (int r = lane; r < n; r += 32) b.d[r] = -b.g[r];
             __syncwarp();
             gp = -gn2;
         }
-        float alpha = 1.0f;
+        alpha = 1.0f;
         if (fresh) {
             acc = 0.0;
             for (int r = lane; r < n; r += 32) acc += (double)b.d[r] * (double)b.d[r];
             const double dn = sqrt(warp_sum_d(acc));
             if (dn > 1.0) alpha = (float)(1.0 / dn);
         }
-        bool ok = false;
-        float ft = f;
-        for (int trial = 0; trial < P.max_trials; ++trial) {
-            pose_add_warp(T, b.x, b.d, alpha, b.xt);
-            ft = eval_pose_warp<true>(P, G, L, b.xt, b.gt, b.scratch, nullptr);
-            ++evals;
-            if ((double)ft - (double)f <= (double)P.c1 * (double)alpha * gp) { ok = true; break; }   // Armijo
-            alpha *= P.shrink;
-        }
-        if (!ok) break;
-        double ys = 0.0, yy = 0.0, ss = 0.0;
-        for (int r = lane; r < n; r += 32) {
-            const float s = alpha * b.d[r], yv = b.gt[r] - b.g[r];
-            b.d[r] = s;                        // d now holds s
-            b.y[r] = yv;
-            ys += (double)yv * (double)s; yy += (double)yv * (double)yv; ss += (double)s * (double)s;
-        }
-        ys = warp_sum_d(ys); yy = warp_sum_d(yy); ss = warp_sum_d(ss);
-        for (int k = lane; k < np_; k += 32) b.x[k] = b.xt[k];
-        for (int r = lane; r < n; r += 32) b.g[r] = b.gt[r];
-        f = ft;
-        __syncwarp();
-        if (ys > (double)P.curv_eps * sqrt(ss) * sqrt(yy)) {
-            if (fresh) { set_identity(b.H, n, (float)(ys / yy)); fresh = false; }
-            for (int r = lane; r < n; r += 32) {
-                float a = 0.0f;
-                for (int c = 0; c < n; ++c) a = fmaf(b.H[r * n + c], b.y[c], a);
-                b.hy[r] = a;
-            }
-            __syncwarp();
-            acc = 0.0;
-            for (int r = lane; r < n; r += 32) acc += (double)b.y[r] * (double)b.hy[r];
-            const double yhy = warp_sum_d(acc);
-            const double rho_d = 1.0 / ys;
-            const float rho = (float)rho_d, coef = (float)(rho_d * rho_d * yhy + rho_d);
-            // H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T, expanded for symmetric H
-            for (int r = lane; r < n; r += 32) {
-                const float sr = b.d[r], hr = b.hy[r];
-                for (int c = 0; c < n; ++c) {
-                    const float sc = b.d[c], hc = b.hy[c];
-                    b.H[r * n + c] += fmaf(coef * sr, sc, -rho * fmaf(sr, hc, hr * sc));
-                }
-            }
-            __syncwarp();
-        }
+        trial = 0;
+        pose_add_warp(T, b.x, b.d, alpha, b.xt);
     }
     iters = it;
     return f;
@@ -233,37 +247,43 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
     float *cur = base, *best = base + pad4(row);
     const OptBuf b = carve(base + 2 * pad4(row), T, L.n_pad);
 
-    for (int k = lane; k < np_; k += 32) b.x[k] = init[gw * row + k];
-    __syncwarp();
     int iters, evals;
     unsigned long long total_evals = 0;
-    float e_cur = local_opt_warp(P, G, L, b, cap, iters, evals);
-    total_evals += evals;
-    for (int k = lane; k < np_; k += 32) { cur[k] = b.x[k]; best[k] = b.x[k]; }
-    __syncwarp();
-    float e_best = e_cur;
-
-    for (int step = 0; step < steps; ++step) {
-        uint32_t r[4];
-        philox4x32_10(copy, (uint32_t)step, 0u, sys, seed_lo, seed_hi, r);
-        const uint32_t K = T > 0 ? 3u : 2u;
-        const int kind = (int)__umulhi(r[0], K);
-        for (int k = lane; k < np_; k += 32) b.x[k] = cur[k];
-        __syncwarp();
-        if (lane == 0) {
-            if (kind == 0) {
-                for (int c = 0; c < 3; ++c) b.x[c] = cur[c] + P.amp_trans * (2.0f * u24(r[1 + c]) - 1.0f);
-            } else if (kind == 1) {
-                rotate_quat(P.amp_rot * (2.0f * u24(r[1]) - 1.0f), P.amp_rot * (2.0f * u24(r[2]) - 1.0f),
-                            P.amp_rot * (2.0f * u24(r[3]) - 1.0f), cur + 3, b.x + 3);
-            } else {
-                const int k = (int)__umulhi(r[1], (uint32_t)T);
-                b.x[7 + k] = PI_F * (2.0f * u24(r[2]) - 1.0f);
+    float e_cur = 0.0f, e_best = 0.0f;
+    // step -1 = local optimisation of the initial pose (reading S16); one call site of the optimizer
+    for (int step = -1; step < steps; ++step) {
+        uint32_t r[4] = {0u, 0u, 0u, 0u};
+        int kind = 0;
+        if (step < 0) {
+            for (int k = lane; k < np_; k += 32) b.x[k] = init[gw * row + k];
+            __syncwarp();
+        } else {
+            philox4x32_10(copy, (uint32_t)step, 0u, sys, seed_lo, seed_hi, r);
+            const uint32_t K = T > 0 ? 3u : 2u;
+            kind = (int)__umulhi(r[0], K);
+            for (int k = lane; k < np_; k += 32) b.x[k] = cur[k];
+            __syncwarp();
+            if (lane == 0) {
+                if (kind == 0) {
+                    for (int c = 0; c < 3; ++c) b.x[c] = cur[c] + P.amp_trans * (2.0f * u24(r[1 + c]) - 1.0f);
+                } else if (kind == 1) {
+                    rotate_quat(P.amp_rot * (2.0f * u24(r[1]) - 1.0f), P.amp_rot * (2.0f * u24(r[2]) - 1.0f),
+                                P.amp_rot * (2.0f * u24(r[3]) - 1.0f), cur + 3, b.x + 3);
+                } else {
+                    const int k = (int)__umulhi(r[1], (uint32_t)T);
+                    b.x[7 + k] = PI_F * (2.0f * u24(r[2]) - 1.0f);
+                }
             }
+            __syncwarp();
         }
-        __syncwarp();
         const float e_c = local_opt_warp(P, G, L, b, cap, iters, evals);
         total_evals += evals;
+        if (step < 0) {
+            e_cur = e_best = e_c;
+            for (int k = lane; k < np_; k += 32) { cur[k] = b.x[k]; best[k] = b.x[k]; }
+            __syncwarp();
+            continue;
+        }
         uint32_t ra[4];
         philox4x32_10(copy, (uint32_t)step, 1u, sys, seed_lo, seed_hi, ra);
         const float u = u24(ra[0]);
