@@ -132,9 +132,17 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
             if (WANT_GRAD) {
                 const float k = P.sigma * de * rinv;
                 const float fx = k * dx, fy = k * dy, fz = k * dz;
-                if (valid) { gs[i] += fx; gs[np + i] += fy; gs[2 * np + i] += fz; }
+                // all three loads before the stores: the compiler cannot prove the rows distinct and would otherwise
+                // serialise load -> add -> store three times (one shared-memory latency each)
+                if (valid) {
+                    const float a0 = gs[i], a1 = gs[np + i], a2 = gs[2 * np + i];
+                    gs[i] = a0 + fx; gs[np + i] = a1 + fy; gs[2 * np + i] = a2 + fz;
+                }
                 __syncwarp();
-                if (valid) { gs[j] -= fx; gs[np + j] -= fy; gs[2 * np + j] -= fz; }
+                if (valid) {
+                    const float a0 = gs[j], a1 = gs[np + j], a2 = gs[2 * np + j];
+                    gs[j] = a0 - fx; gs[np + j] = a1 - fy; gs[2 * np + j] = a2 - fz;
+                }
                 __syncwarp();
             }
         }
