@@ -402,3 +402,67 @@ def test_end_to_end_host_call(dk, orc, torch, tiny):
     assert r["evals"] == int(r2["evals"][0])
     chk = orc.score_batch(op, og, oL, r["topk_pose"][:r["count"]].astype(np.float64), want_grad=False)[0]
     assert np.all(np.abs(r["topk_e"][:r["count"]] - chk) <= tol(chk))
+
+
+# ----------------------------------------------------------------------------------- configs 3 and 4
+@pytest.mark.parametrize("index", [0, 5])
+def test_config3_systems_score_and_local_opt(dk, orc, torch, index):
+    """Two systems of the screening batch (BASELINE.json configs[3]) at their drawn sizes: grid at every node,
+    per-pose scores and gradients, and local-optimisation energies against the oracle."""
+    s = make_system(3, seed=0, index=index)
+    p, box, grid, lig = gpu_side(dk, s)
+    op, og, oL = oracle_side(orc, s)
+    err = np.abs(grid.data.cpu().numpy().astype(np.float64) - og.maps) / tol(og.maps)
+    assert err.max() <= 1.0
+    rng = np.random.default_rng(30 + index)
+    poses = random_poses(rng, 2053, s.box_center, s.box_size, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, f"cfg3[{index}]",
+                        cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
+    _log(f"score_cfg3_{index}", dict(st, N=lig.N, T=lig.T, P=lig.P, n_prot=int(s.protein_xyz.shape[0])))
+    # local optimisation never increases the energy and ends where the oracle's evaluation agrees
+    n = 64
+    out_pose, out_e, iters = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:n]).cuda(), 300)
+    fin = out_pose.cpu().numpy()
+    oe2, _, _, d2 = orc.score_batch(op, og, oL, fin.astype(np.float64))
+    ok = d2["cutoff_margin"] > 1e-4
+    assert np.all(np.abs(out_e.cpu().numpy() - oe2)[ok] <= tol(oe2)[ok])
+    assert np.all(out_e.cpu().numpy() <= e[:n].cpu().numpy() + 1e-3)
+
+
+def test_config4_large_box_grid_score_and_search_properties(dk, orc, torch):
+    """BASELINE.json configs[4]: 8000-atom protein, 161^3 x 8 maps, 60-atom / 15-torsion ligand.  The grid is
+    compared at EVERY node (the oracle's brute force takes ~30 s on the box's cores), scores on a sample;
+    the search runs with the config's 2048 copies for a few steps and is checked through properties that hold
+    at any size (bitwise determinism, best <= initial local optimum, oracle re-evaluation of the winners)."""
+    s = make_system(4, seed=0)
+    p, box, grid, lig = gpu_side(dk, s)
+    op, og, oL = oracle_side(orc, s)
+    assert tuple(grid.dims) == (161, 161, 161)
+    gm = grid.data.cpu().numpy().astype(np.float64)
+    err = np.abs(gm - og.maps) / tol(og.maps)
+    assert err.max() <= 1.0
+    del gm, err
+    rng = np.random.default_rng(4)
+    poses = random_poses(rng, 8192, s.box_center, s.box_size, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, "cfg4",
+                        cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
+    _log("score_cfg4", dict(st, N=lig.N, T=lig.T, P=lig.P))
+    steps = 3
+    r1 = dk.dock_search(p, [grid], [lig], [box], s.copies, steps, s.bfgs_cap, 11)
+    r2 = dk.dock_search(p, [grid], [lig], [box], s.copies, steps, s.bfgs_cap, 11)
+    assert torch.equal(r1["best_e"], r2["best_e"]) and torch.equal(r1["best_pose"], r2["best_pose"])
+    r0 = dk.dock_search(p, [grid], [lig], [box], s.copies, 0, s.bfgs_cap, 11)
+    assert bool((r1["best_e"] <= r0["best_e"] + 1e-6).all())          # best only improves on the optimised start
+    k = int(r1["topk_count"][0])
+    assert 1 <= k <= 10
+    tp = r1["topk_pose"][0, :k].cpu().numpy().astype(np.float64)
+    te = r1["topk_e"][0, :k].cpu().numpy()
+    oe3, _, _, d3 = orc.score_batch(op, og, oL, tp)
+    ok = d3["cutoff_margin"] > 1e-4
+    assert np.all(np.abs(te - oe3)[ok] <= tol(oe3)[ok])
+    assert np.all(np.diff(te) >= 0)
+    _log("search_cfg4", dict(copies=s.copies, steps=steps, evals=int(r1["evals"][0]), best=float(te[0])))
