@@ -194,10 +194,6 @@ __device__ __forceinline__ void record_class(const DevParams &P, const TppLigand
                                              PairAcc *acc,
                                              const char *xy, const char *zz, char *gxy, char *gz)
 {
-#ifdef ABL_NORECORDS
-    pos += n2 * (1 + 2 * (1 + CLS)) + n1 * (2 + CLS);
-    if (n1 >= 0) return;
-#endif
     if (n2 > 0) {
         // the partners of double record r+1 are read ahead of record r's arithmetic (measured +3 %, profiles/r1f.md:
         // the LDS latency is otherwise exposed at the top of every record); partners are distinct within a group,
@@ -332,11 +328,7 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
                 t.fx[k] = t.fy[k] = t.fz[k] = 0.0f;
                 cr[k] = locate_cell(G, t.x[k] + tx, t.y[k] + ty, t.z[k] + tz);
                 const Cell8 *e0 = G.packed + (size_t)__float_as_int(L.atom_ref[i].w) + cr[k].idx;
-#ifdef ABL_NOGATHER
-                q0[k] = make_float4(t.x[k], t.y[k], t.z[k], 1.f); q1[k] = q0[k]; (void)e0;
-#else
                 ldg_cell(e0, q0[k], q1[k]);                                     // consumed after the records
-#endif
             }
             record_class<0, WANT_GRAD, SCHED_PARAM>(P, L, pos, (int)(hdr.y & 0xffu), (int)((hdr.y >> 8) & 0xffu), t, acc, xyb, zzb, gxyb, gzb);
             record_class<1, WANT_GRAD, SCHED_PARAM>(P, L, pos, (int)((hdr.y >> 16) & 0xffu), (int)(hdr.y >> 24), t, acc, xyb, zzb, gxyb, gzb);
