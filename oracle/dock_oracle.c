@@ -66,6 +66,9 @@ void orc_default_params(orc_params *p)
     p->bfgs_curv_eps = 1e-8;
     p->cluster_rmsd = 2.0;
     p->topk = 10;
+    p->optimizer = 0;
+    p->bb_step = 1.0;
+    p->bb_fallback = 0.1;
 }
 
 /* ---------------------------------------------------------------------------------------
@@ -657,6 +660,54 @@ double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
 }
 
 typedef struct { const orc_params *p; const orc_grid *g; const orc_ligand *L; } dock_ctx;
+/* ---------------------------------------------------------------------------------------
+ * O8' Barzilai-Borwein ("BB only needs a vector inner product to estimate the step
+ * length and does not need to perform line search"; ref. 37).  Reading S13:
+ *   alpha_0 = bb_step / |g_0|;  alpha_k = s.s / s.y  (s = x_k - x_{k-1} in tangent coordinates,
+ *   y = g_k - g_{k-1}) if s.y > curv_eps |s| |y|, else bb_fallback / |g_k|;  alpha_k |g_k| <= bb_step.
+ * ------------------------------------------------------------------------------------- */
+double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
+              orc_objective_fn fn, orc_retract_fn add, void *ctx,
+              double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx)
+{
+    double *x = (double *)malloc(sizeof(double) * np_), *xn = (double *)malloc(sizeof(double) * np_);
+    double *gr = (double *)malloc(sizeof(double) * n), *gn = (double *)malloc(sizeof(double) * n);
+    double *s = (double *)malloc(sizeof(double) * n), *y = (double *)malloc(sizeof(double) * n);
+    int it = 0, ne = 0;
+    memcpy(x, x0, sizeof(double) * np_);
+    double f = fn(ctx, x, gr);
+    ++ne;
+    double fbest = f;
+    memcpy(x_out, x, sizeof(double) * np_);
+    for (it = 0; it < cap; ++it) {
+        double g2 = 0.0;
+        for (int k = 0; k < n; ++k) g2 += gr[k] * gr[k];
+        const double gnorm = sqrt(g2);
+        if (gnorm < p->bfgs_gtol) break;
+        double alpha;
+        if (it == 0) alpha = p->bb_step / gnorm;
+        else {
+            double sy = 0.0, ss = 0.0, yy = 0.0;
+            for (int k = 0; k < n; ++k) { sy += s[k] * y[k]; ss += s[k] * s[k]; yy += y[k] * y[k]; }
+            alpha = (sy > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) ? ss / sy : p->bb_fallback / gnorm;
+        }
+        if (alpha * gnorm > p->bb_step) alpha = p->bb_step / gnorm;
+        for (int k = 0; k < n; ++k) s[k] = -alpha * gr[k];
+        add(ctx, x, s, xn);
+        const double fnew = fn(ctx, xn, gn);
+        ++ne;
+        for (int k = 0; k < n; ++k) { y[k] = gn[k] - gr[k]; gr[k] = gn[k]; }
+        memcpy(x, xn, sizeof(double) * np_);
+        f = fnew;
+        if (obs) obs(obs_ctx, it, f, NULL, s, y, 1);
+        if (f < fbest) { fbest = f; memcpy(x_out, x, sizeof(double) * np_); }
+    }
+    if (iters) *iters = it;
+    if (evals) *evals = ne;
+    free(x); free(xn); free(gr); free(gn); free(s); free(y);
+    return fbest;
+}
+
 static double dock_fn(void *c, const double *x, double *grad)
 {
     dock_ctx *k = (dock_ctx *)c;
@@ -675,7 +726,7 @@ double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L
     double *x0 = (double *)malloc(sizeof(double) * (7 + T));
     memcpy(x0, pose_in, sizeof(double) * (7 + T));
     quat_normalize(x0 + 3);
-    double f = orc_bfgs(p, 6 + T, 7 + T, cap, x0, dock_fn, dock_add, &ctx, pose_out, iters, evals, NULL, NULL);
+    double f = (p->optimizer == 1 ? orc_bb : orc_bfgs)(p, 6 + T, 7 + T, cap, x0, dock_fn, dock_add, &ctx, pose_out, iters, evals, NULL, NULL);
     free(x0);
     return f;
 }

@@ -16,6 +16,8 @@
  *   O5  intra-ligand pair terms        : PAPER.md:49
  *   O6  chain rule to force/torque/torsion derivatives
  *   O8  BFGS local optimisation        : PAPER.md:53 (Vina's BFGS, ref. 36 at 183) -- constants are readings (S12): PARITY UNPINNED for the constants
+ *   O8' Barzilai-Borwein local optimisation : PAPER.md:53 ("only needs a vector inner product ... no line search"), ref. 37 at 184;
+ *       step rule and safeguards are readings (S13): PARITY UNPINNED for the constants, algorithm pinned on quadratics
  *   O9  many-copy Monte-Carlo          : PAPER.md:65-67 (reading S14-S16); search outcome: PARITY UNPINNED beyond GPU-vs-oracle
  *   O10 ranking + RMSD clustering      : PAPER.md:67, 81 (reading S19)
  *   Philox4x32-10                      : Salmon et al. SC'11, as restated in SURVEY.md 8(c) R-rules
@@ -54,6 +56,9 @@ typedef struct {
     double bfgs_curv_eps;   /* skip the update if y.s <= eps*||s||*||y|| */
     double cluster_rmsd;    /* O10 */
     int    topk;            /* O10 */
+    int    optimizer;       /* 0 = BFGS (O8), 1 = Barzilai-Borwein (O8'; reading S13) */
+    double bb_step;         /* O8': length of the first step and cap on every step, pose units (A / rad) */
+    double bb_fallback;     /* O8': step length used when s.y is not safely positive */
 } orc_params;
 
 typedef struct {
@@ -127,6 +132,12 @@ typedef double (*orc_objective_fn)(void *ctx, const double *x, double *grad);
 typedef void   (*orc_retract_fn)(void *ctx, const double *x, const double *s, double *out);
 typedef void   (*orc_observer_fn)(void *ctx, int it, double f, const double *H, const double *s, const double *y, int updated);
 double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
+                orc_objective_fn fn, orc_retract_fn add, void *ctx,
+                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx);
+/* O8': x_{k+1} = x_k (+) (-alpha_k g_k), alpha_0 = bb_step/|g|, alpha_k = s.s/s.y (BB1) when
+ * s.y > curv_eps |s||y| else bb_fallback/|g|, every step capped at length bb_step; one evaluation per iteration,
+ * no line search; returns the best point seen (the method is non-monotone).  Same signature as orc_bfgs. */
+double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
                 orc_objective_fn fn, orc_retract_fn add, void *ctx,
                 double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx);
 

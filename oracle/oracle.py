@@ -51,6 +51,9 @@ class Params(C.Structure):
         ("bfgs_curv_eps", C.c_double),
         ("cluster_rmsd", C.c_double),
         ("topk", C.c_int),
+        ("optimizer", C.c_int),
+        ("bb_step", C.c_double),
+        ("bb_fallback", C.c_double),
     ]
 
 
@@ -139,7 +142,7 @@ def params_as_fp32(p: Params) -> Params:
     for i in range(5):
         q.w[i] = float(np.float32(p.w[i]))
     for name in ("cutoff", "k_wall", "t_mc", "amp_trans", "amp_rot", "bfgs_c1", "bfgs_shrink",
-                 "bfgs_gtol", "bfgs_curv_eps", "cluster_rmsd"):
+                 "bfgs_gtol", "bfgs_curv_eps", "cluster_rmsd", "bb_step", "bb_fallback"):
         setattr(q, name, float(np.float32(getattr(p, name))))
     return q
 
@@ -365,4 +368,35 @@ def bfgs_generic(p: Params, x0, fn, cap: int, observer=None):
     l.orc_bfgs.restype = C.c_double
     f = l.orc_bfgs(C.byref(p), n, n, int(cap), _p(x0), _OBJ_FN(_fn), _ADD_FN(_add), None, _p(out),
                    C.byref(it), C.byref(ne), _OBS_FN(_obs), None)
+    return float(f), out, it.value, ne.value
+
+
+def bb_generic(p: Params, x0, fn, cap: int, observer=None):
+    """Run the oracle's O8' Barzilai-Borwein optimizer on a Python objective fn(x)->(f, grad) with the
+    Euclidean retraction x+s.  observer(it, f, s, y) is optional.  Pin tests only."""
+    x0 = _f64(x0)
+    n = x0.shape[0]
+
+    def _fn(_ctx, xp, gp):
+        x = np.ctypeslib.as_array(xp, shape=(n,))
+        f, g = fn(x.copy())
+        for k in range(n):
+            gp[k] = float(g[k])
+        return float(f)
+
+    def _add(_ctx, xp, sp, op):
+        for k in range(n):
+            op[k] = xp[k] + sp[k]
+
+    def _obs(_ctx, it, f, Hp, sp, yp, updated):
+        if observer is not None:
+            observer(int(it), float(f), np.ctypeslib.as_array(sp, shape=(n,)).copy(),
+                     np.ctypeslib.as_array(yp, shape=(n,)).copy())
+
+    out = np.zeros(n)
+    it, ne = C.c_int(), C.c_int()
+    l = lib()
+    l.orc_bb.restype = C.c_double
+    f = l.orc_bb(C.byref(p), n, n, int(cap), _p(x0), _OBJ_FN(_fn), _ADD_FN(_add), None, _p(out),
+                 C.byref(it), C.byref(ne), _OBS_FN(_obs), None)
     return float(f), out, it.value, ne.value

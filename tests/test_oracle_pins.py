@@ -586,3 +586,71 @@ def test_gradient_conditioning_scale_bounds_the_gradient(orc, tiny):
     _, g1, _, _ = orc.score_batch(op, og, one, p1)
     A1 = orc.grad_cond(op, og, one, p1)
     assert np.allclose(A1[:, :3], np.abs(g1[:, :3]), rtol=1e-12, atol=1e-300) and np.all(A1[:, 3:] < 1e-9)
+
+
+# ----------------------------------------------------------------------------------- O8' Barzilai-Borwein (NEXT-1)
+def test_bb_is_exact_in_two_steps_on_an_isotropic_quadratic(orc):
+    """PAPER.md:53 / ref. 37: for f = c/2 |x - m|^2 the BB1 step s.s/s.y equals 1/c, so the iterate after the
+    first (length-capped) step lands exactly on the minimiser: a closed form no implementation detail can fake."""
+    p = orc.default_params()
+    c, m = 3.7, np.array([0.3, -1.2, 2.0, 0.5])
+    fn = lambda x: (0.5 * c * float((x - m) @ (x - m)), c * (x - m))
+    x0 = m + np.array([1.28, -0.96, 0.0, 0.0])                   # 1.6 away: one capped step (length 1), then 0.6 left
+    steps = []
+    f, x, it, ne = orc.bb_generic(p, x0, fn, 50, observer=lambda i, fv, s, y: steps.append((i, fv, s.copy())))
+    assert np.allclose(x, m, atol=1e-12) and f < 1e-24
+    assert it == 2 and ne == 3                                   # start, capped first step, exact second step, then |g| < gtol
+    assert abs(np.linalg.norm(steps[0][2]) - p.bb_step) < 1e-12   # first step has length bb_step along -g
+    assert np.allclose(steps[0][2] / np.linalg.norm(steps[0][2]), -(x0 - m) / np.linalg.norm(x0 - m))
+
+
+def test_bb_reaches_closed_form_minimiser_of_convex_quadratic_and_returns_best_seen(orc):
+    p = orc.default_params()
+    rng = np.random.default_rng(5)
+    n = 9
+    Q = rng.normal(size=(n, n))
+    A = Q @ Q.T + n * np.eye(n)
+    b = rng.normal(size=n)
+    fn = lambda x: (0.5 * float(x @ A @ x) - float(b @ x), A @ x - b)
+    xs = np.linalg.solve(A, b)
+    hist = []
+    f, x, it, ne = orc.bb_generic(p, rng.normal(size=n) * 3, fn, 400, observer=lambda i, fv, s, y: hist.append((fv, np.linalg.norm(s))))
+    assert np.allclose(x, xs, atol=1e-3 / n) and ne == it + 1    # one evaluation per iteration, no line search
+    fv = np.array([h[0] for h in hist])
+    assert abs(f - min(fv.min(), fn(x)[0])) < 1e-12             # the best point seen is what is returned
+    assert np.any(np.diff(fv) > 0)                               # the method is non-monotone (that is BB)
+    assert max(h[1] for h in hist) <= p.bb_step + 1e-12          # every step is capped
+
+
+def test_bb_secant_step_and_fallback(orc):
+    """alpha_k = s.s / s.y on the observer's (s, y); with negative curvature the fallback length is used."""
+    p = orc.default_params()
+    A = np.diag([1.0, 10.0])
+    fn = lambda x: (0.5 * float(x @ A @ x), A @ x)
+    rec = []
+    orc.bb_generic(p, np.array([0.2, 0.1]), fn, 6, observer=lambda i, fv, s, y: rec.append((s.copy(), y.copy())))
+    # step k+1 = -alpha g_{k+1} with alpha = s_k.s_k / s_k.y_k and g_{k+1} = g_k + y_k
+    g = A @ np.array([0.2, 0.1])
+    for k in range(len(rec) - 1):
+        s, y = rec[k]
+        g = g + y
+        alpha = float(s @ s) / float(s @ y)
+        if alpha * np.linalg.norm(g) <= p.bb_step:
+            assert np.allclose(rec[k + 1][0], -alpha * g, rtol=1e-12, atol=1e-15)
+    conc = lambda x: (-0.5 * float(x @ x), -x)                   # concave: s.y < 0 on every step
+    rec2 = []
+    orc.bb_generic(p, np.array([0.3, 0.4]), conc, 3, observer=lambda i, fv, s, y: rec2.append(np.linalg.norm(s)))
+    assert abs(rec2[0] - p.bb_step) < 1e-12 and all(abs(v - p.bb_fallback) < 1e-12 for v in rec2[1:])
+
+
+def test_bb_local_opt_on_the_docking_objective(orc, tiny):
+    s, op, og, oL = tiny
+    q = orc.params_as_fp32(orc.default_params())
+    q.optimizer = 1
+    rng = np.random.default_rng(3)
+    poses = random_poses(rng, 24, s.box_center, s.box_size * 0.6, oL.T).astype(np.float64)
+    e0 = orc.score_batch(q, og, oL, poses, want_grad=False)[0]
+    for i in range(len(poses)):
+        f, x, it, ne = orc.local_opt(q, og, oL, poses[i], 150)
+        assert f <= e0[i] + 1e-12 and ne == it + 1
+        assert abs(orc.score_batch(q, og, oL, x[None, :], want_grad=False)[0][0] - f) < 1e-9
