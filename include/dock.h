@@ -66,6 +66,9 @@ typedef struct dock_params {
     float   bfgs_curv_eps;                    /* skip the update if y.s <= eps ||s|| ||y|| */
     float   cluster_rmsd;                     /* top-k clustering radius, A (PAPER.md:81 RMSD) */
     int32_t topk;                             /* number of poses to report, <= DOCK_MAX_TOPK */
+    int32_t optimizer;                        /* local optimizer: 0 = BFGS + backtracking, 1 = Barzilai-Borwein */
+    float   bb_step;                          /* BB: length of the first step and cap on every step (A / rad) */
+    float   bb_fallback;                      /* BB: step length when s.y is not safely positive */
 } dock_params;
 
 /* Search / interpolation box: n_axis = round(size/spacing)+1 nodes,

@@ -48,6 +48,8 @@ struct DevParams {
     float amp_trans, amp_rot;
     float c1, shrink, gtol, curv_eps;
     int   max_trials;
+    int   optimizer;           // 0 = BFGS, 1 = Barzilai-Borwein
+    float bb_step, bb_fallback;
     // pair term of the thread-per-pose evaluator (eval_thread.cuh), weights folded into the exponents:
     //   A = 8|w1| exp(-(d/0.5)^2) = ex2(cA d^2 + lw1),   B = |w2|/2 exp(-((d-3)/2)^2) = ex2(cB (d-3)^2 + lw2)
     // with sigma = -sign(w1):  sigma dE/dd = d (A + q B) - 3 q B + c4 min(d,0) + wh' [hyd ramp] + whb' [hb ramp]

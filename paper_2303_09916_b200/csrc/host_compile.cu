@@ -48,6 +48,9 @@ extern "C" int dock_default_params(dock_params *p)
     p->bfgs_curv_eps = 1e-8f;
     p->cluster_rmsd = 2.0f;
     p->topk = 10;
+    p->optimizer = 0;
+    p->bb_step = 1.0f;          // reading S13
+    p->bb_fallback = 0.1f;
     return DOCK_OK;
 }
 
@@ -59,6 +62,8 @@ int dock_validate_params(const dock_params *p)
     if (p->bfgs_max_trials < 1 || p->bfgs_max_trials > 64) return DOCK_EINVAL;
     if (!(p->bfgs_shrink > 0.f && p->bfgs_shrink < 1.f)) return DOCK_EINVAL;
     if (p->topk < 1 || p->topk > DOCK_MAX_TOPK) return DOCK_EINVAL;
+    if (p->optimizer < 0 || p->optimizer > 1) return DOCK_EINVAL;
+    if (p->optimizer == 1 && (!(p->bb_step > 0.f) || !(p->bb_fallback > 0.f))) return DOCK_EINVAL;
     return DOCK_OK;
 }
 
@@ -77,6 +82,9 @@ int dock_make_dev_params(const dock_params *p, DevParams *o)
     o->gtol = p->bfgs_gtol;
     o->curv_eps = p->bfgs_curv_eps;
     o->max_trials = p->bfgs_max_trials;
+    o->optimizer = p->optimizer;
+    o->bb_step = p->bb_step;
+    o->bb_fallback = p->bb_fallback;
     const double s1 = p->w[0] < 0.f ? -1.0 : 1.0, s2 = p->w[1] < 0.f ? -1.0 : 1.0;
     o->lw1 = p->w[0] != 0.f ? (float)std::log2(8.0 * std::fabs((double)p->w[0])) : -INFINITY;
     o->lw2 = p->w[1] != 0.f ? (float)std::log2(0.5 * std::fabs((double)p->w[1])) : -INFINITY;

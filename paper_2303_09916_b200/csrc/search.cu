@@ -111,9 +111,11 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
     __syncwarp();
     for (int k = lane; k < np_; k += 32) b.xt[k] = b.x[k];
     __syncwarp();
-    float f = 0.0f, alpha = 1.0f;
+    float f = 0.0f, alpha = 1.0f, f_best = 0.0f;
     double gp = 0.0;
     bool init = true, fresh = true;
+    const bool bb = P.optimizer == 1;          // Barzilai-Borwein (reading S13): no H, no line search;
+    float *const x_best = b.H;                 // the best point seen is kept in the (unused) H buffer
     int it = 0, trial = 0;
     evals = 0;
     for (;;) {
@@ -123,7 +125,25 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
             init = false;
             f = ft;
             for (int r = lane; r < n; r += 32) b.g[r] = b.gt[r];
-            set_identity(b.H, n, 1.0f);
+            if (bb) {
+                f_best = f;
+                for (int k = lane; k < np_; k += 32) x_best[k] = b.x[k];
+                __syncwarp();
+            } else set_identity(b.H, n, 1.0f);
+        } else if (bb) {                           // every BB step is taken: s = alpha d, y = g_new - g
+            for (int r = lane; r < n; r += 32) {
+                b.d[r] = alpha * b.d[r];
+                b.y[r] = b.gt[r] - b.g[r];
+                b.g[r] = b.gt[r];
+            }
+            for (int k = lane; k < np_; k += 32) b.x[k] = b.xt[k];
+            f = ft;
+            if (f < f_best) {
+                f_best = f;
+                for (int k = lane; k < np_; k += 32) x_best[k] = b.xt[k];
+            }
+            __syncwarp();
+            ++it;
         } else if ((double)ft - (double)f <= (double)P.c1 * (double)alpha * gp) {   // Armijo: accept the step
             double ys = 0.0, yy = 0.0, ss = 0.0;
             for (int r = lane; r < n; r += 32) {
@@ -173,6 +193,27 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
         for (int r = lane; r < n; r += 32) acc += (double)b.g[r] * (double)b.g[r];
         const double gn2 = warp_sum_d(acc);
         if (sqrt(gn2) < (double)P.gtol) break;
+        if (bb) {
+            const double gnorm = sqrt(gn2);
+            double al;
+            if (it == 0) al = (double)P.bb_step / gnorm;
+            else {
+                double sy = 0.0, ss = 0.0, yy = 0.0;
+                for (int r = lane; r < n; r += 32) {
+                    const double sv = (double)b.d[r], yv = (double)b.y[r];
+                    sy += sv * yv; ss += sv * sv; yy += yv * yv;
+                }
+                sy = warp_sum_d(sy); ss = warp_sum_d(ss); yy = warp_sum_d(yy);
+                al = (sy > (double)P.curv_eps * sqrt(ss) * sqrt(yy)) ? ss / sy : (double)P.bb_fallback / gnorm;
+            }
+            if (al * gnorm > (double)P.bb_step) al = (double)P.bb_step / gnorm;
+            alpha = (float)al;
+            __syncwarp();
+            for (int r = lane; r < n; r += 32) b.d[r] = -b.g[r];
+            __syncwarp();
+            pose_add_warp(T, b.x, b.d, alpha, b.xt);
+            continue;
+        }
         for (int r = lane; r < n; r += 32) {
             float a = 0.0f;
             for (int c = 0; c < n; ++c) a = fmaf(b.H[r * n + c], b.g[c], a);
@@ -198,6 +239,12 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
         }
         trial = 0;
         pose_add_warp(T, b.x, b.d, alpha, b.xt);
+    }
+    if (bb) {                                      // non-monotone method: report the best point seen
+        __syncwarp();
+        for (int k = lane; k < np_; k += 32) b.x[k] = x_best[k];
+        __syncwarp();
+        f = f_best;
     }
     iters = it;
     return f;

@@ -466,3 +466,66 @@ def test_config4_large_box_grid_score_and_search_properties(dk, orc, torch):
     assert np.all(np.abs(te - oe3)[ok] <= tol(oe3)[ok])
     assert np.all(np.diff(te) >= 0)
     _log("search_cfg4", dict(copies=s.copies, steps=steps, evals=int(r1["evals"][0]), best=float(te[0])))
+
+
+# ----------------------------------------------------------------------------------- NEXT-1: Barzilai-Borwein
+@pytest.mark.parametrize("cfg,n", [(0, 256), (1, 256)])
+def test_bb_local_opt(dk, orc, torch, tiny, micro, cfg, n):
+    """The paper's own local optimizer (reading S13) on both sides: one evaluation per iteration,
+    best point seen returned.  Deterministic prefix (1 and 2 iterations) against the oracle under S20; the
+    free-running 150-iteration result as a distribution (BB is non-monotone, so round-off decides the path)."""
+    s, (p0, box, grid, lig), (op0, og, oL) = tiny if cfg == 0 else micro
+    p = dk.dock_default_params()
+    p.optimizer = 1
+    op = orc.params_as_fp32(orc.default_params())
+    op.optimizer = 1
+    rng = np.random.default_rng(17)
+    poses = random_poses(rng, n, s.box_center, s.box_size * 0.6, lig.T)
+    pd = torch.from_numpy(poses).cuda()
+    e0 = orc.score_batch(op, og, oL, poses.astype(np.float64), want_grad=False)[0]
+    for cap in (1, 2):
+        o, e, it = dk.dock_local_opt_batch(p, grid, lig, pd, cap)
+        ref = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), cap)[0] for i in range(n)])
+        chk, _, _, dg = orc.score_batch(op, og, oL, o.cpu().numpy().astype(np.float64))
+        ok = dg["cutoff_margin"] > KINK_MARGIN
+        ge = e.cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(ge - chk)[ok] <= tol(chk)[ok])                  # reported E = E of the reported pose
+        assert np.all(it.cpu().numpy()[:, 1] == it.cpu().numpy()[:, 0] + 1)  # evaluations = iterations + 1
+        agree = (np.abs(ge - ref) <= 10 * tol(ref))[ok]
+        assert agree.mean() >= 0.97, (cap, float(agree.mean()))
+    cap = 150
+    o, e, it = dk.dock_local_opt_batch(p, grid, lig, pd, cap)
+    ge = e.cpu().numpy().astype(np.float64)
+    ref = [orc.local_opt(op, og, oL, poses[i].astype(np.float64), cap) for i in range(n)]
+    re_ = np.array([r[0] for r in ref])
+    chk, _, _, dg = orc.score_batch(op, og, oL, o.cpu().numpy().astype(np.float64))
+    ok = dg["cutoff_margin"] > KINK_MARGIN
+    assert np.all(np.abs(ge - chk)[ok] <= tol(chk)[ok])
+    assert np.all(ge <= e0 + tol(e0))                                        # best-seen never exceeds the start
+    qg, qr = np.quantile(ge, [0.25, 0.5, 0.75]), np.quantile(re_, [0.25, 0.5, 0.75])
+    st = dict(cfg=cfg, n=n, cap=cap, agree_1e3=float((np.abs(ge - re_) <= 1e-3).mean()),
+              gpu_quartiles=qg.tolist(), ref_quartiles=qr.tolist(), gpu_mean=float(ge.mean()), ref_mean=float(re_.mean()),
+              gpu_iters=float(it.cpu().numpy()[:, 0].mean()), ref_iters=float(np.mean([r[2] for r in ref])))
+    _log("bb_local_opt", st)
+    assert np.all(np.abs(qg - qr) <= 0.75 + 0.15 * np.abs(qr)), st
+
+
+def test_bb_search_properties(dk, orc, torch, tiny):
+    """Search driven by BB: bitwise determinism, zero steps = local optimum of the start, winners re-scored by the oracle."""
+    s, (p0, box, grid, lig), (op0, og, oL) = tiny
+    p = dk.dock_default_params()
+    p.optimizer = 1
+    r1 = dk.dock_search(p, [grid], [lig], [box], s.copies, s.steps, 150, 5)
+    r2 = dk.dock_search(p, [grid], [lig], [box], s.copies, s.steps, 150, 5)
+    assert torch.equal(r1["best_e"], r2["best_e"]) and torch.equal(r1["best_pose"], r2["best_pose"])
+    r0 = dk.dock_search(p, [grid], [lig], [box], s.copies, 0, 150, 5)
+    assert bool((r1["best_e"] <= r0["best_e"] + 1e-6).all())
+    k = int(r1["topk_count"][0])
+    tp = r1["topk_pose"][0, :k].cpu().numpy().astype(np.float64)
+    te = r1["topk_e"][0, :k].cpu().numpy()
+    op = orc.params_as_fp32(orc.default_params())
+    oe, _, _, d = orc.score_batch(op, og, oL, tp)
+    ok = d["cutoff_margin"] > KINK_MARGIN
+    assert np.all(np.abs(te - oe)[ok] <= tol(oe)[ok])
+    ev = int(r1["evals"][0])
+    _log("bb_search", dict(copies=s.copies, steps=s.steps, evals=ev, best=float(te[0])))
