@@ -358,8 +358,8 @@ def run_ours(args) -> dict:
 
 
 # per-launch DRAM traffic of the score kernel from the committed `ncu --set full` capture
-# (profiles/r1f_score_thread_kernel_details.txt, commit 43d6884).
-TRAFFIC_BYTES_PER_LAUNCH = 823.1e6   # profiles/r1f.md: dram__bytes_read.sum 756.75 MB + dram__bytes_write.sum 66.37 MB
+# (profiles/r1i_score_thread_kernel_details.txt, commit 917e8f1).
+TRAFFIC_BYTES_PER_LAUNCH = 823.0e6   # profiles/r1i.md: dram__bytes_read.sum 757.2 MB + dram__bytes_write.sum 65.8 MB
 
 
 def main():
