@@ -171,37 +171,3 @@ __device__ __forceinline__ float trilinear(const DevGrid &G, const CellRef &c,
     e_wall = fmaf(G.kw_e, fmaf(c.ox, c.ox, fmaf(c.oy, c.oy, c.oz * c.oz)), e_wall);   // k h^2 * sum overshoot_cells^2
     return e;
 }
-
-// ---- pose algebra shared by the search kernels ------------------------------------------------------
-constexpr float PI_F = 3.14159265358979323846f;
-
-// u = (r >> 8) 2^-24: exact in fp32 and fp64 (R-rules)
-__device__ __forceinline__ float u24(uint32_t r) { return (float)(r >> 8) * (1.0f / 16777216.0f); }
-
-__device__ __forceinline__ void quat_mul_norm(float aw, float ax, float ay, float az,
-                                              float bw, float bx, float by, float bz, float *out)
-{
-    float w = aw * bw - ax * bx - ay * by - az * bz;
-    float x = aw * bx + ax * bw + ay * bz - az * by;
-    float y = aw * by - ax * bz + ay * bw + az * bx;
-    float z = aw * bz + ax * by - ay * bx + az * bw;
-    const float inv = 1.0f / sqrtf(w * w + x * x + y * y + z * z);
-    out[0] = w * inv; out[1] = x * inv; out[2] = y * inv; out[3] = z * inv;
-}
-
-// q <- normalize(quat(rotation vector w) (x) q)   (left-multiplied, lab frame)
-__device__ __forceinline__ void rotate_quat(float wx, float wy, float wz, const float *q, float *out)
-{
-    const float phi = sqrtf(wx * wx + wy * wy + wz * wz);
-    float qw, s;
-    if (phi < 1e-6f) { qw = 1.0f; s = 0.5f; }
-    else {
-        float sn, cs;
-        sincosf(0.5f * phi, &sn, &cs);
-        qw = cs; s = sn / phi;
-    }
-    float ax = s * wx, ay = s * wy, az = s * wz;
-    const float inv = 1.0f / sqrtf(qw * qw + ax * ax + ay * ay + az * az);
-    quat_mul_norm(qw * inv, ax * inv, ay * inv, az * inv, q[0], q[1], q[2], q[3], out);
-}
-
