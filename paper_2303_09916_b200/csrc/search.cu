@@ -276,7 +276,9 @@ local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap
 // ---- A7 Monte-Carlo ------------------------------------------------------------------------------
 __device__ __forceinline__ float u24(uint32_t r) { return (float)(r >> 8) * (1.0f / 16777216.0f); }
 
-__global__ void __launch_bounds__(SEARCH_WARPS * 32)
+// 4 CTAs per SM = 128 registers, no spills: 16 resident warps for the screening batches (143 vs 126 M evals/s on a
+// 64-system config-3 slice), same latency for the 384-copy case (profiles/r1i.md)
+__global__ void __launch_bounds__(SEARCH_WARPS * 32, 4)
 search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems, int copies, int steps,
               int cap, uint32_t seed_lo, uint32_t seed_hi, int t_max, int warp_floats,
               const float *__restrict__ init, float *__restrict__ best_pose, float *__restrict__ best_e,
