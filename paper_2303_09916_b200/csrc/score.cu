@@ -76,12 +76,13 @@ int launch(const ScorePlan &pl, long long n_poses, const float *poses_dev, float
 
 // `ws` receives the overflow schedule (if any); pl.L.sched_global is pointed at it.
 int score_launch(ScorePlan &pl, long long n_poses, const float *poses_dev, float *energy_dev, float *grad_dev,
-                 float *terms_dev, void *ws, cudaStream_t stream)
+                 float *terms_dev, void *ws, cudaStream_t stream, bool upload = true)
 {
     if (n_poses < 1) return DOCK_OK;
     if (!pl.L.sched_in_param) {
-        DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.overflow.data(), pl.overflow.size() * sizeof(uint4),
-                                        cudaMemcpyHostToDevice, stream));
+        if (upload)
+            DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.overflow.data(), pl.overflow.size() * sizeof(uint4),
+                                            cudaMemcpyHostToDevice, stream));
         pl.L.sched_global = (const uint4 *)ws;
         return grad_dev ? launch<true, false>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream)
                         : launch<false, false>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
@@ -132,12 +133,44 @@ extern "C" int dock_score_batch_host(const dock_params *params, const dock_grid 
     float *d_pose = (float *)(ws + b_blob), *d_e = (float *)(ws + b_blob + b_pose);
     float *d_g = grad_host ? (float *)(ws + b_blob + b_pose + b_e) : nullptr;
     float *d_t = terms_host ? (float *)(ws + b_blob + b_pose + b_e + b_g) : nullptr;
-    DOCK_CUDA_CHECK(cudaMemcpyAsync(d_pose, poses_host, (size_t)n_poses * np_ * sizeof(float), cudaMemcpyHostToDevice, stream));
-    const int rc2 = score_launch(pl, n_poses, d_pose, d_e, d_g, d_t, ws, stream);
-    if (rc2 != DOCK_OK) return rc2;
-    DOCK_CUDA_CHECK(cudaMemcpyAsync(energy_host, d_e, (size_t)n_poses * sizeof(float), cudaMemcpyDeviceToHost, stream));
-    if (grad_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(grad_host, d_g, (size_t)n_poses * ng * sizeof(float), cudaMemcpyDeviceToHost, stream));
-    if (terms_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(terms_host, d_t, (size_t)n_poses * 3 * sizeof(float), cudaMemcpyDeviceToHost, stream));
+    // Three-stage pipeline over chunks of the batch: host->device copies on one side stream, kernels on the
+    // caller's stream, device->host copies on another side stream, so that PCIe in, compute and PCIe out
+    // overlap (the buses are full duplex).  The side streams and events belong to the library and are created once.
+    static cudaStream_t s_in = nullptr, s_out = nullptr;
+    constexpr int MAX_CHUNKS = 8;
+    static cudaEvent_t ev_in[MAX_CHUNKS], ev_k[MAX_CHUNKS], ev_begin, ev_end;
+    if (!s_in) {
+        DOCK_CUDA_CHECK(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+        DOCK_CUDA_CHECK(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+        for (int c = 0; c < MAX_CHUNKS; ++c) {
+            DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming));
+            DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_k[c], cudaEventDisableTiming));
+        }
+        DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
+        DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
+    }
+    const int n_chunks = (int)std::min<int64_t>(MAX_CHUNKS, (n_poses + 65535) / 65536);      // >= 64 Ki poses per chunk
+    const int64_t per = ((n_poses + n_chunks - 1) / n_chunks + 31) / 32 * 32;
+    DOCK_CUDA_CHECK(cudaEventRecord(ev_begin, stream));                  // the workspace may still be in use upstream
+    DOCK_CUDA_CHECK(cudaStreamWaitEvent(s_in, ev_begin, 0));
+    DOCK_CUDA_CHECK(cudaStreamWaitEvent(s_out, ev_begin, 0));
+    for (int c = 0; c < n_chunks; ++c) {
+        const int64_t o = c * per, m = std::min<int64_t>(per, n_poses - o);
+        if (m <= 0) break;
+        DOCK_CUDA_CHECK(cudaMemcpyAsync(d_pose + o * np_, poses_host + o * np_, (size_t)m * np_ * sizeof(float), cudaMemcpyHostToDevice, s_in));
+        DOCK_CUDA_CHECK(cudaEventRecord(ev_in[c], s_in));
+        DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, ev_in[c], 0));
+        const int rc2 = score_launch(pl, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr, d_t ? d_t + o * 3 : nullptr,
+                                     ws, stream, c == 0);
+        if (rc2 != DOCK_OK) return rc2;
+        DOCK_CUDA_CHECK(cudaEventRecord(ev_k[c], stream));
+        DOCK_CUDA_CHECK(cudaStreamWaitEvent(s_out, ev_k[c], 0));
+        DOCK_CUDA_CHECK(cudaMemcpyAsync(energy_host + o, d_e + o, (size_t)m * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+        if (grad_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(grad_host + o * ng, d_g + o * ng, (size_t)m * ng * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+        if (terms_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(terms_host + o * 3, d_t + o * 3, (size_t)m * 3 * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+    }
+    DOCK_CUDA_CHECK(cudaEventRecord(ev_end, s_out));
+    DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, ev_end, 0));
     DOCK_CUDA_CHECK(cudaStreamSynchronize(stream));
     return DOCK_OK;
 }
