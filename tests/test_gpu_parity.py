@@ -137,9 +137,11 @@ def test_score_edge_cases(dk, orc, torch, tiny):
     assert np.all(np.abs(g3.cpu().numpy() - ograd) <= tol(ograd))
 
 
-@pytest.mark.parametrize("N,T", [(1, 0), (5, 0), (33, 3), (60, 15), (100, 9)])
+@pytest.mark.parametrize("N,T", [(1, 0), (5, 0), (33, 3), (60, 15), (100, 9), (128, 32)])
 def test_score_other_ligand_shapes(dk, orc, torch, micro, N, T):
-    """Degenerate and large ligands on the config-1 grid: single atom, rigid, N > 32 (two atoms per lane), T = 15."""
+    """Degenerate and large ligands on the config-1 grid: single atom, rigid, N > 32 (two atoms per lane), T = 15,
+    and the maxima of include/dock.h (N = 128, T = 32: the pair schedule overflows the kernel-parameter bank and is
+    read from global memory)."""
     s0, (p, box, grid, _), (op, og, _) = micro
     import dock_synth
     from dock_synth.generators import LIG_TYPES_FULL
@@ -529,3 +531,26 @@ def test_bb_search_properties(dk, orc, torch, tiny):
     assert np.all(np.abs(te - oe)[ok] <= tol(oe)[ok])
     ev = int(r1["evals"][0])
     _log("bb_search", dict(copies=s.copies, steps=s.steps, evals=ev, best=float(te[0])))
+
+
+def test_maximum_ligand_size_local_opt_and_search(dk, orc, torch, micro):
+    """DOCK_MAX_ATOMS x DOCK_MAX_TORSIONS through the optimizer and the search (4 atoms per lane, 38 x 38 inverse
+    Hessian per warp): the optimizer never raises the energy, the reported energies are the oracle's energies of the
+    reported poses, the search is deterministic."""
+    s0, (p, box, grid, _), (op, og, _) = micro
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    rng = np.random.default_rng(228)
+    ligd = dock_synth.make_ligand(rng, 128, 32, LIG_TYPES_FULL)
+    lig, oL = dk.LigandHandle(ligd), orc.Ligand(ligd)
+    poses = random_poses(rng, 64, s0.box_center, s0.box_size * 0.5, 32)
+    e0, _, _ = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    o, e, it = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), 30)
+    assert bool((e <= e0 + 1e-3 + 1e-4 * e0.abs()).all())
+    chk, _, _, dg = orc.score_batch(op, og, oL, o.cpu().numpy().astype(np.float64))
+    ok = dg["cutoff_margin"] > KINK_MARGIN
+    assert ok.any() and np.all(np.abs(e.cpu().numpy() - chk)[ok] <= tol(chk)[ok])
+    r1 = dk.dock_search(p, [grid], [lig], [box], 32, 2, 20, 9)
+    r2 = dk.dock_search(p, [grid], [lig], [box], 32, 2, 20, 9)
+    assert torch.equal(r1["best_e"], r2["best_e"]) and int(r1["topk_count"][0]) >= 1
+    assert bool(torch.isfinite(r1["best_e"]).all())
