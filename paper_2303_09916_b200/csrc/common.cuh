@@ -118,11 +118,11 @@ struct DevSystem {
 //                      n2_hb | n1_hb << 8 | n_live << 16, 0}
 //             then per class (plain, hyd, hb) n2 double records and n1 (0/1) single records.
 //   record  : one partner slot j against the 4 tile atoms.  A pair that is not listed gets
-//             R_i+R_j = TPP_MASKED_RSUM: its surface distance is then +1e18 and every term and
+//             -(R_i+R_j) = -TPP_MASKED_RSUM: its surface distance is then +1e18 and every term and
 //             derivative evaluates to exactly 0 -- no mask test in the instruction stream.
 //             class plain: no pair of the record has a hydrophobic or H-bond term; hyd: some pair has
 //             the hydrophobic term, none the H-bond term; hb: some pair has the H-bond term.
-//     single : {j, 0, 0, 0} {rsum[4]} [{wh'[4]}  (hyd, hb)] [{whb'[4]}  (hb)]
+//     single : {j, 0, 0, 0} {-rsum[4]} [{wh'[4]}  (hyd, hb)] [{whb'[4]}  (hb)]      (the NEGATED radius sum: d = r + (-rsum))
 //     double : {jA, jB, 0, 0} then the single-record payload of A, then that of B
 //   j is stored as the byte offset of the slot's z column (j * 128); the (x,y) column is at twice that.
 //   wh' = -sigma w4 or 0, whb' = -sigma w5 / 0.7 or 0 per pair (see DevParams).
@@ -162,6 +162,45 @@ __device__ __forceinline__ void ldg_cell(const Cell8 *p, float4 &lo, float4 &hi)
     hi.x = __uint_as_float((unsigned)c); hi.y = __uint_as_float((unsigned)(c >> 32));
     hi.z = __uint_as_float((unsigned)d); hi.w = __uint_as_float((unsigned)(d >> 32));
 }
+// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2) ------------------------------------
+// Two IEEE fp32 operations in ONE issue slot (the FMA pipe still spends two cycles): the thread-per-pose
+// evaluator is bound by issue slots, not by the FMA pipe, so its pair arithmetic runs on register pairs
+// (profiles/r1j.md).  Scalars, immediates and uniform registers broadcast for free in SASS.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ f32x2 bc2(float v) { return pk2(v, v); }
+__device__ __forceinline__ void up2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ float sum2(f32x2 v) { float a, b; up2(v, a, b); return a + b; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 __device__ __forceinline__ float fast_ex2(float x)
 {
     float y;

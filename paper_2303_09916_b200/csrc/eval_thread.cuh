@@ -58,18 +58,21 @@ __device__ __forceinline__ uint4 tpp_quad(const TppLigand &L, int pos)
 }
 
 // Accumulators of the pair phase (DevParams): E_intra = eA a + eB b + sigma/2 rep - sigma hyd - 0.7 sigma hb.
+// Packed pairs: the two halves belong to tile atoms (0,1) / (2,3) and are added at the very end.
 struct PairAcc {
-    float a, b, rep, hyd, hb;
+    f32x2 a, b, rep, hyd, hb;
 };
 
-// The register tile of the pair phase: TPP_TILE atoms with their force accumulators.
+// The register tile of the pair phase: TPP_TILE = 4 atoms as two packed halves h = 0: atoms (0,1), h = 1: atoms
+// (2,3), with their force accumulators.
 struct PairTile {
-    float x[TPP_TILE], y[TPP_TILE], z[TPP_TILE], fx[TPP_TILE], fy[TPP_TILE], fz[TPP_TILE];
+    f32x2 x[2], y[2], z[2], fx[2], fy[2], fz[2];
 };
 
-__device__ __forceinline__ void quad_floats(const uint4 q, float v[4])
+__device__ __forceinline__ void quad_halves(const uint4 q, f32x2 v[2])
 {
-    v[0] = __uint_as_float(q.x); v[1] = __uint_as_float(q.y); v[2] = __uint_as_float(q.z); v[3] = __uint_as_float(q.w);
+    v[0] = pk2(__uint_as_float(q.x), __uint_as_float(q.y));
+    v[1] = pk2(__uint_as_float(q.z), __uint_as_float(q.w));
 }
 
 // A partner atom's coordinates and force accumulator, read one record ahead (record_class).
@@ -104,15 +107,15 @@ __device__ __forceinline__ void record_block(const DevParams &P, const TppLigand
                                              const PartnerRegs *pre = nullptr)
 {
     constexpr int S = 1 + CLS;                 // payload quads of one record
-    constexpr int NQ = NP * TPP_TILE;          // pairs of the block; pair p = partner p / TPP_TILE, tile atom p % TPP_TILE
+    constexpr int NC = NP * 2;                 // packed chains of the block; chain c = partner c / 2, tile half c % 2
     const uint4 h = tpp_quad<SCHED_PARAM>(L, pos);
     const unsigned off[2] = {h.x, h.y};
-    float rs[NQ], wh[NQ], wb[NQ];
+    f32x2 nrs[NC], wh[NC], wb[NC];
 #pragma unroll
     for (int a = 0; a < NP; ++a) {
-        quad_floats(tpp_quad<SCHED_PARAM>(L, pos + 1 + a * S), rs + a * TPP_TILE);
-        if (CLS >= 1) quad_floats(tpp_quad<SCHED_PARAM>(L, pos + 2 + a * S), wh + a * TPP_TILE);
-        if (CLS >= 2) quad_floats(tpp_quad<SCHED_PARAM>(L, pos + 3 + a * S), wb + a * TPP_TILE);
+        quad_halves(tpp_quad<SCHED_PARAM>(L, pos + 1 + a * S), nrs + 2 * a);
+        if (CLS >= 1) quad_halves(tpp_quad<SCHED_PARAM>(L, pos + 2 + a * S), wh + 2 * a);
+        if (CLS >= 2) quad_halves(tpp_quad<SCHED_PARAM>(L, pos + 3 + a * S), wb + 2 * a);
     }
     pos += 1 + NP * S;
     float jx[NP], jy[NP], jz[NP];
@@ -124,66 +127,86 @@ __device__ __forceinline__ void record_block(const DevParams &P, const TppLigand
             jx[a] = c.x; jy[a] = c.y; jz[a] = *reinterpret_cast<const float *>(zz + off[a]);
         }
     }
-    float dx[NQ], dy[NQ], dz[NQ], r2[NQ], rinv[NQ], d[NQ], argA[NQ], argB[NQ], c4m[NQ], eA[NQ], eB[NQ];
+    f32x2 dx[NC], dy[NC], dz[NC], r2[NC], rinv[NC], d[NC], argA[NC], argB[NC], c4m[NC], eA[NC], eB[NC];
 #pragma unroll
-    for (int p = 0; p < NQ; ++p) {
-        const int a = p / TPP_TILE, k = p % TPP_TILE;
-        dx[p] = t.x[k] - jx[a]; dy[p] = t.y[k] - jy[a]; dz[p] = t.z[k] - jz[a];
-        r2[p] = fmaf(dz[p], dz[p], fmaf(dy[p], dy[p], fmaf(dx[p], dx[p], 1e-12f)));
+    for (int c = 0; c < NC; ++c) {
+        const int a = c / 2, hf = c % 2;
+        dx[c] = sub2(t.x[hf], bc2(jx[a])); dy[c] = sub2(t.y[hf], bc2(jy[a])); dz[c] = sub2(t.z[hf], bc2(jz[a]));
+        r2[c] = fma2(dz[c], dz[c], fma2(dy[c], dy[c], fma2(dx[c], dx[c], bc2(1e-12f))));
     }
 #pragma unroll
-    for (int p = 0; p < NQ; ++p) rinv[p] = fast_rsqrt(r2[p]);
+    for (int c = 0; c < NC; ++c) {
+        float r0, r1;
+        up2(r2[c], r0, r1);
+        rinv[c] = pk2(fast_rsqrt(r0), fast_rsqrt(r1));
+    }
 #pragma unroll
-    for (int p = 0; p < NQ; ++p) {
-        const int a = p / TPP_TILE;
+    for (int c = 0; c < NC; ++c) {
+        const int a = c / 2;
         // out of range (r >= cutoff, decided on r^2 in fp32) -> the same "infinitely far" surface distance as a
         // masked pair: every term and derivative below is then exactly 0, with no branch in the instruction stream
-        d[p] = (r2[p] < P.cutoff2) ? fmaf(r2[p], rinv[p], -rs[p]) : 1.0e18f;
-        argA[p] = fmaf(d[p] * -5.770780163555854f, d[p], P.lw1);                 // log2 of 8|w1| exp(-(d/0.5)^2)
+        const f32x2 d0 = fma2(r2[c], rinv[c], nrs[c]);
+        float r0, r1, d0l, d0h;
+        up2(r2[c], r0, r1);
+        up2(d0, d0l, d0h);
+        const float dl = (r0 < P.cutoff2) ? d0l : 1.0e18f, dh = (r1 < P.cutoff2) ? d0h : 1.0e18f;
+        d[c] = pk2(dl, dh);
+        argA[c] = fma2(mul2(d[c], bc2(-5.770780163555854f)), d[c], bc2(P.lw1));  // log2 of 8|w1| exp(-(d/0.5)^2)
         // -log2(e)/4 (d-3)^2 + lw2 expanded in d
-        argB[p] = fmaf(d[p], fmaf(d[p], -0.36067376022224085f, 2.1640425613334453f), P.lw2 - 3.2460638420001677f);
-        const float m = fminf(d[p], 0.0f);
-        c4m[p] = P.c4 * m;
-        acc[a].rep = fmaf(c4m[p], m, acc[a].rep);
+        argB[c] = fma2(d[c], fma2(d[c], bc2(-0.36067376022224085f), bc2(2.1640425613334453f)), bc2(P.lw2 - 3.2460638420001677f));
+        const f32x2 m = pk2(fminf(dl, 0.0f), fminf(dh, 0.0f));
+        c4m[c] = mul2(m, bc2(P.c4));
+        acc[a].rep = fma2(c4m[c], m, acc[a].rep);
     }
 #pragma unroll
-    for (int p = 0; p < NQ; ++p) { eA[p] = fast_ex2(argA[p]); eB[p] = fast_ex2(argB[p]); }
-    float gx[NP], gy[NP], gzz[NP];
+    for (int c = 0; c < NC; ++c) {
+        float a0, a1, b0, b1;
+        up2(argA[c], a0, a1);
+        up2(argB[c], b0, b1);
+        eA[c] = pk2(fast_ex2(a0), fast_ex2(a1));
+        eB[c] = pk2(fast_ex2(b0), fast_ex2(b1));
+    }
+    f32x2 gx[NP], gy[NP], gzz[NP];                 // force on the partner, sign flipped (subtracted at the end)
 #pragma unroll
-    for (int a = 0; a < NP; ++a) gx[a] = gy[a] = gzz[a] = 0.0f;
+    for (int a = 0; a < NP; ++a) gx[a] = gy[a] = gzz[a] = bc2(0.0f);
 #pragma unroll
-    for (int p = 0; p < NQ; ++p) {
-        const int a = p / TPP_TILE, k = p % TPP_TILE;
-        acc[a].a += eA[p];
-        acc[a].b += eB[p];
-        float de = fmaf(d[p], fmaf(P.q, eB[p], eA[p]), fmaf(P.m3q, eB[p], c4m[p]));   // sigma dE/dd
+    for (int c = 0; c < NC; ++c) {
+        const int a = c / 2, hf = c % 2;
+        acc[a].a = add2(acc[a].a, eA[c]);
+        acc[a].b = add2(acc[a].b, eB[c]);
+        f32x2 de = fma2(d[c], fma2(bc2(P.q), eB[c], eA[c]), fma2(bc2(P.m3q), eB[c], c4m[c]));   // sigma dE/dd
         if (CLS >= 1) {
-            const float th = 1.5f - d[p], hh = __saturatef(th);                   // hydrophobic: 1 | 1.5 - d | 0
-            acc[a].hyd = fmaf(wh[p], hh, acc[a].hyd);
-            de = fmaf(wh[p], (hh == th) ? 1.0f : 0.0f, de);                       // on the ramp iff the clamp did nothing
+            float t0, t1;
+            up2(sub2(bc2(1.5f), d[c]), t0, t1);                                   // hydrophobic: 1 | 1.5 - d | 0
+            const float h0 = __saturatef(t0), h1 = __saturatef(t1);
+            acc[a].hyd = fma2(wh[c], pk2(h0, h1), acc[a].hyd);
+            de = fma2(wh[c], pk2((h0 == t0) ? 1.0f : 0.0f, (h1 == t1) ? 1.0f : 0.0f), de);   // on the ramp iff the clamp did nothing
         }
         if (CLS >= 2) {
-            const float tb = d[p] * -1.4285714285714286f, hb = __saturatef(tb);   // H-bond: 1 | -d/0.7 | 0
-            acc[a].hb = fmaf(wb[p], hb, acc[a].hb);
-            de = fmaf(wb[p], (hb == tb) ? 1.0f : 0.0f, de);
+            float t0, t1;
+            up2(mul2(d[c], bc2(-1.4285714285714286f)), t0, t1);                   // H-bond: 1 | -d/0.7 | 0
+            const float h0 = __saturatef(t0), h1 = __saturatef(t1);
+            acc[a].hb = fma2(wb[c], pk2(h0, h1), acc[a].hb);
+            de = fma2(wb[c], pk2((h0 == t0) ? 1.0f : 0.0f, (h1 == t1) ? 1.0f : 0.0f), de);
         }
         if (WANT_GRAD) {
-            const float kk = de * rinv[p];
-            t.fx[k] = fmaf(kk, dx[p], t.fx[k]); t.fy[k] = fmaf(kk, dy[p], t.fy[k]); t.fz[k] = fmaf(kk, dz[p], t.fz[k]);
-            gx[a] = fmaf(-kk, dx[p], gx[a]); gy[a] = fmaf(-kk, dy[p], gy[a]); gzz[a] = fmaf(-kk, dz[p], gzz[a]);
+            const f32x2 kk = mul2(de, rinv[c]);
+            t.fx[hf] = fma2(kk, dx[c], t.fx[hf]); t.fy[hf] = fma2(kk, dy[c], t.fy[hf]); t.fz[hf] = fma2(kk, dz[c], t.fz[hf]);
+            gx[a] = fma2(kk, dx[c], gx[a]); gy[a] = fma2(kk, dy[c], gy[a]); gzz[a] = fma2(kk, dz[c], gzz[a]);
         }
     }
     if (WANT_GRAD) {
 #pragma unroll
         for (int a = 0; a < NP; ++a) {
+            const float sx = sum2(gx[a]), sy = sum2(gy[a]), sz = sum2(gzz[a]);
             if (PRE) {
-                *reinterpret_cast<float2 *>(gxy + 2 * off[a]) = make_float2(pre[a].gx + gx[a], pre[a].gy + gy[a]);
-                *reinterpret_cast<float *>(gz + off[a]) = pre[a].gz + gzz[a];
+                *reinterpret_cast<float2 *>(gxy + 2 * off[a]) = make_float2(pre[a].gx - sx, pre[a].gy - sy);
+                *reinterpret_cast<float *>(gz + off[a]) = pre[a].gz - sz;
             } else {
                 float2 g = *reinterpret_cast<float2 *>(gxy + 2 * off[a]);
-                g.x += gx[a]; g.y += gy[a];
+                g.x -= sx; g.y -= sy;
                 *reinterpret_cast<float2 *>(gxy + 2 * off[a]) = g;
-                *reinterpret_cast<float *>(gz + off[a]) += gzz[a];
+                *reinterpret_cast<float *>(gz + off[a]) -= sz;
             }
         }
     }
@@ -313,27 +336,38 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
     {
         const char *xyb = reinterpret_cast<const char *>(xy), *zzb = reinterpret_cast<const char *>(zz);
         char *gxyb = reinterpret_cast<char *>(gxy), *gzb = reinterpret_cast<char *>(gz);
-        PairAcc acc[2] = {{0.f, 0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f, 0.f}};
+        const f32x2 z2 = bc2(0.0f);
+        PairAcc acc[2] = {{z2, z2, z2, z2, z2}, {z2, z2, z2, z2, z2}};
         int pos = 0;
         for (int g = 0; g < L.n_groups; ++g) {
             const uint4 hdr = tpp_quad<SCHED_PARAM>(L, pos++);
             PairTile t;
             CellRef cr[TPP_TILE];
             float4 q0[TPP_TILE], q1[TPP_TILE];
+            float ax[TPP_TILE], ay[TPP_TILE], az[TPP_TILE];
 #pragma unroll
             for (int k = 0; k < TPP_TILE; ++k) {
                 const int i = (int)((hdr.x >> (8 * k)) & 0xffu);
                 const float2 a = xy[i * 32];
-                t.x[k] = a.x; t.y[k] = a.y; t.z[k] = zz[i * 32];
-                t.fx[k] = t.fy[k] = t.fz[k] = 0.0f;
-                cr[k] = locate_cell(G, t.x[k] + tx, t.y[k] + ty, t.z[k] + tz);
+                ax[k] = a.x; ay[k] = a.y; az[k] = zz[i * 32];
+                cr[k] = locate_cell(G, ax[k] + tx, ay[k] + ty, az[k] + tz);
                 const Cell8 *e0 = G.packed + (size_t)__float_as_int(L.atom_ref[i].w) + cr[k].idx;
                 ldg_cell(e0, q0[k], q1[k]);                                     // consumed after the records
+            }
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                t.x[hf] = pk2(ax[2 * hf], ax[2 * hf + 1]); t.y[hf] = pk2(ay[2 * hf], ay[2 * hf + 1]); t.z[hf] = pk2(az[2 * hf], az[2 * hf + 1]);
+                t.fx[hf] = t.fy[hf] = t.fz[hf] = z2;
             }
             record_class<0, WANT_GRAD, SCHED_PARAM>(P, L, pos, (int)(hdr.y & 0xffu), (int)((hdr.y >> 8) & 0xffu), t, acc, xyb, zzb, gxyb, gzb);
             record_class<1, WANT_GRAD, SCHED_PARAM>(P, L, pos, (int)((hdr.y >> 16) & 0xffu), (int)(hdr.y >> 24), t, acc, xyb, zzb, gxyb, gzb);
             record_class<2, WANT_GRAD, SCHED_PARAM>(P, L, pos, (int)(hdr.z & 0xffu), (int)((hdr.z >> 8) & 0xffu), t, acc, xyb, zzb, gxyb, gzb);
             const int n_live = (int)(hdr.z >> 16);
+            float tfx[TPP_TILE], tfy[TPP_TILE], tfz[TPP_TILE];
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                up2(t.fx[hf], tfx[2 * hf], tfx[2 * hf + 1]); up2(t.fy[hf], tfy[2 * hf], tfy[2 * hf + 1]); up2(t.fz[hf], tfz[2 * hf], tfz[2 * hf + 1]);
+            }
 #pragma unroll
             for (int k = 0; k < TPP_TILE; ++k) {
                 if (k < n_live) {                                               // padding slots of the last tile: skipped
@@ -342,16 +376,16 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
                     if (WANT_GRAD) {
                         const int i = (int)((hdr.x >> (8 * k)) & 0xffu);
                         float2 gi = gxy[i * 32];
-                        gi.x += fmaf(P.sigma, gx, t.fx[k]);
-                        gi.y += fmaf(P.sigma, gy, t.fy[k]);
+                        gi.x += fmaf(P.sigma, gx, tfx[k]);
+                        gi.y += fmaf(P.sigma, gy, tfy[k]);
                         gxy[i * 32] = gi;
-                        gz[i * 32] += fmaf(P.sigma, gz_, t.fz[k]);
+                        gz[i * 32] += fmaf(P.sigma, gz_, tfz[k]);
                     }
                 }
             }
         }
-        const float a = acc[0].a + acc[1].a, b = acc[0].b + acc[1].b, rep = acc[0].rep + acc[1].rep;
-        const float hyd = acc[0].hyd + acc[1].hyd, hb = acc[0].hb + acc[1].hb;
+        const float a = sum2(add2(acc[0].a, acc[1].a)), b = sum2(add2(acc[0].b, acc[1].b)), rep = sum2(add2(acc[0].rep, acc[1].rep));
+        const float hyd = sum2(add2(acc[0].hyd, acc[1].hyd)), hb = sum2(add2(acc[0].hb, acc[1].hb));
         e_intra = fmaf(P.eA, a, fmaf(P.eB, b, P.sigma * fmaf(0.5f, rep, fmaf(-0.7f, hb, -hyd))));
     }
 

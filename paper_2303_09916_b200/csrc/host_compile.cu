@@ -372,13 +372,13 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
             Rec fresh;
             fresh.j = j_slot;
             fresh.cls = 0;
-            for (int t = 0; t < TPP_TILE; ++t) { fresh.rsum[t] = TPP_MASKED_RSUM; fresh.wh[t] = 0.f; fresh.whb[t] = 0.f; }
+            for (int t = 0; t < TPP_TILE; ++t) { fresh.rsum[t] = -TPP_MASKED_RSUM; fresh.wh[t] = 0.f; fresh.whb[t] = 0.f; }   // rsum[] holds -(R_i+R_j)
             grp.push_back(fresh);
             r = &grp.back();
         }
         const int t = i_slot - tile * TPP_TILE;
         const int ti = L->type[atom_of[i_slot]], tj = L->type[atom_of[j_slot]];
-        r->rsum[t] = p->radius[ti] + p->radius[tj];
+        r->rsum[t] = -(p->radius[ti] + p->radius[tj]);
         if (p->hydrophobic[ti] && p->hydrophobic[tj] && p->w[3] != 0.f) { r->wh[t] = whp; r->cls = std::max(r->cls, 1); }
         if (((p->donor[ti] && p->acceptor[tj]) || (p->donor[tj] && p->acceptor[ti])) && p->w[4] != 0.f) { r->whb[t] = whbp; r->cls = 2; }
     };
