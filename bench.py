@@ -358,8 +358,8 @@ def run_ours(args) -> dict:
 
 
 # per-launch DRAM traffic of the score kernel from the committed `ncu --set full` capture
-# (profiles/r1i_score_thread_kernel_details.txt, commit 917e8f1).
-TRAFFIC_BYTES_PER_LAUNCH = 823.0e6   # profiles/r1i.md: dram__bytes_read.sum 757.2 MB + dram__bytes_write.sum 65.8 MB
+# (profiles/r1j_score_thread_kernel_details.txt).
+TRAFFIC_BYTES_PER_LAUNCH = 823.4e6   # profiles/r1j.md: dram__bytes_read.sum 756.8 MB + dram__bytes_write.sum 66.6 MB
 
 
 def main():
