@@ -17,6 +17,7 @@ from .generators import (  # noqa: F401
     make_protein_globule,
     make_ligand,
     make_box,
+    make_site_points,
     random_poses,
     make_system,
     CONFIGS,

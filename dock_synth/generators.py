@@ -267,6 +267,29 @@ def random_poses(rng, n: int, box_center, box_size, T: int) -> np.ndarray:
 
 
 # BASELINE.json:configs, by index.
+def make_site_points(rng: np.random.Generator, box_center, box_size, n: int = 120, step: float = 1.5,
+                     margin: float = 7.0) -> np.ndarray:
+    """Synthetic 'predicted binding site' points (Fig. 3): a connected random-walk cluster of n points on a
+    `step` lattice that starts at the box centre and stays at least `margin` inside the box -- a cavity-shaped blob that
+    stands in for the output of the paper's site-prediction network (out of scope here)."""
+    c = np.asarray(box_center, dtype=np.float64)
+    half = 0.5 * np.asarray(box_size, dtype=np.float64) - margin
+    if int(np.prod(2 * np.floor(np.maximum(half, 0.0) / step) + 1)) < n:
+        raise ValueError("box too small for n site points at this step and margin")
+    pts = {(0, 0, 0)}
+    frontier = [(0, 0, 0)]
+    moves = [(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+    while len(pts) < n:
+        base = frontier[int(rng.integers(len(frontier)))]
+        m = moves[int(rng.integers(6))]
+        q = (base[0] + m[0], base[1] + m[1], base[2] + m[2])
+        if q in pts or np.any(np.abs(np.array(q) * step) > half):
+            continue
+        pts.add(q)
+        frontier.append(q)
+    return (c + step * np.array(sorted(pts), dtype=np.float64)).astype(np.float32)
+
+
 CONFIGS = {
     0: dict(name="tiny", n_prot=200, box=15.0, N=12, T=2, copies=16, steps=20, cap=50),
     1: dict(name="scoring_microbench", n_prot=3000, box=30.0, N=30, T=6, n_poses=1_048_576),

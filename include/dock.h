@@ -170,6 +170,16 @@ int dock_local_opt_batch(const dock_params *params, const dock_grid *grid, const
 int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
                     float *out_host);
 
+/* ---- NEXT-3: initial poses restrained to the adaptive search space (Fig. 3) ------
+ * "A union set of balls with 7 A radius, centered at each discrete points of predicted binding site ... The
+ * intersection of this cube and the union set of balls is taken as the space for binding site search.  The
+ * initial ligand positions are ... restrained to the searching space."  Reading S22: the
+ * translation is drawn uniformly in the box by rejection (Philox slots 0x100 + attempt, 256 attempts, then
+ * the site point copy mod n_site); orientation and torsions as dock_init_poses.  site_xyz_host [n_site][3],
+ * same frame as the box; out_host [copies][7+T], to be passed to dock_search as init poses after upload. */
+int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
+                         int32_t n_site, const float *site_xyz_host, float radius, float *out_host);
+
 /* ---- A6-A8: many-copy Monte-Carlo search + top-k -----------------------------
  * n_systems independent systems in one launch; grids[s], ligands[s], boxes[s] are HOST arrays of
  * descriptors.  T_max = max over systems of T; pose rows are 7+T_max floats wide (unused tail 0).

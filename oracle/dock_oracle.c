@@ -753,6 +753,32 @@ void orc_init_pose(const double box_center[3], const double box_size[3], int T,
     for (int k = 0; k < 7 + T; ++k) pose[k] = (double)(float)pose[k];   /* stored fp32 once (S16) */
 }
 
+/* NEXT-3 (Fig. 3): the search space is the intersection of the box with the union of balls of
+ * radius `radius` centred at the predicted site points; "the initial ligand positions are not fully random but
+ * restrained to the searching space".  Reading S22: rejection sampling of the translation -- attempt a = 0..255
+ * draws t uniform in the box from Philox slot 0x100 + a (counter step 0xFFFFFFFF as in S16) and the first t
+ * inside some ball is kept; if none is, t = site point (copy mod n_site).  Orientation and torsions as S16. */
+void orc_init_pose_site(const double box_center[3], const double box_size[3], int T,
+                        uint64_t seed, uint32_t system, uint32_t copy,
+                        int n_site, const double *site_xyz, double radius, double *pose)
+{
+    orc_init_pose(box_center, box_size, T, seed, system, copy, pose);      /* q, theta (and a t that is replaced) */
+    uint32_t r[4];
+    int found = 0;
+    double t[3];
+    for (int a = 0; a < 256 && !found; ++a) {
+        draw(seed, system, copy, 0xFFFFFFFFu, 0x100u + (uint32_t)a, r);
+        for (int c = 0; c < 3; ++c) t[c] = box_center[c] - 0.5 * box_size[c] + u24(r[c]) * box_size[c];
+        for (int k = 0; k < n_site && !found; ++k) {
+            const double dx = t[0] - site_xyz[3 * k], dy = t[1] - site_xyz[3 * k + 1], dz = t[2] - site_xyz[3 * k + 2];
+            if (dx * dx + dy * dy + dz * dz <= radius * radius) found = 1;
+        }
+    }
+    if (!found)
+        for (int c = 0; c < 3; ++c) t[c] = site_xyz[3 * (copy % (uint32_t)n_site) + c];
+    for (int c = 0; c < 3; ++c) pose[c] = (double)(float)t[c];
+}
+
 int orc_mc_perturb(const orc_params *p, int T, uint64_t seed, uint32_t system, uint32_t copy,
                    uint32_t step, const double *pose, double *cand)
 {

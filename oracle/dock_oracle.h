@@ -148,6 +148,10 @@ double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L
 /* S16 initial pose for (system, copy) from Philox, rounded once to fp32 */
 void   orc_init_pose(const double box_center[3], const double box_size[3], int T,
                      uint64_t seed, uint32_t system, uint32_t copy, double *pose);
+/* NEXT-3: translation restrained to box ∩ union of balls around the site points (reading S22) */
+void   orc_init_pose_site(const double box_center[3], const double box_size[3], int T,
+                          uint64_t seed, uint32_t system, uint32_t copy,
+                          int n_site, const double *site_xyz, double radius, double *pose);
 
 /* O9 perturbation of MC step `step` of (system, copy): writes the candidate start pose, returns kind (0,1,2) */
 int    orc_mc_perturb(const orc_params *p, int T, uint64_t seed, uint32_t system, uint32_t copy,

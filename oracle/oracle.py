@@ -289,6 +289,20 @@ def init_pose(center, size, T, seed, system, copy) -> np.ndarray:
     return out
 
 
+def init_poses_site(center, size, T, seed, system, copies, site_xyz, radius) -> np.ndarray:
+    """NEXT-3: initial poses with the translation restrained to box ∩ union of balls (reading S22)."""
+    site = _f64(site_xyz).reshape(-1, 3)
+    out = np.zeros((copies, 7 + T))
+    for c in range(copies):
+        row = np.zeros(7 + T)
+        lib().orc_init_pose_site((C.c_double * 3)(*[float(x) for x in center]),
+                                 (C.c_double * 3)(*[float(x) for x in size]), int(T),
+                                 C.c_uint64(seed), C.c_uint32(system), C.c_uint32(c),
+                                 int(site.shape[0]), _p(site), C.c_double(radius), _p(row))
+        out[c] = row
+    return out
+
+
 def init_poses(center, size, T, seed, system, copies) -> np.ndarray:
     return np.stack([init_pose(center, size, T, seed, system, c) for c in range(copies)])
 

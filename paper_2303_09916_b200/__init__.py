@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     dock_grid_bytes,
     dock_grid_dims,
     dock_init_poses,
+    dock_init_poses_site,
     dock_ligand,
     dock_local_opt_batch,
     dock_params,

@@ -23,7 +23,7 @@ DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
 
 EXPORTS = [
     "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_score_batch",
-    "dock_score_batch_host", "dock_local_opt_batch", "dock_init_poses", "dock_search", "dock_topk",
+    "dock_score_batch_host", "dock_local_opt_batch", "dock_init_poses", "dock_init_poses_site", "dock_search", "dock_topk",
     "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
 ]
 
@@ -298,6 +298,16 @@ def dock_init_poses(box: dock_box, T: int, seed: int, system: int, copies: int) 
     out = np.zeros((copies, 7 + T), dtype=np.float32)
     _check(load_library().dock_init_poses(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), int(copies),
                                           _np_ptr(out)), "dock_init_poses")
+    return out
+
+
+def dock_init_poses_site(box: dock_box, T: int, seed: int, system: int, copies: int, site_xyz, radius: float = 7.0) -> np.ndarray:
+    """NEXT-3: initial poses with the translation restrained to box ∩ union of balls around the site points."""
+    site = np.ascontiguousarray(site_xyz, dtype=np.float32).reshape(-1, 3)
+    out = np.zeros((copies, 7 + T), dtype=np.float32)
+    _check(load_library().dock_init_poses_site(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), int(copies),
+                                               int(site.shape[0]), _np_ptr(site), C.c_float(radius), _np_ptr(out)),
+           "dock_init_poses_site")
     return out
 
 

@@ -495,6 +495,39 @@ extern "C" int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, ui
     return DOCK_OK;
 }
 
+// NEXT-3 (Fig. 3; reading S22): translation restrained to box (intersected with) the union of balls of
+// `radius` around the predicted site points, by rejection from the Philox slots 0x100 + attempt (256 attempts,
+// then the site point copy mod n_site); orientation and torsions as in dock_init_poses.
+extern "C" int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
+                                    int32_t n_site, const float *site_xyz_host, float radius, float *out_host)
+{
+    if (!box || !out_host || T < 0 || T > DOCK_MAX_TORSIONS || copies < 0) return DOCK_EINVAL;
+    if (n_site < 1 || !site_xyz_host || !(radius > 0.f)) return DOCK_EINVAL;
+    const uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
+    const double r2max = (double)radius * (double)radius;
+    for (int c = 0; c < copies; ++c) {
+        float *out = out_host + (size_t)c * (7 + T);
+        host_init_pose(box, T, seed, system, (uint32_t)c, out);
+        double t[3] = {0, 0, 0};
+        bool found = false;
+        for (int a = 0; a < 256 && !found; ++a) {
+            uint32_t r[4];
+            philox4x32_10((uint32_t)c, 0xffffffffu, 0x100u + (uint32_t)a, system, k0, k1, r);
+            for (int d = 0; d < 3; ++d)
+                t[d] = (double)box->center[d] - 0.5 * (double)box->size[d] + (double)(r[d] >> 8) * (1.0 / 16777216.0) * (double)box->size[d];
+            for (int k = 0; k < n_site && !found; ++k) {
+                const double dx = t[0] - (double)site_xyz_host[3 * k], dy = t[1] - (double)site_xyz_host[3 * k + 1],
+                             dz = t[2] - (double)site_xyz_host[3 * k + 2];
+                if (dx * dx + dy * dy + dz * dz <= r2max) found = true;
+            }
+        }
+        if (!found)
+            for (int d = 0; d < 3; ++d) t[d] = (double)site_xyz_host[3 * (c % n_site) + d];
+        for (int d = 0; d < 3; ++d) out[d] = (float)t[d];
+    }
+    return DOCK_OK;
+}
+
 extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
                                     int64_t n_poses, int32_t max_iters, const float *poses_dev,
                                     float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,

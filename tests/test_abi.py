@@ -142,3 +142,37 @@ def test_init_poses_follow_the_philox_rule(orc, lib):
         assert a.shape == b.shape == (64, 7 + T)
         assert np.max(np.abs(a.astype(np.float64) - b)) <= 1e-6
         assert np.mean(a.astype(np.float64) == b) > 0.99   # same formulas in double, rounded once
+
+
+def test_site_restrained_initial_poses(orc, lib):
+    """NEXT-3 (Fig. 3; reading S22): host logic of dock_init_poses_site against the oracle, and the
+    properties that define it: every translation lies in box ∩ union of 7 A balls, the accepted points are uniform
+    in that set, one ball that covers the box reduces to the plain rule, orientation / torsions are untouched."""
+    from dock_synth import make_site_points
+    center, size = [1.5, -2.25, 3.0], [30.0, 30.0, 30.0]
+    box = dk.make_box(center, size, 0.375)
+    site = make_site_points(np.random.default_rng(1), center, size, n=120)
+    assert site.shape == (120, 3) and np.all(np.abs(site - np.array(center)) <= 8.0 + 1e-6)
+    seed = 0x1234ABCD5678
+    for T in (0, 7):
+        a = dk.dock_init_poses_site(box, T, seed, 2, 512, site, 7.0)
+        b = orc.init_poses_site(center, size, T, seed, 2, 512, site, 7.0)
+        assert np.array_equal(a[:, :3].astype(np.float64), b[:, :3])             # same integers, same affine map, one rounding
+        assert np.max(np.abs(a.astype(np.float64) - b)) <= 1e-6
+        d = np.min(np.linalg.norm(b[:, None, :3] - site[None].astype(np.float64), axis=2), axis=1)
+        assert np.all(d <= 7.0 + 1e-5)
+        assert np.all(np.abs(b[:, :3] - np.array(center)) <= 15.0)
+        plain = orc.init_poses(center, size, T, seed, 2, 512)
+        assert np.array_equal(plain[:, 3:], b[:, 3:])                             # q, theta as S16
+    # uniform in the set: with two far-apart site points, each ball receives about half of the copies
+    two = np.array([[center[0] - 7.5, center[1], center[2]], [center[0] + 7.5, center[1], center[2]]], np.float32)
+    c = orc.init_poses_site(center, size, 0, seed, 0, 2000, two, 7.0)
+    left = (c[:, 0] < center[0]).mean()
+    assert abs(left - 0.5) < 0.04
+    # a ball that contains the whole box accepts attempt 0 -> equals slot 0x100's draw, inside the box
+    big = orc.init_poses_site(center, size, 0, seed, 0, 64, np.array([center], np.float32), 100.0)
+    assert np.all(np.abs(big[:, :3] - np.array(center)) <= 15.0)
+    # no point of the box is within reach -> the fallback site point
+    far = np.array([[500.0, 0.0, 0.0], [600.0, 0.0, 0.0]], np.float32)
+    f = dk.dock_init_poses_site(box, 0, seed, 0, 4, far, 7.0)
+    assert np.array_equal(f[:, :3], far[[0, 1, 0, 1]])

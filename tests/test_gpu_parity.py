@@ -554,3 +554,19 @@ def test_maximum_ligand_size_local_opt_and_search(dk, orc, torch, micro):
     r2 = dk.dock_search(p, [grid], [lig], [box], 32, 2, 20, 9)
     assert torch.equal(r1["best_e"], r2["best_e"]) and int(r1["topk_count"][0]) >= 1
     assert bool(torch.isfinite(r1["best_e"]).all())
+
+
+def test_search_from_site_restrained_initial_poses(dk, torch, tiny):
+    """NEXT-3: copies start inside box ∩ union of balls around synthetic site points; with zero MC steps
+    the search returns exactly the local optima of those poses."""
+    from dock_synth import make_site_points
+    s, (p, box, grid, lig), _ = tiny
+    site = make_site_points(np.random.default_rng(2), s.box_center, s.box_size, n=20, step=1.0, margin=3.0)
+    init = dk.dock_init_poses_site(box, lig.T, 99, 0, 32, site, 3.0)
+    d = np.min(np.linalg.norm(init[:, None, :3] - site[None], axis=2), axis=1)
+    assert np.all(d <= 3.0 + 1e-4)
+    r = dk.dock_search(p, [grid], [lig], [box], 32, 0, 50, 99, init_poses=torch.from_numpy(init[None]).cuda())
+    o, e, it = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(init).cuda(), 50)
+    assert torch.equal(r["best_e"][0], e)
+    r5 = dk.dock_search(p, [grid], [lig], [box], 32, 5, 50, 99, init_poses=torch.from_numpy(init[None]).cuda())
+    assert bool((r5["best_e"] <= r["best_e"] + 1e-6).all())
