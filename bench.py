@@ -365,7 +365,7 @@ TRAFFIC_BYTES_PER_LAUNCH = 823.4e6   # profiles/r1j.md: dram__bytes_read.sum 756
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-sample", type=int, default=1048576, help="poses the CPU oracle scores per step")
