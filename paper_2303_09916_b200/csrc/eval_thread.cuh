@@ -12,9 +12,10 @@
 // Shared memory (6N floats per pose) and registers bound the occupancy (8 warps per SM for a 30-atom
 // ligand), so the kernel is written for instruction-level parallelism instead: the pair phase is
 // branch-free straight-line code over 8 independent pairs (2 partner atoms x a 4-atom register tile),
-// written stage by stage on packed fp32x2 register pairs (two tile atoms per FFMA2 issue slot), and the 32-byte map gathers of a tile's atoms are issued at the top of the tile's
-// pair group and consumed at its end, so their L2 latency hides under the pair arithmetic
-// (profiles/r1a.md -> r1c.md -> r1d.md).
+// written stage by stage on packed fp32x2 register pairs (two tile atoms per FFMA2 issue slot), and
+// the 32-byte map gathers of a tile's atoms are issued at the top of the tile's pair group and
+// consumed at its end, so their L2 latency hides under the pair arithmetic
+// (profiles/r1a.md -> r1f.md -> r1j.md).
 //
 //   phase 1  A2: one rigid frame (rotation + offset) per fragment, parents first, composed from the
 //            parent's frame and one Rodrigues rotation; atoms of a fragment are 9 FMAs each.
