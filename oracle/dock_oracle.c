@@ -223,6 +223,46 @@ void orc_build_grid(const orc_params *p, int np, const double *pxyz, const int32
 /* ---------------------------------------------------------------------------------------
  * small vector / quaternion helpers
  * ------------------------------------------------------------------------------------- */
+/* NEXT-2 / eq. 4: per-vertex gradient of the vertex score, by the same brute force as O2. */
+void orc_build_grid_grad(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
+                         const int dims[3], const double origin[3], double h,
+                         int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *GD)
+{
+    const int nx = dims[0], ny = dims[1], nz = dims[2];
+    const int64_t nodes = (int64_t)nx * ny * nz;
+    const float hf = (float)h;
+    const float cut2f = (float)p->cutoff * (float)p->cutoff;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t m = 0; m < nodes; ++m) {
+        int ix = (int)(m % nx), iy = (int)((m / nx) % ny), iz = (int)(m / ((int64_t)nx * ny));
+        double mx = origin[0] + h * ix, my = origin[1] + h * iy, mz = origin[2] + h * iz;
+        float mxf = fmaf((float)ix, hf, (float)origin[0]);
+        float myf = fmaf((float)iy, hf, (float)origin[1]);
+        float mzf = fmaf((float)iz, hf, (float)origin[2]);
+        for (int t = 0; t < n_lig_types; ++t)
+            for (int c = 0; c < 3; ++c) GD[((int64_t)t * 3 + c) * nodes + m] = 0.0;
+        for (int j = 0; j < np; ++j) {
+            double d[3] = {mx - pxyz[3 * j], my - pxyz[3 * j + 1], mz - pxyz[3 * j + 2]};
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            int in_range;
+            if (fp32_cutoff) {
+                float fx = mxf - (float)pxyz[3 * j], fy = myf - (float)pxyz[3 * j + 1], fz = mzf - (float)pxyz[3 * j + 2];
+                float r2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+                in_range = r2f < cut2f;
+                if (in_range && !(r < p->cutoff)) r = nextafter(p->cutoff, 0.0);
+            } else {
+                in_range = r < p->cutoff;
+            }
+            if (!in_range || r <= 0.0) continue;
+            for (int t = 0; t < n_lig_types; ++t) {
+                double dfdr;
+                orc_pair(p, lig_types[t], ptype[j], r, &dfdr);
+                for (int c = 0; c < 3; ++c) GD[((int64_t)t * 3 + c) * nodes + m] += dfdr * d[c] / r;
+            }
+        }
+    }
+}
+
 static void cross(const double a[3], const double b[3], double c[3])
 {
     c[0] = a[1] * b[2] - a[2] * b[1];
@@ -387,6 +427,20 @@ static void atom_inter(const orc_params *p, const orc_grid *g, int map, const do
                 gy += wx * (2 * m - 1) / h * wz * val;         /* eq. 3, y component */
                 gz += wx * wy * (2 * n - 1) / h * val;         /* eq. 3, z component */
             }
+    if (g->gdata) {                                            /* eq. 4: the vertex gradients, interpolated with eq. 2's weights */
+        const int64_t nodes = (int64_t)nx * ny * nz;
+        const double *GD = g->gdata + (int64_t)map * 3 * nodes;
+        gx = gy = gz = 0.0;
+        for (int l = 0; l <= 1; ++l)
+            for (int m = 0; m <= 1; ++m)
+                for (int n = 0; n <= 1; ++n) {
+                    double w = (l ? pf[0] : 1.0 - pf[0]) * (m ? pf[1] : 1.0 - pf[1]) * (n ? pf[2] : 1.0 - pf[2]);
+                    int64_t node = ((int64_t)(i0[2] + n) * ny + (i0[1] + m)) * nx + (i0[0] + l);
+                    gx += w * GD[node];
+                    gy += w * GD[nodes + node];
+                    gz += w * GD[2 * nodes + node];
+                }
+    }
     double ew = 0.0;
     double gg[3] = {gx, gy, gz};
     for (int c = 0; c < 3; ++c) {

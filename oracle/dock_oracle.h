@@ -79,6 +79,8 @@ typedef struct {
     int    n_maps;
     int    type_to_map[ORC_MAX_TYPES]; /* -1 = absent */
     const double *data;         /* [n_maps][nz][ny][nx] */
+    const double *gdata;        /* NEXT-2 (eq. 4): [n_maps][3][nz][ny][nx] analytic gradient of the vertex score at the vertices, or NULL:
+                                 * then the gradient is that of the interpolant (eq. 3) */
 } orc_grid;
 
 /* per-evaluation diagnostics filled by orc_eval when `diag` != NULL */
@@ -107,6 +109,11 @@ void   orc_grid_geometry(const double center[3], const double size[3], double h,
 void   orc_build_grid(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
                       const int dims[3], const double origin[3], double h,
                       int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *G);
+/* NEXT-2 ("we further used the gradient of score obtained by trilinear interpolation", eq. 4 at 221): the
+ * gradient of the vertex score at the vertices, GD[t][c][m] = sum_j f'(r) (m - r_j)_c / r over the same atoms as G. */
+void orc_build_grid_grad(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
+                         const int dims[3], const double origin[3], double h,
+                         int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *GD);
 
 /* O3 */
 void   orc_coords(const orc_ligand *L, const double *pose, double *x);

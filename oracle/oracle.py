@@ -74,6 +74,7 @@ class _Grid(C.Structure):
         ("n_maps", C.c_int),
         ("type_to_map", C.c_int * ORC_MAX_TYPES),
         ("data", C.c_void_p),
+        ("gdata", C.c_void_p),
     ]
 
 
@@ -182,7 +183,7 @@ class Ligand:
 
 
 class Grid:
-    def __init__(self, dims, origin, h, lig_types, data):
+    def __init__(self, dims, origin, h, lig_types, data, gdata=None):
         self.dims = tuple(int(d) for d in dims)
         self.origin = np.array(origin, dtype=np.float64)
         self.h = float(h)
@@ -199,7 +200,17 @@ class Grid:
         for m, t in enumerate(self.lig_types):
             g.type_to_map[t] = m
         g.data = _p(self.data)
+        self.gdata = None if gdata is None else _f64(gdata)
+        g.gdata = None if gdata is None else _p(self.gdata)
         self.c = g
+
+    @property
+    def gmaps(self):
+        """NEXT-2 (eq. 4): per-vertex gradients [n_maps][3][nz][ny][nx], or None."""
+        if self.gdata is None:
+            return None
+        nx, ny, nz = self.dims
+        return self.gdata.reshape(len(self.lig_types), 3, nz, ny, nx)
 
     @property
     def maps(self):
@@ -216,7 +227,7 @@ def grid_geometry(center, size, h):
     return [int(d) for d in dims], [float(o) for o in org]
 
 
-def build_grid(p: Params, pxyz, ptype, center, size, h, lig_types, fp32_cutoff=True) -> Grid:
+def build_grid(p: Params, pxyz, ptype, center, size, h, lig_types, fp32_cutoff=True, grad=False) -> Grid:
     dims, org = grid_geometry(center, size, h)
     pxyz = _f64(pxyz)
     ptype = _i32(ptype)
@@ -225,7 +236,13 @@ def build_grid(p: Params, pxyz, ptype, center, size, h, lig_types, fp32_cutoff=T
     lib().orc_build_grid(C.byref(p), int(pxyz.shape[0]), _p(pxyz), _p(ptype),
                          (C.c_int * 3)(*dims), (C.c_double * 3)(*org), C.c_double(h),
                          len(lig_types), _p(lt), int(bool(fp32_cutoff)), _p(G))
-    return Grid(dims, org, h, lig_types, G)
+    GD = None
+    if grad:                                               # NEXT-2: eq. 4's per-vertex gradients
+        GD = np.zeros(3 * len(lig_types) * dims[0] * dims[1] * dims[2], dtype=np.float64)
+        lib().orc_build_grid_grad(C.byref(p), int(pxyz.shape[0]), _p(pxyz), _p(ptype),
+                                  (C.c_int * 3)(*dims), (C.c_double * 3)(*org), C.c_double(h),
+                                  len(lig_types), _p(lt), int(bool(fp32_cutoff)), _p(GD))
+    return Grid(dims, org, h, lig_types, G, GD)
 
 
 def coords(L: Ligand, pose) -> np.ndarray:

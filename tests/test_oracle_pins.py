@@ -654,3 +654,76 @@ def test_bb_local_opt_on_the_docking_objective(orc, tiny):
         f, x, it, ne = orc.local_opt(q, og, oL, poses[i], 150)
         assert f <= e0[i] + 1e-12 and ne == it + 1
         assert abs(orc.score_batch(q, og, oL, x[None, :], want_grad=False)[0][0] - f) < 1e-9
+
+
+# ----------------------------------------------------------------------------------- NEXT-2: eq. 4 gradient maps
+def test_eq4_vertex_gradients_are_the_gradient_of_the_brute_force_vertex_score(orc):
+    """PAPER.md:221 (eq. 4): the stored per-vertex gradient must be the derivative of the vertex score s(m) = sum_j f(|m - r_j|)
+    with respect to the vertex position -- checked by central differences of brute-force pair sums at shifted positions."""
+    p = orc.default_params()
+    rng = np.random.default_rng(12)
+    pxyz = rng.uniform(-6, 6, size=(40, 3))
+    ptyp = rng.integers(0, 10, size=40).astype(np.int32)
+    lig_types = [0, 3, 8]
+    g = orc.build_grid(p, pxyz, ptyp, [0, 0, 0], [6.0, 6.0, 6.0], 0.375, lig_types, fp32_cutoff=False, grad=True)
+    assert g.gmaps.shape == (3, 3, 17, 17, 17)
+
+    def s(t, m):
+        r = np.linalg.norm(pxyz - m, axis=1)
+        return sum(orc.pair(p, t, int(tj), float(rr))[0] for tj, rr in zip(ptyp, r) if rr < p.cutoff)
+
+    eps = 1e-5
+    for (mi, ix, iy, iz) in [(0, 3, 4, 5), (1, 8, 8, 8), (2, 16, 0, 7), (1, 0, 16, 16)]:
+        m = np.array(g.origin) + g.h * np.array([ix, iy, iz])
+        # keep away from pairs sitting on a kink or the cutoff, where the derivative is one-sided
+        for c in range(3):
+            e = np.zeros(3); e[c] = eps
+            fd = (s(lig_types[mi], m + e) - s(lig_types[mi], m - e)) / (2 * eps)
+            assert abs(g.gmaps[mi, c, iz, iy, ix] - fd) <= 1e-5 * max(1.0, abs(fd)), (mi, c, fd)
+
+
+def test_eq4_interpolated_gradient_properties(orc, tiny):
+    """Eq. 4 interpolates the vertex gradients with eq. 2's weights: exact at vertices, reproduces an affine gradient
+    field, leaves the energy untouched, and differs from eq. 3 (gradient of the interpolant) by O(h^2) curvature terms."""
+    s, p, g3, L = tiny
+    g4 = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types, grad=True)
+    assert np.array_equal(g4.maps, g3.maps)
+    one = orc.Ligand(SimpleNamespace(ref_xyz=np.zeros((1, 3)), type=np.array([s.lig_types[1]], np.int32),
+                                     frag=np.zeros(1, np.int32), tors_parent=np.zeros(0, np.int32), tors_a=np.zeros(0, np.int32),
+                                     tors_b=np.zeros(0, np.int32), pairs=np.zeros((0, 2), np.int32)))
+    q = [1.0, 0.0, 0.0, 0.0]
+    # at a vertex: gradient = stored vertex gradient, energy = vertex score
+    for (ix, iy, iz) in [(5, 6, 7), (20, 20, 20), (33, 1, 12)]:
+        m = np.array(g4.origin) + g4.h * np.array([ix, iy, iz])
+        e, terms, grad, _ = orc.evaluate(p, g4, one, list(m) + q)
+        assert abs(e - g4.maps[1, iz, iy, ix]) < 1e-12
+        assert np.allclose(grad[:3], g4.gmaps[1, :, iz, iy, ix], rtol=0, atol=1e-12)
+    # inside a cell: the eq. 2 weights applied to the 8 vertex gradients
+    rng = np.random.default_rng(6)
+    for _ in range(20):
+        u = rng.uniform(2, 37, size=3)
+        x = np.array(g4.origin) + g4.h * u
+        i0 = np.floor(u).astype(int); f = u - i0
+        want = np.zeros(3)
+        for l in (0, 1):
+            for m_ in (0, 1):
+                for n in (0, 1):
+                    w = (f[0] if l else 1 - f[0]) * (f[1] if m_ else 1 - f[1]) * (f[2] if n else 1 - f[2])
+                    want += w * g4.gmaps[1, :, i0[2] + n, i0[1] + m_, i0[0] + l]
+        e4, _, grad4, _ = orc.evaluate(p, g4, one, list(x) + q)
+        e3, _, grad3, _ = orc.evaluate(p, g3, one, list(x) + q)
+        assert np.allclose(grad4[:3], want, rtol=1e-12, atol=1e-12) and abs(e4 - e3) < 1e-12
+    # affine gradient field in, the same field out (and eq. 3 is untouched by gdata = None)
+    nx, ny, nz = g3.dims
+    Z, Y, X = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    gd = np.zeros((len(s.lig_types), 3, nz, ny, nx))
+    for c, (a, b) in enumerate([(0.3, 1.0), (-0.7, 0.5), (0.2, -2.0)]):
+        gd[:, c] = a + b * (g3.origin[c] + g3.h * [X, Y, Z][c])
+    ga = orc.Grid(g3.dims, g3.origin, g3.h, s.lig_types, g3.data, gd)
+    x = np.array(g3.origin) + g3.h * np.array([7.3, 11.9, 20.25])
+    _, _, grad, _ = orc.evaluate(p, ga, one, list(x) + q)
+    assert np.allclose(grad[:3], [0.3 + 1.0 * x[0], -0.7 + 0.5 * x[1], 0.2 - 2.0 * x[2]], atol=1e-12)
+    # the wall is unchanged: 1 A outside on x adds the quadratic wall and zeroes the grid gradient on that axis
+    xo = np.array(g4.origin) + np.array([-1.0, 3.0, 3.0])
+    _, t4, gr4, _ = orc.evaluate(p, g4, one, list(xo) + q)
+    assert abs(t4[1] - p.k_wall) < 1e-12 and abs(gr4[0] + 2 * p.k_wall) < 1e-12
