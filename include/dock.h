@@ -69,6 +69,9 @@ typedef struct dock_params {
     int32_t optimizer;                        /* local optimizer: 0 = BFGS + backtracking, 1 = Barzilai-Borwein */
     float   bb_step;                          /* BB: length of the first step and cap on every step (A / rad) */
     float   bb_fallback;                      /* BB: step length when s.y is not safely positive */
+    int32_t grad_mode;                        /* grid gradient: 0 = gradient of the interpolant (eq. 3), 1 = interpolated
+                                               * per-vertex gradients (eq. 4; NEXT-2).  Read by dock_build_grids,
+                                               * which then writes 4 channels per map; the evaluators follow dock_grid.n_channels */
 } dock_params;
 
 /* Search / interpolation box: n_axis = round(size/spacing)+1 nodes,
@@ -117,6 +120,8 @@ typedef struct dock_grid {
     int32_t      type_to_map[DOCK_MAX_XS_TYPES];   /* XS type id -> map index, -1 = absent */
     const float *data_dev;                         /* DEVICE pointer, caller-owned */
     const float *packed_dev;                       /* DEVICE pointer into the same buffer */
+    int32_t      n_channels;                       /* 1: data_dev [n_maps][nz][ny][nx]; 4 (eq. 4): [n_maps][4][nz][ny][nx] with channels
+                                                    * (score, d/dx, d/dy, d/dz) -- packed_dev likewise; 0 is read as 1 */
 } dock_grid;
 
 /* Optional per-(system, copy, step) trace of the search; with the stateless Philox counter it
@@ -133,7 +138,8 @@ int dock_default_params(dock_params *out);
  * out_desc (host) receives the descriptor with data_dev = grid_dev and packed_dev behind it.
  * Errors: DOCK_EINVAL for null pointers, n < 0, spacing <= 0, type ids outside [0, n_types). */
 int dock_grid_dims(const dock_box *box, int32_t dims[3]);
-/* bytes of the caller's grid buffer for n_lig_types maps over `box` (both images); 0 on bad input */
+/* bytes of the caller's grid buffer for n_lig_types maps over `box` (both images); 0 on bad input.
+ * With dock_params.grad_mode = 1 every map has 4 channels: pass 4 * n_lig_types here. */
 size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types);
 int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
                      int32_t n_lig_types, const int32_t *lig_types,

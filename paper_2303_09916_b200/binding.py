@@ -45,7 +45,7 @@ class dock_params(C.Structure):
         ("bfgs_c1", C.c_float), ("bfgs_shrink", C.c_float), ("bfgs_max_trials", C.c_int32),
         ("bfgs_gtol", C.c_float), ("bfgs_curv_eps", C.c_float),
         ("cluster_rmsd", C.c_float), ("topk", C.c_int32),
-        ("optimizer", C.c_int32), ("bb_step", C.c_float), ("bb_fallback", C.c_float),
+        ("optimizer", C.c_int32), ("bb_step", C.c_float), ("bb_fallback", C.c_float), ("grad_mode", C.c_int32),
     ]
 
 
@@ -69,7 +69,7 @@ class dock_grid(C.Structure):
     _fields_ = [
         ("dims", C.c_int32 * 3), ("origin", C.c_float * 3), ("spacing", C.c_float),
         ("n_maps", C.c_int32), ("type_to_map", C.c_int32 * DOCK_MAX_XS_TYPES), ("data_dev", C.c_void_p),
-        ("packed_dev", C.c_void_p),
+        ("packed_dev", C.c_void_p), ("n_channels", C.c_int32),
     ]
 
 
@@ -175,7 +175,7 @@ class LigandHandle:
 
 class GridMaps:
     """Device grid maps + descriptor.  `buf` owns the memory (both images, see dock.h);
-    `data` is the [n_maps, nz, ny, nx] view of the maps themselves."""
+    `data` is the [n_maps, nz, ny, nx] view of the maps themselves ([n_maps, 4, nz, ny, nx] in eq. 4 mode)."""
 
     def __init__(self, buf, data, desc: dock_grid):
         self.buf = buf
@@ -209,8 +209,10 @@ def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_b
     prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
     lt = np.ascontiguousarray(lig_types, dtype=np.int32)
     nx, ny, nz = dock_grid_dims(box)
-    buf = torch.empty(dock_grid_bytes(box, len(lt)), dtype=torch.uint8, device="cuda")
-    data = buf[: len(lt) * nz * ny * nx * 4].view(torch.float32).view(len(lt), nz, ny, nx)
+    ch = 4 if int(params.grad_mode) == 1 else 1                      # eq. 4: (score, d/dx, d/dy, d/dz) per map
+    buf = torch.empty(dock_grid_bytes(box, len(lt) * ch), dtype=torch.uint8, device="cuda")
+    data = buf[: len(lt) * ch * nz * ny * nx * 4].view(torch.float32)
+    data = data.view(len(lt), nz, ny, nx) if ch == 1 else data.view(len(lt), ch, nz, ny, nx)
     desc = dock_grid()
     need = C.c_size_t(0)
     rc = lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
@@ -380,7 +382,8 @@ def dock_system_host(params: dock_params, protein_xyz, protein_type, box: dock_b
     prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
     lt = np.ascontiguousarray(lig_types, dtype=np.int32)
     if grid_buf is None:
-        grid_buf = torch.empty(dock_grid_bytes(box, len(lt)), dtype=torch.uint8, device="cuda")
+        grid_buf = torch.empty(dock_grid_bytes(box, len(lt) * (4 if int(params.grad_mode) == 1 else 1)), dtype=torch.uint8,
+                               device="cuda")
     k = int(params.topk)
     out_pose = np.zeros((k, 7 + ligand.T), dtype=np.float32)
     out_e = np.zeros(k, dtype=np.float32)

@@ -75,6 +75,7 @@ struct DevGrid {
     float hi_x, hi_y, hi_z;         // n-1-ic*
     float h, inv_h, inv_h_lo;       // spacing; fl(1/h) and 1/h - fl(1/h)
     float kw_g, kw_e;               // wall: 2 k h (gradient per cell of overshoot), k h^2
+    int   channels, chan_stride;    // 1, or 4 (eq. 4: score, d/dx, d/dy, d/dz at chan_stride entries apart)
     const Cell8  *packed;           // [n_maps][nz][ny][nx] gather layout: the 8 corners of a cell in one 32-byte entry (see dock.h)
     const float  *data;             // [n_maps][nz][ny][nx]
 };

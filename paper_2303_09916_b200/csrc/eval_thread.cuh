@@ -245,7 +245,7 @@ __device__ __forceinline__ void record_class(const DevParams &P, const TppLigand
 
 // pose[k * ps] = k-th pose component of this thread; grad[k * gs] receives the k-th gradient component.
 // `sm` = this warp's shared memory (tpp_warp_floats floats).  Returns E = e_grid + e_wall + e_intra.
-template <bool WANT_GRAD, bool SCHED_PARAM>
+template <bool WANT_GRAD, bool SCHED_PARAM, bool EQ4 = false>
 __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevGrid &G, const TppLigand &L,
                                                   const float *__restrict__ pose, int ps,
                                                   float *__restrict__ grad, int gs,
@@ -373,7 +373,12 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
             for (int k = 0; k < TPP_TILE; ++k) {
                 if (k < n_live) {                                               // padding slots of the last tile: skipped
                     float gx, gy, gz_;
-                    e_grid += trilinear(G, cr[k], q0[k], q1[k], e_wall, gx, gy, gz_);
+                    if (EQ4 && WANT_GRAD) {                                     // NEXT-2: eq. 4, three more cells per atom (not prefetched)
+                        const int ia = (int)((hdr.x >> (8 * k)) & 0xffu);
+                        const Cell8 *cell = G.packed + (size_t)__float_as_int(L.atom_ref[ia].w) + cr[k].idx;
+                        e_grid += trilinear_eq4(G, cr[k], cell, q0[k], q1[k], e_wall, gx, gy, gz_);
+                    } else
+                        e_grid += trilinear(G, cr[k], q0[k], q1[k], e_wall, gx, gy, gz_);
                     if (WANT_GRAD) {
                         const int i = (int)((hdr.x >> (8 * k)) & 0xffu);
                         float2 gi = gxy[i * 32];

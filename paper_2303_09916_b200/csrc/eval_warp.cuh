@@ -64,7 +64,7 @@ __device__ __forceinline__ void pose_coords_warp(const DevLigand &L, const float
     __syncwarp();
 }
 
-template <bool WANT_GRAD>
+template <bool WANT_GRAD, bool EQ4 = false>
 __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
                                              const float *pose, float *grad, float *scratch, EvalTerms *terms)
 {
@@ -91,8 +91,10 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         xs[i] = x0; xs[np + i] = x1; xs[2 * np + i] = x2;
         const CellRef cr = locate_cell(G, x0, x1, x2);
         float4 q0, q1;
-        ldg_cell(G.packed + (size_t)map_off + cr.idx, q0, q1);
-        e_grid += trilinear(G, cr, q0, q1, e_wall, gx, gy, gz);
+        const Cell8 *cell = G.packed + (size_t)map_off + cr.idx;
+        ldg_cell(cell, q0, q1);
+        if (EQ4 && WANT_GRAD) e_grid += trilinear_eq4(G, cr, cell, q0, q1, e_wall, gx, gy, gz);   // NEXT-2: eq. 4 gradient
+        else e_grid += trilinear(G, cr, q0, q1, e_wall, gx, gy, gz);
         if (WANT_GRAD) { gs[i] = gx; gs[np + i] = gy; gs[2 * np + i] = gz; }
     }
     __syncwarp();

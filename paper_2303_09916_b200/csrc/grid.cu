@@ -32,9 +32,11 @@ struct GridBuildArgs {
     const float4 *atoms;   // sorted by cell; w = bitcast(type)
     const int    *cell_start;
     const float4 *pair_tab;// [n_maps][n_types] {rsum, wh, whb, 0}
-    float        *out;     // [n_maps][nz][ny][nx]
+    float        *out;     // [n_maps][channels][nz][ny][nx]
+    int   channels;        // 1, or 4 = (score, d/dx, d/dy, d/dz): eq. 4's per-vertex gradients (NEXT-2)
 };
 
+template <bool GRAD>
 __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
 {
     __shared__ float4 tab[MAPS_PER_PASS * DOCK_MAX_XS_TYPES];
@@ -60,9 +62,9 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
     const int cy = (int)((my - A.clo[1]) * A.inv_cell);
     const int cz = (int)((mz - A.clo[2]) * A.inv_cell);
 
-    float acc[MAPS_PER_PASS];
+    float acc[MAPS_PER_PASS], agx[MAPS_PER_PASS], agy[MAPS_PER_PASS], agz[MAPS_PER_PASS];
 #pragma unroll
-    for (int m = 0; m < MAPS_PER_PASS; ++m) acc[m] = 0.0f;
+    for (int m = 0; m < MAPS_PER_PASS; ++m) acc[m] = agx[m] = agy[m] = agz[m] = 0.0f;
 
     for (int dz = -1; dz <= 1; ++dz) {
         const int zc = cz + dz;
@@ -95,6 +97,13 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
                             e = fmaf(t.y, __saturatef(1.5f - d), e);
                             e = fmaf(t.z, __saturatef(d * -1.4285714285714286f), e);
                             acc[m] += e;
+                            if (GRAD) {                                   // d f / d(vertex) = f'(r) (m - r_j) / r
+                                float de = fmaf(-8.0f * d, A.w[0] * g1, fmaf(-0.5f * dm3, A.w[1] * g2, 2.0f * A.w[2] * rep));
+                                de -= (d >= 0.5f && d < 1.5f) ? t.y : 0.0f;
+                                de -= (d >= -0.7f && d < 0.0f) ? t.z * 1.4285714285714286f : 0.0f;
+                                const float k = r > 0.0f ? de / r : 0.0f;
+                                agx[m] = fmaf(k, fx, agx[m]); agy[m] = fmaf(k, fy, agy[m]); agz[m] = fmaf(k, fz, agz[m]);
+                            }
                         }
                     }
                 }
@@ -105,7 +114,11 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
     const size_t node = ((size_t)iz * A.ny + iy) * A.nx + ix;
 #pragma unroll
     for (int m = 0; m < MAPS_PER_PASS; ++m)
-        if (m < nm) A.out[(size_t)(m0 + m) * nodes + node] = acc[m];
+        if (m < nm) {
+            float *o = A.out + (size_t)(m0 + m) * A.channels * nodes + node;
+            o[0] = acc[m];
+            if (GRAD) { o[nodes] = agx[m]; o[2 * nodes] = agy[m]; o[3 * nodes] = agz[m]; }
+        }
 }
 
 // Gather layout (Cell8, common.cuh): entry (ix,iy,iz) of map m = the 8 corners of the cell whose low corner is that
@@ -218,7 +231,7 @@ extern "C" int dock_grid_dims(const dock_box *box, int32_t dims[3])
 extern "C" size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types)
 {
     int32_t dims[3];
-    if (n_lig_types < 1 || n_lig_types > DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
+    if (n_lig_types < 1 || n_lig_types > 4 * DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
     const size_t nodes = (size_t)dims[0] * dims[1] * dims[2] * (size_t)n_lig_types;
     return align_up(nodes * sizeof(float), 256) + nodes * sizeof(Cell8);
 }
@@ -260,13 +273,15 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     A.cell_start = (const int *)(ws + b_atoms);
     A.pair_tab = (const float4 *)(ws + b_atoms + b_cells);
     A.out = grid_dev;
+    A.channels = params->grad_mode == 1 ? 4 : 1;
     const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8, tbz = (A.nz + 1) / 2;
     dim3 grid((unsigned)(tbx * tby * tbz), (unsigned)((n_lig_types + MAPS_PER_PASS - 1) / MAPS_PER_PASS));
-    grid_build_kernel<<<grid, 128, 0, stream>>>(A);
+    if (A.channels == 4) grid_build_kernel<true><<<grid, 128, 0, stream>>>(A);
+    else grid_build_kernel<false><<<grid, 128, 0, stream>>>(A);
     DOCK_LAUNCH_CHECK();
-    const size_t nodes = (size_t)A.nx * A.ny * A.nz * (size_t)n_lig_types;
+    const size_t nodes = (size_t)A.nx * A.ny * A.nz * (size_t)n_lig_types * A.channels;
     Cell8 *packed = reinterpret_cast<Cell8 *>(reinterpret_cast<unsigned char *>(grid_dev) + align_up(nodes * sizeof(float), 256));
-    const long long rows = (long long)n_lig_types * A.nz * A.ny;
+    const long long rows = (long long)n_lig_types * A.channels * A.nz * A.ny;
     const unsigned pack_blocks = (unsigned)std::min<long long>((rows * A.nx + 255) / 256, 148LL * 16);
     grid_pack_kernel<<<pack_blocks, 256, 0, stream>>>(grid_dev, packed, A.nx, A.ny, A.nz, rows);
     DOCK_LAUNCH_CHECK();
@@ -279,5 +294,6 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     for (int m = 0; m < n_lig_types; ++m) out_desc->type_to_map[lig_types[m]] = m;
     out_desc->data_dev = grid_dev;
     out_desc->packed_dev = reinterpret_cast<const float *>(packed);
+    out_desc->n_channels = A.channels;
     return DOCK_OK;
 }

@@ -51,6 +51,7 @@ extern "C" int dock_default_params(dock_params *p)
     p->optimizer = 0;
     p->bb_step = 1.0f;          // reading S13
     p->bb_fallback = 0.1f;
+    p->grad_mode = 0;
     return DOCK_OK;
 }
 
@@ -63,6 +64,7 @@ int dock_validate_params(const dock_params *p)
     if (!(p->bfgs_shrink > 0.f && p->bfgs_shrink < 1.f)) return DOCK_EINVAL;
     if (p->topk < 1 || p->topk > DOCK_MAX_TOPK) return DOCK_EINVAL;
     if (p->optimizer < 0 || p->optimizer > 1) return DOCK_EINVAL;
+    if (p->grad_mode < 0 || p->grad_mode > 1) return DOCK_EINVAL;
     if (p->optimizer == 1 && (!(p->bb_step > 0.f) || !(p->bb_fallback > 0.f))) return DOCK_EINVAL;
     return DOCK_OK;
 }
@@ -122,6 +124,9 @@ int dock_make_dev_grid(const dock_params *p, const dock_grid *g, DevGrid *o)
     o->inv_h_lo = (float)(1.0 / h - (double)o->inv_h);
     o->kw_g = (float)(2.0 * (double)p->k_wall * h);
     o->kw_e = (float)((double)p->k_wall * h * h);
+    if (g->n_channels != 0 && g->n_channels != 1 && g->n_channels != 4) return DOCK_EINVAL;
+    o->channels = g->n_channels == 4 ? 4 : 1;
+    o->chan_stride = g->dims[0] * g->dims[1] * g->dims[2];
     o->packed = reinterpret_cast<const Cell8 *>(g->packed_dev);
     o->data = g->data_dev;
     return DOCK_OK;
@@ -239,7 +244,7 @@ int dock_compile_ligand(const dock_params *p, const dock_grid *g, const dock_lig
     for (int i = 0; i < N; ++i) {
         int mask = 0, f = L->atom_fragment[i];
         while (f > 0) { mask |= 1 << (f - 1); f = L->tors_parent[f - 1]; }
-        const long long off = g ? (long long)g->type_to_map[L->type[i]] * map_stride : 0;
+        const long long off = g ? (long long)g->type_to_map[L->type[i]] * map_stride * (g->n_channels == 4 ? 4 : 1) : 0;
         if (off > 0x7fffffffLL) return DOCK_EINVAL;
         atom_ref[i] = make_float4((float)((double)L->ref_xyz[3 * i] - c[0]), (float)((double)L->ref_xyz[3 * i + 1] - c[1]),
                                   (float)((double)L->ref_xyz[3 * i + 2] - c[2]), 0.f);
@@ -322,7 +327,7 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
     int f_cur = 0;
     for (int s = 0; s < N; ++s) {
         const int i = atom_of[s];
-        const long long off = (long long)g->type_to_map[L->type[i]] * map_stride;
+        const long long off = (long long)g->type_to_map[L->type[i]] * map_stride * (g->n_channels == 4 ? 4 : 1);
         if (off > 0x7fffffffLL) return DOCK_EINVAL;
         const int ioff = (int)off;
         out.atom_ref[s] = make_float4((float)((double)L->ref_xyz[3 * i] - c[0]), (float)((double)L->ref_xyz[3 * i + 1] - c[1]),

@@ -144,6 +144,44 @@ __device__ __forceinline__ CellRef locate_cell(const DevGrid &G, float x, float 
     return c;
 }
 
+// Clamped axes get zero grid gradient and the quadratic wall (reading S7).  ggx.. in kcal/mol/A.
+__device__ __forceinline__ void apply_wall(const DevGrid &G, const CellRef &c, float ggx, float ggy, float ggz,
+                                           float &e_wall, float &gx, float &gy, float &gz)
+{
+    if (c.ox != 0.0f) ggx = 0.0f;
+    if (c.oy != 0.0f) ggy = 0.0f;
+    if (c.oz != 0.0f) ggz = 0.0f;
+    gx = fmaf(G.kw_g, c.ox, ggx);                                                     // 2 k h * overshoot_cells
+    gy = fmaf(G.kw_g, c.oy, ggy);
+    gz = fmaf(G.kw_g, c.oz, ggz);
+    e_wall = fmaf(G.kw_e, fmaf(c.ox, c.ox, fmaf(c.oy, c.oy, c.oz * c.oz)), e_wall);   // k h^2 * sum overshoot_cells^2
+}
+
+// Value of the trilinear interpolant (eq. 2) of one channel from its packed cell.
+__device__ __forceinline__ float trilerp(const CellRef &c, const float4 q0, const float4 q1)
+{
+    const float c00 = fmaf(c.px, q0.y - q0.x, q0.x), c10 = fmaf(c.px, q0.w - q0.z, q0.z);
+    const float c01 = fmaf(c.px, q1.y - q1.x, q1.x), c11 = fmaf(c.px, q1.w - q1.z, q1.z);
+    const float c0 = fmaf(c.py, c10 - c00, c00), c1 = fmaf(c.py, c11 - c01, c01);
+    return fmaf(c.pz, c1 - c0, c0);
+}
+
+// NEXT-2 / eq. 4: energy by eq. 2 from the score channel, gradient = the three per-vertex gradient
+// channels interpolated with the same weights.  `cell` = packed entry of the score channel; the gradient channels sit
+// chan_stride entries apart.
+__device__ __forceinline__ float trilinear_eq4(const DevGrid &G, const CellRef &c, const Cell8 *cell,
+                                               const float4 q0, const float4 q1, float &e_wall,
+                                               float &gx, float &gy, float &gz)
+{
+    float4 a0, a1, b0, b1, d0, d1;
+    ldg_cell(cell + (size_t)G.chan_stride, a0, a1);
+    ldg_cell(cell + 2 * (size_t)G.chan_stride, b0, b1);
+    ldg_cell(cell + 3 * (size_t)G.chan_stride, d0, d1);
+    const float e = trilerp(c, q0, q1);
+    apply_wall(G, c, trilerp(c, a0, a1), trilerp(c, b0, b1), trilerp(c, d0, d1), e_wall, gx, gy, gz);
+    return e;
+}
+
 // Trilinear energy (eq. 2) and the gradient of the interpolant (eq. 3) from the two packed entries
 // q0 (plane iz) and q1 (plane iz+1); clamped axes get zero grid gradient and the quadratic wall
 // (reading S7).  Returns e_grid; adds to e_wall; gradient in kcal/mol/A.
@@ -162,12 +200,6 @@ __device__ __forceinline__ float trilinear(const DevGrid &G, const CellRef &c,
     float ggx = fmaf(c.pz, dx1 - dx0, dx0) * G.inv_h;                                 // eq. 3, x
     float ggy = fmaf(c.pz, dy1 - dy0, dy0) * G.inv_h;                                 // eq. 3, y
     float ggz = dz * G.inv_h;                                                         // eq. 3, z
-    if (c.ox != 0.0f) ggx = 0.0f;
-    if (c.oy != 0.0f) ggy = 0.0f;
-    if (c.oz != 0.0f) ggz = 0.0f;
-    gx = fmaf(G.kw_g, c.ox, ggx);                                                     // 2 k h * overshoot_cells
-    gy = fmaf(G.kw_g, c.oy, ggy);
-    gz = fmaf(G.kw_g, c.oz, ggz);
-    e_wall = fmaf(G.kw_e, fmaf(c.ox, c.ox, fmaf(c.oy, c.oy, c.oz * c.oz)), e_wall);   // k h^2 * sum overshoot_cells^2
+    apply_wall(G, c, ggx, ggy, ggz, e_wall, gx, gy, gz);
     return e;
 }

@@ -11,7 +11,7 @@
 
 namespace {
 
-template <bool WANT_GRAD, bool SCHED_PARAM>
+template <bool WANT_GRAD, bool SCHED_PARAM, bool EQ4>
 __global__ void __launch_bounds__(256)
 score_thread_kernel(const DevParams P, const DevGrid G, const __grid_constant__ TppLigand L, long long n_poses,
                     const float *__restrict__ poses, float *__restrict__ energy,
@@ -23,7 +23,7 @@ score_thread_kernel(const DevParams P, const DevGrid G, const __grid_constant__ 
     // idle lanes of the last warp redo the last pose: same inputs, same bits, same stores (benign)
     const long long p = min((long long)blockIdx.x * blockDim.x + threadIdx.x, n_poses - 1);
     EvalTerms t;
-    const float e = eval_pose_thread<WANT_GRAD, SCHED_PARAM>(P, G, L, poses + p * np_, 1, grad + p * ng, 1, smem, t);
+    const float e = eval_pose_thread<WANT_GRAD, SCHED_PARAM, EQ4>(P, G, L, poses + p * np_, 1, grad + p * ng, 1, smem, t);
     energy[p] = e;
     if (terms) { terms[3 * p] = t.e_grid; terms[3 * p + 1] = t.e_wall; terms[3 * p + 2] = t.e_intra; }
 }
@@ -45,11 +45,11 @@ int plan_score(const dock_params *params, const dock_grid *grid, const dock_liga
     return DOCK_OK;
 }
 
-template <bool WANT_GRAD, bool SCHED_PARAM>
+template <bool WANT_GRAD, bool SCHED_PARAM, bool EQ4 = false>
 int launch(const ScorePlan &pl, long long n_poses, const float *poses_dev, float *energy_dev, float *grad_dev,
            float *terms_dev, cudaStream_t stream)
 {
-    auto kern = score_thread_kernel<WANT_GRAD, SCHED_PARAM>;
+    auto kern = score_thread_kernel<WANT_GRAD, SCHED_PARAM, EQ4>;
     const int warp_floats = tpp_warp_floats(pl.L.N, pl.L.T, WANT_GRAD, pl.L.fm_alias != 0);
     const size_t warp_bytes = (size_t)warp_floats * sizeof(float);
     if (warp_bytes > 227 * 1024) return DOCK_EINVAL;
@@ -84,9 +84,11 @@ int score_launch(ScorePlan &pl, long long n_poses, const float *poses_dev, float
             DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.overflow.data(), pl.overflow.size() * sizeof(uint4),
                                             cudaMemcpyHostToDevice, stream));
         pl.L.sched_global = (const uint4 *)ws;
+        if (grad_dev && pl.G.channels == 4) return launch<true, false, true>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
         return grad_dev ? launch<true, false>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream)
                         : launch<false, false>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
     }
+    if (grad_dev && pl.G.channels == 4) return launch<true, true, true>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
     return grad_dev ? launch<true, true>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream)
                     : launch<false, true>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
 }

@@ -97,6 +97,7 @@ __device__ __forceinline__ void set_identity(float *H, int n, float diag)
 // Written as one loop around a SINGLE evaluation site (the start pose is "trial" INIT), so that the evaluator and
 // this routine inline into the kernels once: the compiler then sees that every buffer is shared memory and keeps
 // P, G, L in registers / the constant bank instead of local memory (profiles/r1g.md).
+template <bool EQ4>
 __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
                                                 const OptBuf &b, int cap, int &iters, int &evals)
 {
@@ -119,7 +120,7 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
     int it = 0, trial = 0;
     evals = 0;
     for (;;) {
-        const float ft = eval_pose_warp<true>(P, G, L, b.xt, b.gt, b.scratch, nullptr);
+        const float ft = eval_pose_warp<true, EQ4>(P, G, L, b.xt, b.gt, b.scratch, nullptr);
         ++evals;
         if (init) {
             init = false;
@@ -251,6 +252,7 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
 }
 
 // ---- local optimisation of a batch of poses (level-2 parity entry point) -------------------------
+template <bool EQ4>
 __global__ void __launch_bounds__(SEARCH_WARPS * 32)
 local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap, int warp_floats,
                  const float *__restrict__ poses, float *__restrict__ out_pose, float *__restrict__ out_e,
@@ -265,7 +267,7 @@ local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap
     for (int k = lane; k < np_; k += 32) b.x[k] = poses[p * np_ + k];
     __syncwarp();
     int iters, evals;
-    const float e = local_opt_warp(P, G, L, b, cap, iters, evals);
+    const float e = local_opt_warp<EQ4>(P, G, L, b, cap, iters, evals);
     for (int k = lane; k < np_; k += 32) out_pose[p * np_ + k] = b.x[k];
     if (lane == 0) {
         out_e[p] = e;
@@ -278,6 +280,7 @@ __device__ __forceinline__ float u24(uint32_t r) { return (float)(r >> 8) * (1.0
 
 // 4 CTAs per SM = 128 registers, no spills: 16 resident warps for the screening batches (143 vs 126 M evals/s on a
 // 64-system config-3 slice), same latency for the 384-copy case (profiles/r1i.md)
+template <bool EQ4>
 __global__ void __launch_bounds__(SEARCH_WARPS * 32, 4)
 search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems, int copies, int steps,
               int cap, uint32_t seed_lo, uint32_t seed_hi, int t_max, int warp_floats,
@@ -325,7 +328,7 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
             }
             __syncwarp();
         }
-        const float e_c = local_opt_warp(P, G, L, b, cap, iters, evals);
+        const float e_c = local_opt_warp<EQ4>(P, G, L, b, cap, iters, evals);
         total_evals += evals;
         if (step < 0) {
             e_cur = e_best = e_c;
@@ -549,11 +552,12 @@ extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *
     const int warp_floats = opt_floats(L.T, L.n_pad);
     const size_t smem = (size_t)SEARCH_WARPS * warp_floats * sizeof(float);
     if (smem > 200 * 1024) return DOCK_EINVAL;
+    auto kern = G.channels == 4 ? local_opt_kernel<true> : local_opt_kernel<false>;
     if (smem > 48 * 1024)
-        DOCK_CUDA_CHECK(cudaFuncSetAttribute(local_opt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned blocks = (unsigned)((n_poses + SEARCH_WARPS - 1) / SEARCH_WARPS);
-    local_opt_kernel<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(P, G, L, n_poses, max_iters, warp_floats, poses_dev,
-                                                                 out_pose_dev, out_e_dev, out_iters_dev);
+    kern<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(P, G, L, n_poses, max_iters, warp_floats, poses_dev,
+                                                     out_pose_dev, out_e_dev, out_iters_dev);
     DOCK_LAUNCH_CHECK();
     return DOCK_OK;
 }
@@ -626,11 +630,14 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
     }
     const size_t smem = (size_t)SEARCH_WARPS * wf_max * sizeof(float);
     if (smem > 200 * 1024) return DOCK_EINVAL;
+    for (int s2 = 1; s2 < n_systems; ++s2)
+        if (sys[s2].grid.channels != sys[0].grid.channels) return DOCK_EINVAL;      // one gradient mode per launch
+    auto kern = sys[0].grid.channels == 4 ? search_kernel<true> : search_kernel<false>;
     if (smem > 48 * 1024)
-        DOCK_CUDA_CHECK(cudaFuncSetAttribute(search_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const long long total = (long long)n_systems * copies;
     const unsigned blocks = (unsigned)((total + SEARCH_WARPS - 1) / SEARCH_WARPS);
-    search_kernel<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(
+    kern<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(
         P, sys_dev, n_systems, copies, steps, bfgs_max_iters, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
         t_max, wf_max, init, best_pose_dev, best_e_dev, trace_dev, (unsigned long long *)eval_counter_dev);
     DOCK_LAUNCH_CHECK();

@@ -570,3 +570,48 @@ def test_search_from_site_restrained_initial_poses(dk, torch, tiny):
     assert torch.equal(r["best_e"][0], e)
     r5 = dk.dock_search(p, [grid], [lig], [box], 32, 5, 50, 99, init_poses=torch.from_numpy(init[None]).cuda())
     assert bool((r5["best_e"] <= r["best_e"] + 1e-6).all())
+
+
+# ----------------------------------------------------------------------------------- NEXT-2: eq. 4 gradient maps
+def test_eq4_maps_scores_and_search(dk, orc, torch, tiny):
+    """PAPER.md:51 / eq. 4 (221): four channels per map (score and its per-vertex gradient), gradient of a pose from the
+    interpolated vertex gradients.  Maps at every node, per-pose energies and gradients on both evaluators (batch
+    scoring: thread per pose; local optimisation with zero iterations: warp per pose), and a search on those maps."""
+    s, (p3, box, grid3, lig), (op, og3, oL) = tiny
+    p = dk.dock_default_params()
+    p.grad_mode = 1
+    grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types)
+    og = orc.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types, grad=True)
+    gm = grid.data.cpu().numpy().astype(np.float64)                    # [n_maps, 4, nz, ny, nx]
+    assert gm.shape[1] == 4 and int(grid.desc.n_channels) == 4
+    g3m = grid3.data.cpu().numpy().astype(np.float64)                  # the score channel is the eq. 2 map (to round-off:
+    assert np.all(np.abs(gm[:, 0] - g3m) <= 1e-5 + 1e-6 * np.abs(g3m))  # the two kernel variants contract their FMAs differently)
+    assert np.all(np.abs(gm[:, 0] - og.maps) <= tol(og.maps))
+    assert np.all(np.abs(gm[:, 1:] - og.gmaps) <= tol(og.gmaps))
+    rng = np.random.default_rng(44)
+    poses = random_poses(rng, 2051, s.box_center, s.box_size * 1.2, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    # eq. 4's gradient is continuous across cell faces (only the kinks of the intra pairs remain one-sided)
+    diag4 = diag.copy()
+    diag4["face_margin"] = 1.0
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag4, "eq4",
+                        cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
+    _log("score_eq4", st)
+    e3, g3, _ = dk.dock_score_batch(p3, grid3, lig, torch.from_numpy(poses).cuda())
+    assert torch.allclose(e, e3, rtol=1e-6, atol=1e-5) and not torch.allclose(g, g3, atol=1e-3)   # same E, different gradient
+    # warp evaluator: zero optimizer iterations = one evaluation; its energy matches, and one BFGS step agrees with the oracle
+    o0, e0, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 0)
+    assert torch.allclose(e0, e[:128], rtol=1e-5, atol=1e-4)
+    o1, e1, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 1)
+    r1 = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), 1)[0] for i in range(128)])
+    c1, _, _, d1 = orc.score_batch(op, og, oL, o1.cpu().numpy().astype(np.float64))
+    ok1 = d1["cutoff_margin"] > KINK_MARGIN
+    assert (np.abs(e1.cpu().numpy() - r1) <= 10 * tol(r1))[ok1].mean() >= 0.97
+    r = dk.dock_search(p, [grid], [lig], [box], s.copies, 5, 50, 3)
+    r2 = dk.dock_search(p, [grid], [lig], [box], s.copies, 5, 50, 3)
+    assert torch.equal(r["best_e"], r2["best_e"]) and int(r["topk_count"][0]) >= 1
+    k = int(r["topk_count"][0])
+    oe2, _, _, d2 = orc.score_batch(op, og, oL, r["topk_pose"][0, :k].cpu().numpy().astype(np.float64))
+    ok = d2["cutoff_margin"] > KINK_MARGIN
+    assert np.all(np.abs(r["topk_e"][0, :k].cpu().numpy() - oe2)[ok] <= tol(oe2)[ok])
