@@ -353,6 +353,25 @@ def run_ours(args) -> dict:
                               "search_s": t_3, "grid_build_s": t_g3, "evals": ev3, "evals_per_s": ev3 / t_3,
                               "systems_per_s_search_only": ns / t_3, "systems_per_s_with_grids": ns / (t_3 + t_g3)}
         del gr
+        # configs[4]: large blind box, 161^3 x 8 maps (1.07 GB gather image), 2048 copies x 80 steps, N = 60, T = 15
+        s4 = make_system(4, seed=0)
+        box4 = dk.make_box(s4.box_center, s4.box_size, s4.spacing)
+        lig4 = dk.LigandHandle(s4.ligand)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        grid4 = dk.dock_build_grids(p, s4.protein_xyz, s4.protein_type, box4, s4.lig_types)
+        torch.cuda.synchronize()
+        t_g4 = time.perf_counter() - t0
+        run4 = lambda: dk.dock_search(p, [grid4], [lig4], [box4], s4.copies, s4.steps, s4.bfgs_cap, 2023)
+        t0 = time.perf_counter()
+        r4 = run4()
+        torch.cuda.synchronize()
+        t_4 = time.perf_counter() - t0
+        extra["large_blind_box"] = {"workload": "configs[4]: 8000 atoms, 161^3 x 8 maps, 2048 copies x 80 steps, BFGS<=300",
+                                    "search_s": t_4, "grid_build_s": t_g4, "evals": int(r4["evals"][0]),
+                                    "evals_per_s": int(r4["evals"][0]) / t_4, "systems_per_s_with_grid": 1.0 / (t_4 + t_g4),
+                                    "best_e": float(r4["topk_e"][0, 0])}
+        del grid4
     line["extra"] = extra
     return line
 
