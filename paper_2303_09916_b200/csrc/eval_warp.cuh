@@ -70,8 +70,9 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
 {
     const int lane = threadIdx.x & 31;
     const int N = L.N, T = L.T, np = L.n_pad;
-    float *xs = scratch, *gs = scratch + 3 * np;
-    float *sn = gs + 3 * np, *cs = sn + ((T + 3) & ~3);
+    // coordinates and forces as float4 per atom: one 16-byte shared-memory access instead of three 4-byte ones
+    float4 *xs = reinterpret_cast<float4 *>(scratch), *gs = xs + np;
+    float *sn = scratch + 8 * np, *cs = sn + ((T + 3) & ~3);
 
     if (lane < T) {
         float s, c;
@@ -88,14 +89,14 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         float x0, x1, x2, gx, gy, gz;
         int map_off;
         atom_coords(L, R, tx, ty, tz, sn, cs, i, x0, x1, x2, map_off);
-        xs[i] = x0; xs[np + i] = x1; xs[2 * np + i] = x2;
+        xs[i] = make_float4(x0, x1, x2, 0.0f);
         const CellRef cr = locate_cell(G, x0, x1, x2);
         float4 q0, q1;
         const Cell8 *cell = G.packed + (size_t)map_off + cr.idx;
         ldg_cell(cell, q0, q1);
         if (EQ4 && WANT_GRAD) e_grid += trilinear_eq4(G, cr, cell, q0, q1, e_wall, gx, gy, gz);   // NEXT-2: eq. 4 gradient
         else e_grid += trilinear(G, cr, q0, q1, e_wall, gx, gy, gz);
-        if (WANT_GRAD) { gs[i] = gx; gs[np + i] = gy; gs[2 * np + i] = gz; }
+        if (WANT_GRAD) gs[i] = make_float4(gx, gy, gz, 0.0f);
     }
     __syncwarp();
 
@@ -114,7 +115,8 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
             const int ij = __float_as_int(cur.x);
             const bool valid = ij >= 0;
             const int i = valid ? (ij & 0xffff) : 0, j = valid ? (ij >> 16) : 0;
-            const float dx = xs[i] - xs[j], dy = xs[np + i] - xs[np + j], dz = xs[2 * np + i] - xs[2 * np + j];
+            const float4 pi = xs[i], pj = xs[j];
+            const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, 1e-12f)));
             const float rinv = fast_rsqrt(r2);
             const float d = (valid && r2 < P.cutoff2) ? fmaf(r2, rinv, -cur.y) : 1.0e18f;
@@ -134,16 +136,16 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
             if (WANT_GRAD) {
                 const float k = P.sigma * de * rinv;
                 const float fx = k * dx, fy = k * dy, fz = k * dz;
-                // all three loads before the stores: the compiler cannot prove the rows distinct and would otherwise
-                // serialise load -> add -> store three times (one shared-memory latency each)
                 if (valid) {
-                    const float a0 = gs[i], a1 = gs[np + i], a2 = gs[2 * np + i];
-                    gs[i] = a0 + fx; gs[np + i] = a1 + fy; gs[2 * np + i] = a2 + fz;
+                    float4 v = gs[i];
+                    v.x += fx; v.y += fy; v.z += fz;
+                    gs[i] = v;
                 }
                 __syncwarp();
                 if (valid) {
-                    const float a0 = gs[j], a1 = gs[np + j], a2 = gs[2 * np + j];
-                    gs[j] = a0 - fx; gs[np + j] = a1 - fy; gs[2 * np + j] = a2 - fz;
+                    float4 v = gs[j];
+                    v.x -= fx; v.y -= fy; v.z -= fz;
+                    gs[j] = v;
                 }
                 __syncwarp();
             }
@@ -166,8 +168,9 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         float4 *uw = reinterpret_cast<float4 *>(tsum + 32 * T);                  // [T][2]
         for (int k = lane; k < T; k += 32) {
             const int2 ab = __ldg(&L.tors_ab[k]);
-            const float bx = xs[ab.y], by = xs[np + ab.y], bz = xs[2 * np + ab.y];
-            float ux = bx - xs[ab.x], uy = by - xs[np + ab.x], uz = bz - xs[2 * np + ab.x];
+            const float4 pb = xs[ab.y], pa = xs[ab.x];
+            const float bx = pb.x, by = pb.y, bz = pb.z;
+            float ux = bx - pa.x, uy = by - pa.y, uz = bz - pa.z;
             const float inv = 1.0f / sqrtf(ux * ux + uy * uy + uz * uz);
             ux *= inv; uy *= inv; uz *= inv;
             const float lx = bx - tx, ly = by - ty, lz = bz - tz;
@@ -178,8 +181,9 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         __syncwarp();
         float fx = 0.f, fy = 0.f, fz = 0.f, qx = 0.f, qy = 0.f, qz = 0.f;
         for (int i = lane; i < N; i += 32) {
-            const float gx = gs[i], gy = gs[np + i], gz = gs[2 * np + i];
-            const float px = xs[i] - tx, py = xs[np + i] - ty, pz = xs[2 * np + i] - tz;
+            const float4 gv = gs[i], xv = xs[i];
+            const float gx = gv.x, gy = gv.y, gz = gv.z;
+            const float px = xv.x - tx, py = xv.y - ty, pz = xv.z - tz;
             const float mx = py * gz - pz * gy, my = pz * gx - px * gz, mz = px * gy - py * gx;
             fx += gx; fy += gy; fz += gz;
             qx += mx; qy += my; qz += mz;

@@ -29,4 +29,4 @@ int dock_compile_tpp(const dock_params *p, const dock_grid *g, const dock_ligand
                      std::vector<uint4> &overflow);
 
 // number of floats of per-warp shared memory the warp-per-pose evaluator needs for this ligand
-static inline int eval_scratch_floats(int n_pad, int T) { return 6 * n_pad + 2 * ((T + 3) & ~3) + 40 * T; }
+static inline int eval_scratch_floats(int n_pad, int T) { return 8 * n_pad + 2 * ((T + 3) & ~3) + 40 * T; }

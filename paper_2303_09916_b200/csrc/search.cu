@@ -29,7 +29,7 @@ __host__ __device__ inline int pad4(int v) { return (v + 3) & ~3; }
 __host__ __device__ inline int opt_floats(int T, int n_pad)
 {
     const int n = 6 + T, np_ = 7 + T;
-    return 2 * pad4(np_) + 5 * pad4(n) + pad4(n * n) + 6 * n_pad + 2 * pad4(T) + 40 * T;
+    return 2 * pad4(np_) + 5 * pad4(n) + pad4(n * n) + 8 * n_pad + 2 * pad4(T) + 40 * T;
 }
 
 __device__ __forceinline__ OptBuf carve(float *base, int T, int n_pad)
