@@ -64,14 +64,32 @@ __device__ __forceinline__ void pose_coords_warp(const DevLigand &L, const float
     __syncwarp();
 }
 
-template <bool WANT_GRAD, bool EQ4 = false>
+// Per-atom 3-vectors of the warp evaluator in shared memory, two layouts chosen per launch (search.cu):
+//   VEC4 : float4 per atom -- one 16-byte access instead of three 4-byte ones: fewer instructions on the single
+//          dependent chain of a latency-bound launch (few hundred copies), but random atom indices then collide in the
+//          8 bank groups of a quarter-warp phase (about 3x the shared-memory wavefronts);
+//   !VEC4: three rows [c * n_pad + i] -- conflict-free for N <= 32 and nearly so above; right for throughput-bound
+//          launches with large ligands (configs[4]: 75.6 vs 60.7 M evals/s, profiles/r1l.md).
+template <bool VEC4>
+__device__ __forceinline__ void ld3(const float *base, int np, int i, float &x, float &y, float &z)
+{
+    if (VEC4) { const float4 v = reinterpret_cast<const float4 *>(base)[i]; x = v.x; y = v.y; z = v.z; }
+    else { x = base[i]; y = base[np + i]; z = base[2 * np + i]; }
+}
+template <bool VEC4>
+__device__ __forceinline__ void st3(float *base, int np, int i, float x, float y, float z)
+{
+    if (VEC4) reinterpret_cast<float4 *>(base)[i] = make_float4(x, y, z, 0.0f);
+    else { base[i] = x; base[np + i] = y; base[2 * np + i] = z; }
+}
+
+template <bool WANT_GRAD, bool EQ4 = false, bool VEC4 = true>
 __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
                                              const float *pose, float *grad, float *scratch, EvalTerms *terms)
 {
     const int lane = threadIdx.x & 31;
     const int N = L.N, T = L.T, np = L.n_pad;
-    // coordinates and forces as float4 per atom: one 16-byte shared-memory access instead of three 4-byte ones
-    float4 *xs = reinterpret_cast<float4 *>(scratch), *gs = xs + np;
+    float *xs = scratch, *gs = scratch + 4 * np;                                 // layouts: ld3 / st3 above
     float *sn = scratch + 8 * np, *cs = sn + ((T + 3) & ~3);
 
     if (lane < T) {
@@ -89,14 +107,14 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         float x0, x1, x2, gx, gy, gz;
         int map_off;
         atom_coords(L, R, tx, ty, tz, sn, cs, i, x0, x1, x2, map_off);
-        xs[i] = make_float4(x0, x1, x2, 0.0f);
+        st3<VEC4>(xs, np, i, x0, x1, x2);
         const CellRef cr = locate_cell(G, x0, x1, x2);
         float4 q0, q1;
         const Cell8 *cell = G.packed + (size_t)map_off + cr.idx;
         ldg_cell(cell, q0, q1);
         if (EQ4 && WANT_GRAD) e_grid += trilinear_eq4(G, cr, cell, q0, q1, e_wall, gx, gy, gz);   // NEXT-2: eq. 4 gradient
         else e_grid += trilinear(G, cr, q0, q1, e_wall, gx, gy, gz);
-        if (WANT_GRAD) gs[i] = make_float4(gx, gy, gz, 0.0f);
+        if (WANT_GRAD) st3<VEC4>(gs, np, i, gx, gy, gz);
     }
     __syncwarp();
 
@@ -115,8 +133,10 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
             const int ij = __float_as_int(cur.x);
             const bool valid = ij >= 0;
             const int i = valid ? (ij & 0xffff) : 0, j = valid ? (ij >> 16) : 0;
-            const float4 pi = xs[i], pj = xs[j];
-            const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+            float xi, yi, zi, xj, yj, zj;
+            ld3<VEC4>(xs, np, i, xi, yi, zi);
+            ld3<VEC4>(xs, np, j, xj, yj, zj);
+            const float dx = xi - xj, dy = yi - yj, dz = zi - zj;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, 1e-12f)));
             const float rinv = fast_rsqrt(r2);
             const float d = (valid && r2 < P.cutoff2) ? fmaf(r2, rinv, -cur.y) : 1.0e18f;
@@ -136,16 +156,16 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
             if (WANT_GRAD) {
                 const float k = P.sigma * de * rinv;
                 const float fx = k * dx, fy = k * dy, fz = k * dz;
-                if (valid) {
-                    float4 v = gs[i];
-                    v.x += fx; v.y += fy; v.z += fz;
-                    gs[i] = v;
+                if (valid) {                                                  // loads before stores (the rows may alias for the compiler)
+                    float a0, a1, a2;
+                    ld3<VEC4>(gs, np, i, a0, a1, a2);
+                    st3<VEC4>(gs, np, i, a0 + fx, a1 + fy, a2 + fz);
                 }
                 __syncwarp();
                 if (valid) {
-                    float4 v = gs[j];
-                    v.x -= fx; v.y -= fy; v.z -= fz;
-                    gs[j] = v;
+                    float a0, a1, a2;
+                    ld3<VEC4>(gs, np, j, a0, a1, a2);
+                    st3<VEC4>(gs, np, j, a0 - fx, a1 - fy, a2 - fz);
                 }
                 __syncwarp();
             }
@@ -168,9 +188,10 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         float4 *uw = reinterpret_cast<float4 *>(tsum + 32 * T);                  // [T][2]
         for (int k = lane; k < T; k += 32) {
             const int2 ab = __ldg(&L.tors_ab[k]);
-            const float4 pb = xs[ab.y], pa = xs[ab.x];
-            const float bx = pb.x, by = pb.y, bz = pb.z;
-            float ux = bx - pa.x, uy = by - pa.y, uz = bz - pa.z;
+            float bx, by, bz, ax, ay, az;
+            ld3<VEC4>(xs, np, ab.y, bx, by, bz);
+            ld3<VEC4>(xs, np, ab.x, ax, ay, az);
+            float ux = bx - ax, uy = by - ay, uz = bz - az;
             const float inv = 1.0f / sqrtf(ux * ux + uy * uy + uz * uz);
             ux *= inv; uy *= inv; uz *= inv;
             const float lx = bx - tx, ly = by - ty, lz = bz - tz;
@@ -181,9 +202,10 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         __syncwarp();
         float fx = 0.f, fy = 0.f, fz = 0.f, qx = 0.f, qy = 0.f, qz = 0.f;
         for (int i = lane; i < N; i += 32) {
-            const float4 gv = gs[i], xv = xs[i];
-            const float gx = gv.x, gy = gv.y, gz = gv.z;
-            const float px = xv.x - tx, py = xv.y - ty, pz = xv.z - tz;
+            float gx, gy, gz, px, py, pz;
+            ld3<VEC4>(gs, np, i, gx, gy, gz);
+            ld3<VEC4>(xs, np, i, px, py, pz);
+            px -= tx; py -= ty; pz -= tz;
             const float mx = py * gz - pz * gy, my = pz * gx - px * gz, mz = px * gy - py * gx;
             fx += gx; fy += gy; fz += gz;
             qx += mx; qy += my; qz += mz;

@@ -6,6 +6,7 @@
 // Metropolis test never leave the kernel.  Randomness is stateless Philox4x32-10 with
 // counter = (copy, step, slot, system), so any step can be replayed alone.  Scalar reductions that
 // feed a decision (g.p, y.s, norms, Armijo, Metropolis) are accumulated / compared in fp64.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <vector>
@@ -97,7 +98,7 @@ __device__ __forceinline__ void set_identity(float *H, int n, float diag)
 // Written as one loop around a SINGLE evaluation site (the start pose is "trial" INIT), so that the evaluator and
 // this routine inline into the kernels once: the compiler then sees that every buffer is shared memory and keeps
 // P, G, L in registers / the constant bank instead of local memory (profiles/r1g.md).
-template <bool EQ4>
+template <bool EQ4, bool VEC4>
 __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
                                                 const OptBuf &b, int cap, int &iters, int &evals)
 {
@@ -120,7 +121,7 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
     int it = 0, trial = 0;
     evals = 0;
     for (;;) {
-        const float ft = eval_pose_warp<true, EQ4>(P, G, L, b.xt, b.gt, b.scratch, nullptr);
+        const float ft = eval_pose_warp<true, EQ4, VEC4>(P, G, L, b.xt, b.gt, b.scratch, nullptr);
         ++evals;
         if (init) {
             init = false;
@@ -252,7 +253,7 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
 }
 
 // ---- local optimisation of a batch of poses (level-2 parity entry point) -------------------------
-template <bool EQ4>
+template <bool EQ4, bool VEC4>
 __global__ void __launch_bounds__(SEARCH_WARPS * 32)
 local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap, int warp_floats,
                  const float *__restrict__ poses, float *__restrict__ out_pose, float *__restrict__ out_e,
@@ -267,7 +268,7 @@ local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap
     for (int k = lane; k < np_; k += 32) b.x[k] = poses[p * np_ + k];
     __syncwarp();
     int iters, evals;
-    const float e = local_opt_warp<EQ4>(P, G, L, b, cap, iters, evals);
+    const float e = local_opt_warp<EQ4, VEC4>(P, G, L, b, cap, iters, evals);
     for (int k = lane; k < np_; k += 32) out_pose[p * np_ + k] = b.x[k];
     if (lane == 0) {
         out_e[p] = e;
@@ -280,7 +281,7 @@ __device__ __forceinline__ float u24(uint32_t r) { return (float)(r >> 8) * (1.0
 
 // 4 CTAs per SM = 128 registers, no spills: 16 resident warps for the screening batches (143 vs 126 M evals/s on a
 // 64-system config-3 slice), same latency for the 384-copy case (profiles/r1i.md)
-template <bool EQ4>
+template <bool EQ4, bool VEC4>
 __global__ void __launch_bounds__(SEARCH_WARPS * 32, 4)
 search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems, int copies, int steps,
               int cap, uint32_t seed_lo, uint32_t seed_hi, int t_max, int warp_floats,
@@ -328,7 +329,7 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
             }
             __syncwarp();
         }
-        const float e_c = local_opt_warp<EQ4>(P, G, L, b, cap, iters, evals);
+        const float e_c = local_opt_warp<EQ4, VEC4>(P, G, L, b, cap, iters, evals);
         total_evals += evals;
         if (step < 0) {
             e_cur = e_best = e_c;
@@ -552,7 +553,10 @@ extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *
     const int warp_floats = opt_floats(L.T, L.n_pad);
     const size_t smem = (size_t)SEARCH_WARPS * warp_floats * sizeof(float);
     if (smem > 200 * 1024) return DOCK_EINVAL;
-    auto kern = G.channels == 4 ? local_opt_kernel<true> : local_opt_kernel<false>;
+    // shared-memory layout of the evaluator (eval_warp.cuh): float4 per atom unless the ligand is large
+    const bool vec4 = L.N <= 48;
+    auto kern = G.channels == 4 ? (vec4 ? local_opt_kernel<true, true> : local_opt_kernel<true, false>)
+                                : (vec4 ? local_opt_kernel<false, true> : local_opt_kernel<false, false>);
     if (smem > 48 * 1024)
         DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned blocks = (unsigned)((n_poses + SEARCH_WARPS - 1) / SEARCH_WARPS);
@@ -632,7 +636,11 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
     if (smem > 200 * 1024) return DOCK_EINVAL;
     for (int s2 = 1; s2 < n_systems; ++s2)
         if (sys[s2].grid.channels != sys[0].grid.channels) return DOCK_EINVAL;      // one gradient mode per launch
-    auto kern = sys[0].grid.channels == 4 ? search_kernel<true> : search_kernel<false>;
+    int n_max = 0;
+    for (int s2 = 0; s2 < n_systems; ++s2) n_max = std::max(n_max, (int)ligands[s2].N);
+    const bool vec4 = n_max <= 48;        // float4 per atom unless the ligands are large (eval_warp.cuh)
+    auto kern = sys[0].grid.channels == 4 ? (vec4 ? search_kernel<true, true> : search_kernel<true, false>)
+                                          : (vec4 ? search_kernel<false, true> : search_kernel<false, false>);
     if (smem > 48 * 1024)
         DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const long long total = (long long)n_systems * copies;
