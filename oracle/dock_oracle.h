@@ -20,6 +20,8 @@
  *       step rule and safeguards are readings (S13): PARITY UNPINNED for the constants, algorithm pinned on quadratics
  *   O9  many-copy Monte-Carlo          : PAPER.md:65-67 (reading S14-S16); search outcome: PARITY UNPINNED beyond GPU-vs-oracle
  *   O10 ranking + RMSD clustering      : PAPER.md:67, 81 (reading S19)
+ *   NEXT-2 eq. 4 gradient maps         : PAPER.md:51, 221 -- orc_build_grid_grad + interpolation in orc_eval when orc_grid.gdata != NULL
+ *   NEXT-3 site-restrained start poses : Fig. 3 (reading S22) -- orc_init_pose_site
  *   Philox4x32-10                      : Salmon et al. SC'11, as restated in SURVEY.md 8(c) R-rules
  *
  * Units: Angstrom, kcal/mol, radians.  All arrays C-contiguous, host memory, double / int32.
