@@ -157,8 +157,9 @@ int dock_score_batch(const dock_params *params, const dock_grid *grid, const doc
 /* Same, with HOST buffers for poses / energy / grad / terms (copies inside the call; pinned memory makes them
  * asynchronous).  The batch is processed in up to 8 chunks through a three-stage pipeline -- host->device copy,
  * kernel, device->host copy -- so that both PCIe directions overlap the arithmetic; the kernels run on `stream`,
- * the copies on two side streams that the library creates once (the only resources it owns).  The call returns
- * after everything has completed (`stream` is synchronised once). */
+ * the copies on two side streams that the library creates once (the only resources it owns; because of them this
+ * entry point must not be called from two host threads at once).  The call returns after everything has completed
+ * (`stream` is synchronised once). */
 int dock_score_batch_host(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
                           int64_t n_poses, const float *poses_host,
                           float *energy_host, float *grad_host, float *terms_host,
