@@ -615,3 +615,37 @@ def test_eq4_maps_scores_and_search(dk, orc, torch, tiny):
     oe2, _, _, d2 = orc.score_batch(op, og, oL, r["topk_pose"][0, :k].cpu().numpy().astype(np.float64))
     ok = d2["cutoff_margin"] > KINK_MARGIN
     assert np.all(np.abs(r["topk_e"][0, :k].cpu().numpy() - oe2)[ok] <= tol(oe2)[ok])
+
+
+@pytest.mark.parametrize("w", [(0.05, -0.004, 0.5, -0.03, -0.4), (0.03, 0.006, 0.0, 0.02, 0.3), (-0.02, 0.0, 1.2, 0.0, -0.9),
+                               (0.0, -0.005, 0.84, -0.035, 0.0)])
+def test_other_term_weights_and_signs(dk, orc, torch, tiny, w):
+    """The evaluators fold the weights into exponent arguments and carry forces scaled by -sign(w1): every sign pattern
+    (and zero weights) must reproduce the oracle, on both evaluators (batch scoring and the optimizer's evaluator)."""
+    s, _, _ = tiny
+    p = dk.dock_default_params()
+    op = orc.default_params()
+    for k in range(5):
+        p.w[k] = w[k]
+        op.w[k] = w[k]
+    op = orc.params_as_fp32(op)
+    box = dk.make_box(s.box_center, s.box_size, s.spacing)
+    grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types)
+    lig = dk.LigandHandle(s.ligand)
+    og = orc.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
+    oL = orc.Ligand(s.ligand)
+    assert np.all(np.abs(grid.data.cpu().numpy().astype(np.float64) - og.maps) <= tol(og.maps))
+    rng = np.random.default_rng(91)
+    poses = random_poses(rng, 1031, s.box_center, s.box_size * 1.1, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, f"w={w}",
+                   cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
+    # warp evaluator through the optimizer: zero iterations = one evaluation; one iteration = the oracle's first step
+    o0, e0, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 0)
+    assert torch.allclose(e0, e[:128], rtol=1e-5, atol=1e-4)
+    o1, e1, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 1)
+    r1 = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), 1)[0] for i in range(128)])
+    c1, _, _, d1 = orc.score_batch(op, og, oL, o1.cpu().numpy().astype(np.float64))
+    ok1 = d1["cutoff_margin"] > KINK_MARGIN
+    assert (np.abs(e1.cpu().numpy() - r1) <= 10 * tol(r1))[ok1].mean() >= 0.95
