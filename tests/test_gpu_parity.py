@@ -649,3 +649,34 @@ def test_other_term_weights_and_signs(dk, orc, torch, tiny, w):
     c1, _, _, d1 = orc.score_batch(op, og, oL, o1.cpu().numpy().astype(np.float64))
     ok1 = d1["cutoff_margin"] > KINK_MARGIN
     assert (np.abs(e1.cpu().numpy() - r1) <= 10 * tol(r1))[ok1].mean() >= 0.95
+
+
+def test_non_cubic_box_scores_and_search(dk, orc, torch, tiny):
+    """Box with three different edge lengths (33 x 25 x 41 nodes): index arithmetic of the grid build, the packed
+    cells and both evaluators; atoms outside on every axis exercise the per-axis wall."""
+    s, _, _ = tiny
+    center, size = [10.0, 9.5, 10.5], [12.0, 9.0, 15.0]
+    p = dk.dock_default_params()
+    op = orc.params_as_fp32(orc.default_params())
+    box = dk.make_box(center, size, s.spacing)
+    grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types)
+    assert tuple(grid.dims) == (33, 25, 41)
+    og = orc.build_grid(op, s.protein_xyz, s.protein_type, center, size, s.spacing, s.lig_types)
+    assert np.all(np.abs(grid.data.cpu().numpy().astype(np.float64) - og.maps) <= tol(og.maps))
+    lig, oL = dk.LigandHandle(s.ligand), orc.Ligand(s.ligand)
+    rng = np.random.default_rng(77)
+    poses = random_poses(rng, 1500, np.array(center, np.float32), np.array(size, np.float32) * 1.3, lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, "noncubic",
+                   cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
+    o0, e0, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:96]).cuda(), 0)
+    assert torch.allclose(e0, e[:96], rtol=1e-5, atol=1e-4)
+    r = dk.dock_search(p, [grid], [lig], [box], 32, 4, 40, 21)
+    k = int(r["topk_count"][0])
+    oe2, _, _, d2 = orc.score_batch(op, og, oL, r["topk_pose"][0, :k].cpu().numpy().astype(np.float64))
+    ok = d2["cutoff_margin"] > KINK_MARGIN
+    assert np.all(np.abs(r["topk_e"][0, :k].cpu().numpy() - oe2)[ok] <= tol(oe2)[ok])
+    # the host-generated initial poses lie inside this box
+    init = dk.dock_init_poses(box, lig.T, 21, 0, 32)
+    assert np.all(np.abs(init[:, :3] - np.array(center)) <= np.array(size) / 2 + 1e-5)
