@@ -5,9 +5,9 @@
 //
 // Host: protein atoms are binned into cubic cells of edge = cutoff + 0.01 A over the box grown by the cutoff
 // (counting sort, stable -> fixed summation order).  Device: one thread per node, a warp covers a
-// compact 4x4x2 block of nodes so that its lanes share almost the same in-range atom set; each thread
-// walks the <= 27 cells around its node, decides r < cutoff in fp32 in the stated order
-// (DESIGN.md D-CUT) and accumulates up to 8 maps in registers.
+// compact 4x4x2 block of nodes so that its lanes share almost the same in-range atom set: the warp collects
+// the atoms near its block once (shared-memory candidate list), then each thread walks the list, decides
+// r < cutoff in fp32 in the stated order (DESIGN.md D-CUT) and accumulates up to 8 maps in registers.
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -36,10 +36,17 @@ struct GridBuildArgs {
     int   channels;        // 1, or 4 = (score, d/dx, d/dy, d/dz): eq. 4's per-vertex gradients (NEXT-2)
 };
 
+constexpr int GRID_CAND = 256;       // candidate atoms a warp collects before it evaluates them
+
+// One warp owns a 4 x 4 x 2 block of nodes.  Its lanes first scan the cells around the block TOGETHER -- lane l
+// tests atom j0 + l against the block's centre with the cutoff grown by the block's half-diagonal -- and compact the
+// survivors, in atom order, into a shared-memory list; then every lane walks that list for its own node.  A node's
+// own 27 cells hold about 6.5 times as many atoms as its cutoff sphere, the list about 1.3 times (profiles/r1k.md).
 template <bool GRAD>
 __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
 {
     __shared__ float4 tab[MAPS_PER_PASS * DOCK_MAX_XS_TYPES];
+    __shared__ float4 cand_all[4][GRID_CAND];
     const int m0 = blockIdx.y * MAPS_PER_PASS;
     const int nm = min(MAPS_PER_PASS, A.n_maps - m0);
     for (int k = threadIdx.x; k < nm * A.n_types; k += blockDim.x) tab[k] = A.pair_tab[m0 * A.n_types + k];
@@ -49,35 +56,34 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
     const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8;
     const int bx = blockIdx.x % tbx, by = (blockIdx.x / tbx) % tby, bz = blockIdx.x / (tbx * tby);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int ix = bx * 8 + (warp & 1) * 4 + (lane & 3);
-    const int iy = by * 8 + (warp >> 1) * 4 + ((lane >> 2) & 3);
-    const int iz = bz * 2 + (lane >> 4);
-    if (ix >= A.nx || iy >= A.ny || iz >= A.nz) return;
+    const int wx0 = bx * 8 + (warp & 1) * 4, wy0 = by * 8 + (warp >> 1) * 4, wz0 = bz * 2;
+    if (wx0 >= A.nx || wy0 >= A.ny || wz0 >= A.nz) return;            // whole warp outside the lattice
+    const int ix = wx0 + (lane & 3), iy = wy0 + ((lane >> 2) & 3), iz = wz0 + (lane >> 4);
+    const bool live = ix < A.nx && iy < A.ny && iz < A.nz;
+    float4 *cand = cand_all[warp];
 
     // node coordinate exactly as the oracle's fp32 cutoff rule states it: fmaf(i, h, origin)
     const float mx = __fmaf_rn((float)ix, A.h, A.ox);
     const float my = __fmaf_rn((float)iy, A.h, A.oy);
     const float mz = __fmaf_rn((float)iz, A.h, A.oz);
-    const int cx = (int)((mx - A.clo[0]) * A.inv_cell);
-    const int cy = (int)((my - A.clo[1]) * A.inv_cell);
-    const int cz = (int)((mz - A.clo[2]) * A.inv_cell);
+    // the warp's block: centre, and the cutoff grown by its half-diagonal (1.5, 1.5, 0.5 spacings) plus a guard band
+    const float cxw = fmaf((float)wx0 + 1.5f, A.h, A.ox), cyw = fmaf((float)wy0 + 1.5f, A.h, A.oy), czw = fmaf((float)wz0 + 0.5f, A.h, A.oz);
+    const float reach = A.cutoff + 2.18f * A.h + 0.01f;
+    const float reach2 = reach * reach;
+    const int cx_lo = max((int)floorf((cxw - reach - A.clo[0]) * A.inv_cell), 0), cx_hi = min((int)floorf((cxw + reach - A.clo[0]) * A.inv_cell), A.ncx - 1);
+    const int cy_lo = max((int)floorf((cyw - reach - A.clo[1]) * A.inv_cell), 0), cy_hi = min((int)floorf((cyw + reach - A.clo[1]) * A.inv_cell), A.ncy - 1);
+    const int cz_lo = max((int)floorf((czw - reach - A.clo[2]) * A.inv_cell), 0), cz_hi = min((int)floorf((czw + reach - A.clo[2]) * A.inv_cell), A.ncz - 1);
 
     float acc[MAPS_PER_PASS], agx[MAPS_PER_PASS], agy[MAPS_PER_PASS], agz[MAPS_PER_PASS];
 #pragma unroll
     for (int m = 0; m < MAPS_PER_PASS; ++m) acc[m] = agx[m] = agy[m] = agz[m] = 0.0f;
 
-    for (int dz = -1; dz <= 1; ++dz) {
-        const int zc = cz + dz;
-        if (zc < 0 || zc >= A.ncz) continue;
-        for (int dy = -1; dy <= 1; ++dy) {
-            const int yc = cy + dy;
-            if (yc < 0 || yc >= A.ncy) continue;
-            // the three x-cells are contiguous in the sorted atom array
-            const int xlo = max(cx - 1, 0), xhi = min(cx + 1, A.ncx - 1);
-            const int base = (zc * A.ncy + yc) * A.ncx;
-            const int j0 = __ldg(&A.cell_start[base + xlo]), j1 = __ldg(&A.cell_start[base + xhi + 1]);
-            for (int j = j0; j < j1; ++j) {
-                const float4 a = __ldg(&A.atoms[j]);
+    // every lane adds the listed atoms to its own node, in list (= atom) order
+    auto flush = [&](int n_cand) {
+        __syncwarp();
+        if (live)
+            for (int k = 0; k < n_cand; ++k) {
+                const float4 a = cand[k];
                 const float fx = __fsub_rn(mx, a.x), fy = __fsub_rn(my, a.y), fz = __fsub_rn(mz, a.z);
                 const float r2 = __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx)));
                 if (r2 < A.cutoff2) {
@@ -101,15 +107,40 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
                                 float de = fmaf(-8.0f * d, A.w[0] * g1, fmaf(-0.5f * dm3, A.w[1] * g2, 2.0f * A.w[2] * rep));
                                 de -= (d >= 0.5f && d < 1.5f) ? t.y : 0.0f;
                                 de -= (d >= -0.7f && d < 0.0f) ? t.z * 1.4285714285714286f : 0.0f;
-                                const float k = r > 0.0f ? de / r : 0.0f;
-                                agx[m] = fmaf(k, fx, agx[m]); agy[m] = fmaf(k, fy, agy[m]); agz[m] = fmaf(k, fz, agz[m]);
+                                const float k2 = r > 0.0f ? de / r : 0.0f;
+                                agx[m] = fmaf(k2, fx, agx[m]); agy[m] = fmaf(k2, fy, agy[m]); agz[m] = fmaf(k2, fz, agz[m]);
                             }
                         }
                     }
                 }
             }
+        __syncwarp();
+    };
+
+    int n_cand = 0;
+    for (int zc = cz_lo; zc <= cz_hi; ++zc)
+        for (int yc = cy_lo; yc <= cy_hi; ++yc) {
+            // the x-cells of a row are contiguous in the sorted atom array
+            const int base = (zc * A.ncy + yc) * A.ncx;
+            const int j0 = __ldg(&A.cell_start[base + cx_lo]), j1 = __ldg(&A.cell_start[base + cx_hi + 1]);
+            for (int jb = j0; jb < j1; jb += 32) {
+                const int j = jb + lane;
+                float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+                bool near = false;
+                if (j < j1) {
+                    a = __ldg(&A.atoms[j]);
+                    const float dx = a.x - cxw, dy = a.y - cyw, dz = a.z - czw;
+                    near = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < reach2;
+                }
+                const unsigned mask = __ballot_sync(FULL_MASK, near);
+                if (n_cand + __popc(mask) > GRID_CAND) { flush(n_cand); n_cand = 0; }
+                if (near) cand[n_cand + __popc(mask & ((1u << lane) - 1u))] = a;
+                n_cand += __popc(mask);
+            }
         }
-    }
+    flush(n_cand);
+    if (!live) return;
+
     const size_t nodes = (size_t)A.nx * A.ny * A.nz;
     const size_t node = ((size_t)iz * A.ny + iy) * A.nx + ix;
 #pragma unroll
