@@ -34,6 +34,11 @@ struct GridBuildArgs {
     const float4 *pair_tab;// [n_maps][n_types] {rsum, wh, whb, 0}
     float        *out;     // [n_maps][channels][nz][ny][nx]
     int   channels;        // 1, or 4 = (score, d/dx, d/dy, d/dz): eq. 4's per-vertex gradients (NEXT-2)
+    // maps are processed in order of ligand radius: slot k writes map map_of[k]; bit k of fresh says that slot k
+    // has another radius than slot k-1 (or opens a pass), i.e. the distance-only part of the term must be recomputed.
+    // The two Gaussians and the repulsion depend on the ligand type only through its radius.
+    int      map_of[DOCK_MAX_XS_TYPES];
+    unsigned fresh;
 };
 
 constexpr int GRID_CAND = 256;       // candidate atoms a warp collects before it evaluates them
@@ -89,22 +94,25 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
                 if (r2 < A.cutoff2) {
                     const float r = sqrtf(r2);
                     const int tj = __float_as_int(a.w);
+                    float d = 0.f, dm3 = 0.f, rep = 0.f, base = 0.f, dbase = 0.f;
 #pragma unroll
                     for (int m = 0; m < MAPS_PER_PASS; ++m) {
                         if (m < nm) {
                             const float4 t = tab[m * A.n_types + tj];
-                            const float d = r - t.x;
-                            const float g1 = fast_ex2(-5.770780163555854f * d * d);
-                            const float dm3 = d - 3.0f;
-                            const float g2 = fast_ex2(-0.36067376022224085f * dm3 * dm3);
-                            const float rep = fminf(d, 0.0f);
-                            float e = A.w[0] * g1 + A.w[1] * g2;
-                            e = fmaf(A.w[2] * rep, rep, e);
-                            e = fmaf(t.y, __saturatef(1.5f - d), e);
+                            if ((A.fresh >> (m0 + m)) & 1u) {             // uniform: a new ligand radius
+                                d = r - t.x;
+                                const float g1 = A.w[0] * fast_ex2(-5.770780163555854f * d * d);
+                                dm3 = d - 3.0f;
+                                const float g2 = A.w[1] * fast_ex2(-0.36067376022224085f * dm3 * dm3);
+                                rep = fminf(d, 0.0f);
+                                base = fmaf(A.w[2] * rep, rep, g1 + g2);
+                                if (GRAD) dbase = fmaf(-8.0f * d, g1, fmaf(-0.5f * dm3, g2, 2.0f * A.w[2] * rep));
+                            }
+                            float e = fmaf(t.y, __saturatef(1.5f - d), base);
                             e = fmaf(t.z, __saturatef(d * -1.4285714285714286f), e);
                             acc[m] += e;
                             if (GRAD) {                                   // d f / d(vertex) = f'(r) (m - r_j) / r
-                                float de = fmaf(-8.0f * d, A.w[0] * g1, fmaf(-0.5f * dm3, A.w[1] * g2, 2.0f * A.w[2] * rep));
+                                float de = dbase;
                                 de -= (d >= 0.5f && d < 1.5f) ? t.y : 0.0f;
                                 de -= (d >= -0.7f && d < 0.0f) ? t.z * 1.4285714285714286f : 0.0f;
                                 const float k2 = r > 0.0f ? de / r : 0.0f;
@@ -146,7 +154,7 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
 #pragma unroll
     for (int m = 0; m < MAPS_PER_PASS; ++m)
         if (m < nm) {
-            float *o = A.out + (size_t)(m0 + m) * A.channels * nodes + node;
+            float *o = A.out + (size_t)A.map_of[m0 + m] * A.channels * nodes + node;
             o[0] = acc[m];
             if (GRAD) { o[nodes] = agx[m]; o[2 * nodes] = agy[m]; o[3 * nodes] = agz[m]; }
         }
@@ -183,7 +191,9 @@ struct GridPlan {
     float inv_cell;
     std::vector<float4> atoms;
     std::vector<int> cell_start;
-    std::vector<float4> pair_tab;
+    std::vector<float4> pair_tab;   // rows in processing order (maps sorted by ligand radius)
+    int map_of[DOCK_MAX_XS_TYPES];
+    unsigned fresh;
 };
 
 int plan_grid(const dock_params *p, const dock_protein *prot, const dock_box *box, int n_lig_types,
@@ -235,14 +245,22 @@ int plan_grid(const dock_params *p, const dock_protein *prot, const dock_box *bo
         std::memcpy(&a.w, &t, 4);
         pl.atoms[cursor[cell_of[j]]++] = a;
     }
+    // processing order: maps sorted by ligand radius, so that maps of equal radius share the distance-only terms
+    std::vector<int> order(n_lig_types);
+    for (int m = 0; m < n_lig_types; ++m) order[m] = m;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->radius[lig_types[a]] < p->radius[lig_types[b]]; });
+    pl.fresh = 0u;
     pl.pair_tab.resize((size_t)n_lig_types * p->n_types);
-    for (int m = 0; m < n_lig_types; ++m)
+    for (int k = 0; k < n_lig_types; ++k) {
+        const int m = order[k], a = lig_types[m];
+        pl.map_of[k] = m;
+        if (k % MAPS_PER_PASS == 0 || p->radius[a] != p->radius[lig_types[order[k - 1]]]) pl.fresh |= 1u << k;
         for (int t = 0; t < p->n_types; ++t) {
-            const int a = lig_types[m];
             const float wh = (p->hydrophobic[a] && p->hydrophobic[t]) ? p->w[3] : 0.f;
             const float whb = ((p->donor[a] && p->acceptor[t]) || (p->donor[t] && p->acceptor[a])) ? p->w[4] : 0.f;
-            pl.pair_tab[(size_t)m * p->n_types + t] = make_float4(p->radius[a] + p->radius[t], wh, whb, 0.f);
+            pl.pair_tab[(size_t)k * p->n_types + t] = make_float4(p->radius[a] + p->radius[t], wh, whb, 0.f);
         }
+    }
     return DOCK_OK;
 }
 
@@ -305,6 +323,8 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     A.pair_tab = (const float4 *)(ws + b_atoms + b_cells);
     A.out = grid_dev;
     A.channels = params->grad_mode == 1 ? 4 : 1;
+    for (int k = 0; k < DOCK_MAX_XS_TYPES; ++k) A.map_of[k] = k < n_lig_types ? pl.map_of[k] : 0;
+    A.fresh = pl.fresh;
     const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8, tbz = (A.nz + 1) / 2;
     dim3 grid((unsigned)(tbx * tby * tbz), (unsigned)((n_lig_types + MAPS_PER_PASS - 1) / MAPS_PER_PASS));
     if (A.channels == 4) grid_build_kernel<true><<<grid, 128, 0, stream>>>(A);
