@@ -338,7 +338,7 @@ def run_ours(args) -> dict:
         bx = [dk.make_box(q.box_center, q.box_size, q.spacing) for q in sy]
         lg = [dk.LigandHandle(q.ligand) for q in sy]
         t0 = time.perf_counter()
-        gr = [dk.dock_build_grids(p, q.protein_xyz, q.protein_type, b, q.lig_types) for q, b in zip(sy, bx)]
+        gr = dk.dock_build_grids_batch(p, [(q.protein_xyz, q.protein_type) for q in sy], bx, sy[0].lig_types)
         torch.cuda.synchronize()
         t_g3 = time.perf_counter() - t0
         run3 = lambda: dk.dock_search(p, gr, lg, bx, 128, 40, 300, 2023)

@@ -146,6 +146,14 @@ int dock_build_grids(const dock_params *params, const dock_protein *protein, con
                      float *grid_dev, dock_grid *out_desc,
                      void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
+/* Batched form (BASELINE.json configs[3]): n_systems (protein, box) pairs with one ligand-type list, enqueued back to
+ * back on `stream`.  proteins, boxes, out_descs: HOST arrays [n_systems]; grid_dev: HOST array of n_systems DEVICE
+ * buffers (dock_grid_bytes each).  One workspace serves all systems (the stream orders them); *needed = the largest. */
+int dock_build_grids_batch(const dock_params *params, int32_t n_systems, const dock_protein *proteins,
+                           const dock_box *boxes, int32_t n_lig_types, const int32_t *lig_types,
+                           float *const *grid_dev, dock_grid *out_descs,
+                           void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
 /* ---- A2-A5: fused pose -> coordinates -> energy + gradient (eq. 2-3 at 198-219) --
  * poses_dev [n_poses][7+T]; energy_dev [n_poses]; grad_dev [n_poses][6+T] or NULL;
  * terms_dev [n_poses][3] = (E_grid, E_wall, E_intra) or NULL.  E = sum of the three terms. */

@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     LigandHandle,
     dock_box,
     dock_build_grids,
+    dock_build_grids_batch,
     dock_default_params,
     dock_grid,
     dock_grid_bytes,

@@ -22,7 +22,7 @@ DOCK_TRACE_HEADER = 8
 DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
 
 EXPORTS = [
-    "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_score_batch",
+    "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_build_grids_batch", "dock_score_batch",
     "dock_score_batch_host", "dock_local_opt_batch", "dock_init_poses", "dock_init_poses_site", "dock_search", "dock_topk",
     "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
 ]
@@ -224,6 +224,48 @@ def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_b
                                 _ptr(buf), C.byref(desc), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
                                 _stream(stream)), "dock_build_grids")
     return GridMaps(buf, data, desc)
+
+
+def dock_build_grids_batch(params: dock_params, proteins, boxes: Sequence[dock_box], lig_types: Sequence[int],
+                           stream=None):
+    """proteins: sequence of (xyz [n,3], type [n]).  One C call for all systems (BASELINE.json configs[3]); returns a
+    list of GridMaps."""
+    torch = _torch()
+    lib = load_library()
+    ns = len(proteins)
+    assert len(boxes) == ns
+    lt = np.ascontiguousarray(lig_types, dtype=np.int32)
+    ch = 4 if int(params.grad_mode) == 1 else 1
+    keep, prots, bxs = [], (dock_protein * ns)(), (dock_box * ns)()
+    bufs, datas = [], []
+    ptrs = (C.c_void_p * ns)()
+    for s, (xyz, typ) in enumerate(proteins):
+        xyz = np.ascontiguousarray(xyz, dtype=np.float32).reshape(-1, 3)
+        typ = np.ascontiguousarray(typ, dtype=np.int32)
+        keep.append((xyz, typ))
+        prots[s] = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
+        bxs[s] = boxes[s]
+        nx, ny, nz = dock_grid_dims(boxes[s])
+        buf = torch.empty(dock_grid_bytes(boxes[s], len(lt) * ch), dtype=torch.uint8, device="cuda")
+        data = buf[: len(lt) * ch * nz * ny * nx * 4].view(torch.float32)
+        datas.append(data.view(len(lt), nz, ny, nx) if ch == 1 else data.view(len(lt), ch, nz, ny, nx))
+        bufs.append(buf)
+        ptrs[s] = buf.data_ptr()
+    descs = (dock_grid * ns)()
+    need = C.c_size_t(0)
+    rc = lib.dock_build_grids_batch(C.byref(params), ns, prots, bxs, len(lt), _np_ptr(lt), None, None, None,
+                                    C.c_size_t(0), C.byref(need), None)
+    if rc not in (DOCK_EWORKSPACE, DOCK_OK):
+        _check(rc, "dock_build_grids_batch(size query)")
+    ws = _ws.get(max(need.value, 256))
+    _check(lib.dock_build_grids_batch(C.byref(params), ns, prots, bxs, len(lt), _np_ptr(lt), ptrs, descs, _ptr(ws),
+                                      C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_build_grids_batch")
+    out = []
+    for s in range(ns):
+        d = dock_grid()
+        C.memmove(C.byref(d), C.byref(descs[s]), C.sizeof(dock_grid))
+        out.append(GridMaps(bufs[s], datas[s], d))
+    return out
 
 
 def dock_score_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses,

@@ -348,3 +348,32 @@ extern "C" int dock_build_grids(const dock_params *params, const dock_protein *p
     out_desc->n_channels = A.channels;
     return DOCK_OK;
 }
+
+// Batched form (BASELINE.json configs[3]): n_systems independent (protein, box) pairs with the same
+// ligand-type list, enqueued back to back on one stream.  The systems share one workspace: uploads and kernels of
+// consecutive systems are ordered by the stream.
+extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_systems, const dock_protein *proteins,
+                                      const dock_box *boxes, int32_t n_lig_types, const int32_t *lig_types,
+                                      float *const *grid_dev, dock_grid *out_descs,
+                                      void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+{
+    if (n_systems < 0 || (n_systems > 0 && (!proteins || !boxes))) return DOCK_EINVAL;
+    size_t need = 0;
+    for (int s = 0; s < n_systems; ++s) {
+        size_t n1 = 0;
+        const int rc = dock_build_grids(params, &proteins[s], &boxes[s], n_lig_types, lig_types, nullptr, nullptr, nullptr, 0,
+                                        &n1, nullptr);
+        if (rc != DOCK_EWORKSPACE) return rc == DOCK_OK ? DOCK_EINVAL : rc;
+        need = std::max(need, n1);
+    }
+    if (needed) *needed = need;
+    if (n_systems == 0) return DOCK_OK;
+    if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
+    if (!grid_dev || !out_descs) return DOCK_EINVAL;
+    for (int s = 0; s < n_systems; ++s) {
+        const int rc = dock_build_grids(params, &proteins[s], &boxes[s], n_lig_types, lig_types, grid_dev[s], &out_descs[s],
+                                        ws_dev, ws_bytes, nullptr, stream_);
+        if (rc != DOCK_OK) return rc;
+    }
+    return DOCK_OK;
+}

@@ -680,3 +680,22 @@ def test_non_cubic_box_scores_and_search(dk, orc, torch, tiny):
     # the host-generated initial poses lie inside this box
     init = dk.dock_init_poses(box, lig.T, 21, 0, 32)
     assert np.all(np.abs(init[:, :3] - np.array(center)) <= np.array(size) / 2 + 1e-5)
+
+
+def test_batched_grid_build_equals_single_builds(dk, torch):
+    """dock_build_grids_batch (SURVEY.md 8(b), configs[3]): heterogeneous proteins and boxes in one call give bitwise
+    the maps of one call per system, in both images."""
+    systems = [make_system(3, seed=0, index=i, n_prot=400 + 150 * i) for i in range(4)]
+    p = dk.dock_default_params()
+    boxes = [dk.make_box(s.box_center, s.box_size if i != 2 else s.box_size * np.array([0.5, 0.75, 1.0], np.float32), s.spacing)
+             for i, s in enumerate(systems)]
+    lt = systems[0].lig_types
+    batch = dk.dock_build_grids_batch(p, [(s.protein_xyz, s.protein_type) for s in systems], boxes, lt)
+    assert len(batch) == 4
+    for s, b, g in zip(systems, boxes, batch):
+        one = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, b, lt)
+        assert tuple(g.dims) == tuple(one.dims)
+        assert torch.equal(g.data, one.data)                                 # the maps ...
+        off = (g.data.numel() * 4 + 255) // 256 * 256                        # ... and the packed gather image behind them
+        assert torch.equal(g.buf[off:], one.buf[off:])
+    assert dk.dock_build_grids_batch(p, [], [], lt) == []
