@@ -186,74 +186,67 @@ void orc_grid_geometry(const double center[3], const double size[3], double h, i
 
 void orc_build_grid(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
                     const int dims[3], const double origin[3], double h,
-                    int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *G)
+                    int n_lig_types, const int32_t *lig_types, double *G)
 {
     const int nx = dims[0], ny = dims[1], nz = dims[2];
     const int64_t nodes = (int64_t)nx * ny * nz;
-    const float hf = (float)h;
-    const float cut2f = (float)p->cutoff * (float)p->cutoff;
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t m = 0; m < nodes; ++m) {
         int ix = (int)(m % nx), iy = (int)((m / nx) % ny), iz = (int)(m / ((int64_t)nx * ny));
         double mx = origin[0] + h * ix, my = origin[1] + h * iy, mz = origin[2] + h * iz;
-        /* fp32 node coordinate, as the kernel forms it: fmaf(i, h, origin) */
-        float mxf = fmaf((float)ix, hf, (float)origin[0]);
-        float myf = fmaf((float)iy, hf, (float)origin[1]);
-        float mzf = fmaf((float)iz, hf, (float)origin[2]);
         for (int t = 0; t < n_lig_types; ++t) G[(int64_t)t * nodes + m] = 0.0;
         for (int j = 0; j < np; ++j) {
             double dx = mx - pxyz[3 * j], dy = my - pxyz[3 * j + 1], dz = mz - pxyz[3 * j + 2];
             double r = sqrt(dx * dx + dy * dy + dz * dz);
-            int in_range;
-            if (fp32_cutoff) {
-                float fx = mxf - (float)pxyz[3 * j], fy = myf - (float)pxyz[3 * j + 1], fz = mzf - (float)pxyz[3 * j + 2];
-                float r2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
-                in_range = r2f < cut2f;
-                if (in_range && !(r < p->cutoff)) r = nextafter(p->cutoff, 0.0); /* value side of the same decision */
-            } else {
-                in_range = r < p->cutoff;
-            }
-            if (!in_range) continue;
+            if (!(r < p->cutoff)) continue;                    /* S3: strict, decided in double */
             for (int t = 0; t < n_lig_types; ++t)
                 G[(int64_t)t * nodes + m] += orc_pair(p, lig_types[t], ptype[j], r, NULL);
         }
     }
 }
 
-/* ---------------------------------------------------------------------------------------
- * small vector / quaternion helpers
- * ------------------------------------------------------------------------------------- */
-/* NEXT-2 / eq. 4 (PAPER.md:221): per-vertex gradient of the vertex score, by the same brute force as O2. */
-void orc_build_grid_grad(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
-                         const int dims[3], const double origin[3], double h,
-                         int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *GD)
+/* Diagnostic only (changes no result): flags[node] = 1 iff some protein atom lies within `margin` of the cutoff
+ * sphere of that node, i.e. | |node - r_j| - cutoff | < margin.  The vertex score jumps by f(cutoff^-) (about
+ * -0.004 per atom, reading S3) there, so an implementation in another precision may legitimately count that atom
+ * on the other side; the parity tests exempt these nodes and assert that they are few.  Returns the number flagged. */
+int64_t orc_grid_cutoff_flags(int np, const double *pxyz, const int dims[3], const double origin[3], double h,
+                              double cutoff, double margin, uint8_t *flags)
 {
     const int nx = dims[0], ny = dims[1], nz = dims[2];
     const int64_t nodes = (int64_t)nx * ny * nz;
-    const float hf = (float)h;
-    const float cut2f = (float)p->cutoff * (float)p->cutoff;
+    int64_t count = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : count)
+    for (int64_t m = 0; m < nodes; ++m) {
+        int ix = (int)(m % nx), iy = (int)((m / nx) % ny), iz = (int)(m / ((int64_t)nx * ny));
+        double mx = origin[0] + h * ix, my = origin[1] + h * iy, mz = origin[2] + h * iz;
+        int near = 0;
+        for (int j = 0; j < np && !near; ++j) {
+            double dx = mx - pxyz[3 * j], dy = my - pxyz[3 * j + 1], dz = mz - pxyz[3 * j + 2];
+            if (fabs(sqrt(dx * dx + dy * dy + dz * dz) - cutoff) < margin) near = 1;
+        }
+        flags[m] = (uint8_t)near;
+        count += near;
+    }
+    return count;
+}
+
+/* NEXT-2 / eq. 4 (PAPER.md:221): per-vertex gradient of the vertex score, by the same brute force as O2. */
+void orc_build_grid_grad(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
+                         const int dims[3], const double origin[3], double h,
+                         int n_lig_types, const int32_t *lig_types, double *GD)
+{
+    const int nx = dims[0], ny = dims[1], nz = dims[2];
+    const int64_t nodes = (int64_t)nx * ny * nz;
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t m = 0; m < nodes; ++m) {
         int ix = (int)(m % nx), iy = (int)((m / nx) % ny), iz = (int)(m / ((int64_t)nx * ny));
         double mx = origin[0] + h * ix, my = origin[1] + h * iy, mz = origin[2] + h * iz;
-        float mxf = fmaf((float)ix, hf, (float)origin[0]);
-        float myf = fmaf((float)iy, hf, (float)origin[1]);
-        float mzf = fmaf((float)iz, hf, (float)origin[2]);
         for (int t = 0; t < n_lig_types; ++t)
             for (int c = 0; c < 3; ++c) GD[((int64_t)t * 3 + c) * nodes + m] = 0.0;
         for (int j = 0; j < np; ++j) {
             double d[3] = {mx - pxyz[3 * j], my - pxyz[3 * j + 1], mz - pxyz[3 * j + 2]};
             double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-            int in_range;
-            if (fp32_cutoff) {
-                float fx = mxf - (float)pxyz[3 * j], fy = myf - (float)pxyz[3 * j + 1], fz = mzf - (float)pxyz[3 * j + 2];
-                float r2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
-                in_range = r2f < cut2f;
-                if (in_range && !(r < p->cutoff)) r = nextafter(p->cutoff, 0.0);
-            } else {
-                in_range = r < p->cutoff;
-            }
-            if (!in_range || r <= 0.0) continue;
+            if (!(r < p->cutoff) || r <= 0.0) continue;
             for (int t = 0; t < n_lig_types; ++t) {
                 double dfdr;
                 orc_pair(p, lig_types[t], ptype[j], r, &dfdr);
@@ -263,6 +256,9 @@ void orc_build_grid_grad(const orc_params *p, int np, const double *pxyz, const 
     }
 }
 
+/* ---------------------------------------------------------------------------------------
+ * small vector / quaternion helpers
+ * ------------------------------------------------------------------------------------- */
 static void cross(const double a[3], const double b[3], double c[3])
 {
     c[0] = a[1] * b[2] - a[2] * b[1];
@@ -623,93 +619,144 @@ void orc_grad_cond_batch(const orc_params *p, const orc_grid *g, const orc_ligan
  * over the retraction x (+) s (`add`), so that the pin tests can run it on closed-form
  * quadratics; orc_local_opt instantiates it with the docking objective and orc_pose_add.
  * `obs` (nullable) is called after every accepted iteration with (it, f, H, s, y, updated).
+ *
+ * One iteration is written once (bfgs_iteration) and used by the full loop (orc_bfgs) and by the
+ * single-step replay of the iteration-level teacher-forced parity test (orc_bfgs_step).
  * ------------------------------------------------------------------------------------- */
+typedef struct {
+    int n, np_;
+    double *H, *A, *B, *x, *xt, *gr, *gt, *d, *s, *y;
+    double f;
+    int fresh;        /* H is still the identity (no update applied since the start or the last reset) */
+    int ne;           /* evaluations so far */
+} bfgs_state;
+
+static void bfgs_alloc(bfgs_state *S, int n, int np_)
+{
+    S->n = n; S->np_ = np_;
+    S->H = (double *)malloc(sizeof(double) * n * n);
+    S->A = (double *)malloc(sizeof(double) * n * n);
+    S->B = (double *)malloc(sizeof(double) * n * n);
+    S->x = (double *)malloc(sizeof(double) * np_); S->xt = (double *)malloc(sizeof(double) * np_);
+    S->gr = (double *)malloc(sizeof(double) * n); S->gt = (double *)malloc(sizeof(double) * n);
+    S->d = (double *)malloc(sizeof(double) * n); S->s = (double *)malloc(sizeof(double) * n); S->y = (double *)malloc(sizeof(double) * n);
+    S->f = 0.0; S->fresh = 1; S->ne = 0;
+}
+static void bfgs_free(bfgs_state *S)
+{
+    free(S->H); free(S->A); free(S->B); free(S->x); free(S->xt); free(S->gr); free(S->gt); free(S->d); free(S->s); free(S->y);
+}
+
+/* One iteration from the state (x, f, gr, H, fresh).  Returns 0 if a step was accepted (state advanced),
+ * ORC_EXIT_GTOL if ||g|| < gtol (nothing done), ORC_EXIT_LINESEARCH if no trial was acceptable (state unchanged).
+ * `rec` (nullable) receives the decision scalars of the iteration. */
+static int bfgs_iteration(const orc_params *p, bfgs_state *S, orc_objective_fn fn, orc_retract_fn add, void *ctx,
+                          orc_iter_rec *rec)
+{
+    const int n = S->n, np_ = S->np_;
+    double *H = S->H, *A = S->A, *B = S->B, *x = S->x, *xt = S->xt, *gr = S->gr, *gt = S->gt, *d = S->d, *s = S->s, *y = S->y;
+    if (rec) { memset(rec, 0, sizeof(*rec)); rec->f = S->f; rec->fresh_in = S->fresh; }
+    double gn = 0.0;
+    for (int k = 0; k < n; ++k) gn += gr[k] * gr[k];
+    if (rec) rec->gnorm = sqrt(gn);
+    if (sqrt(gn) < p->bfgs_gtol) { if (rec) rec->status = ORC_EXIT_GTOL; return ORC_EXIT_GTOL; }
+    double gp = 0.0;
+    for (int r = 0; r < n; ++r) {                      /* d = -H g */
+        double a = 0.0;
+        for (int c = 0; c < n; ++c) a += H[r * n + c] * gr[c];
+        d[r] = -a;
+        gp += gr[r] * d[r];
+    }
+    if (gp >= 0.0) {                                   /* not a descent direction: reset H = I */
+        for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? 1.0 : 0.0;
+        S->fresh = 1;
+        gp = 0.0;
+        for (int r = 0; r < n; ++r) { d[r] = -gr[r]; gp += gr[r] * d[r]; }
+        if (rec) rec->reset = 1;
+    }
+    double alpha = 1.0;
+    if (S->fresh) {                                    /* alpha0 = min(1, 1/||d||) while H = I */
+        double dn = 0.0;
+        for (int k = 0; k < n; ++k) dn += d[k] * d[k];
+        dn = sqrt(dn);
+        if (dn > 1.0) alpha = 1.0 / dn;
+    }
+    if (rec) { rec->gp = gp; rec->alpha0 = alpha; }
+    int ok = 0;
+    double ft = S->f;
+    for (int trial = 0; trial < p->bfgs_max_trials; ++trial) {
+        for (int k = 0; k < n; ++k) s[k] = alpha * d[k];
+        add(ctx, x, s, xt);
+        ft = fn(ctx, xt, gt);
+        ++S->ne;
+        if (rec) {
+            rec->trials = trial + 1;
+            rec->alpha = alpha;
+            if (trial < ORC_MAX_TRIALS) rec->armijo_margin[trial] = (ft - S->f) - p->bfgs_c1 * alpha * gp;
+        }
+        if (ft - S->f <= p->bfgs_c1 * alpha * gp) { ok = 1; break; }   /* Armijo */
+        alpha *= p->bfgs_shrink;
+    }
+    if (!ok) { if (rec) rec->status = ORC_EXIT_LINESEARCH; return ORC_EXIT_LINESEARCH; }
+    double ys = 0.0, yy = 0.0, ss = 0.0;
+    for (int k = 0; k < n; ++k) {
+        y[k] = gt[k] - gr[k];
+        ys += y[k] * s[k]; yy += y[k] * y[k]; ss += s[k] * s[k];
+    }
+    memcpy(x, xt, sizeof(double) * np_);
+    memcpy(gr, gt, sizeof(double) * n);
+    S->f = ft;
+    int updated = 0;
+    if (rec) { rec->f_new = ft; rec->curv_margin = ys - p->bfgs_curv_eps * sqrt(ss) * sqrt(yy); }
+    if (ys > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) {
+        if (S->fresh) {                                /* first update: H = (y.s / y.y) I */
+            double sc = ys / yy;
+            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? sc : 0.0;
+            S->fresh = 0;
+        }
+        /* H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T */
+        double rho = 1.0 / ys;
+        for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {   /* A = (I - rho s y^T) H */
+            double a = H[r * n + c];
+            for (int k = 0; k < n; ++k) a -= rho * s[r] * y[k] * H[k * n + c];
+            A[r * n + c] = a;
+        }
+        for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {   /* B = A (I - rho y s^T) + rho s s^T */
+            double a = A[r * n + c];
+            for (int k = 0; k < n; ++k) a -= A[r * n + k] * rho * y[k] * s[c];
+            B[r * n + c] = a + rho * s[r] * s[c];
+        }
+        memcpy(H, B, sizeof(double) * n * n);
+        updated = 1;
+    }
+    if (rec) { rec->updated = updated; rec->fresh_out = S->fresh; }
+    return 0;
+}
+
 double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
                 orc_objective_fn fn, orc_retract_fn add, void *ctx,
-                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx)
+                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx,
+                int *exit_reason, orc_iter_rec *recs, int max_recs)
 {
-    double *H = (double *)malloc(sizeof(double) * n * n);
-    double *A = (double *)malloc(sizeof(double) * n * n);
-    double *B = (double *)malloc(sizeof(double) * n * n);
-    double *x = (double *)malloc(sizeof(double) * np_), *xt = (double *)malloc(sizeof(double) * np_);
-    double *gr = (double *)malloc(sizeof(double) * n), *gt = (double *)malloc(sizeof(double) * n);
-    double *d = (double *)malloc(sizeof(double) * n), *s = (double *)malloc(sizeof(double) * n), *y = (double *)malloc(sizeof(double) * n);
-    int it = 0, ne = 0, fresh = 1;
-    memcpy(x, x0, sizeof(double) * np_);
-    double f = fn(ctx, x, gr);
-    ++ne;
-    for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? 1.0 : 0.0;
+    bfgs_state S;
+    bfgs_alloc(&S, n, np_);
+    int it = 0, why = ORC_EXIT_CAP;
+    memcpy(S.x, x0, sizeof(double) * np_);
+    S.f = fn(ctx, S.x, S.gr);
+    ++S.ne;
+    for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) S.H[r * n + c] = (r == c) ? 1.0 : 0.0;
     for (it = 0; it < cap; ++it) {
-        double gn = 0.0;
-        for (int k = 0; k < n; ++k) gn += gr[k] * gr[k];
-        if (sqrt(gn) < p->bfgs_gtol) break;
-        double gp = 0.0;
-        for (int r = 0; r < n; ++r) {                      /* d = -H g */
-            double a = 0.0;
-            for (int c = 0; c < n; ++c) a += H[r * n + c] * gr[c];
-            d[r] = -a;
-            gp += gr[r] * d[r];
-        }
-        if (gp >= 0.0) {                                   /* not a descent direction: reset H = I */
-            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? 1.0 : 0.0;
-            fresh = 1;
-            gp = 0.0;
-            for (int r = 0; r < n; ++r) { d[r] = -gr[r]; gp += gr[r] * d[r]; }
-        }
-        double alpha = 1.0;
-        if (fresh) {                                       /* alpha0 = min(1, 1/||d||) while H = I */
-            double dn = 0.0;
-            for (int k = 0; k < n; ++k) dn += d[k] * d[k];
-            dn = sqrt(dn);
-            if (dn > 1.0) alpha = 1.0 / dn;
-        }
-        int ok = 0;
-        double ft = f;
-        for (int trial = 0; trial < p->bfgs_max_trials; ++trial) {
-            for (int k = 0; k < n; ++k) s[k] = alpha * d[k];
-            add(ctx, x, s, xt);
-            ft = fn(ctx, xt, gt);
-            ++ne;
-            if (ft - f <= p->bfgs_c1 * alpha * gp) { ok = 1; break; }   /* Armijo */
-            alpha *= p->bfgs_shrink;
-        }
-        if (!ok) break;
-        double ys = 0.0, yy = 0.0, ss = 0.0;
-        for (int k = 0; k < n; ++k) {
-            y[k] = gt[k] - gr[k];
-            ys += y[k] * s[k]; yy += y[k] * y[k]; ss += s[k] * s[k];
-        }
-        memcpy(x, xt, sizeof(double) * np_);
-        memcpy(gr, gt, sizeof(double) * n);
-        f = ft;
-        int updated = 0;
-        if (ys > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) {
-            if (fresh) {                                   /* first update: H = (y.s / y.y) I */
-                double sc = ys / yy;
-                for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) H[r * n + c] = (r == c) ? sc : 0.0;
-                fresh = 0;
-            }
-            /* H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T */
-            double rho = 1.0 / ys;
-            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {   /* A = (I - rho s y^T) H */
-                double a = H[r * n + c];
-                for (int k = 0; k < n; ++k) a -= rho * s[r] * y[k] * H[k * n + c];
-                A[r * n + c] = a;
-            }
-            for (int r = 0; r < n; ++r) for (int c = 0; c < n; ++c) {   /* B = A (I - rho y s^T) + rho s s^T */
-                double a = A[r * n + c];
-                for (int k = 0; k < n; ++k) a -= A[r * n + k] * rho * y[k] * s[c];
-                B[r * n + c] = a + rho * s[r] * s[c];
-            }
-            memcpy(H, B, sizeof(double) * n * n);
-            updated = 1;
-        }
-        if (obs) obs(obs_ctx, it, f, H, s, y, updated);
+        orc_iter_rec tmp;
+        const int st = bfgs_iteration(p, &S, fn, add, ctx, (recs && it < max_recs) ? &recs[it] : &tmp);
+        if (st != 0) { why = st; break; }
+        if (obs) obs(obs_ctx, it, S.f, S.H, S.s, S.y, (recs && it < max_recs) ? recs[it].updated : tmp.updated);
     }
-    memcpy(x_out, x, sizeof(double) * np_);
+    memcpy(x_out, S.x, sizeof(double) * np_);
     if (iters) *iters = it;
-    if (evals) *evals = ne;
-    free(H); free(A); free(B); free(x); free(xt); free(gr); free(gt); free(d); free(s); free(y);
+    if (evals) *evals = S.ne;
+    if (exit_reason) *exit_reason = why;
+    const double f = S.f;
+    bfgs_free(&S);
     return f;
 }
 
@@ -722,8 +769,9 @@ typedef struct { const orc_params *p; const orc_grid *g; const orc_ligand *L; } 
  * ------------------------------------------------------------------------------------- */
 double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
               orc_objective_fn fn, orc_retract_fn add, void *ctx,
-              double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx)
+              double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx, int *exit_reason)
 {
+    int why = ORC_EXIT_CAP;
     double *x = (double *)malloc(sizeof(double) * np_), *xn = (double *)malloc(sizeof(double) * np_);
     double *gr = (double *)malloc(sizeof(double) * n), *gn = (double *)malloc(sizeof(double) * n);
     double *s = (double *)malloc(sizeof(double) * n), *y = (double *)malloc(sizeof(double) * n);
@@ -737,7 +785,7 @@ double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
         double g2 = 0.0;
         for (int k = 0; k < n; ++k) g2 += gr[k] * gr[k];
         const double gnorm = sqrt(g2);
-        if (gnorm < p->bfgs_gtol) break;
+        if (gnorm < p->bfgs_gtol) { why = ORC_EXIT_GTOL; break; }
         double alpha;
         if (it == 0) alpha = p->bb_step / gnorm;
         else {
@@ -758,6 +806,7 @@ double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
     }
     if (iters) *iters = it;
     if (evals) *evals = ne;
+    if (exit_reason) *exit_reason = why;
     free(x); free(xn); free(gr); free(gn); free(s); free(y);
     return fbest;
 }
@@ -772,17 +821,74 @@ static void dock_add(void *c, const double *x, const double *s, double *out)
     orc_pose_add(((dock_ctx *)c)->L->T, x, s, out);
 }
 
-double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap,
-                     const double *pose_in, double *pose_out, int *iters, int *evals)
+double orc_local_opt_ex(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap,
+                        const double *pose_in, double *pose_out, int *iters, int *evals, int *exit_reason,
+                        orc_iter_rec *recs, int max_recs)
 {
     const int T = L->T;
     dock_ctx ctx = {p, g, L};
     double *x0 = (double *)malloc(sizeof(double) * (7 + T));
     memcpy(x0, pose_in, sizeof(double) * (7 + T));
     quat_normalize(x0 + 3);
-    double f = (p->optimizer == 1 ? orc_bb : orc_bfgs)(p, 6 + T, 7 + T, cap, x0, dock_fn, dock_add, &ctx, pose_out, iters, evals, NULL, NULL);
+    double f;
+    if (p->optimizer == 1) f = orc_bb(p, 6 + T, 7 + T, cap, x0, dock_fn, dock_add, &ctx, pose_out, iters, evals, NULL, NULL, exit_reason);
+    else f = orc_bfgs(p, 6 + T, 7 + T, cap, x0, dock_fn, dock_add, &ctx, pose_out, iters, evals, NULL, NULL, exit_reason, recs, max_recs);
     free(x0);
     return f;
+}
+
+double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap,
+                     const double *pose_in, double *pose_out, int *iters, int *evals)
+{
+    return orc_local_opt_ex(p, g, L, cap, pose_in, pose_out, iters, evals, NULL, NULL, 0);
+}
+
+/* Diagnostic for the iteration-level teacher-forced parity test (SURVEY.md 8(c) parity protocol; DESIGN.md
+ * "Parity levels"): ONE iteration of O8 on the docking objective from a GIVEN state -- pose x (quaternion used
+ * as given), inverse Hessian H [n][n] and the flag `fresh` (H is the identity of the start / of a reset).
+ * The energy and gradient at x are evaluated here, in double.  Returns the status (0 = step accepted,
+ * ORC_EXIT_GTOL, ORC_EXIT_LINESEARCH); x_new / H_new (nullable) receive the state after the iteration. */
+int orc_bfgs_step(const orc_params *p, const orc_grid *g, const orc_ligand *L,
+                  const double *x, const double *H, int fresh, orc_iter_rec *rec, double *x_new, double *H_new)
+{
+    const int n = 6 + L->T, np_ = 7 + L->T;
+    dock_ctx ctx = {p, g, L};
+    bfgs_state S;
+    bfgs_alloc(&S, n, np_);
+    memcpy(S.x, x, sizeof(double) * np_);
+    memcpy(S.H, H, sizeof(double) * n * n);
+    S.fresh = fresh;
+    S.f = dock_fn(&ctx, S.x, S.gr);
+    const int st = bfgs_iteration(p, &S, dock_fn, dock_add, &ctx, rec);
+    if (x_new) memcpy(x_new, S.x, sizeof(double) * np_);
+    if (H_new) memcpy(H_new, S.H, sizeof(double) * n * n);
+    bfgs_free(&S);
+    return st;
+}
+
+void orc_bfgs_step_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n_states,
+                         const double *x, const double *H, const int32_t *fresh,
+                         orc_iter_rec *recs, double *x_new, double *H_new)
+{
+    const int n = 6 + L->T, np_ = 7 + L->T;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t k = 0; k < n_states; ++k)
+        orc_bfgs_step(p, g, L, x + k * np_, H + k * n * n, fresh[k], recs + k,
+                      x_new ? x_new + k * np_ : NULL, H_new ? H_new + k * n * n : NULL);
+}
+
+/* batch of independent local optimisations (OpenMP over poses): poses [n][7+T] -> out_pose, out_e [n],
+ * out_info [n][3] = (iters, evals, exit reason) */
+void orc_local_opt_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap, int64_t n,
+                         const double *poses, double *out_pose, double *out_e, int32_t *out_info)
+{
+    const int np_ = 7 + L->T;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < n; ++k) {
+        int it, ne, why;
+        out_e[k] = orc_local_opt_ex(p, g, L, cap, poses + k * np_, out_pose + k * np_, &it, &ne, &why, NULL, 0);
+        out_info[3 * k] = it; out_info[3 * k + 1] = ne; out_info[3 * k + 2] = why;
+    }
 }
 
 /* ---------------------------------------------------------------------------------------
@@ -911,6 +1017,38 @@ int64_t orc_search(const orc_params *p, const orc_grid *g, const orc_ligand *L,
         if (tr) for (int s = 0; s < steps; ++s) total += tr[s].evals;
     }
     return total;
+}
+
+/* Teacher-forced replay of recorded MC steps (parity level 3'): for record k the current pose
+ * before the step is given (pre_pose [n][7+T], any implementation's); the oracle evaluates it, draws the
+ * perturbation of (system, copy[k], step[k]), relaxes the candidate and takes the Metropolis decision with its own
+ * numbers.  OpenMP over records.  Outputs per record: e_cur, cutoff margin of the pre-step pose, kind, e_cand, u,
+ * accept, iters, evals (all nullable). */
+void orc_replay_steps(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap, uint64_t seed,
+                      uint32_t system, int64_t n, const double *pre_pose, const int32_t *copy, const int32_t *step,
+                      double *e_cur, double *cur_cutoff_margin, int32_t *kind, double *e_cand, double *u,
+                      int32_t *accept, int32_t *iters, int32_t *evals)
+{
+    const int np_ = 7 + L->T;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < n; ++k) {
+        double *c0 = (double *)malloc(sizeof(double) * np_), *c1 = (double *)malloc(sizeof(double) * np_);
+        orc_diag dg;
+        const double ec = orc_eval(p, g, L, pre_pose + k * np_, NULL, NULL, &dg);
+        const int kd = orc_mc_perturb(p, L->T, seed, system, (uint32_t)copy[k], (uint32_t)step[k], pre_pose + k * np_, c0);
+        int it, ne;
+        const double en = orc_local_opt(p, g, L, cap, c0, c1, &it, &ne);
+        const double uu = orc_mc_uniform(seed, system, (uint32_t)copy[k], (uint32_t)step[k]);
+        if (e_cur) e_cur[k] = ec;
+        if (cur_cutoff_margin) cur_cutoff_margin[k] = dg.cutoff_margin;
+        if (kind) kind[k] = kd;
+        if (e_cand) e_cand[k] = en;
+        if (u) u[k] = uu;
+        if (accept) accept[k] = (en < ec) || (uu < exp((ec - en) / p->t_mc));
+        if (iters) iters[k] = it;
+        if (evals) evals[k] = ne;
+        free(c0); free(c1);
+    }
 }
 
 /* ---------------------------------------------------------------------------------------

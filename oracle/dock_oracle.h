@@ -105,17 +105,19 @@ void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t 
 /* grid geometry: n = round(size/h)+1, origin = center - size/2 */
 void   orc_grid_geometry(const double center[3], const double size[3], double h, int dims[3], double origin[3]);
 
-/* O2: brute-force maps.  G is [n_lig_types][nz][ny][nx].  fp32_cutoff != 0: the in-range
- * predicate r<cutoff is evaluated in float arithmetic in the CUDA kernel's stated order
- * (reading D-CUT); the value f() is always evaluated in double. */
+/* O2: brute-force maps.  G is [n_lig_types][nz][ny][nx].  An atom counts iff r < cutoff, decided in double (S3). */
 void   orc_build_grid(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
                       const int dims[3], const double origin[3], double h,
-                      int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *G);
+                      int n_lig_types, const int32_t *lig_types, double *G);
+/* diagnostic (changes no result): flags[node] = 1 iff some atom lies within `margin` of that node's cutoff sphere;
+ * the vertex score jumps there (S3), so the parity tests exempt these nodes and assert they are few.  Returns the count. */
+int64_t orc_grid_cutoff_flags(int np, const double *pxyz, const int dims[3], const double origin[3], double h,
+                              double cutoff, double margin, uint8_t *flags);
 /* NEXT-2 ("we further used the gradient of score obtained by trilinear interpolation", eq. 4 at 221): the
  * gradient of the vertex score at the vertices, GD[t][c][m] = sum_j f'(r) (m - r_j)_c / r over the same atoms as G. */
 void orc_build_grid_grad(const orc_params *p, int np, const double *pxyz, const int32_t *ptype,
                          const int dims[3], const double origin[3], double h,
-                         int n_lig_types, const int32_t *lig_types, int fp32_cutoff, double *GD);
+                         int n_lig_types, const int32_t *lig_types, double *GD);
 
 /* O3 */
 void   orc_coords(const orc_ligand *L, const double *pose, double *x);
@@ -140,19 +142,54 @@ void   orc_pose_add(int T, const double *pose, const double *s, double *out);
 typedef double (*orc_objective_fn)(void *ctx, const double *x, double *grad);
 typedef void   (*orc_retract_fn)(void *ctx, const double *x, const double *s, double *out);
 typedef void   (*orc_observer_fn)(void *ctx, int it, double f, const double *H, const double *s, const double *y, int updated);
+
+/* why a local optimisation ended */
+#define ORC_EXIT_GTOL       1   /* ||g||_2 < gtol */
+#define ORC_EXIT_CAP        2   /* iteration cap reached */
+#define ORC_EXIT_LINESEARCH 3   /* no acceptable trial in bfgs_max_trials backtracking steps */
+#define ORC_MAX_TRIALS     64
+
+/* decision scalars of one O8 iteration (diagnostic; filled by orc_bfgs / orc_bfgs_step) */
+typedef struct {
+    int    status;      /* 0 = step accepted, else ORC_EXIT_GTOL / ORC_EXIT_LINESEARCH */
+    int    reset;       /* g.d >= 0: H was reset to the identity */
+    int    fresh_in, fresh_out;   /* "H is the identity" flag before / after the iteration */
+    int    trials;      /* evaluations spent in the line search */
+    int    updated;     /* inverse-Hessian update applied (curvature guard passed) */
+    double f, gnorm, gp, alpha0, alpha, f_new;
+    double armijo_margin[ORC_MAX_TRIALS];  /* (f_trial - f) - c1 alpha g.d of every trial: <= 0 accepts */
+    double curv_margin; /* y.s - curv_eps |s| |y|: > 0 updates */
+} orc_iter_rec;
+
+/* recs (nullable, capacity max_recs) receives one record per iteration started; exit_reason nullable */
 double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
                 orc_objective_fn fn, orc_retract_fn add, void *ctx,
-                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx);
+                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx,
+                int *exit_reason, orc_iter_rec *recs, int max_recs);
 /* O8': x_{k+1} = x_k (+) (-alpha_k g_k), alpha_0 = bb_step/|g|, alpha_k = s.s/s.y (BB1) when
  * s.y > curv_eps |s||y| else bb_fallback/|g|, every step capped at length bb_step; one evaluation per iteration,
  * no line search; returns the best point seen (the method is non-monotone).  Same signature as orc_bfgs. */
 double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
                 orc_objective_fn fn, orc_retract_fn add, void *ctx,
-                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx);
+                double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx, int *exit_reason);
 
 /* O8 on the docking objective.  Returns the final energy. */
 double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap,
                      const double *pose_in, double *pose_out, int *iters, int *evals);
+/* same, also reporting why it ended and (BFGS only; nullable) the per-iteration decision records */
+double orc_local_opt_ex(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap,
+                        const double *pose_in, double *pose_out, int *iters, int *evals, int *exit_reason,
+                        orc_iter_rec *recs, int max_recs);
+/* OpenMP over poses: poses [n][7+T] -> out_pose [n][7+T], out_e [n], out_info [n][3] = (iters, evals, exit reason) */
+void   orc_local_opt_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap, int64_t n,
+                           const double *poses, double *out_pose, double *out_e, int32_t *out_info);
+/* ONE O8 iteration on the docking objective from a GIVEN state (x, H [n][n], fresh); E and gradient at x are
+ * evaluated here in double.  For the iteration-level teacher-forced parity test.  x_new / H_new nullable. */
+int    orc_bfgs_step(const orc_params *p, const orc_grid *g, const orc_ligand *L,
+                     const double *x, const double *H, int fresh, orc_iter_rec *rec, double *x_new, double *H_new);
+void   orc_bfgs_step_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n_states,
+                           const double *x, const double *H, const int32_t *fresh,
+                           orc_iter_rec *recs, double *x_new, double *H_new);
 
 /* S16 initial pose for (system, copy) from Philox, rounded once to fp32 */
 void   orc_init_pose(const double box_center[3], const double box_size[3], int T,
@@ -191,6 +228,12 @@ int64_t orc_search(const orc_params *p, const orc_grid *g, const orc_ligand *L,
                    int copies, int steps, int cap, uint64_t seed, uint32_t system,
                    const double *init_poses, double *best_pose, double *best_e,
                    double *trace_pose, orc_step_rec *trace, orc_step_rec *init_rec);
+
+/* teacher-forced replay of recorded MC steps (parity level 3'): see dock_oracle.c.  OpenMP over records. */
+void   orc_replay_steps(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap, uint64_t seed,
+                        uint32_t system, int64_t n, const double *pre_pose, const int32_t *copy, const int32_t *step,
+                        double *e_cur, double *cur_cutoff_margin, int32_t *kind, double *e_cand, double *u,
+                        int32_t *accept, int32_t *iters, int32_t *evals);
 
 /* heavy-atom RMSD between two poses, atom order as given, no symmetry correction */
 double orc_rmsd(const orc_ligand *L, const double *pose_a, const double *pose_b);

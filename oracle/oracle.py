@@ -88,6 +88,13 @@ class StepRec(C.Structure):
                 ("accept", C.c_int), ("iters", C.c_int), ("evals", C.c_int)]
 
 
+ORC_MAX_TRIALS = 64
+EXIT_GTOL, EXIT_CAP, EXIT_LINESEARCH = 1, 2, 3
+ITER_DTYPE = np.dtype([("status", "i4"), ("reset", "i4"), ("fresh_in", "i4"), ("fresh_out", "i4"), ("trials", "i4"),
+                       ("updated", "i4"), ("f", "f8"), ("gnorm", "f8"), ("gp", "f8"), ("alpha0", "f8"), ("alpha", "f8"),
+                       ("f_new", "f8"), ("armijo_margin", "f8", (ORC_MAX_TRIALS,)), ("curv_margin", "f8")])
+assert ITER_DTYPE.itemsize == 6 * 4 + 8 * (6 + ORC_MAX_TRIALS + 1)
+
 STEP_DTYPE = np.dtype([("e_cur", "f8"), ("e_cand", "f8"), ("u", "f8"),
                        ("accept", "i4"), ("iters", "i4"), ("evals", "i4"), ("_pad", "i4")])
 DIAG_DTYPE = np.dtype([("face_margin", "f8"), ("kink_margin", "f8"), ("cutoff_margin", "f8"),
@@ -112,6 +119,9 @@ def lib():
         _lib.orc_topk.restype = C.c_int
         _lib.orc_mc_perturb.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_local_opt_ex.restype = C.c_double
+        _lib.orc_bfgs_step.restype = C.c_int
+        _lib.orc_grid_cutoff_flags.restype = C.c_int64
     return _lib
 
 
@@ -227,7 +237,7 @@ def grid_geometry(center, size, h):
     return [int(d) for d in dims], [float(o) for o in org]
 
 
-def build_grid(p: Params, pxyz, ptype, center, size, h, lig_types, fp32_cutoff=True, grad=False) -> Grid:
+def build_grid(p: Params, pxyz, ptype, center, size, h, lig_types, grad=False) -> Grid:
     dims, org = grid_geometry(center, size, h)
     pxyz = _f64(pxyz)
     ptype = _i32(ptype)
@@ -235,14 +245,24 @@ def build_grid(p: Params, pxyz, ptype, center, size, h, lig_types, fp32_cutoff=T
     G = np.zeros(len(lig_types) * dims[0] * dims[1] * dims[2], dtype=np.float64)
     lib().orc_build_grid(C.byref(p), int(pxyz.shape[0]), _p(pxyz), _p(ptype),
                          (C.c_int * 3)(*dims), (C.c_double * 3)(*org), C.c_double(h),
-                         len(lig_types), _p(lt), int(bool(fp32_cutoff)), _p(G))
+                         len(lig_types), _p(lt), _p(G))
     GD = None
     if grad:                                               # NEXT-2: eq. 4's per-vertex gradients
         GD = np.zeros(3 * len(lig_types) * dims[0] * dims[1] * dims[2], dtype=np.float64)
         lib().orc_build_grid_grad(C.byref(p), int(pxyz.shape[0]), _p(pxyz), _p(ptype),
                                   (C.c_int * 3)(*dims), (C.c_double * 3)(*org), C.c_double(h),
-                                  len(lig_types), _p(lt), int(bool(fp32_cutoff)), _p(GD))
+                                  len(lig_types), _p(lt), _p(GD))
     return Grid(dims, org, h, lig_types, G, GD)
+
+
+def grid_cutoff_flags(p: Params, pxyz, g: Grid, margin: float = 1e-5) -> np.ndarray:
+    """Diagnostic: bool [nz, ny, nx], True where some atom lies within `margin` of the node's cutoff sphere."""
+    pxyz = _f64(pxyz)
+    nx, ny, nz = g.dims
+    flags = np.zeros(nx * ny * nz, dtype=np.uint8)
+    lib().orc_grid_cutoff_flags(int(pxyz.shape[0]), _p(pxyz), (C.c_int * 3)(*g.dims), (C.c_double * 3)(*g.origin),
+                                C.c_double(g.h), C.c_double(p.cutoff), C.c_double(margin), _p(flags))
+    return flags.reshape(nz, ny, nx).astype(bool)
 
 
 def coords(L: Ligand, pose) -> np.ndarray:
@@ -296,6 +316,57 @@ def local_opt(p: Params, g: Grid, L: Ligand, pose, cap: int):
     e = lib().orc_local_opt(C.byref(p), C.byref(g.c), C.byref(L.c), int(cap), _p(pose), _p(out),
                             C.byref(it), C.byref(ne))
     return float(e), out, it.value, ne.value
+
+
+def local_opt_ex(p: Params, g: Grid, L: Ligand, pose, cap: int, max_recs: int = 0):
+    """local_opt plus the exit reason and (BFGS) the per-iteration decision records."""
+    pose = _f64(pose)
+    out = np.zeros(7 + L.T)
+    it, ne, why = C.c_int(), C.c_int(), C.c_int()
+    recs = np.zeros(max(1, max_recs), dtype=ITER_DTYPE)
+    e = lib().orc_local_opt_ex(C.byref(p), C.byref(g.c), C.byref(L.c), int(cap), _p(pose), _p(out),
+                               C.byref(it), C.byref(ne), C.byref(why), _p(recs) if max_recs else None, int(max_recs))
+    started = it.value + (0 if why.value == EXIT_CAP else 1)          # iterations started = records written
+    return float(e), out, it.value, ne.value, why.value, recs[:min(max_recs, started)]
+
+
+def local_opt_batch(p: Params, g: Grid, L: Ligand, poses, cap: int):
+    """OpenMP over poses.  Returns (e [n], pose [n,7+T], info [n,3] = iters, evals, exit reason)."""
+    poses = _f64(poses).reshape(-1, 7 + L.T)
+    n = poses.shape[0]
+    out = np.zeros_like(poses)
+    e = np.zeros(n)
+    info = np.zeros((n, 3), dtype=np.int32)
+    lib().orc_local_opt_batch(C.byref(p), C.byref(g.c), C.byref(L.c), int(cap), C.c_int64(n), _p(poses), _p(out), _p(e), _p(info))
+    return e, out, info
+
+
+def bfgs_step_batch(p: Params, g: Grid, L: Ligand, x, H, fresh):
+    """One O8 iteration from each given state (x [m,7+T], H [m,n,n], fresh [m]).  Returns (recs, x_new, H_new)."""
+    n = 6 + L.T
+    x = _f64(x).reshape(-1, 7 + L.T)
+    m = x.shape[0]
+    H = _f64(H).reshape(m, n, n)
+    fresh = _i32(fresh).reshape(m)
+    recs = np.zeros(m, dtype=ITER_DTYPE)
+    x_new, H_new = np.zeros_like(x), np.zeros_like(H)
+    lib().orc_bfgs_step_batch(C.byref(p), C.byref(g.c), C.byref(L.c), C.c_int64(m), _p(x), _p(H), _p(fresh),
+                              _p(recs), _p(x_new), _p(H_new))
+    return recs, x_new, H_new
+
+
+def replay_steps(p: Params, g: Grid, L: Ligand, cap: int, seed: int, system: int, pre_pose, copy, step):
+    """Teacher-forced replay of recorded MC steps (level 3'), OpenMP over records."""
+    pre = _f64(pre_pose).reshape(-1, 7 + L.T)
+    n = pre.shape[0]
+    copy, step = _i32(copy).reshape(n), _i32(step).reshape(n)
+    out = dict(e_cur=np.zeros(n), cur_cutoff_margin=np.zeros(n), kind=np.zeros(n, np.int32), e_cand=np.zeros(n),
+               u=np.zeros(n), accept=np.zeros(n, np.int32), iters=np.zeros(n, np.int32), evals=np.zeros(n, np.int32))
+    lib().orc_replay_steps(C.byref(p), C.byref(g.c), C.byref(L.c), int(cap), C.c_uint64(seed), C.c_uint32(system),
+                           C.c_int64(n), _p(pre), _p(copy), _p(step), _p(out["e_cur"]), _p(out["cur_cutoff_margin"]),
+                           _p(out["kind"]), _p(out["e_cand"]), _p(out["u"]), _p(out["accept"]), _p(out["iters"]),
+                           _p(out["evals"]))
+    return out
 
 
 def init_pose(center, size, T, seed, system, copy) -> np.ndarray:
@@ -398,7 +469,7 @@ def bfgs_generic(p: Params, x0, fn, cap: int, observer=None):
     l = lib()
     l.orc_bfgs.restype = C.c_double
     f = l.orc_bfgs(C.byref(p), n, n, int(cap), _p(x0), _OBJ_FN(_fn), _ADD_FN(_add), None, _p(out),
-                   C.byref(it), C.byref(ne), _OBS_FN(_obs), None)
+                   C.byref(it), C.byref(ne), _OBS_FN(_obs), None, None, None, 0)
     return float(f), out, it.value, ne.value
 
 
@@ -429,5 +500,5 @@ def bb_generic(p: Params, x0, fn, cap: int, observer=None):
     l = lib()
     l.orc_bb.restype = C.c_double
     f = l.orc_bb(C.byref(p), n, n, int(cap), _p(x0), _OBJ_FN(_fn), _ADD_FN(_add), None, _p(out),
-                 C.byref(it), C.byref(ne), _OBS_FN(_obs), None)
+                 C.byref(it), C.byref(ne), _OBS_FN(_obs), None, None)
     return float(f), out, it.value, ne.value

@@ -67,3 +67,19 @@ def compare_scores(gpu_e, gpu_grad, gpu_terms, ref_e, ref_grad, ref_terms, diag,
                                             np.unravel_index(int(np.argmax(np.where(ok_g[:, None], err_c, 0))), err_c.shape))
         stats["max_err_g"] = float(err_c[ok_g].max())
     return stats
+
+
+def oracle_self_agreement(O, op, og, oL, poses, cap, eps=6e-8, seeds=(1, 2, 3), tol_e=1e-3):
+    """The chaos ceiling of a free-running local optimisation: fraction of poses whose
+    final energy the ORACLE reproduces within tol_e when its start pose is perturbed by a relative eps (6e-8 = half an
+    fp32 ulp: the smallest difference any single-precision implementation must introduce).  Mean over `seeds`."""
+    poses = np.asarray(poses, np.float64)
+    e0, _, info0 = O.local_opt_batch(op, og, oL, poses, cap)
+    rates, med = [], []
+    for sd in seeds:
+        r = np.random.default_rng(sd)
+        pp = poses * (1.0 + eps * (2.0 * r.random(poses.shape) - 1.0))
+        e1, _, _ = O.local_opt_batch(op, og, oL, pp, cap)
+        rates.append(float(np.mean(np.abs(e1 - e0) <= tol_e)))
+        med.append(float(np.median(np.abs(e1 - e0))))
+    return dict(agree=float(np.mean(rates)), median_abs=float(np.mean(med)), n=int(len(poses)), e0=e0, info0=info0)

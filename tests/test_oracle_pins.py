@@ -126,17 +126,16 @@ def test_single_atom_grid_equals_pair_values(orc):
     p = orc.default_params()
     atom = np.array([[0.3, -0.2, 0.1]])
     lig_types = [XS["C_H"], XS["N_D"], XS["O_A"]]
-    for fp32 in (False, True):
-        g = orc.build_grid(p, atom, [XS["O_A"]], [0, 0, 0], [6, 6, 6], 0.375, lig_types, fp32_cutoff=fp32)
-        assert g.dims == (17, 17, 17)
-        assert np.allclose(g.origin, [-3, -3, -3])
-        rng = np.random.default_rng(0)
-        for _ in range(300):
-            ix, iy, iz = rng.integers(17, size=3)
-            m = g.origin + 0.375 * np.array([ix, iy, iz])
-            r = float(np.linalg.norm(m - atom[0]))
-            for k, t in enumerate(lig_types):
-                assert abs(g.maps[k, iz, iy, ix] - orc.pair(p, t, XS["O_A"], r)[0]) < 1e-14
+    g = orc.build_grid(p, atom, [XS["O_A"]], [0, 0, 0], [6, 6, 6], 0.375, lig_types)
+    assert g.dims == (17, 17, 17)
+    assert np.allclose(g.origin, [-3, -3, -3])
+    rng = np.random.default_rng(0)
+    for _ in range(300):
+        ix, iy, iz = rng.integers(17, size=3)
+        m = g.origin + 0.375 * np.array([ix, iy, iz])
+        r = float(np.linalg.norm(m - atom[0]))
+        for k, t in enumerate(lig_types):
+            assert abs(g.maps[k, iz, iy, ix] - orc.pair(p, t, XS["O_A"], r)[0]) < 1e-14
 
 
 def test_grid_is_plain_sum_over_atoms_within_cutoff(orc, tiny):
@@ -154,15 +153,31 @@ def test_grid_is_plain_sum_over_atoms_within_cutoff(orc, tiny):
                 assert abs(g.maps[k, iz, iy, ix] - ref) < 1e-12
 
 
-def test_fp32_cutoff_rule_only_matters_at_the_cutoff(orc):
-    s = make_system(0, seed=0)
+def test_cutoff_is_decided_in_double_and_the_near_cutoff_diagnostic_is_the_plain_definition(orc):
+    """S3: an atom counts iff r < 8 in double.  Two atoms 1e-9 A inside / outside the cutoff sphere of a node; and
+    orc_grid_cutoff_flags against the same statement written with numpy."""
     p = orc.default_params()
-    a = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, 0.375, s.lig_types, fp32_cutoff=True)
-    b = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, 0.375, s.lig_types, fp32_cutoff=False)
-    diff = np.abs(a.maps - b.maps)
-    # a flipped pair changes a node by |f(cutoff^-)| <= ~0.006; everything else is identical
-    assert diff.max() < 0.01
-    assert (diff > 0).mean() < 1e-3
+    h, lt = 0.375, [XS["C_H"]]
+    g0 = orc.build_grid(p, np.zeros((0, 3)), np.zeros(0, np.int32), [0, 0, 0], [3, 3, 3], h, lt)
+    node = g0.origin + h * np.array([4, 4, 4])                      # the centre node (0, 0, 0)
+    for dr, inside in ((-1e-9, True), (1e-9, False)):
+        atom = (node + np.array([8.0 + dr, 0.0, 0.0]))[None]
+        g = orc.build_grid(p, atom, [XS["C_H"]], [0, 0, 0], [3, 3, 3], h, lt)
+        want = orc.pair(p, XS["C_H"], XS["C_H"], 8.0 + dr)[0]
+        assert (want != 0.0) == inside
+        assert g.maps[0, 4, 4, 4] == want
+    s = make_system(0, seed=0)
+    g = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, 0.375, s.lig_types)
+    flags = orc.grid_cutoff_flags(p, s.protein_xyz, g, margin=1e-4)
+    nx, ny, nz = g.dims
+    ax = [g.origin[c] + g.h * np.arange(g.dims[c]) for c in range(3)]
+    Z, Y, X = np.meshgrid(ax[2], ax[1], ax[0], indexing="ij")
+    nodes = np.stack([X, Y, Z], axis=-1).reshape(-1, 3)
+    near = np.zeros(len(nodes), bool)
+    for a in s.protein_xyz.astype(np.float64):
+        near |= np.abs(np.linalg.norm(nodes - a, axis=1) - 8.0) < 1e-4
+    assert np.array_equal(flags.ravel(), near)
+    assert 0 < flags.mean() < 5e-3        # a thin shell: ~ 4 pi 64 * 2e-4 A^3 per atom
 
 
 def test_grid_geometry(orc):
@@ -451,6 +466,78 @@ def test_local_opt_never_increases_energy(orc, tiny):
         assert ne >= it + 1
 
 
+def test_exit_reasons_and_iteration_records(orc, tiny):
+    """Why a local optimisation ends (gtol / cap / line search exhausted), and the per-iteration decision records:
+    consistency with the closed form on a quadratic and with the plain run on the docking objective."""
+    s, p, g, L = tiny
+    n = 9
+    g0 = orc.Grid((n, n, n), [0.0, 0.0, 0.0], 0.375, [0], np.zeros((1, n, n, n)))
+    L1 = _single_atom_ligand(orc, 0)
+    start = [5.0, -1.0, 4.5, 1, 0, 0, 0]               # outside a zero map: E = k_wall |overshoot|^2, a quadratic in t
+    e, pose, it, ne, why, recs = orc.local_opt_ex(p, g0, L1, start, 100, max_recs=100)
+    assert why == orc.EXIT_GTOL and e < 1e-6
+    r0 = recs[0]                                        # first iteration: H = I, d = -g, alpha0 = 1/|g|, f = 72.5
+    gvec = 2 * 10.0 * np.array([2.0, -1.0, 1.5])
+    assert r0["fresh_in"] == 1 and abs(r0["f"] - 72.5) < 1e-12 and abs(r0["gnorm"] - np.linalg.norm(gvec)) < 1e-12
+    assert abs(r0["gp"] + gvec @ gvec) < 1e-9 and abs(r0["alpha0"] - 1 / np.linalg.norm(gvec)) < 1e-15
+    assert r0["trials"] == 1 and r0["status"] == 0 and r0["armijo_margin"][0] <= 0
+    assert recs[-1]["status"] == orc.EXIT_GTOL and len(recs) == it + 1      # the last record is the stop itself
+    e2, _, it2, _, why2, _ = orc.local_opt_ex(p, g0, L1, start, 1)
+    assert why2 == orc.EXIT_CAP and it2 == 1
+    # docking objective: records of the plain run == one teacher-forced step from each of its own states
+    rng = np.random.default_rng(31)
+    whys = []
+    for _ in range(6):
+        pose = _random_pose(rng, L.T, s.box_center, spread=6.0)
+        e, out, it, ne, why, recs = orc.local_opt_ex(p, g, L, pose, 50, max_recs=64)
+        whys.append(why)
+        assert (e, it, ne) == orc.local_opt(p, g, L, pose, 50)[0:1] + orc.local_opt(p, g, L, pose, 50)[2:4]
+        assert ne == 1 + int(recs["trials"].sum())
+        nn = 6 + L.T
+        x, H, fresh = pose.copy(), np.eye(nn), 1
+        x[3:7] /= math.sqrt(x[3] * x[3] + x[4] * x[4] + x[5] * x[5] + x[6] * x[6])   # as quat_normalize does
+        for k in range(len(recs)):
+            rk, xn, Hn = orc.bfgs_step_batch(p, g, L, x[None], H[None], [fresh])
+            for f in ("status", "trials", "updated", "reset", "f", "gp", "alpha", "f_new"):
+                assert rk[0][f] == recs[k][f], (k, f)
+            x, H, fresh = xn[0], Hn[0], int(rk[0]["fresh_out"])
+        assert np.array_equal(x, out)
+    assert set(whys) <= {orc.EXIT_GTOL, orc.EXIT_CAP, orc.EXIT_LINESEARCH}
+
+
+def test_replay_steps_equals_the_search_it_replays(orc, tiny):
+    """orc_replay_steps (teacher-forced diagnostic) fed with the oracle's own pre-step poses reproduces its search."""
+    s, p, g, L = tiny
+    init = orc.init_poses(s.box_center, s.box_size, L.T, 5, 0, 4)
+    r = orc.search(p, g, L, init, 6, 30, 5)
+    cc, ss = np.meshgrid(np.arange(4), np.arange(6), indexing="ij")
+    rp = orc.replay_steps(p, g, L, 30, 5, 0, r["trace_pose"].reshape(-1, 7 + L.T), cc.ravel(), ss.ravel())
+    tr = r["trace"].ravel()
+    assert np.array_equal(rp["e_cand"], tr["e_cand"]) and np.array_equal(rp["accept"], tr["accept"])
+    assert np.array_equal(rp["u"], tr["u"]) and np.array_equal(rp["evals"], tr["evals"])
+    assert np.allclose(rp["e_cur"], tr["e_cur"], atol=1e-12)
+
+
+def test_local_optimisation_is_chaotic_at_fp32_resolution(orc):
+    """BASELINE.json's level 2 ("local-opt final energies within 1e-3 kcal/mol") cannot be
+    met by ANY single-precision evaluator, because the oracle does not meet it against itself: the same double
+    precision optimisation started from poses that differ by half an fp32 ulp (6e-8 relative) -- or even by 1e-12 --
+    ends more than 1e-3 away on most poses (gradient of eq. 3 jumps at every cell face, the cutoff is hard, 50-300
+    BFGS iterations amplify the difference).  The GPU parity tests therefore gate on this ceiling, measured the same
+    way (tests/parity.py: oracle_self_agreement), and on the iteration-level teacher-forced replay."""
+    from tests.parity import oracle_self_agreement
+    s = make_system(0, seed=0)
+    p = orc.params_as_fp32(orc.default_params())
+    g = orc.build_grid(p, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
+    L = orc.Ligand(s.ligand)
+    rng = np.random.default_rng(7)
+    poses = random_poses(rng, 256, s.box_center, s.box_size * 0.6, L.T).astype(np.float64)
+    a12 = oracle_self_agreement(orc, p, g, L, poses, 50, eps=1e-12)
+    a32 = oracle_self_agreement(orc, p, g, L, poses, 50, eps=6e-8)
+    assert 0.02 < a32["agree"] < 0.6 and a12["agree"] < 0.85, (a12, a32)
+    assert a32["agree"] <= a12["agree"] + 0.1
+
+
 # ----------------------------------------------------------------------------- O9 Monte Carlo
 def test_initial_poses_are_fp32_inside_the_box_with_unit_quaternions(orc):
     c, sz = [1.0, -2.0, 3.0], [30.0, 30.0, 30.0]
@@ -466,6 +553,44 @@ def test_initial_poses_are_fp32_inside_the_box_with_unit_quaternions(orc):
     # uniformity of t (coarse): mean near centre, std near size/sqrt(12)
     assert np.all(np.abs(P[:, :3].mean(axis=0) - np.array(c)) < 3.0)
     assert np.all(np.abs(P[:, :3].std(axis=0) - 30 / math.sqrt(12)) < 2.0)
+
+
+def _rng_pins():
+    rows = {}
+    words = []
+    for l in open(os.path.join(GOLD, "rng_mapping_pins.txt")):
+        if not l.strip() or l.startswith("#"):
+            continue
+        k, *v = l.split()
+        if k == "philox":
+            words.append([int(x, 16) for x in v])
+        else:
+            rows[k] = [float(x) for x in v]
+    return words, rows
+
+
+def test_rng_word_to_field_mapping_hand_worked(orc):
+    """S16 / S14 / O9: which Philox word lands in which pose field (tests/golden/rng_mapping_pins.txt, hand-worked
+    from the words; a swapped quaternion component, slot, word or a right- instead of left-multiplied rotation fails)."""
+    words, rows = _rng_pins()
+    for w in words:                                       # the words themselves: oracle's Philox (KAT-pinned) agrees
+        assert orc.philox(w[0:4], [0, 0]) == w[4:8]
+    pose = orc.init_pose([1.0, -2.0, 3.0], [30.0, 20.0, 10.0], 5, 0, 0, 0)
+    want = np.array(rows["init_pose"])
+    assert np.array_equal(pose, want.astype(np.float32).astype(np.float64))          # rounded once to fp32
+    p = orc.default_params()
+    base = np.array([3.0, -1.0, 2.0, 0.5, 0.5, 0.5, 0.5, 0.1, -0.2, 0.3, -0.4, 0.5])
+    kind, cand = orc.mc_perturb(p, 0, 0, 0, 0, 0, base[:7])                           # T = 0: K = 2 -> translate
+    assert kind == 0 and np.allclose(cand[:3] - base[:3], rows["perturb_translate"], atol=1e-15)
+    assert np.array_equal(cand[3:], base[3:7])
+    kind, cand = orc.mc_perturb(p, 5, 0, 0, 0, 0, base)                               # T = 5: K = 3 -> rotate (left product)
+    assert kind == 1 and np.allclose(cand[3:7], rows["perturb_rotate"], atol=1e-15)
+    assert np.array_equal(cand[:3], base[:3]) and np.array_equal(cand[7:], base[7:])
+    kind, cand = orc.mc_perturb(p, 5, 0, 0, 0, 3, base)                               # step 3: torsion 4 resampled
+    k = int(rows["perturb_torsion"][0])
+    assert kind == 2 and k == 4 and abs(cand[7 + k] - rows["perturb_torsion"][1]) < 1e-15
+    assert np.array_equal(np.delete(cand, 7 + k), np.delete(base, 7 + k))
+    assert orc.mc_uniform(0, 0, 0, 0) == rows["accept_uniform"][0]
 
 
 def test_perturbation_kinds_and_amplitudes(orc, tiny):
@@ -665,7 +790,7 @@ def test_eq4_vertex_gradients_are_the_gradient_of_the_brute_force_vertex_score(o
     pxyz = rng.uniform(-6, 6, size=(40, 3))
     ptyp = rng.integers(0, 10, size=40).astype(np.int32)
     lig_types = [0, 3, 8]
-    g = orc.build_grid(p, pxyz, ptyp, [0, 0, 0], [6.0, 6.0, 6.0], 0.375, lig_types, fp32_cutoff=False, grad=True)
+    g = orc.build_grid(p, pxyz, ptyp, [0, 0, 0], [6.0, 6.0, 6.0], 0.375, lig_types, grad=True)
     assert g.gmaps.shape == (3, 3, 17, 17, 17)
 
     def s(t, m):
