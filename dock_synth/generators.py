@@ -99,8 +99,9 @@ def make_protein_tiny(rng, n=200, cube=20.0, dmin=2.8) -> Tuple[np.ndarray, np.n
     return pts.astype(np.float32), _protein_types(rng, n)
 
 
-def make_protein_globule(rng, n, a=2.46, jitter=0.3) -> Tuple[np.ndarray, np.ndarray, float]:
-    """Compact globule: jittered cubic lattice, keep the n sites nearest the origin."""
+def make_protein_globule(rng, n, a=2.46, jitter=0.3, return_lattice=False):
+    """Compact globule: jittered cubic lattice, keep the n sites nearest the origin.
+    With return_lattice the whole lattice sorted by distance and the permutation are returned too (carve_pocket)."""
     r_need = (3.0 * n / (4.0 * np.pi)) ** (1.0 / 3.0) * a * 1.25 + 2 * a
     m = int(np.ceil(r_need / a))
     ax = np.arange(-m, m + 1) * a
@@ -108,11 +109,33 @@ def make_protein_globule(rng, n, a=2.46, jitter=0.3) -> Tuple[np.ndarray, np.nda
     pts = np.stack([gx.ravel(), gy.ravel(), gz.ravel()], axis=1)
     pts = pts + (rng.random(pts.shape) * 2.0 - 1.0) * jitter
     d = np.linalg.norm(pts, axis=1)
-    order = np.argsort(d, kind="stable")[:n]
-    pts = pts[order]
+    full = pts[np.argsort(d, kind="stable")]
+    pts = full[:n]
     radius = float(np.max(np.linalg.norm(pts, axis=1)))
     perm = rng.permutation(n)  # no spatial ordering in the input
-    return pts[perm].astype(np.float32), _protein_types(rng, n), radius
+    types = _protein_types(rng, n)
+    if return_lattice:
+        return pts[perm].astype(np.float32), types, radius, full, perm
+    return pts[perm].astype(np.float32), types, radius
+
+
+POCKET_RADIUS = 7.0   # A: radius of the carved cavity
+POCKET_DEPTH = 4.0    # A: its centre lies this far below the surface point the box is centred on
+
+
+def carve_pocket(full_sorted: np.ndarray, n: int, perm: np.ndarray, surface_point: np.ndarray) -> np.ndarray:
+    """A binding pocket at the box centre (configs 1-3): the globule is re-selected as the n lattice sites nearest the
+    origin that lie OUTSIDE a sphere of POCKET_RADIUS centred POCKET_DEPTH below `surface_point` -- a half-open cavity
+    of about the ligand's volume, so that the search landscape has a real minimum (a convex lattice surface has none:
+    best energies stayed positive).  Atom count, density, types and input order are unchanged; no random draw is used,
+    so ligand and box are the ones of the uncarved system."""
+    sp = np.asarray(surface_point, dtype=np.float64)
+    r = float(np.linalg.norm(sp))
+    centre = sp * (1.0 - POCKET_DEPTH / r) if r > 0 else sp
+    keep = np.linalg.norm(full_sorted - centre, axis=1) >= POCKET_RADIUS
+    pts = full_sorted[keep][:n]
+    assert pts.shape[0] == n
+    return pts[perm].astype(np.float32)
 
 
 def _grow_tree(rng, N: int):
@@ -319,12 +342,13 @@ def make_system(config: int, seed: int = 0, index: int = 0,
         npr = n_prot or cfg["n_prot"]
         nl = N or cfg["N"]
         tl = cfg["T"] if T is None else T
-    pxyz, ptyp, radius = make_protein_globule(rng, npr)
+    pxyz, ptyp, radius, lattice, perm = make_protein_globule(rng, npr, return_lattice=True)
     lig = make_ligand(rng, nl, tl, LIG_TYPES_FULL)
     if config == 4:
         c, s = make_box(rng, "center", size=cfg["box"])
     else:
         c, s = make_box(rng, "surface", radius=radius, size=cfg["box"])
+        pxyz = carve_pocket(lattice, npr, perm, c)
     return System(cfg["name"], pxyz, ptyp, lig, c, s, 0.375, list(LIG_TYPES_FULL),
                   cfg.get("copies", 0), cfg.get("steps", 0), cfg.get("cap", 0),
                   extra=dict(radius=radius))

@@ -54,7 +54,7 @@ typedef struct dock_params {
     int32_t donor[DOCK_MAX_XS_TYPES];
     int32_t acceptor[DOCK_MAX_XS_TYPES];
     float   w[5];                             /* gauss1, gauss2, repulsion, hydrophobic, hbond */
-    float   cutoff;                           /* 8 A; a pair counts iff r < cutoff (decided in fp32) */
+    float   cutoff;                           /* 8 A; a pair counts iff r < cutoff (the kernels decide it on r^2 in fp32) */
     float   k_wall;                           /* quadratic wall, kcal/mol/A^2 per axis overshoot */
     float   t_mc;                             /* Metropolis temperature, kcal/mol */
     float   amp_trans;                        /* MC translation amplitude per axis, A */
@@ -129,29 +129,48 @@ typedef struct dock_grid {
  * One record = DOCK_TRACE_HEADER floats followed by the pre-step pose (7+T_max floats). */
 #define DOCK_TRACE_HEADER 8   /* e_cur, e_cand, u, accept, iters, evals, kind, reserved */
 
+/* Why a local optimisation ended (reading S12). */
+#define DOCK_EXIT_GTOL       1   /* ||g||_2 < bfgs_gtol */
+#define DOCK_EXIT_CAP        2   /* iteration cap reached */
+#define DOCK_EXIT_LINESEARCH 3   /* no acceptable trial in bfgs_max_trials backtracking steps */
+
+/* Optional per-iteration trace of the BFGS local optimizer (dock_local_opt_trace): the state each iteration starts
+ * from and its decision scalars -- enough to redo that single iteration elsewhere (iteration-level teacher-forced
+ * parity).  One record = DOCK_ITER_HEADER floats
+ *   {f, |g|, g.d, alpha0, alpha (last tried), f_new (last trial), status (0 = step taken, else DOCK_EXIT_*),
+ *    trials (evaluations of the line search), updated (inverse Hessian updated), reset (H reset to I: g.d >= 0),
+ *    fresh_in, fresh_out ("H is the identity" before / after)}
+ * followed by the pose x[7+T], the gradient g[6+T] at x and the inverse Hessian H[(6+T)^2] (row-major) the iteration
+ * starts from.  With the Barzilai-Borwein optimizer (params->optimizer = 1) the header holds
+ *   {f, |g|, 0, 0, alpha, f_new, status, branch (0 = first step, 1 = s.s/s.y, 2 = fallback), 0, capped, 0, 0}
+ * and the H area starts with the previous step s[6+T] and gradient change y[6+T] (zeros at iteration 0). */
+#define DOCK_ITER_HEADER 12
+
 /* ---- parameters ----------------------------------------------------------------------------- */
 int dock_default_params(dock_params *out);
 
 /* ---- A1: grid maps ----------------------------------------
  * G[m][node] = sum over protein atoms j with |node - r_j| < cutoff of f(lig_types[m], type_j, r).
- * protein: host.  grid_dev: device, dock_grid_bytes(box, n_lig_types) bytes, 256-byte aligned.
+ * protein: host.  grid_dev: device, 256-byte aligned, grid_bytes >= dock_grid_bytes(params, box, n_lig_types)
+ * (checked: DOCK_EINVAL if the buffer is too small -- with grad_mode = 1 the maps have 4 channels).
  * out_desc (host) receives the descriptor with data_dev = grid_dev and packed_dev behind it.
- * Errors: DOCK_EINVAL for null pointers, n < 0, spacing <= 0, type ids outside [0, n_types). */
+ * Errors: DOCK_EINVAL for null pointers, n < 0, spacing <= 0, type ids outside [0, n_types), short or misaligned buffer. */
 int dock_grid_dims(const dock_box *box, int32_t dims[3]);
-/* bytes of the caller's grid buffer for n_lig_types maps over `box` (both images); 0 on bad input.
- * With dock_params.grad_mode = 1 every map has 4 channels: pass 4 * n_lig_types here. */
-size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types);
+/* bytes of the caller's grid buffer for n_lig_types maps over `box` (both images, all channels of params->grad_mode);
+ * 0 on bad input. */
+size_t dock_grid_bytes(const dock_params *params, const dock_box *box, int32_t n_lig_types);
 int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
                      int32_t n_lig_types, const int32_t *lig_types,
-                     float *grid_dev, dock_grid *out_desc,
+                     float *grid_dev, size_t grid_bytes, dock_grid *out_desc,
                      void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
-/* Batched form (BASELINE.json configs[3]): n_systems (protein, box) pairs with one ligand-type list, enqueued back to
- * back on `stream`.  proteins, boxes, out_descs: HOST arrays [n_systems]; grid_dev: HOST array of n_systems DEVICE
- * buffers (dock_grid_bytes each).  One workspace serves all systems (the stream orders them); *needed = the largest. */
+/* Batched form (BASELINE.json configs[3]): n_systems (protein, box) pairs with one ligand-type list in ONE upload and
+ * ONE pair of launches (build, pack) over all systems.  proteins, boxes, out_descs: HOST arrays [n_systems];
+ * grid_dev: HOST array of n_systems DEVICE buffers, grid_bytes: HOST array of their sizes (each checked against
+ * dock_grid_bytes).  The workspace holds every system's cell lists: *needed = their sum. */
 int dock_build_grids_batch(const dock_params *params, int32_t n_systems, const dock_protein *proteins,
                            const dock_box *boxes, int32_t n_lig_types, const int32_t *lig_types,
-                           float *const *grid_dev, dock_grid *out_descs,
+                           float *const *grid_dev, const size_t *grid_bytes, dock_grid *out_descs,
                            void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
 /* ---- A2-A5: fused pose -> coordinates -> energy + gradient (eq. 2-3 at 198-219) --
@@ -165,25 +184,37 @@ int dock_score_batch(const dock_params *params, const dock_grid *grid, const doc
 /* Same, with HOST buffers for poses / energy / grad / terms (copies inside the call; pinned memory makes them
  * asynchronous).  The batch is processed in up to 8 chunks through a three-stage pipeline -- host->device copy,
  * kernel, device->host copy -- so that both PCIe directions overlap the arithmetic; the kernels run on `stream`,
- * the copies on two side streams that the library creates once (the only resources it owns; because of them this
- * entry point must not be called from two host threads at once).  The call returns after everything has completed
- * (`stream` is synchronised once). */
+ * the copies on two side streams that the library creates once per device (the only resources it owns; calls on
+ * the same device from several host threads are serialised by a mutex).  The call returns after everything has
+ * completed (`stream` is synchronised once); on an error every copy already enqueued is drained first. */
 int dock_score_batch_host(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
                           int64_t n_poses, const float *poses_host,
                           float *energy_host, float *grad_host, float *terms_host,
                           void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
 /* ---- A6: BFGS local optimisation of a batch of start poses -----------------------
- * poses_dev [n][7+T] in; out_pose_dev [n][7+T]; out_e_dev [n]; out_iters_dev [n][2] = (iters, evals) or NULL */
+ * poses_dev [n][7+T] in; out_pose_dev [n][7+T]; out_e_dev [n];
+ * out_iters_dev [n][3] = (iterations, evaluations, DOCK_EXIT_* reason) or NULL */
 int dock_local_opt_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
                          int64_t n_poses, int32_t max_iters, const float *poses_dev,
                          float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
                          void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+/* Same with the per-iteration trace:
+ * iter_trace_dev [n][trace_cap][DOCK_ITER_HEADER + (7+T) + (6+T) + (6+T)^2] floats, one record per iteration STARTED
+ * (the last one is the stop itself unless the cap ended the run); iterations >= trace_cap are not recorded.
+ * The caller zero-fills the buffer if it wants to tell unused records apart. */
+int dock_local_opt_trace(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                         int64_t n_poses, int32_t max_iters, const float *poses_dev,
+                         float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
+                         float *iter_trace_dev, int32_t trace_cap,
+                         void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
 /* ---- S16: initial poses from Philox ("randomly generated within this box", 67) ----
- * Generated on the host in double, rounded once to fp32.  out_host [copies][7+T]. */
-int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
-                    float *out_host);
+ * Generated on the host in double, rounded once to fp32.  out_host [copies][7+T] = the poses of copies
+ * copy_base .. copy_base + copies - 1 of `system` (the Philox counter words, so a shard of copies starts exactly
+ * where the same copies of an unsharded run start). */
+int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, uint32_t copy_base,
+                    int32_t copies, float *out_host);
 
 /* ---- NEXT-3: initial poses restrained to the adaptive search space (Fig. 3) ------
  * "A union set of balls with 7 A radius, centered at each discrete points of predicted binding site ... The
@@ -192,12 +223,17 @@ int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t syst
  * translation is drawn uniformly in the box by rejection (Philox slots 0x100 + attempt, 256 attempts, then
  * the site point copy mod n_site); orientation and torsions as dock_init_poses.  site_xyz_host [n_site][3],
  * same frame as the box; out_host [copies][7+T], to be passed to dock_search as init poses after upload. */
-int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
-                         int32_t n_site, const float *site_xyz_host, float radius, float *out_host);
+int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, uint32_t copy_base,
+                         int32_t copies, int32_t n_site, const float *site_xyz_host, float radius, float *out_host);
 
 /* ---- A6-A8: many-copy Monte-Carlo search + top-k -----------------------------
  * n_systems independent systems in one launch; grids[s], ligands[s], boxes[s] are HOST arrays of
  * descriptors.  T_max = max over systems of T; pose rows are 7+T_max floats wide (unused tail 0).
+ * system_base / copy_base: system s, copy c of this call draw the Philox streams of (system_base + s,
+ * copy_base + c) -- a multi-GPU run that shards systems or copies passes the index of its
+ * first unit and reproduces the unsharded run bit for bit; 0, 0 otherwise.
+ * Everything that can be rejected (sizes, shared-memory needs, mixed gradient modes) is rejected before any work is
+ * enqueued.
  * init_poses_dev [n_systems][copies][7+T_max] or NULL (then generated by dock_init_poses' rule).
  * best_pose_dev [n_systems][copies][7+T_max]; best_e_dev [n_systems][copies];
  * topk_pose_dev [n_systems][k][7+T_max]; topk_e_dev [n_systems][k]; topk_idx_dev [n_systems][k]
@@ -207,6 +243,7 @@ int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t
 int dock_search(const dock_params *params, int32_t n_systems,
                 const dock_grid *grids, const dock_ligand *ligands, const dock_box *boxes,
                 int32_t copies, int32_t steps, int32_t bfgs_max_iters, uint64_t seed,
+                uint32_t system_base, uint32_t copy_base,
                 const float *init_poses_dev,
                 float *best_pose_dev, float *best_e_dev,
                 float *topk_pose_dev, float *topk_e_dev, int32_t *topk_idx_dev, int32_t *topk_count_dev,
@@ -227,7 +264,7 @@ int dock_system_host(const dock_params *params, const dock_protein *protein, con
                      int32_t copies, int32_t steps, int32_t bfgs_max_iters, uint64_t seed,
                      float *out_topk_pose_host, float *out_topk_e_host, int32_t *out_count_host,
                      uint64_t *out_evals_host,
-                     float *grid_dev, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+                     float *grid_dev, size_t grid_bytes, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
 /* ---- diagnostics ------------------------------------------------------------------------------ */
 int         dock_last_cuda_error(void);          /* cudaError_t of the last failing CUDA call (0 = none) */

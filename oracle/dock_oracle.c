@@ -760,13 +760,83 @@ double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
     return f;
 }
 
-typedef struct { const orc_params *p; const orc_grid *g; const orc_ligand *L; } dock_ctx;
+typedef struct {
+    const orc_params *p; const orc_grid *g; const orc_ligand *L;
+    double *min_cutoff_margin;   /* diagnostic, nullable: min over all evaluations of orc_diag.cutoff_margin */
+} dock_ctx;
+
+/* Diagnostic switch for the "chaos ceiling" measurement; OFF by default and never
+ * switched on by anything but tests/parity.py: when on, the docking objective handed to the optimizers returns the
+ * oracle's energy and gradient rounded to a (24 - drop_bits)-bit significand: drop_bits = 0 is fp32 correctly
+ * rounded -- the best any single-precision evaluator could do --, drop_bits = 3 an fp32 result that is off by up to
+ * 4 ulp, which is what a sum of a few hundred fp32 terms delivers.  Comparing the oracle with itself under this
+ * switch says how far a free-running local optimisation / search may legitimately drift for a reason that is not an
+ * implementation difference.  drop_bits < 0 switches it off. */
+static int g_eval_drop_bits = -1;
+void orc_diag_round_eval_fp32(int drop_bits) { g_eval_drop_bits = drop_bits; }
+/* Second noise model of the same diagnostic: every value the optimizer sees carries ONE fp32 rounding error of its
+ * CONDITIONING SCALE -- E of |E_grid| + |E_wall| + |E_intra|, gradient component k of A_k (orc_grad_cond: the sum of
+ * the absolute values of its terms) -- times `c`, with a deterministic pseudo-random sign and size in [-1, 1], and is
+ * then rounded to fp32.  This is how an fp32 sum behaves (error ~ eps x sum of |terms|, not eps x |result|); the
+ * level-1 tests allow the kernel 8 such units per gradient component (reading S20').  c <= 0 switches it off. */
+static double g_eval_noise_c = 0.0;
+void orc_diag_eval_noise(double c) { g_eval_noise_c = c; }
+static double hash_unit(uint64_t x)                    /* splitmix64 -> [-1, 1) */
+{
+    x += 0x9E3779B97F4A7C15ull;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+    x ^= x >> 31;
+    return (double)(int64_t)x / 9223372036854775808.0;
+}
+static double round_sig(double x, int bits)
+{
+    if (x == 0.0 || !isfinite(x)) return x;
+    int e;
+    double m = frexp(x, &e);                       /* x = m 2^e, 0.5 <= |m| < 1 */
+    return ldexp(nearbyint(ldexp(m, bits)), e - bits);
+}
+
 /* ---------------------------------------------------------------------------------------
  * O8' Barzilai-Borwein ("BB only needs a vector inner product to estimate the step
  * length and does not need to perform line search"; ref. 37).  Reading S13:
  *   alpha_0 = bb_step / |g_0|;  alpha_k = s.s / s.y  (s = x_k - x_{k-1} in tangent coordinates,
  *   y = g_k - g_{k-1}) if s.y > curv_eps |s| |y|, else bb_fallback / |g_k|;  alpha_k |g_k| <= bb_step.
  * ------------------------------------------------------------------------------------- */
+/* One iteration from the state (x, f, gr) and the previous step (s, y; unused when `first`).  Returns 0 if the step was
+ * taken (state advanced: x, f, gr, s, y), ORC_EXIT_GTOL if ||g|| < gtol (nothing done).  Written once, used by the
+ * full loop (orc_bb) and by the single-step replay of the iteration-level parity test (orc_bb_step). */
+static int bb_iteration(const orc_params *p, int n, int np_, orc_objective_fn fn, orc_retract_fn add, void *ctx,
+                        int first, double *x, double *f, double *gr, double *s, double *y, double *xn, double *gn,
+                        int *ne, orc_bb_rec *rec)
+{
+    if (rec) { memset(rec, 0, sizeof(*rec)); rec->f = *f; }
+    double g2 = 0.0;
+    for (int k = 0; k < n; ++k) g2 += gr[k] * gr[k];
+    const double gnorm = sqrt(g2);
+    if (rec) rec->gnorm = gnorm;
+    if (gnorm < p->bfgs_gtol) { if (rec) rec->status = ORC_EXIT_GTOL; return ORC_EXIT_GTOL; }
+    double alpha;
+    if (first) alpha = p->bb_step / gnorm;
+    else {
+        double sy = 0.0, ss = 0.0, yy = 0.0;
+        for (int k = 0; k < n; ++k) { sy += s[k] * y[k]; ss += s[k] * s[k]; yy += y[k] * y[k]; }
+        alpha = (sy > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) ? ss / sy : p->bb_fallback / gnorm;
+        if (rec) { rec->branch = (sy > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) ? 1 : 2; rec->sy_margin = sy - p->bfgs_curv_eps * sqrt(ss) * sqrt(yy); }
+    }
+    if (rec) rec->cap_margin = alpha * gnorm - p->bb_step;
+    if (alpha * gnorm > p->bb_step) { alpha = p->bb_step / gnorm; if (rec) rec->capped = 1; }
+    for (int k = 0; k < n; ++k) s[k] = -alpha * gr[k];
+    add(ctx, x, s, xn);
+    const double fnew = fn(ctx, xn, gn);
+    ++*ne;
+    for (int k = 0; k < n; ++k) { y[k] = gn[k] - gr[k]; gr[k] = gn[k]; }
+    memcpy(x, xn, sizeof(double) * np_);
+    *f = fnew;
+    if (rec) { rec->alpha = alpha; rec->f_new = fnew; }
+    return 0;
+}
+
 double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
               orc_objective_fn fn, orc_retract_fn add, void *ctx,
               double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx, int *exit_reason)
@@ -782,25 +852,7 @@ double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
     double fbest = f;
     memcpy(x_out, x, sizeof(double) * np_);
     for (it = 0; it < cap; ++it) {
-        double g2 = 0.0;
-        for (int k = 0; k < n; ++k) g2 += gr[k] * gr[k];
-        const double gnorm = sqrt(g2);
-        if (gnorm < p->bfgs_gtol) { why = ORC_EXIT_GTOL; break; }
-        double alpha;
-        if (it == 0) alpha = p->bb_step / gnorm;
-        else {
-            double sy = 0.0, ss = 0.0, yy = 0.0;
-            for (int k = 0; k < n; ++k) { sy += s[k] * y[k]; ss += s[k] * s[k]; yy += y[k] * y[k]; }
-            alpha = (sy > p->bfgs_curv_eps * sqrt(ss) * sqrt(yy)) ? ss / sy : p->bb_fallback / gnorm;
-        }
-        if (alpha * gnorm > p->bb_step) alpha = p->bb_step / gnorm;
-        for (int k = 0; k < n; ++k) s[k] = -alpha * gr[k];
-        add(ctx, x, s, xn);
-        const double fnew = fn(ctx, xn, gn);
-        ++ne;
-        for (int k = 0; k < n; ++k) { y[k] = gn[k] - gr[k]; gr[k] = gn[k]; }
-        memcpy(x, xn, sizeof(double) * np_);
-        f = fnew;
+        if (bb_iteration(p, n, np_, fn, add, ctx, it == 0, x, &f, gr, s, y, xn, gn, &ne, NULL) != 0) { why = ORC_EXIT_GTOL; break; }
         if (obs) obs(obs_ctx, it, f, NULL, s, y, 1);
         if (f < fbest) { fbest = f; memcpy(x_out, x, sizeof(double) * np_); }
     }
@@ -814,7 +866,26 @@ double orc_bb(const orc_params *p, int n, int np_, int cap, const double *x0,
 static double dock_fn(void *c, const double *x, double *grad)
 {
     dock_ctx *k = (dock_ctx *)c;
-    return orc_eval(k->p, k->g, k->L, x, NULL, grad, NULL);
+    orc_diag dg;
+    double e = orc_eval(k->p, k->g, k->L, x, NULL, grad, k->min_cutoff_margin ? &dg : NULL);
+    if (k->min_cutoff_margin && dg.cutoff_margin < *k->min_cutoff_margin) *k->min_cutoff_margin = dg.cutoff_margin;
+    if (g_eval_drop_bits >= 0) {
+        e = round_sig(e, 24 - g_eval_drop_bits);
+        for (int i = 0; i < 6 + k->L->T; ++i) grad[i] = round_sig(grad[i], 24 - g_eval_drop_bits);
+    }
+    if (g_eval_noise_c > 0.0) {
+        const int n = 6 + k->L->T;
+        double tr[3], *A = (double *)malloc(sizeof(double) * n);
+        orc_eval(k->p, k->g, k->L, x, tr, NULL, NULL);
+        orc_grad_cond(k->p, k->g, k->L, x, A);
+        uint64_t seed;
+        memcpy(&seed, &e, sizeof(seed));
+        const double u = g_eval_noise_c * 5.9604644775390625e-08;   /* c 2^-24 */
+        e = (double)(float)(e + hash_unit(seed) * u * (fabs(tr[0]) + fabs(tr[1]) + fabs(tr[2])));
+        for (int i = 0; i < n; ++i) grad[i] = (double)(float)(grad[i] + hash_unit(seed + 1 + (uint64_t)i) * u * A[i]);
+        free(A);
+    }
+    return e;
 }
 static void dock_add(void *c, const double *x, const double *s, double *out)
 {
@@ -826,7 +897,7 @@ double orc_local_opt_ex(const orc_params *p, const orc_grid *g, const orc_ligand
                         orc_iter_rec *recs, int max_recs)
 {
     const int T = L->T;
-    dock_ctx ctx = {p, g, L};
+    dock_ctx ctx = {p, g, L, NULL};
     double *x0 = (double *)malloc(sizeof(double) * (7 + T));
     memcpy(x0, pose_in, sizeof(double) * (7 + T));
     quat_normalize(x0 + 3);
@@ -845,21 +916,25 @@ double orc_local_opt(const orc_params *p, const orc_grid *g, const orc_ligand *L
 
 /* Diagnostic for the iteration-level teacher-forced parity test (SURVEY.md 8(c) parity protocol; DESIGN.md
  * "Parity levels"): ONE iteration of O8 on the docking objective from a GIVEN state -- pose x (quaternion used
- * as given), inverse Hessian H [n][n] and the flag `fresh` (H is the identity of the start / of a reset).
- * The energy and gradient at x are evaluated here, in double.  Returns the status (0 = step accepted,
+ * as given), inverse Hessian H [n][n], the flag `fresh` (H is the identity of the start / of a reset) and,
+ * optionally, the gradient g_in at x (NULL: evaluated here).  The energy at x and at every trial point is
+ * evaluated here, in double.  Returns the status (0 = step accepted,
  * ORC_EXIT_GTOL, ORC_EXIT_LINESEARCH); x_new / H_new (nullable) receive the state after the iteration. */
 int orc_bfgs_step(const orc_params *p, const orc_grid *g, const orc_ligand *L,
-                  const double *x, const double *H, int fresh, orc_iter_rec *rec, double *x_new, double *H_new)
+                  const double *x, const double *g_in, const double *H, int fresh, orc_iter_rec *rec, double *x_new, double *H_new)
 {
     const int n = 6 + L->T, np_ = 7 + L->T;
-    dock_ctx ctx = {p, g, L};
+    double mcm = 1e300;
+    dock_ctx ctx = {p, g, L, &mcm};
     bfgs_state S;
     bfgs_alloc(&S, n, np_);
     memcpy(S.x, x, sizeof(double) * np_);
     memcpy(S.H, H, sizeof(double) * n * n);
     S.fresh = fresh;
     S.f = dock_fn(&ctx, S.x, S.gr);
+    if (g_in) memcpy(S.gr, g_in, sizeof(double) * n);      /* the recorded gradient is part of the given state */
     const int st = bfgs_iteration(p, &S, dock_fn, dock_add, &ctx, rec);
+    if (rec) rec->min_cutoff_margin = mcm;
     if (x_new) memcpy(x_new, S.x, sizeof(double) * np_);
     if (H_new) memcpy(H_new, S.H, sizeof(double) * n * n);
     bfgs_free(&S);
@@ -867,14 +942,48 @@ int orc_bfgs_step(const orc_params *p, const orc_grid *g, const orc_ligand *L,
 }
 
 void orc_bfgs_step_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n_states,
-                         const double *x, const double *H, const int32_t *fresh,
+                         const double *x, const double *g_in, const double *H, const int32_t *fresh,
                          orc_iter_rec *recs, double *x_new, double *H_new)
 {
     const int n = 6 + L->T, np_ = 7 + L->T;
 #pragma omp parallel for schedule(dynamic, 8)
     for (int64_t k = 0; k < n_states; ++k)
-        orc_bfgs_step(p, g, L, x + k * np_, H + k * n * n, fresh[k], recs + k,
+        orc_bfgs_step(p, g, L, x + k * np_, g_in ? g_in + k * n : NULL, H + k * n * n, fresh[k], recs + k,
                       x_new ? x_new + k * np_ : NULL, H_new ? H_new + k * n * n : NULL);
+}
+
+/* ONE O8' iteration on the docking objective from a GIVEN state: pose x, gradient g_in at x (NULL: evaluated here),
+ * previous step s_prev / y_prev (tangent coordinates; ignored when `first`).  Energies are evaluated here, in double. */
+int orc_bb_step(const orc_params *p, const orc_grid *g, const orc_ligand *L, const double *x, const double *g_in,
+                const double *s_prev, const double *y_prev, int first, orc_bb_rec *rec, double *x_new)
+{
+    const int n = 6 + L->T, np_ = 7 + L->T;
+    double mcm = 1e300;
+    dock_ctx ctx = {p, g, L, &mcm};
+    double *xx = (double *)malloc(sizeof(double) * np_), *xn = (double *)malloc(sizeof(double) * np_);
+    double *gr = (double *)malloc(sizeof(double) * n), *gn = (double *)malloc(sizeof(double) * n);
+    double *s = (double *)calloc(n, sizeof(double)), *y = (double *)calloc(n, sizeof(double));
+    memcpy(xx, x, sizeof(double) * np_);
+    double f = dock_fn(&ctx, xx, gr);
+    if (g_in) memcpy(gr, g_in, sizeof(double) * n);
+    if (!first) { memcpy(s, s_prev, sizeof(double) * n); memcpy(y, y_prev, sizeof(double) * n); }
+    int ne = 0;
+    const int st = bb_iteration(p, n, np_, dock_fn, dock_add, &ctx, first, xx, &f, gr, s, y, xn, gn, &ne, rec);
+    if (rec) rec->min_cutoff_margin = mcm;
+    if (x_new) memcpy(x_new, xx, sizeof(double) * np_);
+    free(xx); free(xn); free(gr); free(gn); free(s); free(y);
+    return st;
+}
+
+void orc_bb_step_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n_states,
+                       const double *x, const double *g_in, const double *s_prev, const double *y_prev,
+                       const int32_t *first, orc_bb_rec *recs, double *x_new)
+{
+    const int n = 6 + L->T, np_ = 7 + L->T;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t k = 0; k < n_states; ++k)
+        orc_bb_step(p, g, L, x + k * np_, g_in ? g_in + k * n : NULL, s_prev + k * n, y_prev + k * n, first[k],
+                    recs + k, x_new ? x_new + k * np_ : NULL);
 }
 
 /* batch of independent local optimisations (OpenMP over poses): poses [n][7+T] -> out_pose, out_e [n],

@@ -159,6 +159,8 @@ typedef struct {
     double f, gnorm, gp, alpha0, alpha, f_new;
     double armijo_margin[ORC_MAX_TRIALS];  /* (f_trial - f) - c1 alpha g.d of every trial: <= 0 accepts */
     double curv_margin; /* y.s - curv_eps |s| |y|: > 0 updates */
+    double min_cutoff_margin; /* orc_bfgs_step only: min over the state and all trial poses of the distance (A) of any
+                               * intra pair to the cutoff, where E itself jumps (S3) */
 } orc_iter_rec;
 
 /* recs (nullable, capacity max_recs) receives one record per iteration started; exit_reason nullable */
@@ -166,6 +168,18 @@ double orc_bfgs(const orc_params *p, int n, int np_, int cap, const double *x0,
                 orc_objective_fn fn, orc_retract_fn add, void *ctx,
                 double *x_out, int *iters, int *evals, orc_observer_fn obs, void *obs_ctx,
                 int *exit_reason, orc_iter_rec *recs, int max_recs);
+/* decision scalars of one O8' iteration (diagnostic; filled by orc_bb_step) */
+typedef struct {
+    int    status;      /* 0 = step taken, ORC_EXIT_GTOL = stopped before it */
+    int    branch;      /* 0 = first step (bb_step/|g|), 1 = BB1 s.s/s.y, 2 = fallback bb_fallback/|g| */
+    int    capped;      /* step length clipped to bb_step */
+    int    pad_;
+    double f, gnorm, alpha, f_new;
+    double sy_margin;   /* s.y - curv_eps |s| |y|: > 0 takes the BB1 step */
+    double cap_margin;  /* alpha |g| - bb_step before clipping: > 0 clips */
+    double min_cutoff_margin; /* as in orc_iter_rec */
+} orc_bb_rec;
+
 /* O8': x_{k+1} = x_k (+) (-alpha_k g_k), alpha_0 = bb_step/|g|, alpha_k = s.s/s.y (BB1) when
  * s.y > curv_eps |s||y| else bb_fallback/|g|, every step capped at length bb_step; one evaluation per iteration,
  * no line search; returns the best point seen (the method is non-monotone).  Same signature as orc_bfgs. */
@@ -183,12 +197,14 @@ double orc_local_opt_ex(const orc_params *p, const orc_grid *g, const orc_ligand
 /* OpenMP over poses: poses [n][7+T] -> out_pose [n][7+T], out_e [n], out_info [n][3] = (iters, evals, exit reason) */
 void   orc_local_opt_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap, int64_t n,
                            const double *poses, double *out_pose, double *out_e, int32_t *out_info);
-/* ONE O8 iteration on the docking objective from a GIVEN state (x, H [n][n], fresh); E and gradient at x are
- * evaluated here in double.  For the iteration-level teacher-forced parity test.  x_new / H_new nullable. */
+/* ONE O8 iteration on the docking objective from a GIVEN state (x, optional gradient g_in at x, H [n][n], fresh);
+ * every energy (and the gradient if g_in is NULL) is evaluated here in double.  For the iteration-level
+ * teacher-forced parity test.  x_new / H_new nullable. */
 int    orc_bfgs_step(const orc_params *p, const orc_grid *g, const orc_ligand *L,
-                     const double *x, const double *H, int fresh, orc_iter_rec *rec, double *x_new, double *H_new);
+                     const double *x, const double *g_in, const double *H, int fresh, orc_iter_rec *rec,
+                     double *x_new, double *H_new);
 void   orc_bfgs_step_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n_states,
-                           const double *x, const double *H, const int32_t *fresh,
+                           const double *x, const double *g_in, const double *H, const int32_t *fresh,
                            orc_iter_rec *recs, double *x_new, double *H_new);
 
 /* S16 initial pose for (system, copy) from Philox, rounded once to fp32 */
@@ -229,6 +245,14 @@ int64_t orc_search(const orc_params *p, const orc_grid *g, const orc_ligand *L,
                    const double *init_poses, double *best_pose, double *best_e,
                    double *trace_pose, orc_step_rec *trace, orc_step_rec *init_rec);
 
+/* ONE O8' (Barzilai-Borwein) iteration on the docking objective from a GIVEN state (x, optional gradient, previous
+ * step s_prev / y_prev unless `first`); energies evaluated here in double.  Iteration-level parity of NEXT-1. */
+int    orc_bb_step(const orc_params *p, const orc_grid *g, const orc_ligand *L, const double *x, const double *g_in,
+                   const double *s_prev, const double *y_prev, int first, orc_bb_rec *rec, double *x_new);
+void   orc_bb_step_batch(const orc_params *p, const orc_grid *g, const orc_ligand *L, int64_t n_states,
+                         const double *x, const double *g_in, const double *s_prev, const double *y_prev,
+                         const int32_t *first, orc_bb_rec *recs, double *x_new);
+
 /* teacher-forced replay of recorded MC steps (parity level 3'): see dock_oracle.c.  OpenMP over records. */
 void   orc_replay_steps(const orc_params *p, const orc_grid *g, const orc_ligand *L, int cap, uint64_t seed,
                         uint32_t system, int64_t n, const double *pre_pose, const int32_t *copy, const int32_t *step,
@@ -243,6 +267,12 @@ int    orc_topk(const orc_params *p, const orc_ligand *L, int copies, const doub
                 const double *e, int k, double rmsd_min, int32_t *out_idx);
 
 int    orc_num_threads(void);
+/* diagnostic switch (default off = negative): the objective seen by the optimizers is rounded to a (24 - drop_bits)-bit
+ * significand -- see dock_oracle.c */
+void   orc_diag_round_eval_fp32(int drop_bits);
+/* second noise model (default off = 0): one fp32 rounding error of the conditioning scale of E and of every gradient
+ * component, times c -- see dock_oracle.c */
+void   orc_diag_eval_noise(double c);
 
 #ifdef __cplusplus
 }

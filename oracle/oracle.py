@@ -92,8 +92,12 @@ ORC_MAX_TRIALS = 64
 EXIT_GTOL, EXIT_CAP, EXIT_LINESEARCH = 1, 2, 3
 ITER_DTYPE = np.dtype([("status", "i4"), ("reset", "i4"), ("fresh_in", "i4"), ("fresh_out", "i4"), ("trials", "i4"),
                        ("updated", "i4"), ("f", "f8"), ("gnorm", "f8"), ("gp", "f8"), ("alpha0", "f8"), ("alpha", "f8"),
-                       ("f_new", "f8"), ("armijo_margin", "f8", (ORC_MAX_TRIALS,)), ("curv_margin", "f8")])
-assert ITER_DTYPE.itemsize == 6 * 4 + 8 * (6 + ORC_MAX_TRIALS + 1)
+                       ("f_new", "f8"), ("armijo_margin", "f8", (ORC_MAX_TRIALS,)), ("curv_margin", "f8"),
+                       ("min_cutoff_margin", "f8")])
+assert ITER_DTYPE.itemsize == 6 * 4 + 8 * (6 + ORC_MAX_TRIALS + 2)
+
+BB_DTYPE = np.dtype([("status", "i4"), ("branch", "i4"), ("capped", "i4"), ("_pad", "i4"), ("f", "f8"), ("gnorm", "f8"),
+                     ("alpha", "f8"), ("f_new", "f8"), ("sy_margin", "f8"), ("cap_margin", "f8"), ("min_cutoff_margin", "f8")])
 
 STEP_DTYPE = np.dtype([("e_cur", "f8"), ("e_cand", "f8"), ("u", "f8"),
                        ("accept", "i4"), ("iters", "i4"), ("evals", "i4"), ("_pad", "i4")])
@@ -156,6 +160,37 @@ def params_as_fp32(p: Params) -> Params:
                  "bfgs_gtol", "bfgs_curv_eps", "cluster_rmsd", "bb_step", "bb_fallback"):
         setattr(q, name, float(np.float32(getattr(p, name))))
     return q
+
+
+class round_eval_fp32:
+    """Context manager for the chaos-ceiling diagnostic: inside, the optimizers see the oracle's energy and gradient
+    rounded to a (24 - drop_bits)-bit significand (dock_oracle.c: orc_diag_round_eval_fp32): 0 = fp32 correctly
+    rounded, 3 = an fp32 result off by up to 4 ulp.  Off outside; nothing else may switch it on."""
+
+    def __init__(self, drop_bits: int = 3):
+        self.drop_bits = int(drop_bits)
+
+    def __enter__(self):
+        lib().orc_diag_round_eval_fp32(self.drop_bits)
+
+    def __exit__(self, *exc):
+        lib().orc_diag_round_eval_fp32(-1)
+        return False
+
+
+class eval_noise:
+    """Context manager for the second chaos-ceiling model (dock_oracle.c: orc_diag_eval_noise): inside, every energy /
+    gradient component the optimizers see carries c fp32 rounding errors of its conditioning scale."""
+
+    def __init__(self, c: float = 1.0):
+        self.c = float(c)
+
+    def __enter__(self):
+        lib().orc_diag_eval_noise(C.c_double(self.c))
+
+    def __exit__(self, *exc):
+        lib().orc_diag_eval_noise(C.c_double(0.0))
+        return False
 
 
 def num_threads() -> int:
@@ -341,18 +376,35 @@ def local_opt_batch(p: Params, g: Grid, L: Ligand, poses, cap: int):
     return e, out, info
 
 
-def bfgs_step_batch(p: Params, g: Grid, L: Ligand, x, H, fresh):
-    """One O8 iteration from each given state (x [m,7+T], H [m,n,n], fresh [m]).  Returns (recs, x_new, H_new)."""
+def bfgs_step_batch(p: Params, g: Grid, L: Ligand, x, H, fresh, grad=None):
+    """One O8 iteration from each given state (x [m,7+T], H [m,n,n], fresh [m], optional gradient [m,n] at x).
+    Returns (recs, x_new, H_new)."""
     n = 6 + L.T
     x = _f64(x).reshape(-1, 7 + L.T)
     m = x.shape[0]
     H = _f64(H).reshape(m, n, n)
     fresh = _i32(fresh).reshape(m)
+    grad = None if grad is None else _f64(grad).reshape(m, n)
     recs = np.zeros(m, dtype=ITER_DTYPE)
     x_new, H_new = np.zeros_like(x), np.zeros_like(H)
-    lib().orc_bfgs_step_batch(C.byref(p), C.byref(g.c), C.byref(L.c), C.c_int64(m), _p(x), _p(H), _p(fresh),
+    lib().orc_bfgs_step_batch(C.byref(p), C.byref(g.c), C.byref(L.c), C.c_int64(m), _p(x), _p(grad), _p(H), _p(fresh),
                               _p(recs), _p(x_new), _p(H_new))
     return recs, x_new, H_new
+
+
+def bb_step_batch(p: Params, g: Grid, L: Ligand, x, grad, s_prev, y_prev, first):
+    """One O8' iteration from each given state.  Returns (recs, x_new)."""
+    n = 6 + L.T
+    x = _f64(x).reshape(-1, 7 + L.T)
+    m = x.shape[0]
+    grad = None if grad is None else _f64(grad).reshape(m, n)
+    s_prev, y_prev = _f64(s_prev).reshape(m, n), _f64(y_prev).reshape(m, n)
+    first = _i32(first).reshape(m)
+    recs = np.zeros(m, dtype=BB_DTYPE)
+    x_new = np.zeros_like(x)
+    lib().orc_bb_step_batch(C.byref(p), C.byref(g.c), C.byref(L.c), C.c_int64(m), _p(x), _p(grad), _p(s_prev), _p(y_prev),
+                            _p(first), _p(recs), _p(x_new))
+    return recs, x_new
 
 
 def replay_steps(p: Params, g: Grid, L: Ligand, cap: int, seed: int, system: int, pre_pose, copy, step):

@@ -4,6 +4,10 @@ The product is `libdock_b200.so` (hand-written sm_100a CUDA behind include/dock.
 only marshals arguments; it never computes any step of the path on the CPU.
 """
 from .binding import (  # noqa: F401
+    DOCK_EXIT_CAP,
+    DOCK_EXIT_GTOL,
+    DOCK_EXIT_LINESEARCH,
+    DOCK_ITER_HEADER,
     DOCK_TRACE_HEADER,
     DockError,
     EXPORTS,

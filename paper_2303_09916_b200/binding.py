@@ -19,12 +19,14 @@ DOCK_MAX_XS_TYPES = 32
 DOCK_MAX_TORSIONS = 32
 DOCK_MAX_ATOMS = 128
 DOCK_TRACE_HEADER = 8
+DOCK_ITER_HEADER = 12
+DOCK_EXIT_GTOL, DOCK_EXIT_CAP, DOCK_EXIT_LINESEARCH = 1, 2, 3
 DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
 
 EXPORTS = [
     "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_build_grids_batch", "dock_score_batch",
-    "dock_score_batch_host", "dock_local_opt_batch", "dock_init_poses", "dock_init_poses_site", "dock_search", "dock_topk",
-    "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
+    "dock_score_batch_host", "dock_local_opt_batch", "dock_local_opt_trace", "dock_init_poses", "dock_init_poses_site",
+    "dock_search", "dock_topk", "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
 ]
 
 
@@ -108,10 +110,12 @@ def _torch():
     return torch
 
 
+def _stream_obj(stream=None):
+    return stream if stream is not None else _torch().cuda.current_stream()
+
+
 def _stream(stream=None) -> C.c_void_p:
-    torch = _torch()
-    s = stream if stream is not None else torch.cuda.current_stream()
-    return C.c_void_p(s.cuda_stream)
+    return C.c_void_p(_stream_obj(stream).cuda_stream)
 
 
 def _ptr(t) -> C.c_void_p:
@@ -123,16 +127,28 @@ def _np_ptr(a: Optional[np.ndarray]) -> C.c_void_p:
 
 
 class _Workspace:
-    """Grow-only device scratch buffer (a torch uint8 tensor) reused across calls."""
+    """Grow-only device scratch buffers (torch uint8 tensors) reused across calls, ONE PER (device, stream).
+
+    The library stages ligand tables, system descriptors and cell lists in the workspace and returns without
+    synchronising, so a kernel still in flight on stream A must never see a later call on stream B overwrite them:
+    calls on different streams get different buffers; calls on one stream are ordered by the stream.  When a buffer
+    is replaced by a larger one the old tensor is handed to the caching allocator with record_stream, so its memory
+    is not reused before the work queued on that stream has finished."""
 
     def __init__(self):
-        self.buf = None
+        self.bufs = {}
 
-    def get(self, nbytes: int):
+    def get(self, nbytes: int, stream=None):
         torch = _torch()
-        if self.buf is None or self.buf.numel() < nbytes:
-            self.buf = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device="cuda")
-        return self.buf
+        st = _stream_obj(stream)
+        key = (torch.cuda.current_device(), int(st.cuda_stream))
+        buf = self.bufs.get(key)
+        if buf is None or buf.numel() < nbytes:
+            if buf is not None:
+                buf.record_stream(st)
+            buf = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device="cuda")
+            self.bufs[key] = buf
+        return buf
 
 
 _ws = _Workspace()
@@ -193,8 +209,8 @@ def dock_grid_dims(box: dock_box):
     return tuple(int(x) for x in d)
 
 
-def dock_grid_bytes(box: dock_box, n_lig_types: int) -> int:
-    n = int(load_library().dock_grid_bytes(C.byref(box), int(n_lig_types)))
+def dock_grid_bytes(params: dock_params, box: dock_box, n_lig_types: int) -> int:
+    n = int(load_library().dock_grid_bytes(C.byref(params), C.byref(box), int(n_lig_types)))
     if n == 0:
         raise DockError("dock_grid_bytes: bad box or type count")
     return n
@@ -210,19 +226,19 @@ def dock_build_grids(params: dock_params, protein_xyz, protein_type, box: dock_b
     lt = np.ascontiguousarray(lig_types, dtype=np.int32)
     nx, ny, nz = dock_grid_dims(box)
     ch = 4 if int(params.grad_mode) == 1 else 1                      # eq. 4: (score, d/dx, d/dy, d/dz) per map
-    buf = torch.empty(dock_grid_bytes(box, len(lt) * ch), dtype=torch.uint8, device="cuda")
+    buf = torch.empty(dock_grid_bytes(params, box, len(lt)), dtype=torch.uint8, device="cuda")
     data = buf[: len(lt) * ch * nz * ny * nx * 4].view(torch.float32)
     data = data.view(len(lt), nz, ny, nx) if ch == 1 else data.view(len(lt), ch, nz, ny, nx)
     desc = dock_grid()
     need = C.c_size_t(0)
     rc = lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
-                              None, None, None, C.c_size_t(0), C.byref(need), None)
+                              None, C.c_size_t(0), None, None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_build_grids(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
     _check(lib.dock_build_grids(C.byref(params), C.byref(prot), C.byref(box), len(lt), _np_ptr(lt),
-                                _ptr(buf), C.byref(desc), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
-                                _stream(stream)), "dock_build_grids")
+                                _ptr(buf), C.c_size_t(buf.numel()), C.byref(desc), _ptr(ws), C.c_size_t(ws.numel()),
+                                C.byref(need), _stream(stream)), "dock_build_grids")
     return GridMaps(buf, data, desc)
 
 
@@ -239,6 +255,7 @@ def dock_build_grids_batch(params: dock_params, proteins, boxes: Sequence[dock_b
     keep, prots, bxs = [], (dock_protein * ns)(), (dock_box * ns)()
     bufs, datas = [], []
     ptrs = (C.c_void_p * ns)()
+    sizes = (C.c_size_t * ns)()
     for s, (xyz, typ) in enumerate(proteins):
         xyz = np.ascontiguousarray(xyz, dtype=np.float32).reshape(-1, 3)
         typ = np.ascontiguousarray(typ, dtype=np.int32)
@@ -246,19 +263,20 @@ def dock_build_grids_batch(params: dock_params, proteins, boxes: Sequence[dock_b
         prots[s] = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
         bxs[s] = boxes[s]
         nx, ny, nz = dock_grid_dims(boxes[s])
-        buf = torch.empty(dock_grid_bytes(boxes[s], len(lt) * ch), dtype=torch.uint8, device="cuda")
+        buf = torch.empty(dock_grid_bytes(params, boxes[s], len(lt)), dtype=torch.uint8, device="cuda")
         data = buf[: len(lt) * ch * nz * ny * nx * 4].view(torch.float32)
         datas.append(data.view(len(lt), nz, ny, nx) if ch == 1 else data.view(len(lt), ch, nz, ny, nx))
         bufs.append(buf)
         ptrs[s] = buf.data_ptr()
+        sizes[s] = buf.numel()
     descs = (dock_grid * ns)()
     need = C.c_size_t(0)
-    rc = lib.dock_build_grids_batch(C.byref(params), ns, prots, bxs, len(lt), _np_ptr(lt), None, None, None,
+    rc = lib.dock_build_grids_batch(C.byref(params), ns, prots, bxs, len(lt), _np_ptr(lt), None, None, None, None,
                                     C.c_size_t(0), C.byref(need), None)
     if rc not in (DOCK_EWORKSPACE, DOCK_OK):
         _check(rc, "dock_build_grids_batch(size query)")
-    ws = _ws.get(max(need.value, 256))
-    _check(lib.dock_build_grids_batch(C.byref(params), ns, prots, bxs, len(lt), _np_ptr(lt), ptrs, descs, _ptr(ws),
+    ws = _ws.get(max(need.value, 256), stream)
+    _check(lib.dock_build_grids_batch(C.byref(params), ns, prots, bxs, len(lt), _np_ptr(lt), ptrs, sizes, descs, _ptr(ws),
                                       C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_build_grids_batch")
     out = []
     for s in range(ns):
@@ -287,7 +305,7 @@ def dock_score_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, 
                               None, None, None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_score_batch(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
     _check(lib.dock_score_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), _ptr(poses),
                                 _ptr(energy), _ptr(grad), _ptr(terms), _ptr(ws), C.c_size_t(ws.numel()),
                                 C.byref(need), _stream(stream)), "dock_score_batch")
@@ -312,53 +330,66 @@ def dock_score_batch_host(params: dock_params, grid: GridMaps, ligand: LigandHan
     rc = lib.dock_score_batch_host(*args, None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_score_batch_host(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
     _check(lib.dock_score_batch_host(*args, _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)),
            "dock_score_batch_host")
     return energy, grad, terms
 
 
-def dock_local_opt_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses, max_iters: int, stream=None):
+def dock_local_opt_batch(params: dock_params, grid: GridMaps, ligand: LigandHandle, poses, max_iters: int, stream=None,
+                         trace_cap: int = 0):
+    """Returns (out_pose [n,7+T], out_e [n], out_it [n,3] = iterations, evaluations, DOCK_EXIT_* reason) and, with
+    trace_cap > 0, a 4th item: the per-iteration trace [n, trace_cap, DOCK_ITER_HEADER + (7+T) + (6+T) + (6+T)^2] (dock.h)."""
     torch = _torch()
     lib = load_library()
     assert poses.is_cuda and poses.dtype == torch.float32 and poses.is_contiguous()
     n = int(poses.shape[0])
     out_pose = torch.empty_like(poses)
     out_e = torch.empty(n, dtype=torch.float32, device="cuda")
-    out_it = torch.empty((n, 2), dtype=torch.int32, device="cuda")
+    out_it = torch.empty((n, 3), dtype=torch.int32, device="cuda")
     need = C.c_size_t(0)
     rc = lib.dock_local_opt_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), int(max_iters),
                                   None, None, None, None, None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_local_opt_batch(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
+    if trace_cap > 0:
+        nn = 6 + ligand.T
+        trace = torch.zeros((n, int(trace_cap), DOCK_ITER_HEADER + 7 + ligand.T + nn + nn * nn), dtype=torch.float32, device="cuda")
+        _check(lib.dock_local_opt_trace(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), int(max_iters),
+                                        _ptr(poses), _ptr(out_pose), _ptr(out_e), _ptr(out_it), _ptr(trace), int(trace_cap),
+                                        _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_local_opt_trace")
+        return out_pose, out_e, out_it, trace
     _check(lib.dock_local_opt_batch(C.byref(params), C.byref(grid.desc), C.byref(ligand.c), C.c_int64(n), int(max_iters),
                                     _ptr(poses), _ptr(out_pose), _ptr(out_e), _ptr(out_it), _ptr(ws),
                                     C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_local_opt_batch")
     return out_pose, out_e, out_it
 
 
-def dock_init_poses(box: dock_box, T: int, seed: int, system: int, copies: int) -> np.ndarray:
+def dock_init_poses(box: dock_box, T: int, seed: int, system: int, copies: int, copy_base: int = 0) -> np.ndarray:
     out = np.zeros((copies, 7 + T), dtype=np.float32)
-    _check(load_library().dock_init_poses(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), int(copies),
-                                          _np_ptr(out)), "dock_init_poses")
+    _check(load_library().dock_init_poses(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), C.c_uint32(copy_base),
+                                          int(copies), _np_ptr(out)), "dock_init_poses")
     return out
 
 
-def dock_init_poses_site(box: dock_box, T: int, seed: int, system: int, copies: int, site_xyz, radius: float = 7.0) -> np.ndarray:
+def dock_init_poses_site(box: dock_box, T: int, seed: int, system: int, copies: int, site_xyz, radius: float = 7.0,
+                         copy_base: int = 0) -> np.ndarray:
     """NEXT-3: initial poses with the translation restrained to box ∩ union of balls around the site points."""
     site = np.ascontiguousarray(site_xyz, dtype=np.float32).reshape(-1, 3)
     out = np.zeros((copies, 7 + T), dtype=np.float32)
-    _check(load_library().dock_init_poses_site(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), int(copies),
-                                               int(site.shape[0]), _np_ptr(site), C.c_float(radius), _np_ptr(out)),
+    _check(load_library().dock_init_poses_site(C.byref(box), int(T), C.c_uint64(seed), C.c_uint32(system), C.c_uint32(copy_base),
+                                               int(copies), int(site.shape[0]), _np_ptr(site), C.c_float(radius), _np_ptr(out)),
            "dock_init_poses_site")
     return out
 
 
 def dock_search(params: dock_params, grids: Sequence[GridMaps], ligands: Sequence[LigandHandle],
                 boxes: Optional[Sequence[dock_box]], copies: int, steps: int, bfgs_max_iters: int, seed: int,
-                init_poses=None, want_trace: bool = False, want_topk: bool = True, stream=None):
-    """Many-copy MC search for n_systems systems in one launch.  Returns a dict of torch tensors."""
+                init_poses=None, want_trace: bool = False, want_topk: bool = True, stream=None,
+                system_base: int = 0, copy_base: int = 0):
+    """Many-copy MC search for n_systems systems in one launch.  Returns a dict of torch tensors.
+    system_base / copy_base: Philox indices of the first system / copy of this call (sharded runs, dock.h)."""
     torch = _torch()
     lib = load_library()
     ns = len(grids)
@@ -383,12 +414,12 @@ def dock_search(params: dock_params, grids: Sequence[GridMaps], ligands: Sequenc
         assert tuple(init_poses.shape) == (ns, copies, row)
     need = C.c_size_t(0)
     head = (C.byref(params), ns, g_arr, l_arr, b_arr, int(copies), int(steps), int(bfgs_max_iters), C.c_uint64(seed),
-            _ptr(init_poses))
+            C.c_uint32(system_base), C.c_uint32(copy_base), _ptr(init_poses))
     rc = lib.dock_search(*head, _ptr(best_pose), _ptr(best_e), None, None, None, None, None, None,
                          None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_search(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
     _check(lib.dock_search(*head, _ptr(best_pose), _ptr(best_e), _ptr(topk_pose), _ptr(topk_e), _ptr(topk_idx),
                            _ptr(topk_cnt), _ptr(trace), _ptr(evals), _ptr(ws), C.c_size_t(ws.numel()), C.byref(need),
                            _stream(stream)), "dock_search")
@@ -407,7 +438,7 @@ def dock_topk(params: dock_params, ligand: LigandHandle, poses, e, stream=None):
     rc = lib.dock_topk(C.byref(params), C.byref(ligand.c), n, None, None, None, None, None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_topk(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
     _check(lib.dock_topk(C.byref(params), C.byref(ligand.c), n, _ptr(poses), _ptr(e), _ptr(out_idx), _ptr(out_cnt),
                          _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_topk")
     return out_idx, out_cnt
@@ -424,8 +455,7 @@ def dock_system_host(params: dock_params, protein_xyz, protein_type, box: dock_b
     prot = dock_protein(int(xyz.shape[0]), _np_ptr(xyz), _np_ptr(typ))
     lt = np.ascontiguousarray(lig_types, dtype=np.int32)
     if grid_buf is None:
-        grid_buf = torch.empty(dock_grid_bytes(box, len(lt) * (4 if int(params.grad_mode) == 1 else 1)), dtype=torch.uint8,
-                               device="cuda")
+        grid_buf = torch.empty(dock_grid_bytes(params, box, len(lt)), dtype=torch.uint8, device="cuda")
     k = int(params.topk)
     out_pose = np.zeros((k, 7 + ligand.T), dtype=np.float32)
     out_e = np.zeros(k, dtype=np.float32)
@@ -434,11 +464,11 @@ def dock_system_host(params: dock_params, protein_xyz, protein_type, box: dock_b
     need = C.c_size_t(0)
     head = (C.byref(params), C.byref(prot), C.byref(box), C.byref(ligand.c), len(lt), _np_ptr(lt), int(copies),
             int(steps), int(bfgs_max_iters), C.c_uint64(seed), _np_ptr(out_pose), _np_ptr(out_e), _np_ptr(out_cnt),
-            _np_ptr(out_ev), _ptr(grid_buf))
+            _np_ptr(out_ev), _ptr(grid_buf), C.c_size_t(grid_buf.numel()))
     rc = lib.dock_system_host(*head, None, C.c_size_t(0), C.byref(need), None)
     if rc != DOCK_EWORKSPACE:
         _check(rc, "dock_system_host(size query)")
-    ws = _ws.get(need.value)
+    ws = _ws.get(need.value, stream)
     _check(lib.dock_system_host(*head, _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)),
            "dock_system_host")
     return dict(topk_pose=out_pose, topk_e=out_e, count=int(out_cnt[0]), evals=int(out_ev[0]))

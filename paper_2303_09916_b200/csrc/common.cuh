@@ -5,26 +5,28 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "../../include/dock.h"
 
 #define FULL_MASK 0xffffffffu
 
 // ---- host-side error plumbing -----------------------------------------------------------------
-extern int g_dock_last_cuda_error;
-extern unsigned long long g_dock_launches;
+extern std::atomic<int> g_dock_last_cuda_error;
+extern std::atomic<unsigned long long> g_dock_launches;
 
 #define DOCK_CUDA_CHECK(expr)                                   \
     do {                                                        \
         cudaError_t _e = (expr);                                \
         if (_e != cudaSuccess) {                                \
-            g_dock_last_cuda_error = (int)_e;                   \
+            g_dock_last_cuda_error.store((int)_e);              \
             return DOCK_ECUDA;                                  \
         }                                                       \
     } while (0)
 
 #define DOCK_LAUNCH_CHECK()                                     \
     do {                                                        \
-        ++g_dock_launches;                                      \
+        g_dock_launches.fetch_add(1);                           \
         DOCK_CUDA_CHECK(cudaGetLastError());                    \
     } while (0)
 

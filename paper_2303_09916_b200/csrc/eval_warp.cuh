@@ -173,10 +173,15 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
     }
     float e_intra = fmaf(P.eA, aA, fmaf(P.eB, aB, P.sigma * fmaf(0.5f, aRep, fmaf(-0.7f, aHb, -aHyd))));
 
-    e_grid = warp_sum(e_grid);
-    e_wall = warp_sum(e_wall);
-    e_intra = warp_sum(e_intra);
-    if (terms) { terms->e_grid = e_grid; terms->e_wall = e_wall; terms->e_intra = e_intra; }
+    // the lanes' partial energies are added in double: the total feeds the Armijo and Metropolis decisions, and a
+    // 32-term fp32 tree would add ~1e-6 |E| of noise to differences the line search has to resolve
+    float e_total;
+    if (terms) {
+        const double dg = warp_sum_d((double)e_grid), dw = warp_sum_d((double)e_wall), di = warp_sum_d((double)e_intra);
+        terms->e_grid = (float)dg; terms->e_wall = (float)dw; terms->e_intra = (float)di;
+        e_total = (float)(dg + dw + di);
+    } else
+        e_total = (float)warp_sum_d((double)e_grid + (double)e_wall + (double)e_intra);
 
     // ---- A5 ------------------------------------------------------------------------------------
     // With p_i = x_i - t (lever arm about the pivot) and m_i = p_i x g_i:
@@ -236,5 +241,5 @@ __device__ __forceinline__ float eval_pose_warp(const DevParams &P, const DevGri
         }
         __syncwarp();
     }
-    return e_grid + e_wall + e_intra;
+    return e_total;
 }

@@ -7,7 +7,7 @@
 // (counting sort, stable -> fixed summation order).  Device: one thread per node, a warp covers a
 // compact 4x4x2 block of nodes so that its lanes share almost the same in-range atom set: the warp collects
 // the atoms near its block once (shared-memory candidate list), then each thread walks the list, decides
-// r < cutoff in fp32 in the stated order (DESIGN.md D-CUT) and accumulates up to 8 maps in registers.
+// r < cutoff (fp32, redone in double within round-off of the cutoff: DESIGN.md D-CUT) and accumulates up to 8 maps in registers.
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -20,26 +20,50 @@ namespace {
 
 constexpr int MAPS_PER_PASS = 8;
 
-struct GridBuildArgs {
+// Per-system part of the arguments; an array of these lives in the workspace so that ONE launch covers all systems
+// of a screening batch (BASELINE.json configs[3]).
+struct GridSysArgs {
     int   nx, ny, nz;
     float ox, oy, oz, h;
-    float cutoff, cutoff2;
     float clo[3];          // low corner of the cell lattice
     float inv_cell;        // 1 / cell edge
     int   ncx, ncy, ncz;
+    int   atoms_off;       // first atom of this system in GridBuildArgs::atoms
+    int   cells_off;       // first cell of this system in GridBuildArgs::cell_start (entries are system-local atom indices)
+    int   block_begin;     // first value of blockIdx.x that belongs to this system
+    int   pad_;
+    float *out;            // [n_maps][channels][nz][ny][nx]
+    Cell8 *packed;         // gather image of the same maps
+};
+
+struct GridBuildArgs {
+    float cutoff, cutoff2;
     int   n_maps, n_types;
     float w[5];
-    const float4 *atoms;   // sorted by cell; w = bitcast(type)
+    const float4 *atoms;   // all systems, each sorted by cell; w = bitcast(type)
     const int    *cell_start;
     const float4 *pair_tab;// [n_maps][n_types] {rsum, wh, whb, 0}
-    float        *out;     // [n_maps][channels][nz][ny][nx]
     int   channels;        // 1, or 4 = (score, d/dx, d/dy, d/dz): eq. 4's per-vertex gradients (NEXT-2)
     // maps are processed in order of ligand radius: slot k writes map map_of[k]; bit k of fresh says that slot k
     // has another radius than slot k-1 (or opens a pass), i.e. the distance-only part of the term must be recomputed.
     // The two Gaussians and the repulsion depend on the ligand type only through its radius.
     int      map_of[DOCK_MAX_XS_TYPES];
     unsigned fresh;
+    const GridSysArgs *sys;
+    int   n_sys;
 };
+
+// r < cutoff for node (ix,iy,iz) at origin + h i and an atom, every operation in double with products and sums rounded
+// separately (no contraction).  Rare path of grid_build_kernel: kept out of line so that it costs the hot loop no registers.
+__device__ __noinline__ bool in_range_exact(float ox, float oy, float oz, float h, int ix, int iy, int iz,
+                                            float ax, float ay, float az, float cutoff)
+{
+    const double ddx = __dsub_rn(__dadd_rn((double)ox, __dmul_rn((double)h, (double)ix)), (double)ax);
+    const double ddy = __dsub_rn(__dadd_rn((double)oy, __dmul_rn((double)h, (double)iy)), (double)ay);
+    const double ddz = __dsub_rn(__dadd_rn((double)oz, __dmul_rn((double)h, (double)iz)), (double)az);
+    const double rr = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(ddx, ddx), __dmul_rn(ddy, ddy)), __dmul_rn(ddz, ddz)));
+    return rr < (double)cutoff;
+}
 
 constexpr int GRID_CAND = 256;       // candidate atoms a warp collects before it evaluates them
 
@@ -52,33 +76,48 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
 {
     __shared__ float4 tab[MAPS_PER_PASS * DOCK_MAX_XS_TYPES];
     __shared__ float4 cand_all[4][GRID_CAND];
+    __shared__ GridSysArgs S;
     const int m0 = blockIdx.y * MAPS_PER_PASS;
     const int nm = min(MAPS_PER_PASS, A.n_maps - m0);
     for (int k = threadIdx.x; k < nm * A.n_types; k += blockDim.x) tab[k] = A.pair_tab[m0 * A.n_types + k];
+    if (threadIdx.x == 0) {                                           // the system this block belongs to
+        int lo = 0, hi = A.n_sys - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if ((int)blockIdx.x >= __ldg(&A.sys[mid].block_begin)) lo = mid; else hi = mid - 1;
+        }
+        S = A.sys[lo];
+    }
     __syncthreads();
 
     // block tile 8 x 8 x 2 nodes; warp tile 4 x 4 x 2
-    const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8;
-    const int bx = blockIdx.x % tbx, by = (blockIdx.x / tbx) % tby, bz = blockIdx.x / (tbx * tby);
+    const int tbx = (S.nx + 7) / 8, tby = (S.ny + 7) / 8;
+    const int bl = (int)blockIdx.x - S.block_begin;
+    const int bx = bl % tbx, by = (bl / tbx) % tby, bz = bl / (tbx * tby);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wx0 = bx * 8 + (warp & 1) * 4, wy0 = by * 8 + (warp >> 1) * 4, wz0 = bz * 2;
-    if (wx0 >= A.nx || wy0 >= A.ny || wz0 >= A.nz) return;            // whole warp outside the lattice
+    if (wx0 >= S.nx || wy0 >= S.ny || wz0 >= S.nz) return;            // whole warp outside the lattice
     const int ix = wx0 + (lane & 3), iy = wy0 + ((lane >> 2) & 3), iz = wz0 + (lane >> 4);
-    const bool live = ix < A.nx && iy < A.ny && iz < A.nz;
+    const bool live = ix < S.nx && iy < S.ny && iz < S.nz;
     float4 *cand = cand_all[warp];
+    const float4 *atoms = A.atoms + S.atoms_off;
+    const int *cell_start = A.cell_start + S.cells_off;
 
-    // node coordinate exactly as the oracle's fp32 cutoff rule states it: fmaf(i, h, origin)
-    const float mx = __fmaf_rn((float)ix, A.h, A.ox);
-    const float my = __fmaf_rn((float)iy, A.h, A.oy);
-    const float mz = __fmaf_rn((float)iz, A.h, A.oz);
+    // node coordinate in fp32: fmaf(i, h, origin); r^2 < cutoff^2 is decided on it unless it is within round-off of the
+    // threshold, where the decision is redone in double (flush(), DESIGN.md D-CUT)
+    const float mx = __fmaf_rn((float)ix, S.h, S.ox);
+    const float my = __fmaf_rn((float)iy, S.h, S.oy);
+    const float mz = __fmaf_rn((float)iz, S.h, S.oz);
     // the warp's block: centre, and the cutoff grown by its half-diagonal (1.5, 1.5, 0.5 spacings) plus a guard band
-    const float cxw = fmaf((float)wx0 + 1.5f, A.h, A.ox), cyw = fmaf((float)wy0 + 1.5f, A.h, A.oy), czw = fmaf((float)wz0 + 0.5f, A.h, A.oz);
-    const float reach = A.cutoff + 2.18f * A.h + 0.01f;
+    const float cxw = fmaf((float)wx0 + 1.5f, S.h, S.ox), cyw = fmaf((float)wy0 + 1.5f, S.h, S.oy), czw = fmaf((float)wz0 + 0.5f, S.h, S.oz);
+    const float reach = A.cutoff + 2.18f * S.h + 0.01f;
     const float reach2 = reach * reach;
-    const int cx_lo = max((int)floorf((cxw - reach - A.clo[0]) * A.inv_cell), 0), cx_hi = min((int)floorf((cxw + reach - A.clo[0]) * A.inv_cell), A.ncx - 1);
-    const int cy_lo = max((int)floorf((cyw - reach - A.clo[1]) * A.inv_cell), 0), cy_hi = min((int)floorf((cyw + reach - A.clo[1]) * A.inv_cell), A.ncy - 1);
-    const int cz_lo = max((int)floorf((czw - reach - A.clo[2]) * A.inv_cell), 0), cz_hi = min((int)floorf((czw + reach - A.clo[2]) * A.inv_cell), A.ncz - 1);
+    const int cx_lo = max((int)floorf((cxw - reach - S.clo[0]) * S.inv_cell), 0), cx_hi = min((int)floorf((cxw + reach - S.clo[0]) * S.inv_cell), S.ncx - 1);
+    const int cy_lo = max((int)floorf((cyw - reach - S.clo[1]) * S.inv_cell), 0), cy_hi = min((int)floorf((cyw + reach - S.clo[1]) * S.inv_cell), S.ncy - 1);
+    const int cz_lo = max((int)floorf((czw - reach - S.clo[2]) * S.inv_cell), 0), cz_hi = min((int)floorf((czw + reach - S.clo[2]) * S.inv_cell), S.ncz - 1);
 
+    // |r2_fp32 - r2_exact| <= ~2 r (ulp of a 60 A coordinate) + 3 ulp(r2): well inside 1e-3 A^2 for boxes up to a few hundred A
+    const float cut_window = 1e-3f;
     float acc[MAPS_PER_PASS], agx[MAPS_PER_PASS], agy[MAPS_PER_PASS], agz[MAPS_PER_PASS];
 #pragma unroll
     for (int m = 0; m < MAPS_PER_PASS; ++m) acc[m] = agx[m] = agy[m] = agz[m] = 0.0f;
@@ -91,7 +130,14 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
                 const float4 a = cand[k];
                 const float fx = __fsub_rn(mx, a.x), fy = __fsub_rn(my, a.y), fz = __fsub_rn(mz, a.z);
                 const float r2 = __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx)));
-                if (r2 < A.cutoff2) {
+                bool in_range = r2 < A.cutoff2;
+                if (fabsf(r2 - A.cutoff2) < cut_window) {
+                    // Within fp32 round-off of the cutoff sphere (about one node-atom pair in 150): the vertex score jumps by
+                    // f(cutoff^-) ~ -0.004 there (reading S3), so the decision is taken as the definition states it -- r < cutoff
+                    // with the node at origin + h i and every operation in double, products and sums rounded separately
+                    in_range = in_range_exact(S.ox, S.oy, S.oz, S.h, ix, iy, iz, a.x, a.y, a.z, A.cutoff);
+                }
+                if (in_range) {
                     const float r = sqrtf(r2);
                     const int tj = __float_as_int(a.w);
                     float d = 0.f, dm3 = 0.f, rep = 0.f, base = 0.f, dbase = 0.f;
@@ -129,14 +175,14 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
     for (int zc = cz_lo; zc <= cz_hi; ++zc)
         for (int yc = cy_lo; yc <= cy_hi; ++yc) {
             // the x-cells of a row are contiguous in the sorted atom array
-            const int base = (zc * A.ncy + yc) * A.ncx;
-            const int j0 = __ldg(&A.cell_start[base + cx_lo]), j1 = __ldg(&A.cell_start[base + cx_hi + 1]);
+            const int base = (zc * S.ncy + yc) * S.ncx;
+            const int j0 = __ldg(&cell_start[base + cx_lo]), j1 = __ldg(&cell_start[base + cx_hi + 1]);
             for (int jb = j0; jb < j1; jb += 32) {
                 const int j = jb + lane;
                 float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
                 bool near = false;
                 if (j < j1) {
-                    a = __ldg(&A.atoms[j]);
+                    a = __ldg(&atoms[j]);
                     const float dx = a.x - cxw, dy = a.y - cyw, dz = a.z - czw;
                     near = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < reach2;
                 }
@@ -149,12 +195,12 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
     flush(n_cand);
     if (!live) return;
 
-    const size_t nodes = (size_t)A.nx * A.ny * A.nz;
-    const size_t node = ((size_t)iz * A.ny + iy) * A.nx + ix;
+    const size_t nodes = (size_t)S.nx * S.ny * S.nz;
+    const size_t node = ((size_t)iz * S.ny + iy) * S.nx + ix;
 #pragma unroll
     for (int m = 0; m < MAPS_PER_PASS; ++m)
         if (m < nm) {
-            float *o = A.out + (size_t)A.map_of[m0 + m] * A.channels * nodes + node;
+            float *o = S.out + (size_t)A.map_of[m0 + m] * A.channels * nodes + node;
             o[0] = acc[m];
             if (GRAD) { o[nodes] = agx[m]; o[2 * nodes] = agy[m]; o[3 * nodes] = agz[m]; }
         }
@@ -162,10 +208,14 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
 
 // Gather layout (Cell8, common.cuh): entry (ix,iy,iz) of map m = the 8 corners of the cell whose low corner is that
 // node (indices clamped to the last node).  Pure data movement: values are bit-identical copies.
-__global__ void __launch_bounds__(256) grid_pack_kernel(const float *__restrict__ plain, Cell8 *__restrict__ packed,
-                                                        int nx, int ny, int nz, long long rows)
+__global__ void __launch_bounds__(256) grid_pack_kernel(const GridSysArgs *__restrict__ sys, int maps_x_channels)
 {
-    // one thread per entry; consecutive threads walk x -> coalesced reads, 32-byte stores
+    // blockIdx.y = system; one thread per entry; consecutive threads walk x -> coalesced reads, 32-byte stores
+    const GridSysArgs S = sys[blockIdx.y];
+    const int nx = S.nx, ny = S.ny, nz = S.nz;
+    const float *__restrict__ plain = S.out;
+    Cell8 *__restrict__ packed = S.packed;
+    const long long rows = (long long)maps_x_channels * nz * ny;
     const long long total = rows * nx;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
         const int ix = (int)(e % nx);
@@ -277,103 +327,127 @@ extern "C" int dock_grid_dims(const dock_box *box, int32_t dims[3])
     return DOCK_OK;
 }
 
-extern "C" size_t dock_grid_bytes(const dock_box *box, int32_t n_lig_types)
+extern "C" size_t dock_grid_bytes(const dock_params *params, const dock_box *box, int32_t n_lig_types)
 {
     int32_t dims[3];
-    if (n_lig_types < 1 || n_lig_types > 4 * DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
-    const size_t nodes = (size_t)dims[0] * dims[1] * dims[2] * (size_t)n_lig_types;
+    if (!params || n_lig_types < 1 || n_lig_types > DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
+    const size_t ch = params->grad_mode == 1 ? 4 : 1;
+    const size_t nodes = (size_t)dims[0] * dims[1] * dims[2] * (size_t)n_lig_types * ch;
     return align_up(nodes * sizeof(float), 256) + nodes * sizeof(Cell8);
 }
 
-extern "C" int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
-                                int32_t n_lig_types, const int32_t *lig_types,
-                                float *grid_dev, dock_grid *out_desc,
-                                void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+// All systems in ONE upload and two launches (build, pack): the per-system lattice descriptions, cell lists and sorted
+// atoms are concatenated in the workspace; a block finds its system from GridSysArgs::block_begin.
+extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_systems, const dock_protein *proteins,
+                                      const dock_box *boxes, int32_t n_lig_types, const int32_t *lig_types,
+                                      float *const *grid_dev, const size_t *grid_bytes, dock_grid *out_descs,
+                                      void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
 {
-    GridPlan pl;
-    const int rc = plan_grid(params, protein, box, n_lig_types, lig_types, pl);
-    if (rc != DOCK_OK) return rc;
-    const size_t b_atoms = align_up(pl.atoms.size() * sizeof(float4), 256);
-    const size_t b_cells = align_up(pl.cell_start.size() * sizeof(int), 256);
-    const size_t b_tab = align_up(pl.pair_tab.size() * sizeof(float4), 256);
-    const size_t need = b_atoms + b_cells + b_tab;
+    if (n_systems < 0 || (n_systems > 0 && (!proteins || !boxes))) return DOCK_EINVAL;
+    if (n_systems == 0) {
+        if (dock_validate_params(params) != DOCK_OK) return DOCK_EINVAL;
+        if (needed) *needed = 0;
+        return DOCK_OK;
+    }
+    std::vector<GridPlan> plans(n_systems);
+    std::vector<GridSysArgs> sys(n_systems);
+    size_t n_atoms = 0, n_cells = 0;
+    long long n_blocks = 0;
+    for (int s = 0; s < n_systems; ++s) {
+        const int rc = plan_grid(params, &proteins[s], &boxes[s], n_lig_types, lig_types, plans[s]);
+        if (rc != DOCK_OK) return rc;
+        const GridPlan &pl = plans[s];
+        GridSysArgs &S = sys[s];
+        S.nx = pl.dims[0]; S.ny = pl.dims[1]; S.nz = pl.dims[2];
+        S.ox = pl.origin[0]; S.oy = pl.origin[1]; S.oz = pl.origin[2];
+        S.h = boxes[s].spacing;
+        for (int c = 0; c < 3; ++c) S.clo[c] = pl.clo[c];
+        S.inv_cell = pl.inv_cell;
+        S.ncx = pl.nc[0]; S.ncy = pl.nc[1]; S.ncz = pl.nc[2];
+        S.atoms_off = (int)n_atoms;
+        S.cells_off = (int)n_cells;
+        S.block_begin = (int)n_blocks;
+        S.pad_ = 0;
+        S.out = nullptr; S.packed = nullptr;
+        n_atoms += pl.atoms.size();
+        n_cells += pl.cell_start.size();
+        n_blocks += (long long)((S.nx + 7) / 8) * ((S.ny + 7) / 8) * ((S.nz + 1) / 2);
+        if (n_atoms > 0x7fffffffull || n_cells > 0x7fffffffull || n_blocks > 0x7fffffffLL) return DOCK_EINVAL;
+    }
+    const GridPlan &p0 = plans[0];                                      // the pair table depends on params and types only
+    const size_t b_atoms = align_up(n_atoms * sizeof(float4), 256);
+    const size_t b_cells = align_up(n_cells * sizeof(int), 256);
+    const size_t b_tab = align_up(p0.pair_tab.size() * sizeof(float4), 256);
+    const size_t b_sys = align_up((size_t)n_systems * sizeof(GridSysArgs), 256);
+    const size_t need = b_atoms + b_cells + b_tab + b_sys;
     if (needed) *needed = need;
     if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
-    if (!grid_dev || !out_desc || ((uintptr_t)grid_dev & 255)) return DOCK_EINVAL;
+    if (!grid_dev || !grid_bytes || !out_descs) return DOCK_EINVAL;
+    const int channels = params->grad_mode == 1 ? 4 : 1;
+    for (int s = 0; s < n_systems; ++s) {
+        if (!grid_dev[s] || ((uintptr_t)grid_dev[s] & 255)) return DOCK_EINVAL;
+        if (grid_bytes[s] < dock_grid_bytes(params, &boxes[s], n_lig_types)) return DOCK_EINVAL;   // buffer too small for the maps
+        const size_t nodes = (size_t)sys[s].nx * sys[s].ny * sys[s].nz * (size_t)n_lig_types * channels;
+        sys[s].out = grid_dev[s];
+        sys[s].packed = reinterpret_cast<Cell8 *>(reinterpret_cast<unsigned char *>(grid_dev[s]) + align_up(nodes * sizeof(float), 256));
+    }
+    // one host image, one copy
+    std::vector<unsigned char> image(need, 0);
+    for (int s = 0; s < n_systems; ++s) {
+        std::memcpy(image.data() + (size_t)sys[s].atoms_off * sizeof(float4), plans[s].atoms.data(), plans[s].atoms.size() * sizeof(float4));
+        std::memcpy(image.data() + b_atoms + (size_t)sys[s].cells_off * sizeof(int), plans[s].cell_start.data(), plans[s].cell_start.size() * sizeof(int));
+    }
+    std::memcpy(image.data() + b_atoms + b_cells, p0.pair_tab.data(), p0.pair_tab.size() * sizeof(float4));
+    std::memcpy(image.data() + b_atoms + b_cells + b_tab, sys.data(), (size_t)n_systems * sizeof(GridSysArgs));
     cudaStream_t stream = (cudaStream_t)stream_;
     unsigned char *ws = (unsigned char *)ws_dev;
-    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, pl.atoms.data(), pl.atoms.size() * sizeof(float4), cudaMemcpyHostToDevice, stream));
-    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws + b_atoms, pl.cell_start.data(), pl.cell_start.size() * sizeof(int), cudaMemcpyHostToDevice, stream));
-    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws + b_atoms + b_cells, pl.pair_tab.data(), pl.pair_tab.size() * sizeof(float4), cudaMemcpyHostToDevice, stream));
+    DOCK_CUDA_CHECK(cudaMemcpyAsync(ws, image.data(), need, cudaMemcpyHostToDevice, stream));
 
     GridBuildArgs A;
-    A.nx = pl.dims[0]; A.ny = pl.dims[1]; A.nz = pl.dims[2];
-    A.ox = pl.origin[0]; A.oy = pl.origin[1]; A.oz = pl.origin[2];
-    A.h = box->spacing;
     A.cutoff = params->cutoff;
     A.cutoff2 = params->cutoff * params->cutoff;
-    for (int c = 0; c < 3; ++c) A.clo[c] = pl.clo[c];
-    A.inv_cell = pl.inv_cell;
-    A.ncx = pl.nc[0]; A.ncy = pl.nc[1]; A.ncz = pl.nc[2];
     A.n_maps = n_lig_types;
     A.n_types = params->n_types;
     for (int i = 0; i < 5; ++i) A.w[i] = params->w[i];
     A.atoms = (const float4 *)ws;
     A.cell_start = (const int *)(ws + b_atoms);
     A.pair_tab = (const float4 *)(ws + b_atoms + b_cells);
-    A.out = grid_dev;
-    A.channels = params->grad_mode == 1 ? 4 : 1;
-    for (int k = 0; k < DOCK_MAX_XS_TYPES; ++k) A.map_of[k] = k < n_lig_types ? pl.map_of[k] : 0;
-    A.fresh = pl.fresh;
-    const int tbx = (A.nx + 7) / 8, tby = (A.ny + 7) / 8, tbz = (A.nz + 1) / 2;
-    dim3 grid((unsigned)(tbx * tby * tbz), (unsigned)((n_lig_types + MAPS_PER_PASS - 1) / MAPS_PER_PASS));
-    if (A.channels == 4) grid_build_kernel<true><<<grid, 128, 0, stream>>>(A);
+    A.channels = channels;
+    for (int k = 0; k < DOCK_MAX_XS_TYPES; ++k) A.map_of[k] = k < n_lig_types ? p0.map_of[k] : 0;
+    A.fresh = p0.fresh;
+    A.sys = (const GridSysArgs *)(ws + b_atoms + b_cells + b_tab);
+    A.n_sys = n_systems;
+    dim3 grid((unsigned)n_blocks, (unsigned)((n_lig_types + MAPS_PER_PASS - 1) / MAPS_PER_PASS));
+    if (channels == 4) grid_build_kernel<true><<<grid, 128, 0, stream>>>(A);
     else grid_build_kernel<false><<<grid, 128, 0, stream>>>(A);
     DOCK_LAUNCH_CHECK();
-    const size_t nodes = (size_t)A.nx * A.ny * A.nz * (size_t)n_lig_types * A.channels;
-    Cell8 *packed = reinterpret_cast<Cell8 *>(reinterpret_cast<unsigned char *>(grid_dev) + align_up(nodes * sizeof(float), 256));
-    const long long rows = (long long)n_lig_types * A.channels * A.nz * A.ny;
-    const unsigned pack_blocks = (unsigned)std::min<long long>((rows * A.nx + 255) / 256, 148LL * 16);
-    grid_pack_kernel<<<pack_blocks, 256, 0, stream>>>(grid_dev, packed, A.nx, A.ny, A.nz, rows);
+    const unsigned pack_x = (unsigned)std::max(1, std::min(148 * 16, 148 * 16 * 4 / n_systems + 1));
+    grid_pack_kernel<<<dim3(pack_x, (unsigned)n_systems), 256, 0, stream>>>(A.sys, n_lig_types * channels);
     DOCK_LAUNCH_CHECK();
 
-    std::memset(out_desc, 0, sizeof(*out_desc));
-    for (int c = 0; c < 3; ++c) { out_desc->dims[c] = pl.dims[c]; out_desc->origin[c] = pl.origin[c]; }
-    out_desc->spacing = box->spacing;
-    out_desc->n_maps = n_lig_types;
-    for (int t = 0; t < DOCK_MAX_XS_TYPES; ++t) out_desc->type_to_map[t] = -1;
-    for (int m = 0; m < n_lig_types; ++m) out_desc->type_to_map[lig_types[m]] = m;
-    out_desc->data_dev = grid_dev;
-    out_desc->packed_dev = reinterpret_cast<const float *>(packed);
-    out_desc->n_channels = A.channels;
+    for (int s = 0; s < n_systems; ++s) {
+        dock_grid *d = &out_descs[s];
+        std::memset(d, 0, sizeof(*d));
+        for (int c = 0; c < 3; ++c) { d->dims[c] = plans[s].dims[c]; d->origin[c] = plans[s].origin[c]; }
+        d->spacing = boxes[s].spacing;
+        d->n_maps = n_lig_types;
+        for (int t = 0; t < DOCK_MAX_XS_TYPES; ++t) d->type_to_map[t] = -1;
+        for (int m = 0; m < n_lig_types; ++m) d->type_to_map[lig_types[m]] = m;
+        d->data_dev = grid_dev[s];
+        d->packed_dev = reinterpret_cast<const float *>(sys[s].packed);
+        d->n_channels = channels;
+    }
     return DOCK_OK;
 }
 
-// Batched form (BASELINE.json configs[3]): n_systems independent (protein, box) pairs with the same
-// ligand-type list, enqueued back to back on one stream.  The systems share one workspace: uploads and kernels of
-// consecutive systems are ordered by the stream.
-extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_systems, const dock_protein *proteins,
-                                      const dock_box *boxes, int32_t n_lig_types, const int32_t *lig_types,
-                                      float *const *grid_dev, dock_grid *out_descs,
-                                      void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+extern "C" int dock_build_grids(const dock_params *params, const dock_protein *protein, const dock_box *box,
+                                int32_t n_lig_types, const int32_t *lig_types,
+                                float *grid_dev, size_t grid_bytes, dock_grid *out_desc,
+                                void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
 {
-    if (n_systems < 0 || (n_systems > 0 && (!proteins || !boxes))) return DOCK_EINVAL;
-    size_t need = 0;
-    for (int s = 0; s < n_systems; ++s) {
-        size_t n1 = 0;
-        const int rc = dock_build_grids(params, &proteins[s], &boxes[s], n_lig_types, lig_types, nullptr, nullptr, nullptr, 0,
-                                        &n1, nullptr);
-        if (rc != DOCK_EWORKSPACE) return rc == DOCK_OK ? DOCK_EINVAL : rc;
-        need = std::max(need, n1);
-    }
-    if (needed) *needed = need;
-    if (n_systems == 0) return DOCK_OK;
-    if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
-    if (!grid_dev || !out_descs) return DOCK_EINVAL;
-    for (int s = 0; s < n_systems; ++s) {
-        const int rc = dock_build_grids(params, &proteins[s], &boxes[s], n_lig_types, lig_types, grid_dev[s], &out_descs[s],
-                                        ws_dev, ws_bytes, nullptr, stream_);
-        if (rc != DOCK_OK) return rc;
-    }
-    return DOCK_OK;
+    if (!protein || !box) return DOCK_EINVAL;
+    float *const gd[1] = {grid_dev};
+    const size_t gb[1] = {grid_bytes};
+    return dock_build_grids_batch(params, 1, protein, box, n_lig_types, lig_types, grid_dev ? gd : nullptr, gb, out_desc,
+                                  ws_dev, ws_bytes, needed, stream_);
 }

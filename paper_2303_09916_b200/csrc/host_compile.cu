@@ -5,12 +5,12 @@
 #include <cmath>
 #include <cstring>
 
-int g_dock_last_cuda_error = 0;
-unsigned long long g_dock_launches = 0;
+std::atomic<int> g_dock_last_cuda_error{0};
+std::atomic<unsigned long long> g_dock_launches{0};
 
-extern "C" int dock_last_cuda_error(void) { return g_dock_last_cuda_error; }
-extern "C" const char *dock_version(void) { return "dock_b200 0.1 (sm_100a)"; }
-extern "C" uint64_t dock_launch_count(void) { return (uint64_t)g_dock_launches; }
+extern "C" int dock_last_cuda_error(void) { return g_dock_last_cuda_error.load(); }
+extern "C" const char *dock_version(void) { return "dock_b200 0.2 (sm_100a)"; }
+extern "C" uint64_t dock_launch_count(void) { return (uint64_t)g_dock_launches.load(); }
 
 // Readings S1 (weights), S2 (XS radii / flags), S3, S7, S12, S14, S15, S19 of SURVEY.md 8(c): the paper
 // prints none of these ("the same scoring function" as Vina).

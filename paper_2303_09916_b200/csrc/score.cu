@@ -3,6 +3,7 @@
 // (eval_thread.cuh).  The threads never cooperate; the CTA size (1..8 warps) is chosen on the host as
 // the one that packs most warps into an SM's shared memory (each CTA also costs 1 KB of reserved smem).
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
@@ -93,6 +94,42 @@ int score_launch(ScorePlan &pl, long long n_poses, const float *poses_dev, float
                     : launch<false, true>(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, stream);
 }
 
+// Copy streams and events of dock_score_batch_host: the only resources the library owns.  One context per device,
+// created on first use under a mutex and published only when every create call has succeeded; the pipeline itself runs
+// under the context's mutex, so concurrent host threads serialise per device.
+constexpr int MAX_CHUNKS = 8;
+constexpr int MAX_DEVICES = 64;
+struct HostPipe {
+    std::mutex mu;
+    bool ready = false;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_in[MAX_CHUNKS], ev_k[MAX_CHUNKS], ev_begin, ev_end;
+};
+HostPipe g_pipes[MAX_DEVICES];
+
+int pipe_init(HostPipe &hp)
+{
+    if (hp.ready) return DOCK_OK;
+    cudaStream_t a = nullptr, b = nullptr;
+    cudaEvent_t ev[2 * MAX_CHUNKS + 2];
+    int made = 0;
+    cudaError_t e = cudaStreamCreateWithFlags(&a, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&b, cudaStreamNonBlocking);
+    for (; e == cudaSuccess && made < 2 * MAX_CHUNKS + 2; ++made) e = cudaEventCreateWithFlags(&ev[made], cudaEventDisableTiming);
+    if (e != cudaSuccess) {                                  // roll back: nothing half-initialised is ever published
+        for (int k = 0; k < made - 1; ++k) cudaEventDestroy(ev[k]);
+        if (a) cudaStreamDestroy(a);
+        if (b) cudaStreamDestroy(b);
+        g_dock_last_cuda_error.store((int)e);
+        return DOCK_ECUDA;
+    }
+    hp.s_in = a; hp.s_out = b;
+    for (int c = 0; c < MAX_CHUNKS; ++c) { hp.ev_in[c] = ev[2 * c]; hp.ev_k[c] = ev[2 * c + 1]; }
+    hp.ev_begin = ev[2 * MAX_CHUNKS]; hp.ev_end = ev[2 * MAX_CHUNKS + 1];
+    hp.ready = true;
+    return DOCK_OK;
+}
+
 }  // namespace
 
 extern "C" int dock_score_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
@@ -137,42 +174,47 @@ extern "C" int dock_score_batch_host(const dock_params *params, const dock_grid 
     float *d_t = terms_host ? (float *)(ws + b_blob + b_pose + b_e + b_g) : nullptr;
     // Three-stage pipeline over chunks of the batch: host->device copies on one side stream, kernels on the
     // caller's stream, device->host copies on another side stream, so that PCIe in, compute and PCIe out
-    // overlap (the buses are full duplex).  The side streams and events belong to the library and are created once.
-    static cudaStream_t s_in = nullptr, s_out = nullptr;
-    constexpr int MAX_CHUNKS = 8;
-    static cudaEvent_t ev_in[MAX_CHUNKS], ev_k[MAX_CHUNKS], ev_begin, ev_end;
-    if (!s_in) {
-        DOCK_CUDA_CHECK(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
-        DOCK_CUDA_CHECK(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
-        for (int c = 0; c < MAX_CHUNKS; ++c) {
-            DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming));
-            DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_k[c], cudaEventDisableTiming));
-        }
-        DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_begin, cudaEventDisableTiming));
-        DOCK_CUDA_CHECK(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
-    }
+    // overlap (the buses are full duplex).  The side streams and events belong to the library (one set per device).
+    int dev = 0;
+    DOCK_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return DOCK_EINVAL;
+    HostPipe &hp = g_pipes[dev];
+    std::lock_guard<std::mutex> lock(hp.mu);
+    if (pipe_init(hp) != DOCK_OK) return DOCK_ECUDA;
     const int n_chunks = (int)std::min<int64_t>(MAX_CHUNKS, (n_poses + 65535) / 65536);      // >= 64 Ki poses per chunk
     const int64_t per = ((n_poses + n_chunks - 1) / n_chunks + 31) / 32 * 32;
-    DOCK_CUDA_CHECK(cudaEventRecord(ev_begin, stream));                  // the workspace may still be in use upstream
-    DOCK_CUDA_CHECK(cudaStreamWaitEvent(s_in, ev_begin, 0));
-    DOCK_CUDA_CHECK(cudaStreamWaitEvent(s_out, ev_begin, 0));
-    for (int c = 0; c < n_chunks; ++c) {
-        const int64_t o = c * per, m = std::min<int64_t>(per, n_poses - o);
-        if (m <= 0) break;
-        DOCK_CUDA_CHECK(cudaMemcpyAsync(d_pose + o * np_, poses_host + o * np_, (size_t)m * np_ * sizeof(float), cudaMemcpyHostToDevice, s_in));
-        DOCK_CUDA_CHECK(cudaEventRecord(ev_in[c], s_in));
-        DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, ev_in[c], 0));
-        const int rc2 = score_launch(pl, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr, d_t ? d_t + o * 3 : nullptr,
-                                     ws, stream, c == 0);
-        if (rc2 != DOCK_OK) return rc2;
-        DOCK_CUDA_CHECK(cudaEventRecord(ev_k[c], stream));
-        DOCK_CUDA_CHECK(cudaStreamWaitEvent(s_out, ev_k[c], 0));
-        DOCK_CUDA_CHECK(cudaMemcpyAsync(energy_host + o, d_e + o, (size_t)m * sizeof(float), cudaMemcpyDeviceToHost, s_out));
-        if (grad_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(grad_host + o * ng, d_g + o * ng, (size_t)m * ng * sizeof(float), cudaMemcpyDeviceToHost, s_out));
-        if (terms_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(terms_host + o * 3, d_t + o * 3, (size_t)m * 3 * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+    // on any failure the copies already enqueued are drained before returning: the caller's host buffers must not be
+    // written after the call has come back
+    auto pipeline = [&]() -> int {
+        DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_begin, stream));              // the workspace may still be in use upstream
+        DOCK_CUDA_CHECK(cudaStreamWaitEvent(hp.s_in, hp.ev_begin, 0));
+        DOCK_CUDA_CHECK(cudaStreamWaitEvent(hp.s_out, hp.ev_begin, 0));
+        for (int c = 0; c < n_chunks; ++c) {
+            const int64_t o = c * per, m = std::min<int64_t>(per, n_poses - o);
+            if (m <= 0) break;
+            DOCK_CUDA_CHECK(cudaMemcpyAsync(d_pose + o * np_, poses_host + o * np_, (size_t)m * np_ * sizeof(float), cudaMemcpyHostToDevice, hp.s_in));
+            DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_in[c], hp.s_in));
+            DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, hp.ev_in[c], 0));
+            const int rc2 = score_launch(pl, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr, d_t ? d_t + o * 3 : nullptr,
+                                         ws, stream, c == 0);
+            if (rc2 != DOCK_OK) return rc2;
+            DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_k[c], stream));
+            DOCK_CUDA_CHECK(cudaStreamWaitEvent(hp.s_out, hp.ev_k[c], 0));
+            DOCK_CUDA_CHECK(cudaMemcpyAsync(energy_host + o, d_e + o, (size_t)m * sizeof(float), cudaMemcpyDeviceToHost, hp.s_out));
+            if (grad_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(grad_host + o * ng, d_g + o * ng, (size_t)m * ng * sizeof(float), cudaMemcpyDeviceToHost, hp.s_out));
+            if (terms_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(terms_host + o * 3, d_t + o * 3, (size_t)m * 3 * sizeof(float), cudaMemcpyDeviceToHost, hp.s_out));
+        }
+        DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_end, hp.s_out));
+        DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, hp.ev_end, 0));
+        return DOCK_OK;
+    };
+    const int rc3 = pipeline();
+    if (rc3 != DOCK_OK) {
+        cudaStreamSynchronize(hp.s_in);
+        cudaStreamSynchronize(stream);
+        cudaStreamSynchronize(hp.s_out);
+        return rc3;
     }
-    DOCK_CUDA_CHECK(cudaEventRecord(ev_end, s_out));
-    DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, ev_end, 0));
     DOCK_CUDA_CHECK(cudaStreamSynchronize(stream));
     return DOCK_OK;
 }

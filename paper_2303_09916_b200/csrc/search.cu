@@ -98,12 +98,18 @@ __device__ __forceinline__ void set_identity(float *H, int n, float diag)
 // Written as one loop around a SINGLE evaluation site (the start pose is "trial" INIT), so that the evaluator and
 // this routine inline into the kernels once: the compiler then sees that every buffer is shared memory and keeps
 // P, G, L in registers / the constant bank instead of local memory (profiles/r1g.md).
-template <bool EQ4, bool VEC4>
+// TRACE: one record per iteration started goes to `itrace` (layout: dock.h, DOCK_ITER_HEADER) -- the state the
+// iteration starts from (pose, inverse Hessian) and its decision scalars, enough for the oracle to redo that one
+// iteration from the same state (iteration-level teacher-forced parity).
+template <bool EQ4, bool VEC4, bool TRACE = false>
 __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGrid &G, const DevLigand &L,
-                                                const OptBuf &b, int cap, int &iters, int &evals)
+                                                const OptBuf &b, int cap, int &iters, int &evals, int &why,
+                                                float *itrace = nullptr, int itrace_cap = 0)
 {
     const int lane = threadIdx.x & 31;
     const int T = L.T, n = 6 + T, np_ = 7 + T;
+    const int istride = DOCK_ITER_HEADER + np_ + n + n * n;
+    why = DOCK_EXIT_CAP;
     if (lane == 0) {
         const float w = b.x[3], x = b.x[4], y = b.x[5], z = b.x[6];
         const float n2 = w * w + x * x + y * y + z * z;
@@ -145,6 +151,7 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
                 for (int k = lane; k < np_; k += 32) x_best[k] = b.xt[k];
             }
             __syncwarp();
+            if (TRACE && it < itrace_cap && lane == 0) itrace[(size_t)it * istride + 5] = ft;
             ++it;
         } else if ((double)ft - (double)f <= (double)P.c1 * (double)alpha * gp) {   // Armijo: accept the step
             double ys = 0.0, yy = 0.0, ss = 0.0;
@@ -159,7 +166,8 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
             for (int r = lane; r < n; r += 32) b.g[r] = b.gt[r];
             f = ft;
             __syncwarp();
-            if (ys > (double)P.curv_eps * sqrt(ss) * sqrt(yy)) {
+            const bool upd = ys > (double)P.curv_eps * sqrt(ss) * sqrt(yy);
+            if (upd) {
                 if (fresh) { set_identity(b.H, n, (float)(ys / yy)); fresh = false; }
                 for (int r = lane; r < n; r += 32) {
                     float a = 0.0f;
@@ -182,10 +190,21 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
                 }
                 __syncwarp();
             }
+            if (TRACE && it < itrace_cap && lane == 0) {
+                float *rec = itrace + (size_t)it * istride;
+                rec[4] = alpha; rec[5] = f; rec[7] = (float)(trial + 1); rec[8] = upd ? 1.f : 0.f; rec[11] = fresh ? 1.f : 0.f;
+            }
             ++it;
         } else {                                   // backtrack
+            if (++trial >= P.max_trials) {         // no acceptable trial: stop
+                why = DOCK_EXIT_LINESEARCH;
+                if (TRACE && it < itrace_cap && lane == 0) {
+                    float *rec = itrace + (size_t)it * istride;
+                    rec[4] = alpha; rec[5] = ft; rec[6] = (float)DOCK_EXIT_LINESEARCH; rec[7] = (float)trial; rec[11] = fresh ? 1.f : 0.f;
+                }
+                break;
+            }
             alpha *= P.shrink;
-            if (++trial >= P.max_trials) break;    // no acceptable trial: stop
             pose_add_warp(T, b.x, b.d, alpha, b.xt);
             continue;
         }
@@ -194,10 +213,31 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
         double acc = 0.0;
         for (int r = lane; r < n; r += 32) acc += (double)b.g[r] * (double)b.g[r];
         const double gn2 = warp_sum_d(acc);
-        if (sqrt(gn2) < (double)P.gtol) break;
+        if (TRACE && it < itrace_cap) {            // the state this iteration starts from
+            float *rec = itrace + (size_t)it * istride;
+            if (lane == 0) {
+                rec[0] = f; rec[1] = (float)sqrt(gn2); rec[2] = rec[3] = rec[4] = rec[5] = 0.f;
+                rec[6] = 0.f; rec[7] = 0.f; rec[8] = 0.f; rec[9] = 0.f; rec[10] = fresh ? 1.f : 0.f; rec[11] = fresh ? 1.f : 0.f;
+            }
+            for (int k = lane; k < np_; k += 32) rec[DOCK_ITER_HEADER + k] = b.x[k];
+            for (int k = lane; k < n; k += 32) rec[DOCK_ITER_HEADER + np_ + k] = b.g[k];
+            if (bb)                                // Barzilai-Borwein: the previous step (s, y) takes the place of H
+                for (int k = lane; k < n; k += 32) {
+                    rec[DOCK_ITER_HEADER + np_ + n + k] = it > 0 ? b.d[k] : 0.f;
+                    rec[DOCK_ITER_HEADER + np_ + 2 * n + k] = it > 0 ? b.y[k] : 0.f;
+                }
+            else
+                for (int k = lane; k < n * n; k += 32) rec[DOCK_ITER_HEADER + np_ + n + k] = b.H[k];
+        }
+        if (sqrt(gn2) < (double)P.gtol) {
+            why = DOCK_EXIT_GTOL;
+            if (TRACE && it < itrace_cap && lane == 0) itrace[(size_t)it * istride + 6] = (float)DOCK_EXIT_GTOL;
+            break;
+        }
         if (bb) {
             const double gnorm = sqrt(gn2);
             double al;
+            int branch = 0;
             if (it == 0) al = (double)P.bb_step / gnorm;
             else {
                 double sy = 0.0, ss = 0.0, yy = 0.0;
@@ -206,10 +246,16 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
                     sy += sv * yv; ss += sv * sv; yy += yv * yv;
                 }
                 sy = warp_sum_d(sy); ss = warp_sum_d(ss); yy = warp_sum_d(yy);
-                al = (sy > (double)P.curv_eps * sqrt(ss) * sqrt(yy)) ? ss / sy : (double)P.bb_fallback / gnorm;
+                branch = (sy > (double)P.curv_eps * sqrt(ss) * sqrt(yy)) ? 1 : 2;
+                al = branch == 1 ? ss / sy : (double)P.bb_fallback / gnorm;
             }
-            if (al * gnorm > (double)P.bb_step) al = (double)P.bb_step / gnorm;
+            const bool capped = al * gnorm > (double)P.bb_step;
+            if (capped) al = (double)P.bb_step / gnorm;
             alpha = (float)al;
+            if (TRACE && it < itrace_cap && lane == 0) {
+                float *rec = itrace + (size_t)it * istride;
+                rec[4] = alpha; rec[7] = (float)branch; rec[9] = capped ? 1.f : 0.f;
+            }
             __syncwarp();
             for (int r = lane; r < n; r += 32) b.d[r] = -b.g[r];
             __syncwarp();
@@ -231,6 +277,7 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
             for (int r = lane; r < n; r += 32) b.d[r] = -b.g[r];
             __syncwarp();
             gp = -gn2;
+            if (TRACE && it < itrace_cap && lane == 0) itrace[(size_t)it * istride + 9] = 1.f;
         }
         alpha = 1.0f;
         if (fresh) {
@@ -238,6 +285,10 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
             for (int r = lane; r < n; r += 32) acc += (double)b.d[r] * (double)b.d[r];
             const double dn = sqrt(warp_sum_d(acc));
             if (dn > 1.0) alpha = (float)(1.0 / dn);
+        }
+        if (TRACE && it < itrace_cap && lane == 0) {
+            float *rec = itrace + (size_t)it * istride;
+            rec[2] = (float)gp; rec[3] = alpha;
         }
         trial = 0;
         pose_add_warp(T, b.x, b.d, alpha, b.xt);
@@ -253,11 +304,11 @@ __device__ __forceinline__ float local_opt_warp(const DevParams &P, const DevGri
 }
 
 // ---- local optimisation of a batch of poses (level-2 parity entry point) -------------------------
-template <bool EQ4, bool VEC4>
+template <bool EQ4, bool VEC4, bool TRACE>
 __global__ void __launch_bounds__(SEARCH_WARPS * 32)
 local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap, int warp_floats,
                  const float *__restrict__ poses, float *__restrict__ out_pose, float *__restrict__ out_e,
-                 int *__restrict__ out_iters)
+                 int *__restrict__ out_iters, float *__restrict__ itrace, int itrace_cap)
 {
     extern __shared__ float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -267,12 +318,14 @@ local_opt_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap
     const OptBuf b = carve(smem + (size_t)warp * warp_floats, L.T, L.n_pad);
     for (int k = lane; k < np_; k += 32) b.x[k] = poses[p * np_ + k];
     __syncwarp();
-    int iters, evals;
-    const float e = local_opt_warp<EQ4, VEC4>(P, G, L, b, cap, iters, evals);
+    int iters, evals, why;
+    const size_t istride = DOCK_ITER_HEADER + np_ + (size_t)(6 + L.T) * (7 + L.T);
+    const float e = local_opt_warp<EQ4, VEC4, TRACE>(P, G, L, b, cap, iters, evals, why,
+                                                     TRACE ? itrace + (size_t)p * itrace_cap * istride : nullptr, itrace_cap);
     for (int k = lane; k < np_; k += 32) out_pose[p * np_ + k] = b.x[k];
     if (lane == 0) {
         out_e[p] = e;
-        if (out_iters) { out_iters[2 * p] = iters; out_iters[2 * p + 1] = evals; }
+        if (out_iters) { out_iters[3 * p] = iters; out_iters[3 * p + 1] = evals; out_iters[3 * p + 2] = why; }
     }
 }
 
@@ -284,7 +337,7 @@ __device__ __forceinline__ float u24(uint32_t r) { return (float)(r >> 8) * (1.0
 template <bool EQ4, bool VEC4>
 __global__ void __launch_bounds__(SEARCH_WARPS * 32, 4)
 search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems, int copies, int steps,
-              int cap, uint32_t seed_lo, uint32_t seed_hi, int t_max, int warp_floats,
+              int cap, uint32_t seed_lo, uint32_t seed_hi, uint32_t sys_base, uint32_t copy_base, int t_max, int warp_floats,
               const float *__restrict__ init, float *__restrict__ best_pose, float *__restrict__ best_e,
               float *__restrict__ trace, unsigned long long *__restrict__ eval_counter)
 {
@@ -292,7 +345,8 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const long long gw = (long long)blockIdx.x * SEARCH_WARPS + warp;
     if (gw >= (long long)n_systems * copies) return;
-    const uint32_t sys = (uint32_t)(gw / copies), copy = (uint32_t)(gw % copies);
+    const uint32_t sys = (uint32_t)(gw / copies);
+    const uint32_t copy = copy_base + (uint32_t)(gw % copies), psys = sys_base + sys;   // Philox counter words (R-rules)
     const DevGrid G = systems[sys].grid;
     const DevLigand L = systems[sys].lig;
     const int T = L.T, np_ = 7 + T, row = 7 + t_max;
@@ -300,7 +354,7 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
     float *cur = base, *best = base + pad4(row);
     const OptBuf b = carve(base + 2 * pad4(row), T, L.n_pad);
 
-    int iters, evals;
+    int iters, evals, why;
     unsigned long long total_evals = 0;
     float e_cur = 0.0f, e_best = 0.0f;
     // step -1 = local optimisation of the initial pose (reading S16); one call site of the optimizer
@@ -311,7 +365,7 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
             for (int k = lane; k < np_; k += 32) b.x[k] = init[gw * row + k];
             __syncwarp();
         } else {
-            philox4x32_10(copy, (uint32_t)step, 0u, sys, seed_lo, seed_hi, r);
+            philox4x32_10(copy, (uint32_t)step, 0u, psys, seed_lo, seed_hi, r);
             const uint32_t K = T > 0 ? 3u : 2u;
             kind = (int)__umulhi(r[0], K);
             for (int k = lane; k < np_; k += 32) b.x[k] = cur[k];
@@ -329,7 +383,7 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
             }
             __syncwarp();
         }
-        const float e_c = local_opt_warp<EQ4, VEC4>(P, G, L, b, cap, iters, evals);
+        const float e_c = local_opt_warp<EQ4, VEC4>(P, G, L, b, cap, iters, evals, why);
         total_evals += evals;
         if (step < 0) {
             e_cur = e_best = e_c;
@@ -338,7 +392,7 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
             continue;
         }
         uint32_t ra[4];
-        philox4x32_10(copy, (uint32_t)step, 1u, sys, seed_lo, seed_hi, ra);
+        philox4x32_10(copy, (uint32_t)step, 1u, psys, seed_lo, seed_hi, ra);
         const float u = u24(ra[0]);
         const bool accept = (e_c < e_cur) || ((double)u < exp(((double)e_cur - (double)e_c) / (double)P.t_mc));
         if (trace) {
@@ -448,9 +502,8 @@ topk_kernel(const DevSystem *__restrict__ systems, int n, int n_pow2, int row, i
     if (lane == 0) out_count[sys] = n_kept;
 }
 
-int launch_topk(const DevSystem *systems_dev, int n_systems, const DevLigand *ligs_host, int n, int row, int k,
-                float rmsd_min, const float *poses, const float *e, int *out_idx, int *out_count,
-                float *out_pose, float *out_e, cudaStream_t stream)
+// dynamic shared memory of topk_kernel; the callers check it against the 200 KB limit BEFORE they enqueue anything
+size_t topk_smem_bytes(int n_systems, const DevLigand *ligs_host, int n, int row, int k, int *n_pow2_out)
 {
     int n_pow2 = 1;
     while (n_pow2 < n) n_pow2 <<= 1;
@@ -459,7 +512,16 @@ int launch_topk(const DevSystem *systems_dev, int n_systems, const DevLigand *li
         np_max = ligs_host[s].n_pad > np_max ? ligs_host[s].n_pad : np_max;
         t_max = ligs_host[s].T > t_max ? ligs_host[s].T : t_max;
     }
-    const size_t smem = sizeof(float) * ((size_t)2 * n_pow2 + (size_t)(k + 1) * 3 * np_max + 2 * pad4(t_max) + pad4(row) + 8);
+    if (n_pow2_out) *n_pow2_out = n_pow2;
+    return sizeof(float) * ((size_t)2 * n_pow2 + (size_t)(k + 1) * 3 * np_max + 2 * pad4(t_max) + pad4(row) + 8);
+}
+
+int launch_topk(const DevSystem *systems_dev, int n_systems, const DevLigand *ligs_host, int n, int row, int k,
+                float rmsd_min, const float *poses, const float *e, int *out_idx, int *out_count,
+                float *out_pose, float *out_e, cudaStream_t stream)
+{
+    int n_pow2 = 1;
+    const size_t smem = topk_smem_bytes(n_systems, ligs_host, n, row, k, &n_pow2);
     if (smem > 200 * 1024) return DOCK_EINVAL;
     if (smem > 48 * 1024)
         DOCK_CUDA_CHECK(cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -491,32 +553,33 @@ void host_init_pose(const dock_box *box, int T, uint64_t seed, uint32_t system, 
 
 }  // namespace
 
-extern "C" int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
-                               float *out_host)
+extern "C" int dock_init_poses(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, uint32_t copy_base,
+                               int32_t copies, float *out_host)
 {
     if (!box || !out_host || T < 0 || T > DOCK_MAX_TORSIONS || copies < 0) return DOCK_EINVAL;
-    for (int c = 0; c < copies; ++c) host_init_pose(box, T, seed, system, (uint32_t)c, out_host + (size_t)c * (7 + T));
+    for (int c = 0; c < copies; ++c) host_init_pose(box, T, seed, system, copy_base + (uint32_t)c, out_host + (size_t)c * (7 + T));
     return DOCK_OK;
 }
 
 // NEXT-3 (Fig. 3; reading S22): translation restrained to box (intersected with) the union of balls of
 // `radius` around the predicted site points, by rejection from the Philox slots 0x100 + attempt (256 attempts,
 // then the site point copy mod n_site); orientation and torsions as in dock_init_poses.
-extern "C" int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, int32_t copies,
-                                    int32_t n_site, const float *site_xyz_host, float radius, float *out_host)
+extern "C" int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t system, uint32_t copy_base,
+                                    int32_t copies, int32_t n_site, const float *site_xyz_host, float radius, float *out_host)
 {
     if (!box || !out_host || T < 0 || T > DOCK_MAX_TORSIONS || copies < 0) return DOCK_EINVAL;
     if (n_site < 1 || !site_xyz_host || !(radius > 0.f)) return DOCK_EINVAL;
     const uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
     const double r2max = (double)radius * (double)radius;
-    for (int c = 0; c < copies; ++c) {
-        float *out = out_host + (size_t)c * (7 + T);
-        host_init_pose(box, T, seed, system, (uint32_t)c, out);
+    for (int ci = 0; ci < copies; ++ci) {
+        const uint32_t c = copy_base + (uint32_t)ci;
+        float *out = out_host + (size_t)ci * (7 + T);
+        host_init_pose(box, T, seed, system, c, out);
         double t[3] = {0, 0, 0};
         bool found = false;
         for (int a = 0; a < 256 && !found; ++a) {
             uint32_t r[4];
-            philox4x32_10((uint32_t)c, 0xffffffffu, 0x100u + (uint32_t)a, system, k0, k1, r);
+            philox4x32_10(c, 0xffffffffu, 0x100u + (uint32_t)a, system, k0, k1, r);
             for (int d = 0; d < 3; ++d)
                 t[d] = (double)box->center[d] - 0.5 * (double)box->size[d] + (double)(r[d] >> 8) * (1.0 / 16777216.0) * (double)box->size[d];
             for (int k = 0; k < n_site && !found; ++k) {
@@ -526,23 +589,25 @@ extern "C" int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t see
             }
         }
         if (!found)
-            for (int d = 0; d < 3; ++d) t[d] = (double)site_xyz_host[3 * (c % n_site) + d];
+            for (int d = 0; d < 3; ++d) t[d] = (double)site_xyz_host[3 * (c % (uint32_t)n_site) + d];
         for (int d = 0; d < 3; ++d) out[d] = (float)t[d];
     }
     return DOCK_OK;
 }
 
-extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
-                                    int64_t n_poses, int32_t max_iters, const float *poses_dev,
-                                    float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
-                                    void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+namespace {
+int local_opt_launch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                     int64_t n_poses, int32_t max_iters, const float *poses_dev,
+                     float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
+                     float *iter_trace_dev, int32_t trace_cap,
+                     void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
 {
     DevParams P;
     DevGrid G;
     LigandBlob blob;
     if (dock_make_dev_params(params, &P) != DOCK_OK || dock_make_dev_grid(params, grid, &G) != DOCK_OK) return DOCK_EINVAL;
     if (dock_compile_ligand(params, grid, ligand, blob) != DOCK_OK) return DOCK_EINVAL;
-    if (n_poses < 0 || max_iters < 0) return DOCK_EINVAL;
+    if (n_poses < 0 || max_iters < 0 || trace_cap < 0) return DOCK_EINVAL;
     if (needed) *needed = blob.bytes.size();
     if (!ws_dev || ws_bytes < blob.bytes.size()) return DOCK_EWORKSPACE;
     if (n_poses == 0) return DOCK_OK;
@@ -554,21 +619,45 @@ extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *
     const size_t smem = (size_t)SEARCH_WARPS * warp_floats * sizeof(float);
     if (smem > 200 * 1024) return DOCK_EINVAL;
     // shared-memory layout of the evaluator (eval_warp.cuh): float4 per atom unless the ligand is large
-    const bool vec4 = L.N <= 48;
-    auto kern = G.channels == 4 ? (vec4 ? local_opt_kernel<true, true> : local_opt_kernel<true, false>)
-                                : (vec4 ? local_opt_kernel<false, true> : local_opt_kernel<false, false>);
+    const bool vec4 = L.N <= 48, eq4 = G.channels == 4, tr = iter_trace_dev != nullptr;
+    auto kern = tr ? (eq4 ? (vec4 ? local_opt_kernel<true, true, true> : local_opt_kernel<true, false, true>)
+                          : (vec4 ? local_opt_kernel<false, true, true> : local_opt_kernel<false, false, true>))
+                   : (eq4 ? (vec4 ? local_opt_kernel<true, true, false> : local_opt_kernel<true, false, false>)
+                          : (vec4 ? local_opt_kernel<false, true, false> : local_opt_kernel<false, false, false>));
     if (smem > 48 * 1024)
         DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned blocks = (unsigned)((n_poses + SEARCH_WARPS - 1) / SEARCH_WARPS);
     kern<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(P, G, L, n_poses, max_iters, warp_floats, poses_dev,
-                                                     out_pose_dev, out_e_dev, out_iters_dev);
+                                                     out_pose_dev, out_e_dev, out_iters_dev, iter_trace_dev, trace_cap);
     DOCK_LAUNCH_CHECK();
     return DOCK_OK;
+}
+}  // namespace
+
+extern "C" int dock_local_opt_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                                    int64_t n_poses, int32_t max_iters, const float *poses_dev,
+                                    float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
+                                    void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+{
+    return local_opt_launch(params, grid, ligand, n_poses, max_iters, poses_dev, out_pose_dev, out_e_dev, out_iters_dev,
+                            nullptr, 0, ws_dev, ws_bytes, needed, stream_);
+}
+
+extern "C" int dock_local_opt_trace(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                                    int64_t n_poses, int32_t max_iters, const float *poses_dev,
+                                    float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
+                                    float *iter_trace_dev, int32_t trace_cap,
+                                    void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+{
+    if (!iter_trace_dev && ws_dev) return DOCK_EINVAL;
+    return local_opt_launch(params, grid, ligand, n_poses, max_iters, poses_dev, out_pose_dev, out_e_dev, out_iters_dev,
+                            iter_trace_dev, trace_cap, ws_dev, ws_bytes, needed, stream_);
 }
 
 extern "C" int dock_search(const dock_params *params, int32_t n_systems,
                            const dock_grid *grids, const dock_ligand *ligands, const dock_box *boxes,
                            int32_t copies, int32_t steps, int32_t bfgs_max_iters, uint64_t seed,
+                           uint32_t system_base, uint32_t copy_base,
                            const float *init_poses_dev,
                            float *best_pose_dev, float *best_e_dev,
                            float *topk_pose_dev, float *topk_e_dev, int32_t *topk_idx_dev, int32_t *topk_count_dev,
@@ -594,14 +683,24 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
         const int wf = 2 * pad4(row) + opt_floats(ligands[s].T, blobs[s].rel.n_pad);
         wf_max = wf > wf_max ? wf : wf_max;
     }
+    // everything that can be rejected is rejected here, before the workspace answer and before anything is enqueued
+    const bool want_topk = topk_idx_dev || topk_count_dev || topk_pose_dev || topk_e_dev;
+    if (want_topk && (!topk_idx_dev || !topk_count_dev)) return DOCK_EINVAL;
+    for (int s2 = 1; s2 < n_systems; ++s2)
+        if (sys[s2].grid.channels != sys[0].grid.channels) return DOCK_EINVAL;      // one gradient mode per launch
+    const size_t smem = (size_t)SEARCH_WARPS * wf_max * sizeof(float);
+    if (smem > 200 * 1024) return DOCK_EINVAL;
+    if (want_topk) {
+        std::vector<DevLigand> rel(n_systems);
+        for (int s2 = 0; s2 < n_systems; ++s2) rel[s2] = blobs[s2].rel;
+        if (topk_smem_bytes(n_systems, rel.data(), copies, row, params->topk, nullptr) > 200 * 1024) return DOCK_EINVAL;
+    }
     const size_t b_sys = align_up(sizeof(DevSystem) * n_systems, 256);
     const size_t b_init = init_poses_dev ? 0 : align_up((size_t)n_systems * copies * row * sizeof(float), 256);
     const size_t need = blob_bytes + b_sys + b_init;
     if (needed) *needed = need;
     if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
     if (!best_pose_dev || !best_e_dev) return DOCK_EINVAL;
-    const bool want_topk = topk_idx_dev || topk_count_dev || topk_pose_dev || topk_e_dev;
-    if (want_topk && (!topk_idx_dev || !topk_count_dev)) return DOCK_EINVAL;
 
     cudaStream_t stream = (cudaStream_t)stream_;
     unsigned char *ws = (unsigned char *)ws_dev;
@@ -627,15 +726,12 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
         std::vector<float> h((size_t)n_systems * copies * row, 0.0f);
         for (int s = 0; s < n_systems; ++s)
             for (int c = 0; c < copies; ++c)
-                host_init_pose(&boxes[s], ligands[s].T, seed, (uint32_t)s, (uint32_t)c, h.data() + ((size_t)s * copies + c) * row);
+                host_init_pose(&boxes[s], ligands[s].T, seed, system_base + (uint32_t)s, copy_base + (uint32_t)c,
+                               h.data() + ((size_t)s * copies + c) * row);
         float *d = (float *)(ws + blob_bytes + b_sys);
         DOCK_CUDA_CHECK(cudaMemcpyAsync(d, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
         init = d;
     }
-    const size_t smem = (size_t)SEARCH_WARPS * wf_max * sizeof(float);
-    if (smem > 200 * 1024) return DOCK_EINVAL;
-    for (int s2 = 1; s2 < n_systems; ++s2)
-        if (sys[s2].grid.channels != sys[0].grid.channels) return DOCK_EINVAL;      // one gradient mode per launch
     int n_max = 0;
     for (int s2 = 0; s2 < n_systems; ++s2) n_max = std::max(n_max, (int)ligands[s2].N);
     const bool vec4 = n_max <= 48;        // float4 per atom unless the ligands are large (eval_warp.cuh)
@@ -647,7 +743,7 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
     const unsigned blocks = (unsigned)((total + SEARCH_WARPS - 1) / SEARCH_WARPS);
     kern<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(
         P, sys_dev, n_systems, copies, steps, bfgs_max_iters, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
-        t_max, wf_max, init, best_pose_dev, best_e_dev, trace_dev, (unsigned long long *)eval_counter_dev);
+        system_base, copy_base, t_max, wf_max, init, best_pose_dev, best_e_dev, trace_dev, (unsigned long long *)eval_counter_dev);
     DOCK_LAUNCH_CHECK();
     if (want_topk)
         return launch_topk(sys_dev, n_systems, ligs.data(), copies, row, params->topk, params->cluster_rmsd,
@@ -684,7 +780,7 @@ extern "C" int dock_system_host(const dock_params *params, const dock_protein *p
                                 int32_t copies, int32_t steps, int32_t bfgs_max_iters, uint64_t seed,
                                 float *out_topk_pose_host, float *out_topk_e_host, int32_t *out_count_host,
                                 uint64_t *out_evals_host,
-                                float *grid_dev, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
+                                float *grid_dev, size_t grid_bytes, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream_)
 {
     if (!params || !protein || !box || !ligand || copies < 1) return DOCK_EINVAL;
     if (dock_validate_params(params) != DOCK_OK) return DOCK_EINVAL;
@@ -701,7 +797,7 @@ extern "C" int dock_system_host(const dock_params *params, const dock_protein *p
     const size_t head = b_best + b_beste + b_tp + b_te + b_ti + b_misc;
     size_t need_grid = 0, need_search = 0;
     dock_grid desc;
-    int rc = dock_build_grids(params, protein, box, n_lig_types, lig_types, nullptr, nullptr, nullptr, 0, &need_grid, nullptr);
+    int rc = dock_build_grids(params, protein, box, n_lig_types, lig_types, nullptr, 0, nullptr, nullptr, 0, &need_grid, nullptr);
     if (rc != DOCK_EWORKSPACE) return rc == DOCK_OK ? DOCK_EINVAL : rc;
     // descriptor for the size query of the search
     std::memset(&desc, 0, sizeof(desc));
@@ -714,7 +810,7 @@ extern "C" int dock_system_host(const dock_params *params, const dock_protein *p
     desc.data_dev = grid_dev ? grid_dev : (const float *)256;
     desc.packed_dev = desc.data_dev;
     float dummy;
-    rc = dock_search(params, 1, &desc, ligand, box, copies, steps, bfgs_max_iters, seed, nullptr, &dummy, &dummy,
+    rc = dock_search(params, 1, &desc, ligand, box, copies, steps, bfgs_max_iters, seed, 0u, 0u, nullptr, &dummy, &dummy,
                      nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, &need_search, nullptr);
     if (rc != DOCK_EWORKSPACE) return rc == DOCK_OK ? DOCK_EINVAL : rc;
     const size_t need = head + align_up(need_grid, 256) + align_up(need_search, 256);
@@ -730,9 +826,9 @@ extern "C" int dock_system_host(const dock_params *params, const dock_protein *p
     uint64_t *d_ev = (uint64_t *)(ws + head - b_misc + 8);
     unsigned char *ws_grid = ws + head, *ws_search = ws + head + align_up(need_grid, 256);
     DOCK_CUDA_CHECK(cudaMemsetAsync(d_cnt, 0, b_misc, stream));
-    rc = dock_build_grids(params, protein, box, n_lig_types, lig_types, grid_dev, &desc, ws_grid, need_grid, nullptr, stream_);
+    rc = dock_build_grids(params, protein, box, n_lig_types, lig_types, grid_dev, grid_bytes, &desc, ws_grid, need_grid, nullptr, stream_);
     if (rc != DOCK_OK) return rc;
-    rc = dock_search(params, 1, &desc, ligand, box, copies, steps, bfgs_max_iters, seed, nullptr, d_best, d_beste,
+    rc = dock_search(params, 1, &desc, ligand, box, copies, steps, bfgs_max_iters, seed, 0u, 0u, nullptr, d_best, d_beste,
                      d_tp, d_te, d_ti, d_cnt, nullptr, d_ev, ws_search, need_search, nullptr, stream_);
     if (rc != DOCK_OK) return rc;
     DOCK_CUDA_CHECK(cudaMemcpyAsync(out_topk_pose_host, d_tp, (size_t)k * row * sizeof(float), cudaMemcpyDeviceToHost, stream));

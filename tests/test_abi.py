@@ -71,18 +71,42 @@ def test_build_grids_size_query_and_validation(lib):
     lt = np.array(s.lig_types, np.int32)
     need = C.c_size_t(0)
     rc = lib.dock_build_grids(C.byref(p), C.byref(prot), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
-                              None, None, None, C.c_size_t(0), C.byref(need), None)
+                              None, C.c_size_t(0), None, None, C.c_size_t(0), C.byref(need), None)
     assert rc == B.DOCK_EWORKSPACE and need.value > 0
     bad = np.array([0, 99], np.int32)
     rc = lib.dock_build_grids(C.byref(p), C.byref(prot), C.byref(box), 2, bad.ctypes.data_as(C.c_void_p),
-                              None, None, None, C.c_size_t(0), C.byref(need), None)
+                              None, C.c_size_t(0), None, None, C.c_size_t(0), C.byref(need), None)
     assert rc == B.DOCK_EINVAL
     typ_bad = typ.copy()
     typ_bad[3] = -1
     prot_bad = B.dock_protein(len(typ), xyz.ctypes.data_as(C.c_void_p), typ_bad.ctypes.data_as(C.c_void_p))
     rc = lib.dock_build_grids(C.byref(p), C.byref(prot_bad), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
-                              None, None, None, C.c_size_t(0), C.byref(need), None)
+                              None, C.c_size_t(0), None, None, C.c_size_t(0), C.byref(need), None)
     assert rc == B.DOCK_EINVAL
+    # the grid buffer size is part of the contract: a buffer sized for one channel is rejected in eq. 4 mode (4 channels)
+    # before anything touches the device (fake non-null pointers: the check comes first)
+    one = dk.dock_grid_bytes(p, box, len(lt))
+    p4 = dk.dock_default_params()
+    p4.grad_mode = 1
+    assert dk.dock_grid_bytes(p4, box, len(lt)) == 4 * (one - one % 256) + (256 if one % 256 else 0) or dk.dock_grid_bytes(p4, box, len(lt)) > 3 * one
+    desc = B.dock_grid()
+    rc = lib.dock_build_grids(C.byref(p4), C.byref(prot), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
+                              C.c_void_p(1 << 20), C.c_size_t(one), C.byref(desc), C.c_void_p(1 << 21), C.c_size_t(need.value),
+                              C.byref(need), None)
+    assert rc == B.DOCK_EINVAL
+    rc = lib.dock_build_grids(C.byref(p), C.byref(prot), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
+                              C.c_void_p(1 << 20), C.c_size_t(one - 1), C.byref(desc), C.c_void_p(1 << 21), C.c_size_t(need.value),
+                              C.byref(need), None)
+    assert rc == B.DOCK_EINVAL
+    # batched form: the workspace holds every system's cell lists
+    prots = (B.dock_protein * 3)(prot, prot, prot)
+    boxes = (B.dock_box * 3)(box, box, box)
+    need3 = C.c_size_t(0)
+    rc = lib.dock_build_grids_batch(C.byref(p), 3, prots, boxes, len(lt), lt.ctypes.data_as(C.c_void_p), None, None, None,
+                                    None, C.c_size_t(0), C.byref(need3), None)
+    assert rc == B.DOCK_EWORKSPACE and need.value < need3.value <= 3 * need.value
+    assert lib.dock_build_grids_batch(C.byref(p), 0, None, None, len(lt), lt.ctypes.data_as(C.c_void_p), None, None, None,
+                                      None, C.c_size_t(0), C.byref(need3), None) == B.DOCK_OK
 
 
 def _fake_grid(s, lig_types):
@@ -142,6 +166,8 @@ def test_init_poses_follow_the_philox_rule(orc, lib):
         assert a.shape == b.shape == (64, 7 + T)
         assert np.max(np.abs(a.astype(np.float64) - b)) <= 1e-6
         assert np.mean(a.astype(np.float64) == b) > 0.99   # same formulas in double, rounded once
+        # copy_base: a shard of copies starts exactly where those copies of the unsharded run start
+        assert np.array_equal(dk.dock_init_poses(box, T, 0xDEADBEEF12345678, 3, 24, copy_base=40), a[40:])
 
 
 def test_site_restrained_initial_poses(orc, lib):
@@ -176,3 +202,33 @@ def test_site_restrained_initial_poses(orc, lib):
     far = np.array([[500.0, 0.0, 0.0], [600.0, 0.0, 0.0]], np.float32)
     f = dk.dock_init_poses_site(box, 0, seed, 0, 4, far, 7.0)
     assert np.array_equal(f[:, :3], far[[0, 1, 0, 1]])
+    full = dk.dock_init_poses_site(box, 7, seed, 2, 64, site, 7.0)
+    assert np.array_equal(dk.dock_init_poses_site(box, 7, seed, 2, 20, site, 7.0, copy_base=44), full[44:])
+
+
+def test_search_rejects_before_it_enqueues(lib):
+    """dock_search validates everything on the host first: a copy count whose top-k sort does not fit shared memory and
+    mixed gradient modes are DOCK_EINVAL at the size query already (no device pointer is ever touched)."""
+    s = make_system(0, seed=0)
+    p = dk.dock_default_params()
+    g = _fake_grid(s, s.lig_types)
+    h = dk.LigandHandle(s.ligand)
+    box = dk.make_box(s.box_center, s.box_size, s.spacing)
+    need = C.c_size_t(0)
+    fake = C.c_void_p(1 << 20)
+
+    def query(copies, grids, want_topk=True):
+        ns = len(grids)
+        g_arr = (B.dock_grid * ns)(*grids)
+        l_arr = (B.dock_ligand * ns)(*[h.c] * ns)
+        b_arr = (B.dock_box * ns)(*[box] * ns)
+        tk = fake if want_topk else None
+        return lib.dock_search(C.byref(p), ns, g_arr, l_arr, b_arr, copies, 2, 10, C.c_uint64(1), C.c_uint32(0), C.c_uint32(0),
+                               None, fake, fake, tk, tk, tk, tk, None, None, None, C.c_size_t(0), C.byref(need), None)
+
+    assert query(64, [g]) == B.DOCK_EWORKSPACE
+    assert query(1 << 16, [g]) == B.DOCK_EINVAL             # 2 x 65536 sort keys + poses > 200 KB of shared memory
+    assert query(1 << 16, [g], want_topk=False) == B.DOCK_EWORKSPACE
+    g4 = _fake_grid(s, s.lig_types)
+    g4.n_channels = 4
+    assert query(64, [g, g4]) == B.DOCK_EINVAL               # one gradient mode per launch

@@ -8,7 +8,8 @@ import numpy as np
 import pytest
 
 from dock_synth import make_system, random_poses
-from tests.parity import KINK_MARGIN, compare_scores, gpu_side, oracle_side, tol
+from tests.parity import (CEILING_DROP_BITS, KINK_MARGIN, bb_replay, binom_floor, compare_grid, compare_scores, gpu_side, iteration_replay,
+                          oracle_self_agreement, oracle_side, tol, unpack_iter_trace)
 
 pytestmark = pytest.mark.gpu
 
@@ -52,14 +53,11 @@ def micro(dk, orc):
 @pytest.mark.parametrize("cfg", [0, 1])
 def test_grid_maps_match_brute_force_at_every_node(dk, orc, tiny, micro, cfg):
     s, (p, box, grid, lig), (op, og, oL) = tiny if cfg == 0 else micro
-    g = grid.data.cpu().numpy().astype(np.float64)
-    assert g.shape == og.maps.shape
     assert tuple(grid.desc.dims) == og.dims and np.array_equal(np.array(grid.desc.origin, np.float64), og.origin)
-    err = np.abs(g - og.maps) / tol(og.maps)
-    _log("grid", dict(cfg=cfg, nodes=int(g.size), max_err=float(err.max()), max_abs=float(np.abs(g - og.maps).max())))
-    assert err.max() <= 1.0
+    st = compare_grid(orc, op, s.protein_xyz, grid.data.cpu().numpy(), og, f"cfg{cfg}")
+    _log("grid", dict(cfg=cfg, **st))
     # fp32 accumulation of ~150 terms: relative error should really be ~1e-6
-    assert np.abs(g - og.maps).max() <= 2e-5 * max(1.0, np.abs(og.maps).max())
+    assert st["max_abs"] <= 2e-5 * max(1.0, np.abs(og.maps).max())
 
 
 def test_grid_edge_cases(dk, orc, torch):
@@ -75,11 +73,10 @@ def test_grid_edge_cases(dk, orc, torch):
     rng = np.random.default_rng(5)
     xyz = (rng.random((60, 3)) * [10, 8, 6] - [5, 4, 3]).astype(np.float32)
     typ = rng.integers(0, 17, 60).astype(np.int32)
-    all_types = list(range(17))                       # > 8 maps: two passes
+    all_types = list(range(17))                       # > 8 maps: three passes
     g = dk.dock_build_grids(p, xyz, typ, box, all_types)
     og = orc.build_grid(op, xyz, typ, [0, 0, 0], [6.0, 4.5, 3.0], 0.375, all_types)
-    err = np.abs(g.data.cpu().numpy() - og.maps) / tol(og.maps)
-    assert err.max() <= 1.0
+    compare_grid(orc, op, xyz, g.data.cpu().numpy(), og, "17 types")
 
 
 # ----------------------------------------------------------------------------------- A2-A5 per pose
@@ -185,53 +182,104 @@ def test_run_to_run_determinism(dk, torch, tiny):
 
 
 # ----------------------------------------------------------------------------------- A6 local optimisation
-@pytest.mark.parametrize("cfg,n,cap", [(0, 256, 50), (1, 256, 300)])
-def test_local_opt_final_energies(dk, orc, torch, tiny, micro, cfg, n, cap):
-    s, (p, box, grid, lig), (op, og, oL) = tiny if cfg == 0 else micro
+@pytest.mark.parametrize("cfg,n,cap", [(0, 256, 50), (1, 256, 300), (2, 256, 300)])
+def test_local_opt_level2(dk, orc, torch, cfg, n, cap):
+    """Parity level 2 (BASELINE.json:north_star "local-opt final energies within 1e-3 kcal/mol"; DESIGN.md "Parity
+    levels").  Three statements, all numeric:
+      (a) consistency: the reported energy is the oracle's energy of the reported pose (level 1 at the optimum) and
+          never exceeds the start;
+      (b) the ALGORITHM is the oracle's: the oracle redoes every GPU iteration from the GPU's own state (x, g, H) and
+          must take the same decisions (trials, accept / stop, update, reset) except where its own margin to the
+          deciding threshold is a small fraction of the S20 tolerance -- an iteration-level teacher-forced replay;
+      (c) free-running final energies agree within 1e-3 as often as the oracle agrees WITH ITSELF when every energy
+          and gradient it sees is rounded to fp32 (the chaos ceiling: no single-precision evaluator can do better;
+          tests/test_oracle_pins.py::test_local_optimisation_is_chaotic_at_fp32_resolution)."""
+    s = make_system(cfg, seed=0)
+    p, box, grid, lig = gpu_side(dk, s)
+    op, og, oL = oracle_side(orc, s)
     rng = np.random.default_rng(7)
     poses = random_poses(rng, n, s.box_center, s.box_size * 0.6, lig.T)
-    out_pose, out_e, out_it = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap)
+    out_pose, out_e, out_it, trace = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap, trace_cap=cap + 1)
+    plain = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap)
+    assert torch.equal(plain[0], out_pose) and torch.equal(plain[1], out_e) and torch.equal(plain[2], out_it)   # tracing changes nothing
     ge, gp, git = out_e.cpu().numpy().astype(np.float64), out_pose.cpu().numpy(), out_it.cpu().numpy()
-    ref = [orc.local_opt(op, og, oL, poses[i].astype(np.float64), cap) for i in range(n)]
-    re_ = np.array([r[0] for r in ref])
-    # the GPU's reported energy is the oracle's energy of the GPU's final pose (level 1 at the optimum)
-    # A descent that pushes a pair outward cannot cross the hard cutoff (E jumps UP by ~0.0036 at r = 8 A, reading
-    # S3), so the backtracking line search parks that pair at r = 8 - O(1e-7): in about half of all local optima
-    # -- the oracle's own too -- some pair sits closer to the cutoff than fp32 can resolve.  Those poses are
-    # compared with the jump allowed for; all others under S20.
+    # ---- (a) A descent that pushes a pair outward cannot cross the hard cutoff (E jumps UP by ~0.0036 at r = 8 A, reading
+    # S3), so the backtracking line search parks that pair at r = 8 - O(1e-7): in about half of all local optima -- the
+    # oracle's own too -- some pair sits closer to the cutoff than fp32 can resolve; those are compared with the jump allowed.
     chk, _, _, dg = orc.score_batch(op, og, oL, gp.astype(np.float64))
     away = dg["cutoff_margin"] > KINK_MARGIN
     assert away.mean() > 0.25 and np.all(np.abs(ge - chk)[away] <= tol(chk)[away])
     assert np.all(np.abs(ge - chk) <= tol(chk) + 3 * 0.004)
-    # never worse than the start
     e0 = orc.score_batch(op, og, oL, poses.astype(np.float64), want_grad=False)[0]
     assert np.all(ge <= e0 + tol(e0))
-    agree = np.abs(ge - re_) <= 1e-3
-    st = dict(cfg=cfg, n=n, cap=cap, agree_1e3=float(agree.mean()), median_abs=float(np.median(np.abs(ge - re_))),
-              gpu_mean=float(ge.mean()), ref_mean=float(re_.mean()),
-              gpu_iters=float(git[:, 0].mean()), ref_iters=float(np.mean([r[2] for r in ref])))
-    _log("local_opt", st)
-    # Free-running fp32 vs fp64 BFGS on a piecewise-trilinear landscape (the gradient of eq. 3 jumps at
-    # every cell face, so minima sit on faces and the stopping point is round-off sensitive): the
-    # agreement rate is REPORTED; what is asserted is that the two
-    # optimizers are statistically the same optimizer ...
-    qg, qr = np.quantile(ge, [0.25, 0.5, 0.75]), np.quantile(re_, [0.25, 0.5, 0.75])
-    st["gpu_quartiles"], st["ref_quartiles"] = qg.tolist(), qr.tolist()
-    assert np.all(np.abs(qg - qr) <= 0.75 + 0.15 * np.abs(qr)), st
-    assert abs(st["gpu_iters"] - st["ref_iters"]) <= 0.25 * max(st["ref_iters"], 1.0), st
-    # ... that neither side is systematically better (paired sign test, 5 sigma) ...
-    decided = np.abs(ge - re_) > 1e-3
-    wins = int((ge < re_)[decided].sum())
+    assert np.all((git[:, 2] >= 1) & (git[:, 2] <= 3)) and np.all(git[:, 0] <= cap) and np.all(git[:, 1] >= git[:, 0] + 1)
+    # ---- (b) iteration-level teacher-forced replay
+    it = unpack_iter_trace(trace.cpu().numpy(), git, lig.T)
+    assert len(it["f"]) == int((git[:, 0] + (git[:, 2] != dk.DOCK_EXIT_CAP)).sum())
+    assert int(it["trials"].sum()) + n == int(git[:, 1].sum())                     # evaluations = 1 + all line-search trials
+    rp = iteration_replay(orc, op, og, oL, it, float(op.bfgs_gtol))
+    cmp_ = ~rp["near_cut"]
+    same = rp["same"][cmp_]
+    ferr = (np.abs(it["f"] - rp["recs"]["f"]) / tol(rp["recs"]["f"]))[cmp_]        # level 1 at every visited state
+    acc = cmp_ & rp["same"] & (it["status"] == 0)
+    fnerr = np.abs(it["f_new"] - rp["recs"]["f_new"])[acc] / tol(rp["recs"]["f_new"][acc])
+    bad = cmp_ & ~rp["same"]
+    kinds = {k: int((rp["kind"][bad] == k).sum()) for k in ("armijo", "gtol", "descent", "curvature")}
+    worst_margin = float(rp["margin_tol"][bad].max()) if bad.any() else 0.0
+    # state propagation: the GPU's next state against the oracle's result of this iteration
+    key = {(int(a), int(b)): j for j, (a, b) in enumerate(zip(it["pose"], it["iter"]))}
+    nxt = np.array([key.get((int(a), int(b) + 1), -1) for a, b in zip(it["pose"], it["iter"])])
+    prop = acc & (nxt >= 0)
+    ex = np.abs(it["x"][nxt[prop]] - rp["x_new"][prop]).max(axis=1)
+    hn = np.linalg.norm(rp["H_new"][prop].reshape(prop.sum(), -1), axis=1)
+    eh = np.linalg.norm((it["H"][nxt[prop]] - rp["H_new"][prop]).reshape(prop.sum(), -1), axis=1) / np.maximum(hn, 1e-30)
+    # ---- (c) free run against the chaos ceiling
+    oe, _, oinfo = orc.local_opt_batch(op, og, oL, poses.astype(np.float64), cap)
+    ceil = oracle_self_agreement(orc, op, og, oL, poses.astype(np.float64), cap)
+    agree = float(np.mean(np.abs(ge - oe) <= 1e-3))
+    st = dict(cfg=cfg, n=n, cap=cap, iterations=int(len(it["f"])), iterations_compared=int(cmp_.sum()),
+              iter_decisions_identical=float(same.mean()), iter_mismatch_kinds=kinds, iter_mismatch_worst_margin_tol=worst_margin,
+              state_f_max_err_tol=float(ferr.max()), f_new_max_err_tol=float(fnerr.max()),
+              x_new_max_abs=float(ex.max()), H_new_rel_err_median=float(np.median(eh)), H_new_rel_err_q90=float(np.quantile(eh, 0.9)),
+              agree_1e3=agree, ceiling_agree_1e3=ceil["agree"], median_abs=float(np.median(np.abs(ge - oe))),
+              ceiling_median_abs=ceil["median_abs"],
+              gpu_iters=float(git[:, 0].mean()), ref_iters=float(oinfo[:, 0].mean()), ceiling_iters=float(ceil["info1"][:, 0].mean()),
+              gpu_evals=float(git[:, 1].mean()), ref_evals=float(oinfo[:, 1].mean()),
+              exit_gtol_cap_linesearch=dict(gpu=np.bincount(git[:, 2], minlength=4)[1:].tolist(),
+                                            ref=np.bincount(oinfo[:, 2], minlength=4)[1:].tolist(),
+                                            ceiling=np.bincount(ceil["info1"][:, 2], minlength=4)[1:].tolist()))
+    _log("local_opt_level2", st)
+    assert ferr.max() <= 1.0 and fnerr.max() <= 1.0, st                              # S20 at every state and accepted trial
+    assert same.mean() >= 0.975, st                                                  # observed 0.984 - 0.995
+    # a decision may differ only where the oracle itself is within 0.25 S20-tolerances of the threshold (S20 would allow
+    # 2: both energies of an Armijo difference may be off by one tolerance each); observed worst 0.06
+    assert worst_margin <= 0.25, st
+    assert kinds["descent"] == 0 and kinds["curvature"] <= max(2, 0.001 * len(same)), st
+    assert ex.max() <= 1e-5 and np.median(eh) <= 1e-4 and np.quantile(eh, 0.9) <= 1e-2, st
+    assert agree >= binom_floor(ceil["agree"], n), st
+    # neither side is systematically better (paired sign test, 5 sigma)
+    decided = np.abs(ge - oe) > 1e-3
+    wins = int((ge < oe)[decided].sum())
     assert abs(wins - 0.5 * decided.sum()) <= 2.5 * math.sqrt(max(1, decided.sum())), (wins, int(decided.sum()), st)
-    # ... and that the deterministic part agrees: same start, cap = 1 iteration -> same first step
-    o1, e1, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), 1)
-    r1 = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), 1)[0] for i in range(n)])
-    c1, _, _, d1 = orc.score_batch(op, og, oL, o1.cpu().numpy().astype(np.float64))
-    ok1 = d1["cutoff_margin"] > KINK_MARGIN
-    first = np.abs(e1.cpu().numpy() - r1) <= tol(r1) * 10
-    st["first_step_agree"] = float(first[ok1].mean())
-    _log("local_opt_first_step", st)
-    assert first[ok1].mean() >= 0.97, st
+    # stopping: both sides end by the same mechanism, and the GPU does not run longer than its cap or the oracle's horizon
+    assert abs(st["gpu_iters"] - st["ref_iters"]) <= 0.25 * max(st["ref_iters"], 1.0), st
+
+
+def _first_iterations_replay(dk, orc, torch, p, grid, lig, op, og, oL, poses, cap=3):
+    """The first `cap` BFGS iterations of every pose, each redone by the oracle from the GPU's own state: decisions equal
+    (or on the threshold), new energies within S20.  Used where a variant of the evaluator drives the optimizer
+    (eq. 4 maps, other weight signs)."""
+    o, e, it_, trace = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap, trace_cap=cap + 1)
+    it = unpack_iter_trace(trace.cpu().numpy(), it_.cpu().numpy(), lig.T)
+    rp = iteration_replay(orc, op, og, oL, it, float(op.bfgs_gtol))
+    cmp_ = ~rp["near_cut"]
+    acc = cmp_ & rp["same"] & (it["status"] == 0)
+    assert cmp_.sum() >= 0.9 * len(cmp_) and rp["same"][cmp_].mean() >= 0.97, float(rp["same"][cmp_].mean())
+    bad = cmp_ & ~rp["same"]
+    assert not bad.any() or rp["margin_tol"][bad].max() <= 0.25, float(rp["margin_tol"][bad].max())
+    assert np.all(np.abs(it["f"] - rp["recs"]["f"])[cmp_] <= tol(rp["recs"]["f"])[cmp_])
+    assert np.all(np.abs(it["f_new"] - rp["recs"]["f_new"])[acc] <= tol(rp["recs"]["f_new"])[acc])
+    return float(rp["same"][cmp_].mean())
 
 
 def test_local_opt_zero_iterations_is_a_plain_evaluation(dk, orc, torch, tiny):
@@ -242,7 +290,7 @@ def test_local_opt_zero_iterations_is_a_plain_evaluation(dk, orc, torch, tiny):
     e, _, _ = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
     # two evaluators (warp-per-pose in the optimizer, thread-per-pose in the batch call): same value up to summation order
     assert torch.allclose(out_e, e, rtol=1e-5, atol=1e-4)
-    assert np.all(out_it.cpu().numpy() == [0, 1])
+    assert np.all(out_it.cpu().numpy() == [0, 1, dk.DOCK_EXIT_CAP])
 
 
 # ----------------------------------------------------------------------------------- A7 search
@@ -251,86 +299,108 @@ def _trace_fields(tr):
                 iters=tr[..., 4], evals=tr[..., 5], kind=tr[..., 6], pose=tr[..., 8:])
 
 
-@pytest.mark.parametrize("cfg", [0, 2])
-def test_search_free_run_and_teacher_forced(dk, orc, torch, cfg):
-    s = make_system(cfg, seed=0)
-    p, box, grid, lig = gpu_side(dk, s)
-    op, og, oL = oracle_side(orc, s)
-    copies, steps, cap = (s.copies, s.steps, s.bfgs_cap) if cfg == 0 else (64, 10, 300)
-    seed = 2023
-    init = dk.dock_init_poses(box, lig.T, seed, 0, copies)
-    assert np.max(np.abs(init - orc.init_poses(s.box_center, s.box_size, lig.T, seed, 0, copies))) <= 1e-6
-    res = dk.dock_search(p, [grid], [lig], [box], copies, steps, cap, seed,
-                         init_poses=torch.from_numpy(init[None]).cuda(), want_trace=True)
-    tr = _trace_fields(res["trace"][0].cpu().numpy().astype(np.float64))
-    best_e = res["best_e"][0].cpu().numpy().astype(np.float64)
-    best_pose = res["best_pose"][0].cpu().numpy().astype(np.float64)
+def _search_parity(dk, orc, torch, s, gpu_side_, oracle_side_, copies, steps, cap, seed, n_ref, tag, system=0, res=None):
+    """Parity level 3 / 3' for one system: the GPU search over `copies`
+    copies (run here, or given as `res` = its outputs for this system) against the oracle on the first n_ref copies
+    (copies are independent, so a prefix of them is exactly the same sub-problem).  Returns the stats dict."""
+    p, box, grid, lig = gpu_side_
+    op, og, oL = oracle_side_
+    np_ = 7 + lig.T
+    init = dk.dock_init_poses(box, lig.T, seed, system, copies)
+    init_ref = orc.init_poses(s.box_center, s.box_size, lig.T, seed, system, n_ref)
+    assert np.max(np.abs(init[:n_ref] - init_ref)) <= 1e-6
+    if res is None:
+        r = dk.dock_search(p, [grid], [lig], [box], copies, steps, cap, seed,
+                           init_poses=torch.from_numpy(init[None]).cuda(), want_trace=True, system_base=system)
+        res = dict(trace=r["trace"][0], best_e=r["best_e"][0], best_pose=r["best_pose"][0], evals=int(r["evals"][0]))
+    tr = _trace_fields(res["trace"][:n_ref].cpu().numpy().astype(np.float64))
+    tr["pose"] = tr["pose"][..., :np_]
+    best_e = res["best_e"][:n_ref].cpu().numpy().astype(np.float64)
+    best_pose = res["best_pose"][:n_ref, :np_].cpu().numpy().astype(np.float64)
     T_mc = float(p.t_mc)
 
     # --- internal consistency of the GPU trace (logic, exact) ---------------------------------
-    for c in range(copies):
+    for c in range(n_ref):
         for k in range(steps):
-            assert tr["u"][c, k] == orc.mc_uniform(seed, 0, c, k)                  # same Philox stream, bit exact
-            kind, _ = orc.mc_perturb(op, lig.T, seed, 0, c, k, tr["pose"][c, k])
+            assert tr["u"][c, k] == orc.mc_uniform(seed, system, c, k)             # same Philox stream, bit exact
+            kind, _ = orc.mc_perturb(op, lig.T, seed, system, c, k, tr["pose"][c, k])
             assert kind == int(tr["kind"][c, k])
-            de = tr["e_cand"][c, k] - tr["e_cur"][c, k]
-            thr = math.exp(min(50.0, -de / T_mc))
-            if de != 0.0 and abs(tr["u"][c, k] - thr) > 1e-6:                       # margin rule
-                assert bool(tr["accept"][c, k]) == (de < 0 or tr["u"][c, k] < thr), (c, k)
-            if k + 1 < steps:                                                       # chain: next e_cur
-                want = tr["e_cand"][c, k] if tr["accept"][c, k] else tr["e_cur"][c, k]
-                assert tr["e_cur"][c, k + 1] == want
-        acc = [tr["e_cur"][c, 0]] + [tr["e_cand"][c, k] for k in range(steps) if tr["accept"][c, k]]
-        assert best_e[c] == min(acc)
+    de = tr["e_cand"] - tr["e_cur"]
+    thr = np.exp(np.minimum(50.0, -de / T_mc))
+    clear = (de != 0.0) & (np.abs(tr["u"] - thr) > 1e-6)                            # margin rule of north_star
+    assert np.array_equal(tr["accept"][clear], ((de < 0) | (tr["u"] < thr))[clear])
+    nxt = np.where(tr["accept"], tr["e_cand"], tr["e_cur"])
+    assert np.array_equal(tr["e_cur"][:, 1:], nxt[:, :-1])                          # chain: next e_cur
+    run_min = np.minimum(tr["e_cur"][:, 0], np.where(tr["accept"], tr["e_cand"], np.inf).min(axis=1)) if steps else best_e
+    assert np.array_equal(best_e, run_min)
     chk, _, _, dgb = orc.score_batch(op, og, oL, best_pose)
     awayb = dgb["cutoff_margin"] > KINK_MARGIN
     assert np.all(np.abs(best_e - chk)[awayb] <= tol(chk)[awayb])                   # best pose really has that energy
-    assert int(res["evals"][0]) >= int(tr["evals"].sum()) + copies              # + the initial local optimisations
+    if n_ref == copies:
+        assert res["evals"] >= int(tr["evals"].sum()) + copies                      # + the initial local optimisations
 
-    # --- level 3': teacher-forced replay of every recorded step -------------------------------------
-    n_steps = n_e_ok = n_dec = n_dec_ok = 0
-    for c in range(copies):
-        for k in range(steps):
-            _, cand0 = orc.mc_perturb(op, lig.T, seed, 0, c, k, tr["pose"][c, k])
-            e_c, _, _, _ = orc.local_opt(op, og, oL, cand0, cap)
-            e_cur, _, _, dgc = orc.score_batch(op, og, oL, tr["pose"][c, k][None, :7 + lig.T])
-            e_cur = float(e_cur[0])
-            if dgc["cutoff_margin"][0] > KINK_MARGIN:
-                assert abs(e_cur - tr["e_cur"][c, k]) <= tol(e_cur)                 # level 1 on the pre-step pose
-            n_steps += 1
-            ok = abs(e_c - tr["e_cand"][c, k]) <= 1e-3
-            n_e_ok += ok
-            if ok:
-                de = e_c - e_cur
-                thr = math.exp(min(50.0, -de / T_mc))
-                if abs(de) > 2e-3 and abs(tr["u"][c, k] - thr) > 2e-3 * max(thr, 1e-3) / T_mc + 1e-6:
-                    n_dec += 1
-                    n_dec_ok += bool(tr["accept"][c, k]) == (de < 0 or tr["u"][c, k] < thr)
-    # --- level 3: free run from the same initial poses --------------------------------------------
-    ref = orc.search(op, og, oL, init.astype(np.float64), steps, cap, seed, 0)
-    same_prefix = []
-    for c in range(copies):
-        k = 0
-        while k < steps and bool(tr["accept"][c, k]) == bool(ref["trace"]["accept"][c, k]) \
-                and abs(tr["e_cand"][c, k] - ref["trace"]["e_cand"][c, k]) <= 1e-3:
-            k += 1
-        same_prefix.append(k)
+    # --- level 3': teacher-forced replay of every recorded step (oracle restarts from the GPU's pre-step pose) ---
+    cc, kk = np.meshgrid(np.arange(n_ref), np.arange(steps), indexing="ij")
+    pre = tr["pose"].reshape(-1, np_)
+    rp = orc.replay_steps(op, og, oL, cap, seed, system, pre, cc.ravel(), kk.ravel())
+    with orc.round_eval_fp32(CEILING_DROP_BITS):                                    # the chaos ceiling of one relaxed step
+        rp32 = orc.replay_steps(op, og, oL, cap, seed, system, pre, cc.ravel(), kk.ravel())
+    g_ecur, g_ecand, g_acc, g_u = tr["e_cur"].ravel(), tr["e_cand"].ravel(), tr["accept"].ravel(), tr["u"].ravel()
+    away = rp["cur_cutoff_margin"] > KINK_MARGIN
+    assert np.all(np.abs(g_ecur - rp["e_cur"])[away] <= tol(rp["e_cur"])[away])     # level 1 on every pre-step pose
+    assert np.array_equal(rp["kind"], tr["kind"].ravel().astype(np.int32)) and np.array_equal(rp["u"], g_u)
+    e_ok = np.abs(g_ecand - rp["e_cand"]) <= 1e-3
+    tf_ceiling = float(np.mean(np.abs(rp32["e_cand"] - rp["e_cand"]) <= 1e-3))
+    d2 = rp["e_cand"] - rp["e_cur"]
+    thr2 = np.exp(np.minimum(50.0, -d2 / T_mc))
+    decisive = e_ok & (np.abs(d2) > 2e-3) & (np.abs(g_u - thr2) > 2e-3 * np.maximum(thr2, 1e-3) / T_mc + 1e-6)
+    dec_ok = g_acc[decisive] == ((d2 < 0) | (g_u < thr2))[decisive]
+
+    # --- level 3: free run from the same initial poses; ceiling = the oracle against itself with fp32-rounded evaluations ---
+    ref = orc.search(op, og, oL, init[:n_ref].astype(np.float64), steps, cap, seed, system)
+    with orc.round_eval_fp32(CEILING_DROP_BITS):
+        ref32 = orc.search(op, og, oL, init[:n_ref].astype(np.float64), steps, cap, seed, system)
+
+    def prefix(acc_a, ec_a, acc_b, ec_b):
+        same = (acc_a.astype(bool) == acc_b.astype(bool)) & (np.abs(ec_a - ec_b) <= 1e-3)
+        return np.where(same.all(axis=1), steps, np.argmin(same, axis=1)) if steps else np.zeros(len(acc_a), int)
+
+    pg = prefix(tr["accept"], tr["e_cand"], ref["trace"]["accept"], ref["trace"]["e_cand"])
+    pc = prefix(ref32["trace"]["accept"], ref32["trace"]["e_cand"], ref["trace"]["accept"], ref["trace"]["e_cand"])
     best_ok = np.abs(best_e - ref["best_e"]) <= 1e-3
-    st = dict(cfg=cfg, copies=copies, steps=steps, cap=cap,
-              teacher_e_agree=n_e_ok / n_steps, teacher_decisions=n_dec, teacher_decision_agree=(n_dec_ok / max(1, n_dec)),
-              free_full_agree=float(np.mean(np.array(same_prefix) == steps)), free_mean_prefix=float(np.mean(same_prefix)),
-              free_best_agree=float(best_ok.mean()), gpu_best_min=float(best_e.min()), ref_best_min=float(ref["best_e"].min()),
-              gpu_best_mean=float(best_e.mean()), ref_best_mean=float(ref["best_e"].mean()),
-              gpu_evals=int(res["evals"][0]), ref_evals=int(ref["evals"]))
-    _log("search", st)
-    assert n_dec_ok == n_dec, st                         # a decision mismatch with agreeing energies is a bug
-    # teacher_e_agree / free_* are round-off amplification rates of the fp32 path: REPORTED (gpurun_out/parity_stats.jsonl,
-    # DESIGN.md "Parity levels"), not gated -- the gate on search logic is the decision check above plus the exact chain checks
-    # best energies are heavy-tailed (a few copies stay stuck in a clash at E ~ 1e2): compare medians and quartiles
+    best_ok_c = np.abs(ref32["best_e"] - ref["best_e"]) <= 1e-3
     qg, qr = np.quantile(best_e, [0.25, 0.5, 0.75]), np.quantile(ref["best_e"], [0.25, 0.5, 0.75])
-    st["gpu_best_quartiles"], st["ref_best_quartiles"] = qg.tolist(), qr.tolist()
-    _log("search_quartiles", st)
-    assert np.all(np.abs(qg - qr) <= 0.75 + 0.15 * np.abs(qr)), st
+    st = dict(tag=tag, copies=copies, ref_copies=n_ref, steps=steps, cap=cap,
+              teacher_steps=int(len(e_ok)), teacher_e_agree=float(e_ok.mean()), teacher_e_agree_ceiling=tf_ceiling,
+              teacher_decisions=int(decisive.sum()), teacher_decision_agree=float(dec_ok.mean()) if decisive.any() else 1.0,
+              free_full_agree=float(np.mean(pg == steps)), free_full_agree_ceiling=float(np.mean(pc == steps)),
+              free_mean_prefix=float(pg.mean()), free_mean_prefix_ceiling=float(pc.mean()),
+              free_best_agree=float(best_ok.mean()), free_best_agree_ceiling=float(best_ok_c.mean()),
+              gpu_best_min=float(best_e.min()), ref_best_min=float(ref["best_e"].min()),
+              gpu_best_quartiles=qg.tolist(), ref_best_quartiles=qr.tolist(),
+              gpu_evals_traced=int(tr["evals"].sum()), ref_evals=int(ref["evals"]), ceiling_evals=int(ref32["evals"]))
+    _log("search_level3", st)
+    assert dec_ok.all(), st                              # a decision mismatch with agreeing energies is a bug
+    assert st["teacher_e_agree"] >= binom_floor(tf_ceiling, len(e_ok)), st
+    assert st["free_full_agree"] >= binom_floor(st["free_full_agree_ceiling"], n_ref), st
+    assert st["free_best_agree"] >= binom_floor(st["free_best_agree_ceiling"], n_ref), st
+    if n_ref >= 64:                                      # mean length of the agreeing prefix: meaningless on a handful of copies
+        assert st["free_mean_prefix"] >= st["free_mean_prefix_ceiling"] - max(1.0, 0.35 * st["free_mean_prefix_ceiling"]), st
+    # best energies are heavy-tailed (a few copies stay stuck in a clash): compare medians, and quartiles where the
+    # sample is large enough for a quartile to mean something
+    assert abs(qg[1] - qr[1]) <= 0.75 + 0.15 * abs(qr[1]), st
+    if n_ref >= 64:
+        assert np.all(np.abs(qg - qr) <= 0.75 + 0.15 * np.abs(qr)), st
+    return st
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_search_free_run_and_teacher_forced(dk, orc, torch, cfg):
+    """BASELINE.json configs[0] (16 x 20, cap 50) and configs[2] (384 x 40, cap 300) at FULL size, every copy and step
+    replayed by the oracle."""
+    s = make_system(cfg, seed=0)
+    _search_parity(dk, orc, torch, s, gpu_side(dk, s), oracle_side(orc, s), s.copies, s.steps, s.bfgs_cap, 2023,
+                   n_ref=s.copies, tag=f"cfg{cfg}")
 
 
 def test_search_zero_steps_equals_local_opt_and_copy_independence(dk, torch, tiny):
@@ -349,25 +419,44 @@ def test_search_zero_steps_equals_local_opt_and_copy_independence(dk, torch, tin
     assert torch.equal(r3["best_e"][0], r1["best_e"][0, :7])
 
 
-def test_batched_systems_equal_single_system_runs(dk, torch):
-    """Config-3 shape in miniature: heterogeneous systems in one launch == one launch per system."""
-    systems = [make_system(3, seed=0, index=i, n_prot=300 + 50 * i) for i in range(3)]
-    sides = [gpu_side(dk, s) for s in systems]
-    p = sides[0][0]
-    grids, ligs, boxes = [x[2] for x in sides], [x[3] for x in sides], [x[1] for x in sides]
-    rb = dk.dock_search(p, grids, ligs, boxes, 8, 3, 40, 77)
+def test_config3_full_batch_in_one_launch(dk, orc, torch):
+    """BASELINE.json configs[3] at FULL size: 256 heterogeneous systems (1500-6000 protein atoms, ligands of 15-50 atoms
+    with 2-12 torsions), 128 copies x 40 steps, BFGS <= 300 -- maps from ONE dock_build_grids_batch call, search in ONE
+    dock_search launch.  Eight systems (extremes of ligand / protein size and torsion count) are then (1) re-run alone
+    with system_base = their index: bitwise the batch's result, and (2) replayed by the oracle (teacher-forced and
+    free-running, first 16 copies, all 40 steps)."""
+    cfg = 256
+    systems = [make_system(3, seed=0, index=i) for i in range(cfg)]
+    p = dk.dock_default_params()
+    boxes = [dk.make_box(q.box_center, q.box_size, q.spacing) for q in systems]
+    ligs = [dk.LigandHandle(q.ligand) for q in systems]
+    grids = dk.dock_build_grids_batch(p, [(q.protein_xyz, q.protein_type) for q in systems], boxes, systems[0].lig_types)
+    copies, steps, cap, seed = 128, 40, 300, 2023
+    rb = dk.dock_search(p, grids, ligs, boxes, copies, steps, cap, seed, want_trace=True)
+    torch.cuda.synchronize()
     t_max = max(l.T for l in ligs)
-    for i in range(3):
-        # system index enters the Philox counter, so replay system i alone with the same init poses
-        init = np.zeros((8, 7 + ligs[i].T), np.float32)
-        init[:] = dk.dock_init_poses(boxes[i], ligs[i].T, 77, i, 8)
-        rs_e = rb["best_e"][i].cpu().numpy()
-        assert np.all(np.isfinite(rs_e))
-        assert rb["best_pose"].shape[-1] == 7 + t_max
-        assert int(rb["topk_count"][i]) >= 1
-    # the first system has index 0 in both layouts -> identical
-    r0 = dk.dock_search(p, grids[:1], ligs[:1], boxes[:1], 8, 3, 40, 77)
-    assert torch.equal(r0["best_e"][0], rb["best_e"][0])
+    assert rb["best_pose"].shape == (cfg, copies, 7 + t_max)
+    be = rb["best_e"].cpu().numpy()
+    assert np.all(np.isfinite(be)) and bool((rb["topk_count"] >= 1).all())
+    te = rb["topk_e"].cpu().numpy()
+    cnt = rb["topk_count"].cpu().numpy()
+    for i in range(cfg):                                                  # top-k of every system: sorted, = the sorted best energies' head
+        assert np.all(np.diff(te[i, :cnt[i]]) >= 0) and te[i, 0] == be[i].min()
+    N = np.array([l.N for l in ligs]); T = np.array([l.T for l in ligs]); NP = np.array([len(q.protein_type) for q in systems])
+    pick = sorted({int(N.argmin()), int(N.argmax()), int(T.argmin()), int(T.argmax()), int(NP.argmin()), int(NP.argmax()), 0, 5})
+    _log("cfg3_batch", dict(systems=cfg, evals=int(rb["evals"][0]), picked=pick, N=[int(N[i]) for i in pick],
+                            T=[int(T[i]) for i in pick], n_prot=[int(NP[i]) for i in pick],
+                            best_e_median=float(np.median(be.min(axis=1))), negative_best_frac=float((be.min(axis=1) < 0).mean())))
+    for i in pick:
+        one = dk.dock_search(p, [grids[i]], [ligs[i]], [boxes[i]], copies, steps, cap, seed, system_base=i)
+        w = 7 + ligs[i].T
+        assert torch.equal(one["best_e"][0], rb["best_e"][i]), i
+        assert torch.equal(one["best_pose"][0, :, :w], rb["best_pose"][i, :, :w]), i
+        assert torch.equal(one["topk_idx"][0], rb["topk_idx"][i]), i
+        q = systems[i]
+        res = dict(trace=rb["trace"][i], best_e=rb["best_e"][i], best_pose=rb["best_pose"][i], evals=0)
+        _search_parity(dk, orc, torch, q, (p, boxes[i], grids[i], ligs[i]), oracle_side(orc, q), copies, steps, cap, seed,
+                       n_ref=16, tag=f"cfg3[{i}]", system=i, res=res)
 
 
 # ----------------------------------------------------------------------------------- A8 top-k
@@ -414,8 +503,7 @@ def test_config3_systems_score_and_local_opt(dk, orc, torch, index):
     s = make_system(3, seed=0, index=index)
     p, box, grid, lig = gpu_side(dk, s)
     op, og, oL = oracle_side(orc, s)
-    err = np.abs(grid.data.cpu().numpy().astype(np.float64) - og.maps) / tol(og.maps)
-    assert err.max() <= 1.0
+    compare_grid(orc, op, s.protein_xyz, grid.data.cpu().numpy(), og, f"cfg3[{index}]")
     rng = np.random.default_rng(30 + index)
     poses = random_poses(rng, 2053, s.box_center, s.box_size, lig.T)
     e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
@@ -433,19 +521,17 @@ def test_config3_systems_score_and_local_opt(dk, orc, torch, index):
     assert np.all(out_e.cpu().numpy() <= e[:n].cpu().numpy() + 1e-3)
 
 
-def test_config4_large_box_grid_score_and_search_properties(dk, orc, torch):
-    """BASELINE.json configs[4]: 8000-atom protein, 161^3 x 8 maps, 60-atom / 15-torsion ligand.  The grid is
-    compared at EVERY node (the oracle's brute force takes ~30 s on the box's cores), scores on a sample;
-    the search runs with the config's 2048 copies for a few steps and is checked through properties that hold
-    at any size (bitwise determinism, best <= initial local optimum, oracle re-evaluation of the winners)."""
+def test_config4_large_box_grid_score_and_full_search(dk, orc, torch):
+    """BASELINE.json configs[4] at FULL size: 8000-atom protein, 161^3 x 8 maps (compared at EVERY node: the oracle's brute
+    force takes ~30 s on the box's cores), 60-atom / 15-torsion ligand scored on a sample, then the search with all
+    2048 copies x 80 steps, BFGS <= 300; the oracle replays and free-runs the first 128 copies over all 80 steps
+    (copies are independent units, so this is the same sub-problem), properties hold for all 2048."""
     s = make_system(4, seed=0)
     p, box, grid, lig = gpu_side(dk, s)
     op, og, oL = oracle_side(orc, s)
     assert tuple(grid.dims) == (161, 161, 161)
-    gm = grid.data.cpu().numpy().astype(np.float64)
-    err = np.abs(gm - og.maps) / tol(og.maps)
-    assert err.max() <= 1.0
-    del gm, err
+    st = compare_grid(orc, op, s.protein_xyz, grid.data.cpu().numpy(), og, "cfg4")
+    _log("grid_cfg4", st)
     rng = np.random.default_rng(4)
     poses = random_poses(rng, 8192, s.box_center, s.box_size, lig.T)
     e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
@@ -453,11 +539,13 @@ def test_config4_large_box_grid_score_and_search_properties(dk, orc, torch):
     st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, "cfg4",
                         cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
     _log("score_cfg4", dict(st, N=lig.N, T=lig.T, P=lig.P))
-    steps = 3
-    r1 = dk.dock_search(p, [grid], [lig], [box], s.copies, steps, s.bfgs_cap, 11)
-    r2 = dk.dock_search(p, [grid], [lig], [box], s.copies, steps, s.bfgs_cap, 11)
+    seed = 11
+    init = dk.dock_init_poses(box, lig.T, seed, 0, s.copies)
+    ti = torch.from_numpy(init[None]).cuda()
+    r1 = dk.dock_search(p, [grid], [lig], [box], s.copies, s.steps, s.bfgs_cap, seed, init_poses=ti, want_trace=True)
+    r2 = dk.dock_search(p, [grid], [lig], [box], s.copies, s.steps, s.bfgs_cap, seed)       # host-generated start poses
     assert torch.equal(r1["best_e"], r2["best_e"]) and torch.equal(r1["best_pose"], r2["best_pose"])
-    r0 = dk.dock_search(p, [grid], [lig], [box], s.copies, 0, s.bfgs_cap, 11)
+    r0 = dk.dock_search(p, [grid], [lig], [box], s.copies, 0, s.bfgs_cap, seed)
     assert bool((r1["best_e"] <= r0["best_e"] + 1e-6).all())          # best only improves on the optimised start
     k = int(r1["topk_count"][0])
     assert 1 <= k <= 10
@@ -467,15 +555,19 @@ def test_config4_large_box_grid_score_and_search_properties(dk, orc, torch):
     ok = d3["cutoff_margin"] > 1e-4
     assert np.all(np.abs(te - oe3)[ok] <= tol(oe3)[ok])
     assert np.all(np.diff(te) >= 0)
-    _log("search_cfg4", dict(copies=s.copies, steps=steps, evals=int(r1["evals"][0]), best=float(te[0])))
+    _log("search_cfg4", dict(copies=s.copies, steps=s.steps, evals=int(r1["evals"][0]), best=float(te[0])))
+    res = dict(trace=r1["trace"][0], best_e=r1["best_e"][0], best_pose=r1["best_pose"][0], evals=int(r1["evals"][0]))
+    _search_parity(dk, orc, torch, s, (p, box, grid, lig), (op, og, oL), s.copies, s.steps, s.bfgs_cap, seed, n_ref=128,
+                   tag="cfg4", res=res)
 
 
 # ----------------------------------------------------------------------------------- NEXT-1: Barzilai-Borwein
 @pytest.mark.parametrize("cfg,n", [(0, 256), (1, 256)])
 def test_bb_local_opt(dk, orc, torch, tiny, micro, cfg, n):
-    """The paper's own local optimizer (reading S13) on both sides: one evaluation per iteration,
-    best point seen returned.  Deterministic prefix (1 and 2 iterations) against the oracle under S20; the
-    free-running 150-iteration result as a distribution (BB is non-monotone, so round-off decides the path)."""
+    """The paper's own local optimizer (reading S13) on both sides: one evaluation per iteration, best point
+    seen returned.  As for BFGS (test_local_opt_level2): (a) consistency, (b) iteration-level teacher-forced replay --
+    the oracle redoes every GPU iteration from the GPU's state (x, g, s, y): same branch (first / BB1 / fallback), same
+    clipping, same step length and the same new energy under S20 --, (c) free-running result against the chaos ceiling."""
     s, (p0, box, grid, lig), (op0, og, oL) = tiny if cfg == 0 else micro
     p = dk.dock_default_params()
     p.optimizer = 1
@@ -485,30 +577,41 @@ def test_bb_local_opt(dk, orc, torch, tiny, micro, cfg, n):
     poses = random_poses(rng, n, s.box_center, s.box_size * 0.6, lig.T)
     pd = torch.from_numpy(poses).cuda()
     e0 = orc.score_batch(op, og, oL, poses.astype(np.float64), want_grad=False)[0]
-    for cap in (1, 2):
-        o, e, it = dk.dock_local_opt_batch(p, grid, lig, pd, cap)
-        ref = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), cap)[0] for i in range(n)])
-        chk, _, _, dg = orc.score_batch(op, og, oL, o.cpu().numpy().astype(np.float64))
-        ok = dg["cutoff_margin"] > KINK_MARGIN
-        ge = e.cpu().numpy().astype(np.float64)
-        assert np.all(np.abs(ge - chk)[ok] <= tol(chk)[ok])                  # reported E = E of the reported pose
-        assert np.all(it.cpu().numpy()[:, 1] == it.cpu().numpy()[:, 0] + 1)  # evaluations = iterations + 1
-        agree = (np.abs(ge - ref) <= 10 * tol(ref))[ok]
-        assert agree.mean() >= 0.97, (cap, float(agree.mean()))
     cap = 150
-    o, e, it = dk.dock_local_opt_batch(p, grid, lig, pd, cap)
-    ge = e.cpu().numpy().astype(np.float64)
-    ref = [orc.local_opt(op, og, oL, poses[i].astype(np.float64), cap) for i in range(n)]
-    re_ = np.array([r[0] for r in ref])
+    o, e, it_, trace = dk.dock_local_opt_batch(p, grid, lig, pd, cap, trace_cap=cap + 1)
+    plain = dk.dock_local_opt_batch(p, grid, lig, pd, cap)
+    assert torch.equal(plain[0], o) and torch.equal(plain[1], e)
+    ge, git = e.cpu().numpy().astype(np.float64), it_.cpu().numpy()
     chk, _, _, dg = orc.score_batch(op, og, oL, o.cpu().numpy().astype(np.float64))
     ok = dg["cutoff_margin"] > KINK_MARGIN
-    assert np.all(np.abs(ge - chk)[ok] <= tol(chk)[ok])
+    assert np.all(np.abs(ge - chk)[ok] <= tol(chk)[ok])                      # reported E = E of the reported pose
     assert np.all(ge <= e0 + tol(e0))                                        # best-seen never exceeds the start
-    qg, qr = np.quantile(ge, [0.25, 0.5, 0.75]), np.quantile(re_, [0.25, 0.5, 0.75])
-    st = dict(cfg=cfg, n=n, cap=cap, agree_1e3=float((np.abs(ge - re_) <= 1e-3).mean()),
-              gpu_quartiles=qg.tolist(), ref_quartiles=qr.tolist(), gpu_mean=float(ge.mean()), ref_mean=float(re_.mean()),
-              gpu_iters=float(it.cpu().numpy()[:, 0].mean()), ref_iters=float(np.mean([r[2] for r in ref])))
+    assert np.all(git[:, 1] == git[:, 0] + 1)                                # evaluations = iterations + 1
+    it = unpack_iter_trace(trace.cpu().numpy(), git, lig.T)
+    rp = bb_replay(orc, op, og, oL, it)
+    cmp_ = ~rp["near_cut"]
+    taken = cmp_ & rp["same"] & (it["status"] == 0)
+    rel_alpha = np.abs(it["alpha"] - rp["recs"]["alpha"])[taken] / rp["recs"]["alpha"][taken]
+    fnerr = np.abs(it["f_new"] - rp["recs"]["f_new"])[taken] / tol(rp["recs"]["f_new"][taken])
+    ferr = (np.abs(it["f"] - rp["recs"]["f"]) / tol(rp["recs"]["f"]))[cmp_]
+    bad = cmp_ & ~rp["same"]
+    # a differing branch / clipping decision must sit on its threshold: |s.y - eps|s||y|| or |alpha|g| - bb_step| tiny
+    bad_margin = np.minimum(np.abs(rp["recs"]["sy_margin"][bad]) / np.maximum(1e-30, np.abs(rp["recs"]["sy_margin"][bad]) + 1e-6),
+                            np.abs(rp["recs"]["cap_margin"][bad])) if bad.any() else np.zeros(0)
+    ceil = oracle_self_agreement(orc, op, og, oL, poses.astype(np.float64), cap)
+    oe = ceil["e0"]
+    agree = float(np.mean(np.abs(ge - oe) <= 1e-3))
+    qg, qr = np.quantile(ge, [0.25, 0.5, 0.75]), np.quantile(oe, [0.25, 0.5, 0.75])
+    st = dict(cfg=cfg, n=n, cap=cap, iterations=int(len(it["f"])), iter_decisions_identical=float(rp["same"][cmp_].mean()),
+              alpha_rel_err_max=float(rel_alpha.max()), f_new_max_err_tol=float(fnerr.max()), state_f_max_err_tol=float(ferr.max()),
+              mismatches=int(bad.sum()), mismatch_margin_max=float(bad_margin.max()) if bad.any() else 0.0,
+              agree_1e3=agree, ceiling_agree_1e3=ceil["agree"], gpu_quartiles=qg.tolist(), ref_quartiles=qr.tolist(),
+              gpu_iters=float(git[:, 0].mean()), ref_iters=float(ceil["info0"][:, 0].mean()))
     _log("bb_local_opt", st)
+    assert ferr.max() <= 1.0 and fnerr.max() <= 1.0, st
+    assert rp["same"][cmp_].mean() >= 0.995 and (not bad.any() or bad_margin.max() <= 1e-3), st
+    assert rel_alpha.max() <= 1e-5, st                                       # same step length from the same (s, y, g)
+    assert agree >= binom_floor(ceil["agree"], n), st
     assert np.all(np.abs(qg - qr) <= 0.75 + 0.15 * np.abs(qr)), st
 
 
@@ -600,14 +703,10 @@ def test_eq4_maps_scores_and_search(dk, orc, torch, tiny):
     _log("score_eq4", st)
     e3, g3, _ = dk.dock_score_batch(p3, grid3, lig, torch.from_numpy(poses).cuda())
     assert torch.allclose(e, e3, rtol=1e-6, atol=1e-5) and not torch.allclose(g, g3, atol=1e-3)   # same E, different gradient
-    # warp evaluator: zero optimizer iterations = one evaluation; its energy matches, and one BFGS step agrees with the oracle
+    # warp evaluator: zero optimizer iterations = one evaluation; its energy matches, and the first BFGS iterations replay
     o0, e0, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 0)
     assert torch.allclose(e0, e[:128], rtol=1e-5, atol=1e-4)
-    o1, e1, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 1)
-    r1 = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), 1)[0] for i in range(128)])
-    c1, _, _, d1 = orc.score_batch(op, og, oL, o1.cpu().numpy().astype(np.float64))
-    ok1 = d1["cutoff_margin"] > KINK_MARGIN
-    assert (np.abs(e1.cpu().numpy() - r1) <= 10 * tol(r1))[ok1].mean() >= 0.97
+    _first_iterations_replay(dk, orc, torch, p, grid, lig, op, og, oL, poses[:128])
     r = dk.dock_search(p, [grid], [lig], [box], s.copies, 5, 50, 3)
     r2 = dk.dock_search(p, [grid], [lig], [box], s.copies, 5, 50, 3)
     assert torch.equal(r["best_e"], r2["best_e"]) and int(r["topk_count"][0]) >= 1
@@ -634,21 +733,17 @@ def test_other_term_weights_and_signs(dk, orc, torch, tiny, w):
     lig = dk.LigandHandle(s.ligand)
     og = orc.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
     oL = orc.Ligand(s.ligand)
-    assert np.all(np.abs(grid.data.cpu().numpy().astype(np.float64) - og.maps) <= tol(og.maps))
+    compare_grid(orc, op, s.protein_xyz, grid.data.cpu().numpy(), og, f"w={w}")
     rng = np.random.default_rng(91)
     poses = random_poses(rng, 1031, s.box_center, s.box_size * 1.1, lig.T)
     e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
     oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
     compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, f"w={w}",
                    cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
-    # warp evaluator through the optimizer: zero iterations = one evaluation; one iteration = the oracle's first step
+    # warp evaluator through the optimizer: zero iterations = one evaluation; the first iterations replay on the oracle
     o0, e0, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 0)
     assert torch.allclose(e0, e[:128], rtol=1e-5, atol=1e-4)
-    o1, e1, _ = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses[:128]).cuda(), 1)
-    r1 = np.array([orc.local_opt(op, og, oL, poses[i].astype(np.float64), 1)[0] for i in range(128)])
-    c1, _, _, d1 = orc.score_batch(op, og, oL, o1.cpu().numpy().astype(np.float64))
-    ok1 = d1["cutoff_margin"] > KINK_MARGIN
-    assert (np.abs(e1.cpu().numpy() - r1) <= 10 * tol(r1))[ok1].mean() >= 0.95
+    _first_iterations_replay(dk, orc, torch, p, grid, lig, op, og, oL, poses[:128])
 
 
 def test_non_cubic_box_scores_and_search(dk, orc, torch, tiny):
@@ -662,7 +757,7 @@ def test_non_cubic_box_scores_and_search(dk, orc, torch, tiny):
     grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types)
     assert tuple(grid.dims) == (33, 25, 41)
     og = orc.build_grid(op, s.protein_xyz, s.protein_type, center, size, s.spacing, s.lig_types)
-    assert np.all(np.abs(grid.data.cpu().numpy().astype(np.float64) - og.maps) <= tol(og.maps))
+    compare_grid(orc, op, s.protein_xyz, grid.data.cpu().numpy(), og, "noncubic")
     lig, oL = dk.LigandHandle(s.ligand), orc.Ligand(s.ligand)
     rng = np.random.default_rng(77)
     poses = random_poses(rng, 1500, np.array(center, np.float32), np.array(size, np.float32) * 1.3, lig.T)
@@ -699,3 +794,70 @@ def test_batched_grid_build_equals_single_builds(dk, torch):
         off = (g.data.numel() * 4 + 255) // 256 * 256                        # ... and the packed gather image behind them
         assert torch.equal(g.buf[off:], one.buf[off:])
     assert dk.dock_build_grids_batch(p, [], [], lt) == []
+
+
+# ----------------------------------------------------------------------------------- NEXT-4: sharded search, streams
+def test_sharded_search_equals_the_unsharded_run(dk, torch, tiny):
+    """NEXT-4 on one GPU: the shards of a 2- and 3-rank run are executed one after the other and merged
+    by the same host code the ranks use (paper_2303_09916_b200.shard): splitting COPIES (configs[4]-style: copy_base,
+    top-k re-run on the gathered copies) and splitting SYSTEMS (configs[3]-style: system_base) both give the unsharded
+    result bit for bit, top-k included."""
+    from paper_2303_09916_b200.shard import merge_shards, shard_range
+    systems = [make_system(0, seed=3, N=10 + 2 * i, T=1 + i) for i in range(3)]
+    sides = [gpu_side(dk, q) for q in systems]
+    p = sides[0][0]
+    grids, ligs, boxes = [x[2] for x in sides], [x[3] for x in sides], [x[1] for x in sides]
+    copies, steps, cap, seed = 50, 4, 30, 99
+    whole = dk.dock_search(p, grids, ligs, boxes, copies, steps, cap, seed)
+    keys = ("best_pose", "best_e", "topk_idx", "topk_e", "topk_count")
+
+    def topk_fn(s, poses, e):
+        w = 7 + ligs[s].T
+        idx, cnt = dk.dock_topk(p, ligs[s], poses[:, :w].contiguous(), e.contiguous())
+        return idx, cnt[0]
+
+    for world in (2, 3):
+        parts = []
+        for r in range(world):                                         # split the copies
+            b, e = shard_range(copies, r, world)
+            parts.append(dk.dock_search(p, grids, ligs, boxes, e - b, steps, cap, seed, want_topk=False, copy_base=b))
+        m = merge_shards("copies", parts, topk_fn, len(systems))
+        for k in keys:
+            assert torch.equal(m[k], whole[k]), ("copies", world, k)
+        parts = []
+        for r in range(world):                                         # split the systems
+            b, e = shard_range(len(systems), r, world)
+            q = dk.dock_search(p, grids[b:e], ligs[b:e], boxes[b:e], copies, steps, cap, seed, system_base=b)
+            t_here, t_all = q["best_pose"].shape[-1], whole["best_pose"].shape[-1]
+            if t_here < t_all:                                          # rows are 7 + T_max of the CALL wide: pad to the batch's
+                q["best_pose"] = torch.nn.functional.pad(q["best_pose"], (0, t_all - t_here))
+            parts.append(q)
+        m = merge_shards("systems", parts, topk_fn, len(systems))
+        for k in keys:
+            assert torch.equal(m[k], whole[k]), ("systems", world, k)
+
+
+def test_calls_on_two_streams_do_not_share_a_workspace(dk, torch, tiny, micro):
+    """The library stages tables in the caller's workspace and returns without synchronising; the binding therefore
+    keeps one workspace per stream.  A long search on stream A with a grid build and a scoring call enqueued on
+    stream B right behind it gives the serial results."""
+    s, (p, box, grid, lig), _ = tiny
+    s1, (p1, box1, grid1, lig1), _ = micro
+    ref_search = dk.dock_search(p, [grid], [lig], [box], 64, 10, 50, 7)
+    rng = np.random.default_rng(12)
+    poses = torch.from_numpy(random_poses(rng, 4096, s1.box_center, s1.box_size, lig1.T)).cuda()
+    ref_score = dk.dock_score_batch(p1, grid1, lig1, poses)
+    ref_grid = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types)
+    torch.cuda.synchronize()
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(sa):
+        ra = dk.dock_search(p, [grid], [lig], [box], 64, 10, 50, 7, stream=sa)
+    with torch.cuda.stream(sb):
+        gb = dk.dock_build_grids(p, s.protein_xyz, s.protein_type, box, s.lig_types, stream=sb)
+        rb = dk.dock_score_batch(p1, grid1, lig1, poses, stream=sb)
+    torch.cuda.synchronize()
+    assert torch.equal(ra["best_e"], ref_search["best_e"]) and torch.equal(ra["topk_idx"], ref_search["topk_idx"])
+    assert torch.equal(gb.data, ref_grid.data)
+    assert all(torch.equal(x, y) for x, y in zip(rb, ref_score))
+    from paper_2303_09916_b200 import binding
+    assert len({k for k in binding._ws.bufs if k[1] in (sa.cuda_stream, sb.cuda_stream)}) == 2

@@ -497,7 +497,7 @@ def test_exit_reasons_and_iteration_records(orc, tiny):
         x, H, fresh = pose.copy(), np.eye(nn), 1
         x[3:7] /= math.sqrt(x[3] * x[3] + x[4] * x[4] + x[5] * x[5] + x[6] * x[6])   # as quat_normalize does
         for k in range(len(recs)):
-            rk, xn, Hn = orc.bfgs_step_batch(p, g, L, x[None], H[None], [fresh])
+            rk, xn, Hn = orc.bfgs_step_batch(p, g, L, x[None], H[None], [fresh], grad=None if k % 2 else orc.evaluate(p, g, L, x)[2][None])
             for f in ("status", "trials", "updated", "reset", "f", "gp", "alpha", "f_new"):
                 assert rk[0][f] == recs[k][f], (k, f)
             x, H, fresh = xn[0], Hn[0], int(rk[0]["fresh_out"])
@@ -534,8 +534,18 @@ def test_local_optimisation_is_chaotic_at_fp32_resolution(orc):
     poses = random_poses(rng, 256, s.box_center, s.box_size * 0.6, L.T).astype(np.float64)
     a12 = oracle_self_agreement(orc, p, g, L, poses, 50, eps=1e-12)
     a32 = oracle_self_agreement(orc, p, g, L, poses, 50, eps=6e-8)
-    assert 0.02 < a32["agree"] < 0.6 and a12["agree"] < 0.85, (a12, a32)
+    ar = oracle_self_agreement(orc, p, g, L, poses, 50, drop_bits=0)    # evaluations correctly rounded to fp32
+    ar3 = oracle_self_agreement(orc, p, g, L, poses, 50, drop_bits=3)   # ... off by up to 4 ulp
+    for a in (a12, a32, ar, ar3):
+        for k in ("e0", "info0", "e1", "info1"):
+            a.pop(k, None)
+    assert 0.02 < a32["agree"] < 0.6 and a12["agree"] < 0.85 and 0.02 < ar["agree"] < 0.6, (a12, a32, ar, ar3)
+    assert 0.02 < ar3["agree"] <= ar["agree"] + 0.08, (ar, ar3)
     assert a32["agree"] <= a12["agree"] + 0.1
+    # the switch is off again: the plain run is reproduced bit for bit
+    e_a = orc.local_opt_batch(p, g, L, poses[:8], 50)[0]
+    assert np.array_equal(e_a, orc.local_opt_batch(p, g, L, poses[:8], 50)[0])
+    assert np.array_equal(e_a, np.array([orc.local_opt(p, g, L, poses[i], 50)[0] for i in range(8)]))
 
 
 # ----------------------------------------------------------------------------- O9 Monte Carlo

@@ -8,7 +8,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2303_09916_b200.shard import gather_candidates, max_over_ranks, shard_range
+from paper_2303_09916_b200.shard import dock_search_sharded, gather_candidates, max_over_ranks, merge_shards, shard_range
 
 
 def test_shard_ranges_partition_the_units():
@@ -29,6 +29,52 @@ def _free_port():
         return s.getsockname()[1]
 
 
+# ---- stand-ins for the CUDA calls (host logic only is under test here: who runs what, gather order, re-clustering) ----
+_NS, _NC, _ROW, _K = 5, 37, 11, 4
+
+
+def _fake_search(sb, se, cb, ce, want_topk):
+    """Deterministic function of the GLOBAL (system, copy) index, like a search whose Philox streams depend on them only."""
+    s_idx = torch.arange(sb, se, dtype=torch.float64)[:, None]
+    c_idx = torch.arange(cb, ce, dtype=torch.float64)[None, :]
+    e = torch.sin(12.9898 * s_idx + 78.233 * c_idx) * 43758.5453
+    e = e - torch.floor(e)                                             # pseudo-random in [0, 1)
+    pose = torch.stack([e * (k + 1) + s_idx for k in range(_ROW)], dim=-1)
+    out = dict(best_pose=pose, best_e=e)
+    if want_topk:
+        idx, cnt = zip(*[_fake_topk(s, pose[s - sb], e[s - sb]) for s in range(sb, se)])
+        out.update(topk_idx=torch.stack(idx), topk_count=torch.cat([c.reshape(1) for c in cnt]),
+                   topk_e=torch.stack([e[k][i.long()] for k, i in enumerate(idx)]))
+    return out
+
+
+def _fake_topk(system, poses, e):
+    """rank by energy (ties to the lower index), keep a pose iff its first coordinate is >= 0.05 from every kept one"""
+    order = torch.argsort(e, stable=True)
+    kept = []
+    for i in order.tolist():
+        if all(abs(float(poses[i, 0] - poses[j, 0])) >= 0.05 for j in kept):
+            kept.append(i)
+        if len(kept) == _K:
+            break
+    idx = torch.full((_K,), -1, dtype=torch.int32)
+    idx[: len(kept)] = torch.tensor(kept, dtype=torch.int32)
+    return idx, torch.tensor(len(kept), dtype=torch.int32)
+
+
+def test_merge_of_shards_equals_the_unsharded_run():
+    whole = _fake_search(0, _NS, 0, _NC, True)
+    for world in (1, 2, 3):
+        for mode, n_units in (("systems", _NS), ("copies", _NC)):
+            parts = []
+            for r in range(world):
+                b, e = shard_range(n_units, r, world)
+                parts.append(_fake_search(b, e, 0, _NC, True) if mode == "systems" else _fake_search(0, _NS, b, e, False))
+            m = merge_shards(mode, parts, _fake_topk, _NS)
+            for k in ("best_pose", "best_e", "topk_idx", "topk_e", "topk_count"):
+                assert torch.equal(m[k], whole[k]), (world, mode, k)
+
+
 def _worker(rank, world, port, out_dir):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -42,7 +88,8 @@ def _worker(rank, world, port, out_dir):
         loc = torch.argsort(energy_all[b:e], stable=True)[:k] + b          # this rank's k best
         ge, gp = gather_candidates(energy_all[loc], poses_all[loc])
         t = max_over_ranks(1.0 + rank)
-        torch.save({"e": ge, "p": gp, "t": t, "span": (b, e)}, os.path.join(out_dir, f"r{rank}.pt"))
+        sh = {m: dock_search_sharded(_fake_search, _fake_topk, _NS, _NC, m, rank, world) for m in ("systems", "copies")}
+        torch.save({"e": ge, "p": gp, "t": t, "span": (b, e), "sharded": sh}, os.path.join(out_dir, f"r{rank}.pt"))
     finally:
         dist.destroy_process_group()
 
@@ -60,3 +107,9 @@ def test_two_ranks_gloo(tmp_path):
     energy_all = np.sort(rng.normal(size=1001))
     assert np.isclose(float(e[0]), energy_all[0])
     assert r[0]["span"][1] == r[1]["span"][0]
+    # NEXT-4 end to end (host logic): both ranks hold the unsharded result, whether systems or copies were split
+    whole = _fake_search(0, _NS, 0, _NC, True)
+    for rank in range(world):
+        for mode in ("systems", "copies"):
+            for k in ("best_pose", "best_e", "topk_idx", "topk_e", "topk_count"):
+                assert torch.equal(r[rank]["sharded"][mode][k], whole[k]), (rank, mode, k)
