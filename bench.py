@@ -32,7 +32,9 @@ if ROOT not in sys.path:
 METRIC = "score+gradient pose evals/sec"
 UNIT = "evals/s"
 # FP32 ALU roof derived from the guide's unit counts and clocks:
-# 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (clocks.max.sm)
+# 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (clocks.max.sm).  The MEASURED roof (dock_probe_peaks: an FFMA
+# loop on the same GPU, same run) is printed beside it; MEASURED_PEAKS.json holds only HBM and tensor-core peaks,
+# neither of which bounds this path.
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
@@ -104,6 +106,12 @@ def _dist_setup(n_gpus: int):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     import torch
+    if world != n_gpus:
+        # the driver launches N > 1 through torch.distributed.run (one rank per GPU); a plain `python bench.py --gpus N`
+        # would silently measure one GPU, so it is refused
+        sys.stderr.write(f"bench.py: --gpus {n_gpus} but WORLD_SIZE={world}: launch with\n  python -m torch.distributed.run "
+                         f"--nnodes=1 --nproc-per-node {n_gpus} --master-addr 127.0.0.1 --master-port P bench.py --gpus {n_gpus} ...\n")
+        sys.exit(2)
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
@@ -111,7 +119,6 @@ def _dist_setup(n_gpus: int):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     else:
         torch.cuda.set_device(0)
-    assert world == n_gpus or world == 1, f"--gpus {n_gpus} but WORLD_SIZE={world}"
     return rank, world, local
 
 
@@ -162,8 +169,8 @@ def run_reference(args) -> dict:
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "configs[1] scoring microbench (bounded sample)", "n_poses": n, "N": oL.N, "T": oL.T,
-                   "P": oL.P, "grid": "81^3 x 8 fp64"},
+        "config": {"workload": "configs[1] scoring microbench", "n_poses_per_step": n, "N": oL.N, "T": oL.T,
+                   "P": oL.P, "grid": "81^3 x 8 fp64", "bounded_sample": n < poses.shape[0]},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -266,11 +273,54 @@ def run_ours(args) -> dict:
         "clocks": clocks,
         "wall_s_timed_region": wall,
     }
+    # measured roofs of the units this path is bound by (probe kernels in the library, same GPU, same run)
+    peaks = dk.dock_probe_peaks()
+
+    # ---- extras that shard over ranks (N > 1): the screening batch, systems [b, e) per rank, no exchange ----
+    extra = {}
+    if not args.no_search:
+        from paper_2303_09916_b200.shard import shard_range
+        n3 = args.screen_systems
+        b3, e3 = shard_range(n3, rank, world)
+        sy = [make_system(3, seed=0, index=i) for i in range(b3, e3)]
+        bx = [dk.make_box(q.box_center, q.box_size, q.spacing) for q in sy]
+        lg = [dk.LigandHandle(q.ligand) for q in sy]
+        pr = [(q.protein_xyz, q.protein_type) for q in sy]
+        gr = dk.dock_build_grids_batch(p, pr, bx, sy[0].lig_types)            # warm-up (module load, allocator)
+        torch.cuda.synchronize()
+        del gr
+        _barrier(world)
+        t0 = time.perf_counter()
+        gr = dk.dock_build_grids_batch(p, pr, bx, sy[0].lig_types)
+        torch.cuda.synchronize()
+        t_g3 = _max_over_ranks(time.perf_counter() - t0, world)
+        run3 = lambda: dk.dock_search(p, gr, lg, bx, 128, 40, 300, 2023, system_base=b3)
+        run3()
+        _barrier(world)
+        t0 = time.perf_counter()
+        r3 = run3()
+        torch.cuda.synchronize()
+        t_3 = _max_over_ranks(time.perf_counter() - t0, world)
+        ev3 = int(r3["evals"].sum())
+        if world > 1:
+            import torch.distributed as dist
+            tot = torch.tensor([ev3], dtype=torch.int64, device="cuda")
+            dist.all_reduce(tot)
+            ev3 = int(tot.item())
+        best3 = r3["topk_e"][:, 0].cpu().numpy()
+        extra["screening"] = {"workload": f"configs[3]: {n3} systems x 128 copies x 40 steps, BFGS<=300, ONE dock_build_grids_batch + ONE "
+                                          f"dock_search launch per rank ({world} rank(s), systems sharded, no exchange)",
+                              "systems": n3, "search_s": t_3, "grid_build_s": t_g3, "evals": ev3, "evals_per_s": ev3 / t_3,
+                              "systems_per_s_search_only": n3 / t_3, "systems_per_s": n3 / (t_3 + t_g3),
+                              "grid_bytes_resident": int(sum(g.buf.numel() for g in gr)) * world,
+                              "best_e_median_rank0": float(np.median(best3)), "best_e_negative_frac_rank0": float((best3 < 0).mean())}
+        sys3_keep = sy[:2]
+        del gr, r3
     if rank != 0:
         return {}
 
     # roofline of the dominant kernel (score kernel = the whole step)
-    from oracle import oracle as O          # cpu_baseline leg + in-range pair statistics for the flop count
+    from oracle import oracle as O          # cpu_baseline leg + in-range pair statistics / operation count for the flop figure
     O.build()
     op = O.params_as_fp32(O.default_params())
     og = O.build_grid(op, s.protein_xyz, s.protein_type, s.box_center, s.box_size, s.spacing, s.lig_types)
@@ -283,11 +333,25 @@ def run_ours(args) -> dict:
     t_cpu = time.perf_counter() - t0
     p_in = float(diag["pairs_in_range"].mean())
     flops = algorithmic_flops(lig.N, lig.T, p_in, lig.P - p_in)
-    achieved = flops * n / (float(np.mean(ts)) / 1e3) / 1e12
+    counted = O.count_eval_ops(op, og, oL, p64[:2048])                    # the oracle's own statements, operation by operation
+    t_kernel = float(np.mean(ts)) / 1e3
+    achieved = flops * n / t_kernel / 1e12
+    peak_meas = max(peaks["ffma_tflops"], peaks["ffma2_tflops"])
     line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                         "frac": achieved / ALU_PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
-                        "kernel": "score_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
-                        "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+                        "kernel": "score_thread_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
+                        "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                        "peak_measured": peak_meas, "frac_of_measured": achieved / peak_meas,
+                        "peak_measured_source": "dock_probe_peaks: FFMA / FFMA2 loops, 8 independent chains per thread, this run",
+                        "probes": peaks,
+                        "flops_per_eval_opcounted": counted["total"], "opcount": counted,
+                        "achieved_opcounted": counted["total"] * n / t_kernel / 1e12,
+                        "frac_opcounted": counted["total"] * n / t_kernel / 1e12 / ALU_PEAK_TFLOPS,
+                        "flops_note": "frac uses SURVEY.md 8(d)'s formula (93 N + 130 T + 62 P_in + 8 P_out + 50); the *_opcounted "
+                                      "figures count every add/mul/div/compare/sqrt/exp of the unoptimised oracle (oracle/opcount.hpp) "
+                                      "and are reported for reference",
+                        "mufu_frac": (3.0 * p_in + 2.0 * lig.T + 2.0) * n / t_kernel / 1e12 / peaks["mufu_tops"],
+                        "gather_frac": lig.N * n / t_kernel / 1e12 / peaks["gather32_tlanes"]}
     line["cpu_baseline"] = {"value": ns / t_cpu, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
                             "sample": f"first {ns} poses of the same batch, fp64, OpenMP over poses"}
     # spot parity inside the bench run: what is timed is what is correct
@@ -296,8 +360,19 @@ def run_ours(args) -> dict:
     err = np.abs(ge - oe) / (1e-3 + 1e-4 * np.abs(oe))
     line["parity_in_bench"] = {"poses": int(safe.sum()), "max_err_tol_units": float(err[safe].max())}
 
+    def oracle_search_rate(q, n_copies, steps, cap, system=0):
+        """The oracle's own search on the first n_copies copies (copies are independent): evaluations/s on the host cores."""
+        qp = O.params_as_fp32(O.default_params())
+        qg = O.build_grid(qp, q.protein_xyz, q.protein_type, q.box_center, q.box_size, q.spacing, q.lig_types)
+        qL = O.Ligand(q.ligand)
+        init = O.init_poses(q.box_center, q.box_size, qL.T, 2023, system, n_copies)
+        t0 = time.perf_counter()
+        r = O.search(qp, qg, qL, init, steps, cap, 2023, system)
+        dt = time.perf_counter() - t0
+        return r["evals"], dt
+
     # extras: A1 and A6-A8 next to the headline
-    extra = {"grid_build_ms": float(np.median(t_grid)), "grid_nodes": int(np.prod(grid.dims)) * len(s.lig_types)}
+    extra.update({"grid_build_ms": float(np.median(t_grid)), "grid_nodes": int(np.prod(grid.dims)) * len(s.lig_types)})
     if not args.no_search:
         s2 = make_system(2, seed=0)
         box2 = dk.make_box(s2.box_center, s2.box_size, s2.spacing)
@@ -314,10 +389,13 @@ def run_ours(args) -> dict:
         r_h = dk.dock_system_host(p, s2.protein_xyz, s2.protein_type, box2, lig2, s2.lig_types, s2.copies, s2.steps,
                                   s2.bfgs_cap, 2023)
         t_h = time.perf_counter() - t0
+        oev, odt = oracle_search_rate(s2, s2.copies, s2.steps, s2.bfgs_cap)
         extra["site_docking"] = {"workload": "configs[2]: 384 copies x 40 steps, BFGS<=300", "search_s": t_s,
                                  "evals": int(res["evals"][0]), "evals_per_s": int(res["evals"][0]) / t_s,
                                  "systems_per_s_search_only": 1.0 / t_s, "end_to_end_host_s": t_h,
                                  "systems_per_s_end_to_end": 1.0 / t_h, "best_e": float(res["topk_e"][0, 0]),
+                                 "cpu_baseline": {"kind": "oracle", "cores": O.num_threads(), "sample": "all 384 copies x 40 steps (grid build not included)",
+                                                  "search_s": odt, "evals": oev, "evals_per_s": oev / odt, "systems_per_s": 1.0 / odt},
                                  "paper_context": "DSDP 384x40 redocking 0.55 s/system on RTX 2080 SUPER (PAPER.md:108)"}
         # the same site docking driven by the paper's Barzilai-Borwein optimizer (NEXT-1), 150 iterations
         pb = dk.dock_default_params()
@@ -332,45 +410,42 @@ def run_ours(args) -> dict:
         extra["site_docking_bb"] = {"workload": "configs[2] with the Barzilai-Borwein optimizer, <=150 iterations", "search_s": t_b,
                                     "evals": int(rb["evals"][0]), "evals_per_s": int(rb["evals"][0]) / t_b,
                                     "systems_per_s_search_only": 1.0 / t_b, "best_e": float(rb["topk_e"][0, 0])}
-        # configs[3] slice: 32 of the 256 screening systems in one launch (systems are independent units)
-        ns = 32
-        sy = [make_system(3, seed=0, index=i) for i in range(ns)]
-        bx = [dk.make_box(q.box_center, q.box_size, q.spacing) for q in sy]
-        lg = [dk.LigandHandle(q.ligand) for q in sy]
-        t0 = time.perf_counter()
-        gr = dk.dock_build_grids_batch(p, [(q.protein_xyz, q.protein_type) for q in sy], bx, sy[0].lig_types)
-        torch.cuda.synchronize()
-        t_g3 = time.perf_counter() - t0
-        run3 = lambda: dk.dock_search(p, gr, lg, bx, 128, 40, 300, 2023)
-        run3()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        r3 = run3()
-        torch.cuda.synchronize()
-        t_3 = time.perf_counter() - t0
-        ev3 = int(r3["evals"].sum())
-        extra["screening"] = {"workload": f"configs[3] slice: {ns} of 256 systems x 128 copies x 40 steps, BFGS<=300",
-                              "search_s": t_3, "grid_build_s": t_g3, "evals": ev3, "evals_per_s": ev3 / t_3,
-                              "systems_per_s_search_only": ns / t_3, "systems_per_s_with_grids": ns / (t_3 + t_g3)}
-        del gr
+        # configs[3] oracle baseline: the first two systems of the batch, 32 copies x 40 steps each
+        oev = odt = 0.0
+        for i, q in enumerate(sys3_keep):
+            a, b_ = oracle_search_rate(q, 32, 40, 300, system=i)
+            oev += a
+            odt += b_
+        extra["screening"]["cpu_baseline"] = {"kind": "oracle", "cores": O.num_threads(),
+                                              "sample": f"first {len(sys3_keep)} systems, 32 of 128 copies x 40 steps each (grid build not included)",
+                                              "search_s": odt, "evals": int(oev), "evals_per_s": oev / odt,
+                                              "systems_per_s_scaled": len(sys3_keep) / (odt * 128 / 32)}
         # configs[4]: large blind box, 161^3 x 8 maps (1.07 GB gather image), 2048 copies x 80 steps, N = 60, T = 15
         s4 = make_system(4, seed=0)
         box4 = dk.make_box(s4.box_center, s4.box_size, s4.spacing)
         lig4 = dk.LigandHandle(s4.ligand)
+        grid4 = dk.dock_build_grids(p, s4.protein_xyz, s4.protein_type, box4, s4.lig_types)   # warm-up
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         grid4 = dk.dock_build_grids(p, s4.protein_xyz, s4.protein_type, box4, s4.lig_types)
         torch.cuda.synchronize()
         t_g4 = time.perf_counter() - t0
         run4 = lambda: dk.dock_search(p, [grid4], [lig4], [box4], s4.copies, s4.steps, s4.bfgs_cap, 2023)
+        dk.dock_search(p, [grid4], [lig4], [box4], 64, 1, 10, 2023)                             # warm-up: module load, smem attribute
+        torch.cuda.synchronize()
         t0 = time.perf_counter()
         r4 = run4()
         torch.cuda.synchronize()
         t_4 = time.perf_counter() - t0
+        oev, odt = oracle_search_rate(s4, 32, s4.steps, s4.bfgs_cap)
         extra["large_blind_box"] = {"workload": "configs[4]: 8000 atoms, 161^3 x 8 maps, 2048 copies x 80 steps, BFGS<=300",
                                     "search_s": t_4, "grid_build_s": t_g4, "evals": int(r4["evals"][0]),
                                     "evals_per_s": int(r4["evals"][0]) / t_4, "systems_per_s_with_grid": 1.0 / (t_4 + t_g4),
-                                    "best_e": float(r4["topk_e"][0, 0])}
+                                    "best_e": float(r4["topk_e"][0, 0]),
+                                    "cpu_baseline": {"kind": "oracle", "cores": O.num_threads(),
+                                                     "sample": "first 32 of 2048 copies x 80 steps (grid build not included)",
+                                                     "search_s": odt, "evals": oev, "evals_per_s": oev / odt,
+                                                     "systems_per_s_scaled": 1.0 / (odt * 2048 / 32)}}
         del grid4
     line["extra"] = extra
     return line
@@ -390,6 +465,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1048576, help="poses the CPU oracle scores per step")
     ap.add_argument("--no-flush", action="store_true")
     ap.add_argument("--no-search", action="store_true")
+    ap.add_argument("--screen-systems", type=int, default=256, help="systems of the configs[3] screening batch (256 = the config)")
     args = ap.parse_args()
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) != 0:

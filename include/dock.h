@@ -266,6 +266,14 @@ int dock_system_host(const dock_params *params, const dock_protein *protein, con
                      uint64_t *out_evals_host,
                      float *grid_dev, size_t grid_bytes, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
+/* ---- measured roofs --------------------------------------------------
+ * Runs four micro-kernels on `stream` (synchronising it) and writes to out_host[4]:
+ *   [0] FP32 FMA rate, scalar FFMA, TFLOP/s       [1] the same with packed fp32x2 FMAs (FFMA2), TFLOP/s
+ *   [2] MUFU (ex2) rate, T operations/s           [3] fully divergent 32-byte gathers from an L2-resident table, T lanes/s
+ * These are the denominators of bench.py's roofline (nothing on this path is bound by HBM or the tensor cores, the two
+ * peaks MEASURED_PEAKS.json holds).  ws_dev: 32-byte aligned, *needed bytes (about 16 MB). */
+int dock_probe_peaks(float *out_host, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
 /* ---- diagnostics ------------------------------------------------------------------------------ */
 int         dock_last_cuda_error(void);          /* cudaError_t of the last failing CUDA call (0 = none) */
 const char *dock_version(void);

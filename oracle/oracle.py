@@ -31,6 +31,43 @@ def build(force: bool = False) -> str:
     return _SO
 
 
+_SO_COUNT = os.path.join(_HERE, "liboracle_count.so")
+_lib_count = None
+OP_KINDS = ("add_sub", "mul", "div", "compare", "sqrt", "exp", "sin_cos", "floor_abs_min")
+
+
+def build_counted(force: bool = False) -> str:
+    """Compile dock_oracle.c, unchanged, with the operation-counting scalar of opcount.hpp in place of double."""
+    srcs = [_SRC, _HDR, os.path.join(_HERE, "opcount.hpp"), os.path.join(_HERE, "dock_oracle_count.cpp")]
+    if not force and os.path.exists(_SO_COUNT) and os.path.getmtime(_SO_COUNT) >= max(os.path.getmtime(f) for f in srcs):
+        return _SO_COUNT
+    subprocess.check_call(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-w",
+                           "-o", _SO_COUNT, srcs[3], "-lm"], cwd=_HERE)
+    return _SO_COUNT
+
+
+def count_eval_ops(p, g, L, poses, want_grad: bool = True) -> dict:
+    """Mean floating-point operations of ONE score(+gradient) evaluation over `poses`, counted on the oracle's own
+    statements (one per add/sub, mul, div, compare, sqrt, exp, sin/cos, floor/fabs/fmin; nothing fused).  Single-threaded."""
+    global _lib_count
+    if _lib_count is None:
+        _lib_count = C.CDLL(build_counted())
+        _lib_count.orc_eval.restype = C.c_double
+    poses = _f64(poses).reshape(-1, 7 + L.T)
+    terms = np.zeros(3)
+    grad = np.zeros(6 + L.T)
+    _lib_count.orc_count_reset()
+    for k in range(poses.shape[0]):
+        row = np.ascontiguousarray(poses[k])
+        _lib_count.orc_eval(C.byref(p), C.byref(g.c), C.byref(L.c), _p(row), _p(terms), _p(grad) if want_grad else None, None)
+    out = (C.c_uint64 * len(OP_KINDS))()
+    _lib_count.orc_count_get(out)
+    n = max(1, poses.shape[0])
+    per = {k: out[i] / n for i, k in enumerate(OP_KINDS)}
+    per["total"] = float(sum(per.values()))
+    return per
+
+
 class Params(C.Structure):
     _fields_ = [
         ("n_types", C.c_int),

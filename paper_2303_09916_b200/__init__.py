@@ -25,6 +25,7 @@ from .binding import (  # noqa: F401
     dock_ligand,
     dock_local_opt_batch,
     dock_params,
+    dock_probe_peaks,
     dock_score_batch,
     dock_score_batch_host,
     dock_search,

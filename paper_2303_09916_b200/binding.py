@@ -26,7 +26,8 @@ DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
 EXPORTS = [
     "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_build_grids_batch", "dock_score_batch",
     "dock_score_batch_host", "dock_local_opt_batch", "dock_local_opt_trace", "dock_init_poses", "dock_init_poses_site",
-    "dock_search", "dock_topk", "dock_system_host", "dock_last_cuda_error", "dock_version", "dock_launch_count",
+    "dock_search", "dock_topk", "dock_system_host", "dock_probe_peaks", "dock_last_cuda_error", "dock_version",
+    "dock_launch_count",
 ]
 
 
@@ -442,6 +443,19 @@ def dock_topk(params: dock_params, ligand: LigandHandle, poses, e, stream=None):
     _check(lib.dock_topk(C.byref(params), C.byref(ligand.c), n, _ptr(poses), _ptr(e), _ptr(out_idx), _ptr(out_cnt),
                          _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_topk")
     return out_idx, out_cnt
+
+
+def dock_probe_peaks(stream=None) -> dict:
+    """Measured roofs of the units this path is bound by (dock.h): FP32 FMA, packed FMA, MUFU, divergent 32-byte gathers."""
+    lib = load_library()
+    need = C.c_size_t(0)
+    out = (C.c_float * 4)()
+    rc = lib.dock_probe_peaks(out, None, C.c_size_t(0), C.byref(need), None)
+    if rc != DOCK_EWORKSPACE:
+        _check(rc, "dock_probe_peaks(size query)")
+    ws = _ws.get(need.value, stream)
+    _check(lib.dock_probe_peaks(out, _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_probe_peaks")
+    return dict(ffma_tflops=float(out[0]), ffma2_tflops=float(out[1]), mufu_tops=float(out[2]), gather32_tlanes=float(out[3]))
 
 
 def dock_system_host(params: dock_params, protein_xyz, protein_type, box: dock_box, ligand: LigandHandle,
