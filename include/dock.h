@@ -72,6 +72,11 @@ typedef struct dock_params {
     int32_t grad_mode;                        /* grid gradient: 0 = gradient of the interpolant (eq. 3), 1 = interpolated
                                                * per-vertex gradients (eq. 4; NEXT-2).  Read by dock_build_grids,
                                                * which then writes 4 channels per map; the evaluators follow dock_grid.n_channels */
+    int32_t search_kernel;                    /* decomposition of dock_search / dock_local_opt_*: 1 = one warp per copy; 2 = one CTA of
+                                               * 4 warps per copy whose warps evaluate 4 consecutive backtracking trials of the line
+                                               * search at once (the latency form for a few hundred copies);
+                                               * 0 = chosen by the library from n_systems x copies.  Both give bit-identical results;
+                                               * only evaluations the sequential line search would make are counted */
 } dock_params;
 
 /* Search / interpolation box: n_axis = round(size/spacing)+1 nodes,

@@ -49,6 +49,7 @@ class dock_params(C.Structure):
         ("bfgs_gtol", C.c_float), ("bfgs_curv_eps", C.c_float),
         ("cluster_rmsd", C.c_float), ("topk", C.c_int32),
         ("optimizer", C.c_int32), ("bb_step", C.c_float), ("bb_fallback", C.c_float), ("grad_mode", C.c_int32),
+        ("search_kernel", C.c_int32),
     ]
 
 

@@ -94,6 +94,8 @@ __device__ __forceinline__ void set_identity(float *H, int n, float diag)
     __syncwarp();
 }
 
+#include "search_cta.cuh"
+
 // O8: BFGS with backtracking.  b.x holds the start pose (quaternion normalised here) and the result.
 // Written as one loop around a SINGLE evaluation site (the start pose is "trial" INIT), so that the evaluator and
 // this routine inline into the kernels once: the compiler then sees that every buffer is shared memory and keeps
@@ -421,6 +423,115 @@ search_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems,
     }
 }
 
+// ---- the same two kernels with one CTA of CTA_WARPS warps per pose / copy: speculative line search (search_cta.cuh) ----
+template <bool EQ4, bool VEC4, bool TRACE>
+__global__ void __launch_bounds__(CTA_THREADS, 3)
+local_opt_cta_kernel(DevParams P, DevGrid G, DevLigand L, long long n_poses, int cap,
+                     const float *__restrict__ poses, float *__restrict__ out_pose, float *__restrict__ out_e,
+                     int *__restrict__ out_iters, float *__restrict__ itrace, int itrace_cap)
+{
+    extern __shared__ float smem[];
+    const long long p = blockIdx.x;
+    const int tid = threadIdx.x, np_ = 7 + L.T;
+    const SpecBuf b = spec_carve(smem, L.T, L.n_pad);
+    if (tid < np_) b.x[tid] = poses[p * np_ + tid];
+    __syncthreads();
+    int iters, evals, why;
+    const size_t istride = DOCK_ITER_HEADER + np_ + (size_t)(6 + L.T) * (7 + L.T);
+    const float e = local_opt_spec<EQ4, VEC4, TRACE>(P, G, L, b, cap, iters, evals, why,
+                                                     TRACE ? itrace + (size_t)p * itrace_cap * istride : nullptr, itrace_cap);
+    if (tid < np_) out_pose[p * np_ + tid] = b.x[tid];
+    if (tid == 0) {
+        out_e[p] = e;
+        if (out_iters) { out_iters[3 * p] = iters; out_iters[3 * p + 1] = evals; out_iters[3 * p + 2] = why; }
+    }
+}
+
+// 3 CTAs per SM (<= 168 registers): 444 copies resident on 148 SMs, so the paper's 384 copies run in one wave
+template <bool EQ4, bool VEC4>
+__global__ void __launch_bounds__(CTA_THREADS, 3)
+search_cta_kernel(DevParams P, const DevSystem *__restrict__ systems, int n_systems, int copies, int steps,
+                  int cap, uint32_t seed_lo, uint32_t seed_hi, uint32_t sys_base, uint32_t copy_base, int t_max,
+                  const float *__restrict__ init, float *__restrict__ best_pose, float *__restrict__ best_e,
+                  float *__restrict__ trace, unsigned long long *__restrict__ eval_counter)
+{
+    extern __shared__ float smem[];
+    const int tid = threadIdx.x;
+    const long long gw = blockIdx.x;
+    const uint32_t sys = (uint32_t)(gw / copies);
+    const uint32_t copy = copy_base + (uint32_t)(gw % copies), psys = sys_base + sys;
+    const DevGrid G = systems[sys].grid;
+    const DevLigand L = systems[sys].lig;
+    const int T = L.T, np_ = 7 + T, row = 7 + t_max;
+    float *cur = smem, *best = smem + pad4(row);
+    const SpecBuf b = spec_carve(smem + 2 * pad4(row), T, L.n_pad);
+
+    int iters, evals, why;
+    unsigned long long total_evals = 0;
+    float e_cur = 0.0f, e_best = 0.0f;
+    for (int step = -1; step < steps; ++step) {
+        uint32_t r[4] = {0u, 0u, 0u, 0u};
+        int kind = 0;
+        if (step < 0) {
+            if (tid < np_) b.x[tid] = init[gw * row + tid];
+            __syncthreads();
+        } else {
+            philox4x32_10(copy, (uint32_t)step, 0u, psys, seed_lo, seed_hi, r);
+            const uint32_t K = T > 0 ? 3u : 2u;
+            kind = (int)__umulhi(r[0], K);
+            if (tid < np_) b.x[tid] = cur[tid];
+            __syncthreads();
+            if (tid == 0) {
+                if (kind == 0) {
+                    for (int c = 0; c < 3; ++c) b.x[c] = cur[c] + P.amp_trans * (2.0f * u24(r[1 + c]) - 1.0f);
+                } else if (kind == 1) {
+                    rotate_quat(P.amp_rot * (2.0f * u24(r[1]) - 1.0f), P.amp_rot * (2.0f * u24(r[2]) - 1.0f),
+                                P.amp_rot * (2.0f * u24(r[3]) - 1.0f), cur + 3, b.x + 3);
+                } else {
+                    const int k = (int)__umulhi(r[1], (uint32_t)T);
+                    b.x[7 + k] = PI_F * (2.0f * u24(r[2]) - 1.0f);
+                }
+            }
+            __syncthreads();
+        }
+        const float e_c = local_opt_spec<EQ4, VEC4, false>(P, G, L, b, cap, iters, evals, why);
+        total_evals += evals;
+        if (step < 0) {
+            e_cur = e_best = e_c;
+            if (tid < np_) { cur[tid] = b.x[tid]; best[tid] = b.x[tid]; }
+            __syncthreads();
+            continue;
+        }
+        uint32_t ra[4];
+        philox4x32_10(copy, (uint32_t)step, 1u, psys, seed_lo, seed_hi, ra);
+        const float u = u24(ra[0]);
+        const bool accept = (e_c < e_cur) || ((double)u < exp(((double)e_cur - (double)e_c) / (double)P.t_mc));
+        if (trace) {
+            float *rec = trace + ((size_t)gw * steps + step) * (size_t)(DOCK_TRACE_HEADER + row);
+            if (tid == 0) {
+                rec[0] = e_cur; rec[1] = e_c; rec[2] = u; rec[3] = accept ? 1.0f : 0.0f;
+                rec[4] = (float)iters; rec[5] = (float)evals; rec[6] = (float)kind; rec[7] = 0.0f;
+            }
+            if (tid < row) rec[DOCK_TRACE_HEADER + tid] = tid < np_ ? cur[tid] : 0.0f;
+        }
+        __syncthreads();
+        if (accept) {
+            if (tid < np_) cur[tid] = b.x[tid];
+            e_cur = e_c;
+        }
+        if (e_cur < e_best) {
+            e_best = e_cur;
+            if (tid < np_) best[tid] = accept ? b.x[tid] : cur[tid];
+        }
+        __syncthreads();
+    }
+    if (tid < row) best_pose[gw * row + tid] = tid < np_ ? best[tid] : 0.0f;
+    if (tid == 0) {
+        best_e[gw] = e_best;
+        if (eval_counter) atomicAdd(eval_counter, total_evals);
+    }
+}
+
 // ---- A8 top-k + greedy RMSD clustering -------------------------------------------------------------
 // One CTA per system.  Bitonic sort of (E, copy) ascending with ties to the lower copy index, then
 // warp 0 walks the ranking and keeps a pose iff its heavy-atom RMSD to every kept pose is >= rmsd_min.
@@ -596,6 +707,17 @@ extern "C" int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t see
 }
 
 namespace {
+// dock_params.search_kernel: 1 = warp per copy, 2 = CTA of 4 warps per copy with the speculative line search, 0 = by size.
+// Four warps per copy pay while the launch cannot fill the GPU with one warp per copy: up to CTA_AUTO_MAX copies in total
+// (measured, profiles/r2c.md).  The two kernels give bit-identical results.
+constexpr long long CTA_AUTO_MAX = 512;
+bool use_cta_kernel(const dock_params *p, long long total_copies)
+{
+    if (p->search_kernel == 2) return true;
+    if (p->search_kernel == 1) return false;
+    return p->optimizer == 0 && total_copies <= CTA_AUTO_MAX;       // Barzilai-Borwein has no line search to speculate on
+}
+
 int local_opt_launch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
                      int64_t n_poses, int32_t max_iters, const float *poses_dev,
                      float *out_pose_dev, float *out_e_dev, int32_t *out_iters_dev,
@@ -615,11 +737,28 @@ int local_opt_launch(const dock_params *params, const dock_grid *grid, const doc
     cudaStream_t stream = (cudaStream_t)stream_;
     DOCK_CUDA_CHECK(cudaMemcpyAsync(ws_dev, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, stream));
     const DevLigand L = dock_relocate_ligand(blob, (const unsigned char *)ws_dev);
+    const bool eq4 = G.channels == 4, tr = iter_trace_dev != nullptr;
+    if (use_cta_kernel(params, n_poses)) {
+        const size_t smem_c = (size_t)spec_floats(L.T, L.n_pad) * sizeof(float);
+        if (smem_c > 200 * 1024) return DOCK_EINVAL;
+        if (n_poses > 0x7fffffffLL) return DOCK_EINVAL;
+        const bool v4 = L.N <= 48;
+        auto kc = tr ? (eq4 ? (v4 ? local_opt_cta_kernel<true, true, true> : local_opt_cta_kernel<true, false, true>)
+                            : (v4 ? local_opt_cta_kernel<false, true, true> : local_opt_cta_kernel<false, false, true>))
+                     : (eq4 ? (v4 ? local_opt_cta_kernel<true, true, false> : local_opt_cta_kernel<true, false, false>)
+                            : (v4 ? local_opt_cta_kernel<false, true, false> : local_opt_cta_kernel<false, false, false>));
+        if (smem_c > 48 * 1024)
+            DOCK_CUDA_CHECK(cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
+        kc<<<(unsigned)n_poses, CTA_THREADS, smem_c, stream>>>(P, G, L, n_poses, max_iters, poses_dev, out_pose_dev, out_e_dev,
+                                                              out_iters_dev, iter_trace_dev, trace_cap);
+        DOCK_LAUNCH_CHECK();
+        return DOCK_OK;
+    }
     const int warp_floats = opt_floats(L.T, L.n_pad);
     const size_t smem = (size_t)SEARCH_WARPS * warp_floats * sizeof(float);
     if (smem > 200 * 1024) return DOCK_EINVAL;
     // shared-memory layout of the evaluator (eval_warp.cuh): float4 per atom unless the ligand is large
-    const bool vec4 = L.N <= 48, eq4 = G.channels == 4, tr = iter_trace_dev != nullptr;
+    const bool vec4 = L.N <= 48;
     auto kern = tr ? (eq4 ? (vec4 ? local_opt_kernel<true, true, true> : local_opt_kernel<true, false, true>)
                           : (vec4 ? local_opt_kernel<false, true, true> : local_opt_kernel<false, false, true>))
                    : (eq4 ? (vec4 ? local_opt_kernel<true, true, false> : local_opt_kernel<true, false, false>)
@@ -688,7 +827,14 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
     if (want_topk && (!topk_idx_dev || !topk_count_dev)) return DOCK_EINVAL;
     for (int s2 = 1; s2 < n_systems; ++s2)
         if (sys[s2].grid.channels != sys[0].grid.channels) return DOCK_EINVAL;      // one gradient mode per launch
-    const size_t smem = (size_t)SEARCH_WARPS * wf_max * sizeof(float);
+    const bool cta = use_cta_kernel(params, (long long)n_systems * copies);
+    size_t smem = (size_t)SEARCH_WARPS * wf_max * sizeof(float);
+    if (cta) {
+        int cf_max = 0;
+        for (int s2 = 0; s2 < n_systems; ++s2)
+            cf_max = std::max(cf_max, 2 * pad4(row) + spec_floats(ligands[s2].T, blobs[s2].rel.n_pad));
+        smem = (size_t)cf_max * sizeof(float);
+    }
     if (smem > 200 * 1024) return DOCK_EINVAL;
     if (want_topk) {
         std::vector<DevLigand> rel(n_systems);
@@ -732,19 +878,31 @@ extern "C" int dock_search(const dock_params *params, int32_t n_systems,
         DOCK_CUDA_CHECK(cudaMemcpyAsync(d, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, stream));
         init = d;
     }
+    const long long total = (long long)n_systems * copies;
+    if (total > 0x7fffffffLL) return DOCK_EINVAL;
     int n_max = 0;
     for (int s2 = 0; s2 < n_systems; ++s2) n_max = std::max(n_max, (int)ligands[s2].N);
     const bool vec4 = n_max <= 48;        // float4 per atom unless the ligands are large (eval_warp.cuh)
-    auto kern = sys[0].grid.channels == 4 ? (vec4 ? search_kernel<true, true> : search_kernel<true, false>)
-                                          : (vec4 ? search_kernel<false, true> : search_kernel<false, false>);
-    if (smem > 48 * 1024)
-        DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const long long total = (long long)n_systems * copies;
-    const unsigned blocks = (unsigned)((total + SEARCH_WARPS - 1) / SEARCH_WARPS);
-    kern<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(
-        P, sys_dev, n_systems, copies, steps, bfgs_max_iters, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
-        system_base, copy_base, t_max, wf_max, init, best_pose_dev, best_e_dev, trace_dev, (unsigned long long *)eval_counter_dev);
-    DOCK_LAUNCH_CHECK();
+    if (cta) {
+        auto kc = sys[0].grid.channels == 4 ? (vec4 ? search_cta_kernel<true, true> : search_cta_kernel<true, false>)
+                                            : (vec4 ? search_cta_kernel<false, true> : search_cta_kernel<false, false>);
+        if (smem > 48 * 1024)
+            DOCK_CUDA_CHECK(cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kc<<<(unsigned)total, CTA_THREADS, smem, stream>>>(
+            P, sys_dev, n_systems, copies, steps, bfgs_max_iters, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+            system_base, copy_base, t_max, init, best_pose_dev, best_e_dev, trace_dev, (unsigned long long *)eval_counter_dev);
+        DOCK_LAUNCH_CHECK();
+    } else {
+        auto kern = sys[0].grid.channels == 4 ? (vec4 ? search_kernel<true, true> : search_kernel<true, false>)
+                                              : (vec4 ? search_kernel<false, true> : search_kernel<false, false>);
+        if (smem > 48 * 1024)
+            DOCK_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        const unsigned blocks = (unsigned)((total + SEARCH_WARPS - 1) / SEARCH_WARPS);
+        kern<<<blocks, SEARCH_WARPS * 32, smem, stream>>>(
+            P, sys_dev, n_systems, copies, steps, bfgs_max_iters, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+            system_base, copy_base, t_max, wf_max, init, best_pose_dev, best_e_dev, trace_dev, (unsigned long long *)eval_counter_dev);
+        DOCK_LAUNCH_CHECK();
+    }
     if (want_topk)
         return launch_topk(sys_dev, n_systems, ligs.data(), copies, row, params->topk, params->cluster_rmsd,
                            best_pose_dev, best_e_dev, topk_idx_dev, topk_count_dev, topk_pose_dev, topk_e_dev, stream);

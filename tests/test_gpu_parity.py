@@ -861,3 +861,27 @@ def test_calls_on_two_streams_do_not_share_a_workspace(dk, torch, tiny, micro):
     assert all(torch.equal(x, y) for x, y in zip(rb, ref_score))
     from paper_2303_09916_b200 import binding
     assert len({k for k in binding._ws.bufs if k[1] in (sa.cuda_stream, sb.cuda_stream)}) == 2
+
+
+def test_search_kernels_agree_bitwise(dk, torch, tiny):
+    """dock_params.search_kernel: the CTA kernel (four warps per copy evaluating four backtracking trials of the line
+    search at once, search_cta.cuh) returns bit for bit what the warp-per-copy kernel returns -- poses, energies, trace,
+    evaluation counts, per-iteration optimizer trace -- for BFGS and for Barzilai-Borwein, on the tiny and the paper-shaped
+    system."""
+    for s, copies, steps, cap in ((tiny[0], 16, 20, 50), (make_system(2, seed=0), 48, 6, 300)):
+        _, box, grid, lig = gpu_side(dk, s)
+        for opt in (0, 1):
+            out = []
+            for k in (1, 2):
+                p = dk.dock_default_params()
+                p.optimizer, p.search_kernel = opt, k
+                r = dk.dock_search(p, [grid], [lig], [box], copies, steps, 150 if opt else cap, 77, want_trace=True)
+                rng = np.random.default_rng(5)
+                poses = torch.from_numpy(random_poses(rng, 40, s.box_center, s.box_size * 0.6, lig.T)).cuda()
+                lo = dk.dock_local_opt_batch(p, grid, lig, poses, 60, trace_cap=61)
+                out.append((r, lo))
+            (ra, la), (rb, lb) = out
+            for key in ("best_pose", "best_e", "topk_idx", "topk_e", "trace", "evals"):
+                assert torch.equal(ra[key], rb[key]), (opt, key)
+            for a, b in zip(la, lb):
+                assert torch.equal(a, b), opt
