@@ -77,6 +77,11 @@ typedef struct dock_params {
                                                * search at once (the latency form for a few hundred copies);
                                                * 0 = chosen by the library from n_systems x copies.  Both give bit-identical results;
                                                * only evaluations the sequential line search would make are counted */
+    int32_t score_kernel;                     /* dock_score_batch[_host]: 0 or 1 = the generic thread-per-pose kernel; 2 = a kernel specialised
+                                               * for this ligand, generated and compiled at run time (NVRTC, 0.4-6 s per ligand, cached per
+                                               * device / ligand / parameters): DOCK_ECUDA if the compiler is missing, DOCK_EINVAL above 40
+                                               * atoms or with eq. 4 maps.  Same arithmetic per pair / atom / torsion; sums are taken in a
+                                               * different order */
 } dock_params;
 
 /* Search / interpolation box: n_axis = round(size/spacing)+1 nodes,
@@ -280,6 +285,16 @@ int dock_system_host(const dock_params *params, const dock_protein *protein, con
 int dock_probe_peaks(float *out_host, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
 /* ---- diagnostics ------------------------------------------------------------------------------ */
+/* CUDA source of the ligand-specialised score kernel dock_score_batch would compile for (params, grid, ligand)
+ * (score_kernel = 2; A2-A5).  buf: HOST, cap bytes; *needed = length + 1; DOCK_EWORKSPACE if cap is short,
+ * DOCK_EINVAL if the ligand is outside what the generator covers.  No device work. */
+int dock_score_jit_source(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                          int32_t want_grad, char *buf, size_t cap, size_t *needed);
+/* Compiles that source for sm_100a with NVRTC (host only, needs no GPU) and reports the size of the cubin: the "does it build" check
+ * of the run-time kernel.  DOCK_ECUDA if NVRTC (libnvrtc.so.12 of CUDA >= 12.9) is missing or the compilation fails. */
+int dock_score_jit_compile(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
+                           int32_t want_grad, size_t *cubin_bytes);
+const char *dock_score_jit_log(void);            /* compiler log of the last failed run-time compilation ("" = none) */
 int         dock_last_cuda_error(void);          /* cudaError_t of the last failing CUDA call (0 = none) */
 const char *dock_version(void);
 /* number of kernel launches issued by this library since load (for bench.py's gpu_launches) */

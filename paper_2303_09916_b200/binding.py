@@ -27,7 +27,7 @@ EXPORTS = [
     "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_build_grids_batch", "dock_score_batch",
     "dock_score_batch_host", "dock_local_opt_batch", "dock_local_opt_trace", "dock_init_poses", "dock_init_poses_site",
     "dock_search", "dock_topk", "dock_system_host", "dock_probe_peaks", "dock_last_cuda_error", "dock_version",
-    "dock_launch_count",
+    "dock_launch_count", "dock_score_jit_source", "dock_score_jit_compile", "dock_score_jit_log",
 ]
 
 
@@ -49,7 +49,7 @@ class dock_params(C.Structure):
         ("bfgs_gtol", C.c_float), ("bfgs_curv_eps", C.c_float),
         ("cluster_rmsd", C.c_float), ("topk", C.c_int32),
         ("optimizer", C.c_int32), ("bb_step", C.c_float), ("bb_fallback", C.c_float), ("grad_mode", C.c_int32),
-        ("search_kernel", C.c_int32),
+        ("search_kernel", C.c_int32), ("score_kernel", C.c_int32),
     ]
 
 
@@ -90,6 +90,7 @@ def load_library(path: Optional[str] = None):
                             "(there is no CPU fallback)")
         _lib = C.CDLL(path)
         _lib.dock_version.restype = C.c_char_p
+        _lib.dock_score_jit_log.restype = C.c_char_p
         _lib.dock_launch_count.restype = C.c_uint64
         _lib.dock_grid_bytes.restype = C.c_size_t
     return _lib

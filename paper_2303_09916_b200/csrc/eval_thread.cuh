@@ -270,14 +270,18 @@ __device__ __forceinline__ float eval_pose_thread(const DevParams &P, const DevG
 
     // ---- phase 1: A2 -------------------------------------------------------------------------------
     {
+        // The torsion angles are fetched in one burst and parked in the z column: theta_k at slot N-T+k, which phase 1
+        // writes only after fragment k+1 has consumed it (every later fragment owns at least one slot).  One exposed
+        // global-load latency instead of one per fragment.
+        for (int k = 0; k < T; ++k) zz[(N - T + k) * 32] = pose[(7 + k) * ps];
         Rot3 A = quat_to_rot(pose[3 * ps], pose[4 * ps], pose[5 * ps], pose[6 * ps]);
         float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f;                                     // pivot-relative
         int s = 0;
         float sn_n = 0.0f, cs_n = 1.0f;                                            // sin / cos of the NEXT torsion (independent work
-        if (T > 0) sincos_cw(pose[7 * ps], sn_n, cs_n);                            // for the scheduler while a frame is composed)
+        if (T > 0) sincos_cw(zz[(N - T) * 32], sn_n, cs_n);                        // for the scheduler while a frame is composed)
         for (int f = 0; f <= T; ++f) {
             const float sn = sn_n, cs = cs_n;
-            if (f < T && f > 0) sincos_cw(pose[(7 + f) * ps], sn_n, cs_n);
+            if (f < T && f > 0) sincos_cw(zz[(N - T + f) * 32], sn_n, cs_n);
             if (f > 0) {
                 const int k = f - 1;
                 const float4 u = L.tors_axis[k];

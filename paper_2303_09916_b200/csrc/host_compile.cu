@@ -53,6 +53,7 @@ extern "C" int dock_default_params(dock_params *p)
     p->bb_fallback = 0.1f;
     p->grad_mode = 0;
     p->search_kernel = 0;
+    p->score_kernel = 0;
     return DOCK_OK;
 }
 
@@ -67,6 +68,7 @@ int dock_validate_params(const dock_params *p)
     if (p->optimizer < 0 || p->optimizer > 1) return DOCK_EINVAL;
     if (p->grad_mode < 0 || p->grad_mode > 1) return DOCK_EINVAL;
     if (p->search_kernel < 0 || p->search_kernel > 2) return DOCK_EINVAL;
+    if (p->score_kernel < 0 || p->score_kernel > 2) return DOCK_EINVAL;
     if (p->optimizer == 1 && (!(p->bb_step > 0.f) || !(p->bb_fallback > 0.f))) return DOCK_EINVAL;
     return DOCK_OK;
 }

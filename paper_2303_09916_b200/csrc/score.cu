@@ -9,6 +9,7 @@
 #include "common.cuh"
 #include "eval_thread.cuh"
 #include "host_compile.cuh"
+#include "jit_score.cuh"
 
 namespace {
 
@@ -130,6 +131,13 @@ int pipe_init(HostPipe &hp)
     return DOCK_OK;
 }
 
+// The ligand-specialised kernel (jit_score.cu) is opt-in: it costs a run-time compilation per ligand (0.4-6 s, cached) and
+// gains 1.07x on BASELINE configs[1] (profiles/r2b.md), so score_kernel = 0 keeps the generic kernel.
+bool use_jit(const dock_params *params, const dock_grid *grid, const dock_ligand *lig, int64_t n_poses)
+{
+    return params->score_kernel == 2 && n_poses >= 1 && lig && grid;
+}
+
 }  // namespace
 
 extern "C" int dock_score_batch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
@@ -144,6 +152,11 @@ extern "C" int dock_score_batch(const dock_params *params, const dock_grid *grid
     if (needed) *needed = pl.need;
     if (!ws_dev || ws_bytes < pl.need) return DOCK_EWORKSPACE;
     if (n_poses > 0 && (!poses_dev || !energy_dev)) return DOCK_EINVAL;
+    if (use_jit(params, grid, ligand, n_poses)) {
+        const int rj = jit_score_launch(params, grid, ligand, pl.P, pl.G, n_poses, poses_dev, energy_dev, grad_dev, terms_dev,
+                                        (cudaStream_t)stream_);
+        if (rj == DOCK_OK || params->score_kernel == 2) return rj;      // forced: report the failure; auto: generic kernel
+    }
     return score_launch(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, ws_dev, (cudaStream_t)stream_);
 }
 
@@ -185,6 +198,8 @@ extern "C" int dock_score_batch_host(const dock_params *params, const dock_grid 
     const int64_t per = ((n_poses + n_chunks - 1) / n_chunks + 31) / 32 * 32;
     // on any failure the copies already enqueued are drained before returning: the caller's host buffers must not be
     // written after the call has come back
+    const bool jit = use_jit(params, grid, ligand, n_poses);
+    bool uploaded = false;
     auto pipeline = [&]() -> int {
         DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_begin, stream));              // the workspace may still be in use upstream
         DOCK_CUDA_CHECK(cudaStreamWaitEvent(hp.s_in, hp.ev_begin, 0));
@@ -195,8 +210,12 @@ extern "C" int dock_score_batch_host(const dock_params *params, const dock_grid 
             DOCK_CUDA_CHECK(cudaMemcpyAsync(d_pose + o * np_, poses_host + o * np_, (size_t)m * np_ * sizeof(float), cudaMemcpyHostToDevice, hp.s_in));
             DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_in[c], hp.s_in));
             DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, hp.ev_in[c], 0));
-            const int rc2 = score_launch(pl, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr, d_t ? d_t + o * 3 : nullptr,
-                                         ws, stream, c == 0);
+            int rc2 = DOCK_EINVAL;
+            if (jit) rc2 = jit_score_launch(params, grid, ligand, pl.P, pl.G, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr,
+                                            d_t ? d_t + o * 3 : nullptr, stream);
+            if (rc2 != DOCK_OK && !(jit && params->score_kernel == 2))
+                rc2 = score_launch(pl, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr, d_t ? d_t + o * 3 : nullptr,
+                                   ws, stream, !uploaded), uploaded = true;
             if (rc2 != DOCK_OK) return rc2;
             DOCK_CUDA_CHECK(cudaEventRecord(hp.ev_k[c], stream));
             DOCK_CUDA_CHECK(cudaStreamWaitEvent(hp.s_out, hp.ev_k[c], 0));

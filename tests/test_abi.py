@@ -232,3 +232,42 @@ def test_search_rejects_before_it_enqueues(lib):
     g4 = _fake_grid(s, s.lig_types)
     g4.n_channels = 4
     assert query(64, [g, g4]) == B.DOCK_EINVAL               # one gradient mode per launch
+
+
+def test_specialised_score_kernel_source_and_compilation(lib):
+    """score_kernel = 2: the generated CUDA text for configs[0] and a 21-atom ligand compiles for sm_100a with NVRTC on
+    this (GPU-less) box; every listed pair appears in exactly one chain; out-of-range ligands are refused."""
+    import re
+    from dock_synth import make_system, make_ligand
+    from dock_synth.generators import LIG_TYPES_FULL
+    lib.dock_score_jit_log.restype = C.c_char_p
+    p = B.dock_default_params()
+    s = make_system(0, seed=0)
+    g = B.dock_grid()
+    g.dims[0] = g.dims[1] = g.dims[2] = 41
+    g.spacing = 0.375
+    for t in range(32):
+        g.type_to_map[t] = -1
+    for m, t in enumerate(LIG_TYPES_FULL):
+        g.type_to_map[int(t)] = m
+    g.n_maps = len(LIG_TYPES_FULL)
+    g.n_channels = 1
+    g.data_dev, g.packed_dev = 256, 512            # never dereferenced: no device work in these calls
+    for ligd in (s.ligand, make_ligand(np.random.default_rng(3), 21, 4, LIG_TYPES_FULL)):
+        lig = B.LigandHandle(ligd)
+        need = C.c_size_t(0)
+        assert lib.dock_score_jit_source(C.byref(p), C.byref(g), C.byref(lig.c), 1, None, C.c_size_t(0), C.byref(need)) == B.DOCK_EWORKSPACE
+        buf = C.create_string_buffer(need.value)
+        assert lib.dock_score_jit_source(C.byref(p), C.byref(g), C.byref(lig.c), 1, buf, C.c_size_t(need.value), C.byref(need)) == B.DOCK_OK
+        src = buf.value.decode()
+        assert "dock_score_jit" in src and "fma.rn.f32x2" in src
+        m = re.search(r"A4, (\d+) chains for (\d+) pairs", src)
+        assert m and int(m.group(2)) == lig.P and (lig.P + 1) // 2 <= int(m.group(1)) <= lig.P
+        assert src.count("rsq(") - 1 == lig.P          # one reciprocal square root per listed pair (+ the helper's definition)
+        nb = C.c_size_t(0)
+        rc = lib.dock_score_jit_compile(C.byref(p), C.byref(g), C.byref(lig.c), 1, C.byref(nb))
+        assert rc == B.DOCK_OK and nb.value > 10000, (rc, lib.dock_score_jit_log())
+    big = B.LigandHandle(make_ligand(np.random.default_rng(4), 44, 6, LIG_TYPES_FULL))
+    assert lib.dock_score_jit_source(C.byref(p), C.byref(g), C.byref(big.c), 1, None, C.c_size_t(0), C.byref(need)) == B.DOCK_EINVAL
+    g.n_channels = 4
+    assert lib.dock_score_jit_source(C.byref(p), C.byref(g), C.byref(lig.c), 1, None, C.c_size_t(0), C.byref(need)) == B.DOCK_EINVAL

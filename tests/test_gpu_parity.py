@@ -885,3 +885,68 @@ def test_search_kernels_agree_bitwise(dk, torch, tiny):
                 assert torch.equal(ra[key], rb[key]), (opt, key)
             for a, b in zip(la, lb):
                 assert torch.equal(a, b), opt
+
+
+# ---- run-time specialised score kernel (dock_params.score_kernel = 2, jit_score.cu) ------------------------------
+def _jit_params(dk):
+    p = dk.dock_default_params()
+    p.score_kernel = 2
+    return p
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_specialised_score_kernel_matches_the_oracle(dk, orc, torch, tiny, micro, cfg):
+    """A2-A5 through the NVRTC-compiled kernel, element by element against the oracle on configs 0 and 1 (ragged counts,
+    poses in 1.3x the box so the wall is exercised), energy-only variant included."""
+    s, (_, box, grid, lig), (op, og, oL) = tiny if cfg == 0 else micro
+    p = _jit_params(dk)
+    rng = np.random.default_rng(11 + cfg)
+    n = 4099 if cfg == 0 else 8195
+    poses = random_poses(rng, n, s.box_center, s.box_size * (1.3 if cfg == 0 else 1.0), lig.T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, f"jit{cfg}",
+                        cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=lig.N, n_pairs=lig.P)
+    _log("score_specialised", dict(cfg=cfg, **st))
+    e1, g1, t1 = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda(), want_grad=False, want_terms=False)
+    assert g1 is None and torch.allclose(e, e1, rtol=1e-6, atol=1e-5)
+    # host entry point takes the same kernel
+    eh, gh, _ = dk.dock_score_batch_host(p, grid, lig, poses[:1000])
+    assert np.array_equal(eh, e[:1000].cpu().numpy()) and np.array_equal(gh, g[:1000].cpu().numpy())
+
+
+@pytest.mark.parametrize("N,T", [(1, 0), (5, 0), (13, 3), (21, 4), (33, 3)])
+def test_specialised_score_kernel_other_shapes(dk, orc, torch, micro, N, T):
+    """Single atom (no pairs), rigid ligand, odd atom counts (a duo with one atom), and a ligand past the i-cache knee."""
+    s0, (_, box, grid, _), (op, og, _) = micro
+    p = _jit_params(dk)
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    rng = np.random.default_rng(300 + N)
+    if N == 1:
+        from types import SimpleNamespace
+        ligd = SimpleNamespace(ref_xyz=np.zeros((1, 3)), type=np.array([3], np.int32), frag=np.zeros(1, np.int32),
+                               tors_parent=np.zeros(0, np.int32), tors_a=np.zeros(0, np.int32),
+                               tors_b=np.zeros(0, np.int32), pairs=np.zeros((0, 2), np.int32))
+    else:
+        ligd = dock_synth.make_ligand(rng, N, T, LIG_TYPES_FULL)
+    lig, oL = dk.LigandHandle(ligd), orc.Ligand(ligd)
+    poses = random_poses(rng, 777, s0.box_center, s0.box_size * 1.2, T)
+    e, g, t = dk.dock_score_batch(p, grid, lig, torch.from_numpy(poses).cuda())
+    oe, ograd, oterms, diag = orc.score_batch(op, og, oL, poses.astype(np.float64))
+    st = compare_scores(e.cpu().numpy(), g.cpu().numpy(), t.cpu().numpy(), oe, ograd, oterms, diag, f"jitN{N}T{T}",
+                        cond=orc.grad_cond(op, og, oL, poses.astype(np.float64)), n_atoms=N, n_pairs=oL.P)
+    _log("score_specialised_shapes", dict(N=N, T=T, **st))
+
+
+def test_specialised_score_kernel_limits(dk, torch, micro):
+    """Above DOCK_JIT_MAX_ATOMS the forced mode reports DOCK_EINVAL instead of silently taking another kernel."""
+    s0, (_, box, grid, _), _ = micro
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    lig = dk.LigandHandle(dock_synth.make_ligand(np.random.default_rng(5), 44, 6, LIG_TYPES_FULL))
+    poses = torch.from_numpy(random_poses(np.random.default_rng(6), 64, s0.box_center, s0.box_size, lig.T)).cuda()
+    with pytest.raises(dk.DockError, match="DOCK_EINVAL"):
+        dk.dock_score_batch(_jit_params(dk), grid, lig, poses)
+    e, _, _ = dk.dock_score_batch(dk.dock_default_params(), grid, lig, poses)      # default: generic kernel
+    assert bool(torch.isfinite(e).all())
