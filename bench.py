@@ -202,6 +202,7 @@ def run_ours(args) -> dict:
     s, poses_h = _workload(rank)
     p = dk.dock_default_params()
     box = dk.make_box(s.box_center, s.box_size, s.spacing)
+    p.score_kernel = args.score_kernel           # 0 / 1: generic thread-per-pose kernel (default); 2: run-time specialised kernel
     lig = dk.LigandHandle(s.ligand)
     n = poses_h.shape[0]
     np_, ng = 7 + lig.T, 6 + lig.T
@@ -265,6 +266,7 @@ def run_ours(args) -> dict:
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "configs[1] scoring microbench", "n_poses_per_gpu": n, "N": lig.N, "T": lig.T, "P": lig.P,
                    "grid": "81^3 x 8 fp32", "outputs": "energy+gradient+terms",
+                   "score_kernel": "specialised at run time (NVRTC, dock_params.score_kernel = 2)" if args.score_kernel == 2 else "generic (default)",
                    "l2": "flushed between timed steps (256 MiB write)" if not args.no_flush else "not flushed",
                    "parallelism": f"pose-sharded x{world}, no collective"},
         "e2e": {"value": world * n / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -276,8 +278,29 @@ def run_ours(args) -> dict:
     # measured roofs of the units this path is bound by (probe kernels in the library, same GPU, same run)
     peaks = dk.dock_probe_peaks()
 
-    # ---- extras that shard over ranks (N > 1): the screening batch, systems [b, e) per rank, no exchange ----
     extra = {}
+    # the other score kernel next to the headline (rank 0): same batch, same launch configuration, L2 flushed
+    if rank == 0 and not args.no_search:
+        po = dk.dock_default_params()
+        po.score_kernel = 1 if args.score_kernel == 2 else 2
+        name = "generic_score_kernel" if args.score_kernel == 2 else "specialised_score_kernel"
+        try:
+            t0 = time.perf_counter()
+            oo = dk.dock_score_batch(po, grid, lig, poses)
+            torch.cuda.synchronize()
+            t_first = time.perf_counter() - t0
+            to = _time_events(torch, lambda: dk.dock_score_batch(po, grid, lig, poses, out=oo), min(args.steps, 20), flush)
+            de = float((oo[0] - out[0]).abs().max())
+            dg = float(((oo[1] - out[1]).abs() / (1e-3 + 1e-4 * out[1].abs())).max())
+            extra[name] = {"ms_per_step": float(np.mean(to)), "evals_per_s": n / (float(np.mean(to)) / 1e3),
+                           "first_call_s": t_first, "max_abs_dE_vs_headline_kernel": de, "max_dgrad_tol_units_vs_headline_kernel": dg,
+                           "note": "dock_params.score_kernel = 2 (jit_score.cu): first_call_s includes the NVRTC compilation for this ligand"
+                                   if name.startswith("spec") else "dock_params.score_kernel = 1"}
+            del oo
+        except dk.DockError as e:
+            extra[name] = {"unavailable": str(e)}
+
+    # ---- extras that shard over ranks (N > 1): the screening batch, systems [b, e) per rank, no exchange ----
     if not args.no_search:
         from paper_2303_09916_b200.shard import shard_range
         n3 = args.screen_systems
@@ -339,7 +362,7 @@ def run_ours(args) -> dict:
     peak_meas = max(peaks["ffma_tflops"], peaks["ffma2_tflops"])
     line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                         "frac": achieved / ALU_PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
-                        "kernel": "score_thread_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
+                        "kernel": "dock_score_jit" if args.score_kernel == 2 else "score_thread_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
                         "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                         "peak_measured": peak_meas, "frac_of_measured": achieved / peak_meas,
                         "peak_measured_source": "dock_probe_peaks: FFMA / FFMA2 loops, 8 independent chains per thread, this run",
@@ -465,6 +488,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1048576, help="poses the CPU oracle scores per step")
     ap.add_argument("--no-flush", action="store_true")
     ap.add_argument("--no-search", action="store_true")
+    ap.add_argument("--score-kernel", type=int, default=0, choices=[0, 1, 2],
+                    help="dock_params.score_kernel for the headline step: 0/1 generic (default), 2 specialised at run time")
     ap.add_argument("--screen-systems", type=int, default=256, help="systems of the configs[3] screening batch (256 = the config)")
     args = ap.parse_args()
     if args.impl == "reference":
