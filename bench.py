@@ -475,8 +475,8 @@ def run_ours(args) -> dict:
 
 
 # per-launch DRAM traffic of the score kernel from the committed `ncu --set full` capture
-# (profiles/r1j_score_thread_kernel_details.txt).
-TRAFFIC_BYTES_PER_LAUNCH = 823.4e6   # profiles/r1j.md: dram__bytes_read.sum 756.8 MB + dram__bytes_write.sum 66.6 MB
+# (profiles/r2c_score_thread_kernel_details.txt).
+TRAFFIC_BYTES_PER_LAUNCH = 821.8e6   # profiles/r2c.md: dram__bytes_read.sum 755.6 MB + dram__bytes_write.sum 66.2 MB
 
 
 def main():
