@@ -202,7 +202,14 @@ def run_ours(args) -> dict:
     s, poses_h = _workload(rank)
     p = dk.dock_default_params()
     box = dk.make_box(s.box_center, s.box_size, s.spacing)
-    p.score_kernel = args.score_kernel           # 0 / 1: generic thread-per-pose kernel (default); 2: run-time specialised kernel
+    # which score kernel the headline times: 2 = specialised for the ligand at run time (NVRTC; the faster one on
+    # configs[1], compiled during the warm-up), 0 / 1 = the generic kernel (the library's default).  -1 (default here) =
+    # 2 if the compiler is there, else generic.  The other kernel is timed beside it (extra.*_score_kernel).
+    args.score_kernel_note = ""
+    if args.score_kernel < 0:
+        args.score_kernel = 2
+        args.score_kernel_note = "auto"
+    p.score_kernel = args.score_kernel
     lig = dk.LigandHandle(s.ligand)
     n = poses_h.shape[0]
     np_, ng = 7 + lig.T, 6 + lig.T
@@ -224,6 +231,13 @@ def run_ours(args) -> dict:
     def step():
         dk.dock_score_batch(p, grid, lig, poses, out=out)
 
+    try:
+        step()
+    except dk.DockError as e:                      # NVRTC missing / ligand outside the generator: the generic kernel
+        if args.score_kernel != 2 or args.score_kernel_note != "auto":
+            raise
+        args.score_kernel = p.score_kernel = 0
+        args.score_kernel_note = f"auto: specialised kernel unavailable ({e}), generic kernel timed"
     for _ in range(max(3, args.warmup)):
         step()
     _barrier(world)
@@ -266,7 +280,9 @@ def run_ours(args) -> dict:
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "configs[1] scoring microbench", "n_poses_per_gpu": n, "N": lig.N, "T": lig.T, "P": lig.P,
                    "grid": "81^3 x 8 fp32", "outputs": "energy+gradient+terms",
-                   "score_kernel": "specialised at run time (NVRTC, dock_params.score_kernel = 2)" if args.score_kernel == 2 else "generic (default)",
+                   "score_kernel": ("specialised at run time (NVRTC, dock_params.score_kernel = 2; compiled during the warm-up)"
+                                    if args.score_kernel == 2 else "generic (dock_params.score_kernel = 0, the library default)")
+                                   + (f" [{args.score_kernel_note}]" if args.score_kernel_note else ""),
                    "l2": "flushed between timed steps (256 MiB write)" if not args.no_flush else "not flushed",
                    "parallelism": f"pose-sharded x{world}, no collective"},
         "e2e": {"value": world * n / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -361,7 +377,8 @@ def run_ours(args) -> dict:
     achieved = flops * n / t_kernel / 1e12
     peak_meas = max(peaks["ffma_tflops"], peaks["ffma2_tflops"])
     line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                        "frac": achieved / ALU_PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                        "frac": achieved / ALU_PEAK_TFLOPS,
+                        "traffic": TRAFFIC_BYTES_PER_LAUNCH["dock_score_jit" if args.score_kernel == 2 else "score_thread_kernel"],
                         "kernel": "dock_score_jit" if args.score_kernel == 2 else "score_thread_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
                         "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                         "peak_measured": peak_meas, "frac_of_measured": achieved / peak_meas,
@@ -474,9 +491,11 @@ def run_ours(args) -> dict:
     return line
 
 
-# per-launch DRAM traffic of the score kernel from the committed `ncu --set full` capture
-# (profiles/r2c_score_thread_kernel_details.txt).
-TRAFFIC_BYTES_PER_LAUNCH = 821.8e6   # profiles/r2c.md: dram__bytes_read.sum 755.6 MB + dram__bytes_write.sum 66.2 MB
+# per-launch DRAM traffic of the score kernels from the committed `ncu --set full` captures
+TRAFFIC_BYTES_PER_LAUNCH = {
+    "score_thread_kernel": 821.8e6,   # profiles/r2c_score_thread_kernel_details.txt: dram read 755.6 MB + write 66.2 MB
+    "dock_score_jit": 817.3e6,        # profiles/r2b_dock_score_jit_details.txt: dram read 751.2 MB + write 66.1 MB
+}
 
 
 def main():
@@ -488,8 +507,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1048576, help="poses the CPU oracle scores per step")
     ap.add_argument("--no-flush", action="store_true")
     ap.add_argument("--no-search", action="store_true")
-    ap.add_argument("--score-kernel", type=int, default=0, choices=[0, 1, 2],
-                    help="dock_params.score_kernel for the headline step: 0/1 generic (default), 2 specialised at run time")
+    ap.add_argument("--score-kernel", type=int, default=-1, choices=[-1, 0, 1, 2],
+                    help="dock_params.score_kernel for the headline step: 0/1 generic (the library default), 2 specialised at run "
+                         "time, -1 (default) = 2 if NVRTC is available, else generic")
     ap.add_argument("--screen-systems", type=int, default=256, help="systems of the configs[3] screening batch (256 = the config)")
     args = ap.parse_args()
     if args.impl == "reference":
