@@ -29,8 +29,8 @@
 //
 // The text is compiled for sm_100a with NVRTC (dlopen'ed: the toolkit's libnvrtc.so.12, CUDA >= 12.9 for the 256-bit
 // load), loaded with cudaLibraryLoadData and cached per (device, ligand, parameters).  Measured on B200
-// (profiles/r2b.md): 1.07x the generic kernel on configs[1] (N = 30, 8.0 k instructions: the unrolled part runs in the
-// 3-cycle regime of the i-cache), 1.2-1.35x for ligands of 12-20 atoms, 0.5x above ~33 atoms (code > 128 KB), and a
+// (profiles/r2b.md): 1.10x the generic kernel on configs[1] (N = 30, 7.8 k instructions: the unrolled part runs in the
+// 3-cycle regime of the i-cache), 1.2-1.3x for ligands of 12-20 atoms, 0.5x above ~33 atoms (code > 128 KB), and a
 // compilation of 0.4-6 s per ligand -- which is why it is opt-in and the generic kernel stays the default.
 #include <dlfcn.h>
 
@@ -153,12 +153,17 @@ __device__ __forceinline__ float rsq(float x) { float y; asm("rsqrt.approx.ftz.f
 __device__ __forceinline__ void ldg_cell(const Cell8 *p, float4 &lo, float4 &hi)
 {
     unsigned long long a, b, c, d;
-    asm("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p));
+    // volatile: the gathers of the NEXT loop iteration must stay ahead of the interpolation of the current one (pin4)
+    asm volatile("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p));
     lo.x = __uint_as_float((unsigned)a); lo.y = __uint_as_float((unsigned)(a >> 32));
     lo.z = __uint_as_float((unsigned)b); lo.w = __uint_as_float((unsigned)(b >> 32));
     hi.x = __uint_as_float((unsigned)c); hi.y = __uint_as_float((unsigned)(c >> 32));
     hi.z = __uint_as_float((unsigned)d); hi.w = __uint_as_float((unsigned)(d >> 32));
 }
+// an empty volatile statement that "rewrites" v: volatile statements keep their order, so everything that uses v afterwards
+// stays behind the volatile loads issued before it (without it the compiler sinks the next iteration's gathers below the
+// interpolation of the current one and their latency is exposed: 16 % of all stall samples, profiles/r2b.md)
+__device__ __forceinline__ void pin4(float4 &v) { asm volatile("" : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)); }
 // volatile: the loads stay where the generator put them (one group ahead of their use) and are not forwarded from
 // the phase-1 stores, which would pin every coordinate in a register
 __device__ __forceinline__ float4 lds4(const float4 *p)
@@ -243,7 +248,7 @@ __device__ __forceinline__ float trilinear(const JitArgs &G, const CellRef &c, c
 int jit_warp_float4(int N, int T, bool want_grad)
 {
     const int D = (N + 1) / 2;
-    const int r2 = std::max(want_grad ? 6 * D : 0, 12 * T);        // floats per lane
+    const int r2 = std::max(want_grad ? 6 * D : 0, 13 * T);        // floats per lane (frames 12 T + staged torsion angles T)
     return D * 48 + (r2 * 32 + 3) / 4;
 }
 
@@ -408,6 +413,11 @@ struct Gen {
         S("        m20 = fmaf(x2, z, -w * y2); m21 = fmaf(y2, z, w * x2); m22 = 1.0f - fmaf(x2, x, y2 * y);");
         S("    }");
         S("    float *const xyf = reinterpret_cast<float *>(xyq), *const zf = reinterpret_cast<float *>(zq);");
+        if (T > 0) {                                          // all torsion angles in one burst (one exposed load latency)
+            S("    float *const thf = reinterpret_cast<float *>(reg2) + %d + lane;", 12 * T * 32);
+            S("    #pragma unroll");
+            S("    for (int k = 0; k < %d; ++k) thf[k * 32] = pose[7 + k];", T);
+        }
         S("    int s = 0;");
         S("    #pragma unroll 1");
         S("    for (int f = 0; f <= %d; ++f) {", T);
@@ -415,7 +425,7 @@ struct Gen {
             S("        if (f > 0) {");
             S("            const JitF3I u = jit_axis[f - 1]; const float4 b = jit_pt[f - 1];");
             S("            const int pf = u.w;");
-            S("            float sn, cs; sincos_cw(pose[6 + f], sn, cs);");
+            S("            float sn, cs; sincos_cw(thf[(f - 1) * 32], sn, cs);");
             S("            const float2 p0 = fr[(6 * pf) * 32], p1 = fr[(6 * pf + 1) * 32], p2 = fr[(6 * pf + 2) * 32];");
             S("            const float2 p3 = fr[(6 * pf + 3) * 32], p4 = fr[(6 * pf + 4) * 32], p5 = fr[(6 * pf + 5) * 32];");
             S("            const float omc = 1.0f - cs;");
@@ -440,7 +450,7 @@ struct Gen {
             S("        }");
         }
         S("        const int s_end = jit_frag_end[f];");
-        S("        #pragma unroll 1");
+        S("        #pragma unroll %d", o.atom_unroll);
         S("        for (; s < s_end; ++s) {");
         S("            const JitF3I r = jit_ref[s];");
         S("            const int sl = r.w, dd = sl >> 1, h = sl & 1;     // duo and lane of this atom");
@@ -486,54 +496,68 @@ struct Gen {
     // the sigma-scaled grid forces go to shared memory and seed the force registers of the pair phase
     void grid_loop()
     {
-        // U duos (2U atoms) per iteration, software-pipelined by one iteration: the cells of the next 2U atoms are
-        // requested before those of the current ones are used (memory-level parallelism 2U per thread, enough to cover
-        // an HBM miss with two warps per scheduler)
+        // Two register sets (A, B) of U duos each, ping-pong: while the cells of one set are interpolated the gathers of the
+        // other are in flight, with no register copies (a copy of a loaded register waits for the load) and no branch
+        // around the requests (ptxas hoists the interpolation above a conditional request).  Indices past the last full
+        // duo are clamped and their results masked.
         const int U = o.grid_unroll;
         const int D2 = d.N / 2;                              // full duos
-        const int n_it = D2 / U;                             // full iterations; the remaining duos / the odd atom follow
-        S("    // ---- phase 2a: A3 (map lookups), %d atoms per iteration ----", 2 * U);
+        const int n_it = (D2 + 2 * U - 1) / (2 * U);
+        const bool ragged = D2 % (2 * U) != 0;
+        S("    // ---- phase 2a: A3 (map lookups), 2 x %d atoms per iteration ----", 2 * U);
         S("    float e_grid = 0.0f, e_wall = 0.0f;");
-        auto issue = [&](const char *pre, const std::string &dd, int u) {      // locate + gather of duo dd into <pre>r<u>a.. regs
-            S("        { const float4 c = xyq[(%s) * 32]; const float2 w = zq[(%s) * 32];", dd.c_str(), dd.c_str());
-            S("          %sr%da = locate_cell(a, c.x + tx, c.z + ty, w.x + tz); %sr%db = locate_cell(a, c.y + tx, c.w + ty, w.y + tz);", pre, u, pre, u);
-            S("          ldg_cell(maps + ((long long)jit_maps[2 * (%s)] * a.map_stride + %sr%da.idx), %sp%da0, %sp%da1);", dd.c_str(), pre, u, pre, u, pre, u);
-            S("          ldg_cell(maps + ((long long)jit_maps[2 * (%s) + 1] * a.map_stride + %sr%db.idx), %sp%db0, %sp%db1); }", dd.c_str(), pre, u, pre, u, pre, u);
+        auto issue = [&](char set, const std::string &dd, int u) {           // locate + gather of duo dd into the set's registers
+            S("        { const int di = min(%s, %d); const float4 c = xyq[di * 32]; const float2 w = zq[di * 32];", dd.c_str(), std::max(D2 - 1, 0));
+            S("          r%c%da = locate_cell(a, c.x + tx, c.z + ty, w.x + tz); r%c%db = locate_cell(a, c.y + tx, c.w + ty, w.y + tz);", set, u, set, u);
+            S("          ldg_cell(maps + ((long long)jit_maps[2 * di] * a.map_stride + r%c%da.idx), p%c%da0, p%c%da1);", set, u, set, u, set, u);
+            S("          ldg_cell(maps + ((long long)jit_maps[2 * di + 1] * a.map_stride + r%c%db.idx), p%c%db0, p%c%db1); }", set, u, set, u, set, u);
         };
-        auto consume = [&](const std::string &dd, int u, bool second) {
-            S("        { float g0x, g0y, g0z, g1x = 0.0f, g1y = 0.0f, g1z = 0.0f;");
-            S("          e_grid += trilinear(a, r%da, p%da0, p%da1, e_wall, g0x, g0y, g0z);", u, u, u);
-            if (second) S("          e_grid += trilinear(a, r%db, p%db0, p%db1, e_wall, g1x, g1y, g1z);", u, u, u);
-            if (o.want_grad) {
-                S("          gq4[(%s) * 32] = make_float4(K_sigma * g0x, K_sigma * g1x, K_sigma * g0y, K_sigma * g1y);", dd.c_str());
-                S("          gq2[(%s) * 32] = make_float2(K_sigma * g0z, K_sigma * g1z); }", dd.c_str());
-            } else
-                S("        }");
+        auto consume = [&](char set, const std::string &dd, int u) {
+            S("        { float g0x, g0y, g0z, g1x, g1y, g1z, ew = 0.0f;");
+            S("          const float e01 = trilinear(a, r%c%da, p%c%da0, p%c%da1, ew, g0x, g0y, g0z) + trilinear(a, r%c%db, p%c%db0, p%c%db1, ew, g1x, g1y, g1z);", set, u, set, u, set, u, set, u, set, u, set, u);
+            if (ragged) {
+                S("          const int dd = %s; const bool live = dd < %d;", dd.c_str(), D2);
+                S("          e_grid += live ? e01 : 0.0f; e_wall += live ? ew : 0.0f;");
+                if (o.want_grad) {
+                    S("          if (live) { gq4[dd * 32] = make_float4(K_sigma * g0x, K_sigma * g1x, K_sigma * g0y, K_sigma * g1y);");
+                    S("                      gq2[dd * 32] = make_float2(K_sigma * g0z, K_sigma * g1z); }");
+                }
+            } else {
+                S("          const int dd = %s;", dd.c_str());
+                S("          e_grid += e01; e_wall += ew;");
+                if (o.want_grad) {
+                    S("          gq4[dd * 32] = make_float4(K_sigma * g0x, K_sigma * g1x, K_sigma * g0y, K_sigma * g1y);");
+                    S("          gq2[dd * 32] = make_float2(K_sigma * g0z, K_sigma * g1z);");
+                }
+            }
+            S("        }");
         };
-        if (n_it > 0) {
+        if (D2 > 0) {
             S("    {");
-            for (int u = 0; u < U; ++u) S("    CellRef r%da, r%db; float4 p%da0, p%da1, p%db0, p%db1;", u, u, u, u, u, u);
-            for (int u = 0; u < U; ++u) issue("", std::to_string(u), u);
+            for (int u = 0; u < U; ++u)
+                S("    CellRef rA%da, rA%db, rB%da, rB%db; float4 pA%da0, pA%da1, pA%db0, pA%db1, pB%da0, pB%da1, pB%db0, pB%db1;", u, u, u, u, u, u, u, u, u, u, u, u);
+            for (int u = 0; u < U; ++u) issue('A', std::to_string(u), u);
             S("    #pragma unroll 1");
             S("    for (int it = 0; it < %d; ++it) {", n_it);
-            for (int u = 0; u < U; ++u) S("        CellRef nr%da = r%da, nr%db = r%db; float4 np%da0 = p%da0, np%da1 = p%da1, np%db0 = p%db0, np%db1 = p%db1;", u, u, u, u, u, u, u, u, u, u, u, u);
-            S("        if (it + 1 < %d) {", n_it);
-            for (int u = 0; u < U; ++u) issue("n", "(it + 1) * " + std::to_string(U) + " + " + std::to_string(u), u);
-            S("        }");
-            for (int u = 0; u < U; ++u) consume("it * " + std::to_string(U) + " + " + std::to_string(u), u, true);
-            for (int u = 0; u < U; ++u) S("        r%da = nr%da; r%db = nr%db; p%da0 = np%da0; p%da1 = np%da1; p%db0 = np%db0; p%db1 = np%db1;", u, u, u, u, u, u, u, u, u, u, u, u);
+            S("        const int base = it * %d;", 2 * U);
+            for (int u = 0; u < U; ++u) issue('B', "base + " + std::to_string(U + u), u);
+            for (int u = 0; u < U; ++u) consume('A', "base + " + std::to_string(u), u);
+            for (int u = 0; u < U; ++u) issue('A', "base + " + std::to_string(2 * U + u), u);
+            for (int u = 0; u < U; ++u) consume('B', "base + " + std::to_string(U + u), u);
             S("    }");
             S("    }");
         }
-        for (int dd = n_it * U; dd < d.D; ++dd) {             // leftover duos (and the single atom of an odd ligand)
-            const bool second = mem[2 * dd + 1] >= 0;
+        if (d.N & 1) {                                      // the single atom of an odd ligand
+            const int dd = d.D - 1;
             S("    {");
-            S("        CellRef r0a, r0b; float4 p0a0, p0a1, p0b0, p0b1;");
-            S("        { const float4 c = xyq[%d]; const float2 w = zq[%d];", dd * 32, dd * 32);
-            S("          r0a = locate_cell(a, c.x + tx, c.z + ty, w.x + tz); ldg_cell(maps + (%dLL * a.map_stride + r0a.idx), p0a0, p0a1);", d.map[mem[2 * dd]]);
-            if (second) S("          r0b = locate_cell(a, c.y + tx, c.w + ty, w.y + tz); ldg_cell(maps + (%dLL * a.map_stride + r0b.idx), p0b0, p0b1);", d.map[mem[2 * dd + 1]]);
-            S("        }");
-            consume(std::to_string(dd), 0, second);
+            S("        const float4 c = xyq[%d]; const float2 w = zq[%d];", dd * 32, dd * 32);
+            S("        const CellRef r0 = locate_cell(a, c.x + tx, c.z + ty, w.x + tz);");
+            S("        float4 p0, p1; ldg_cell(maps + (%dLL * a.map_stride + r0.idx), p0, p1);", d.map[mem[2 * dd]]);
+            S("        float g0x, g0y, g0z; e_grid += trilinear(a, r0, p0, p1, e_wall, g0x, g0y, g0z);");
+            if (o.want_grad) {
+                S("        gq4[%d] = make_float4(K_sigma * g0x, 0.0f, K_sigma * g0y, 0.0f);", dd * 32);
+                S("        gq2[%d] = make_float2(K_sigma * g0z, 0.0f);", dd * 32);
+            }
             S("    }");
         }
     }
@@ -961,7 +985,8 @@ JitOpts jit_default_opts()
     o.maxrreg = 0;
     o.sync_every = 0;
     o.reuse = 1;
-    o.grid_unroll = 3;
+    o.grid_unroll = 1;
+    o.atom_unroll = 2;
     if (const char *e = getenv("DOCK_JIT_TUNE")) {        // tuning aid, e.g. "group=6,warps=8,minb=1,gu=2,reuse=2"
         int v;
         const char *q;
@@ -970,6 +995,7 @@ JitOpts jit_default_opts()
         if ((q = strstr(e, "minb=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 1 && v <= 16) o.min_blocks = v;
         if ((q = strstr(e, "maxrreg=")) && sscanf(q + 8, "%d", &v) == 1 && v >= 0 && v <= 255) o.maxrreg = v;
         if ((q = strstr(e, "sync=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 0 && v <= 1024) o.sync_every = v;
+        if ((q = strstr(e, "au=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 1 && v <= 8) o.atom_unroll = v;
         if ((q = strstr(e, "gu=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 1 && v <= 8) o.grid_unroll = v;
         if ((q = strstr(e, "reuse=")) && sscanf(q + 6, "%d", &v) == 1 && v >= 0 && v <= 1000) o.reuse = v;
     }
