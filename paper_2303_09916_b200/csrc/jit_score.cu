@@ -218,6 +218,16 @@ __device__ __forceinline__ CellRef locate_cell(const JitArgs &G, float x, float 
     c.idx = (iz * G.ny + iy) * G.nx + ix;
     return c;
 }
+// the index part of locate_cell alone, and an L2 prefetch of the cell
+__device__ __forceinline__ int cell_index(const JitArgs &G, float x, float y, float z)
+{
+    const float ux = fmaf(x, G.inv_h_lo, x * G.inv_h), uy = fmaf(y, G.inv_h_lo, y * G.inv_h), uz = fmaf(z, G.inv_h_lo, z * G.inv_h);
+    const float fx = fminf(floorf(fminf(fmaxf(ux, G.lo_x), G.hi_x)), G.hi_x - 1.0f);
+    const float fy = fminf(floorf(fminf(fmaxf(uy, G.lo_y), G.hi_y)), G.hi_y - 1.0f);
+    const float fz = fminf(floorf(fminf(fmaxf(uz, G.lo_z), G.hi_z)), G.hi_z - 1.0f);
+    return (((int)fz + G.icz) * G.ny + (int)fy + G.icy) * G.nx + (int)fx + G.icx;
+}
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 // eq. 2 + eq. 3 + wall (reading S7), same arithmetic as mathx.cuh::trilinear
 __device__ __forceinline__ float trilinear(const JitArgs &G, const CellRef &c, const float4 q0, const float4 q1,
                                            float &e_wall, float &gx, float &gy, float &gz)
@@ -453,10 +463,13 @@ struct Gen {
         S("        #pragma unroll %d", o.atom_unroll);
         S("        for (; s < s_end; ++s) {");
         S("            const JitF3I r = jit_ref[s];");
-        S("            const int sl = r.w, dd = sl >> 1, h = sl & 1;     // duo and lane of this atom");
-        S("            xyf[dd * 128 + h] = fmaf(m00, r.x, fmaf(m01, r.y, fmaf(m02, r.z, c0)));");
-        S("            xyf[dd * 128 + 2 + h] = fmaf(m10, r.x, fmaf(m11, r.y, fmaf(m12, r.z, c1)));");
-        S("            zf[dd * 64 + h] = fmaf(m20, r.x, fmaf(m21, r.y, fmaf(m22, r.z, c2)));");
+        S("            const int sl = r.w & 255, dd = sl >> 1, h = sl & 1;     // duo and lane of this atom (bits 8..: its map)");
+        S("            const float ax = fmaf(m00, r.x, fmaf(m01, r.y, fmaf(m02, r.z, c0)));");
+        S("            const float ay = fmaf(m10, r.x, fmaf(m11, r.y, fmaf(m12, r.z, c1)));");
+        S("            const float az = fmaf(m20, r.x, fmaf(m21, r.y, fmaf(m22, r.z, c2)));");
+        S("            xyf[dd * 128 + h] = ax; xyf[dd * 128 + 2 + h] = ay; zf[dd * 64 + h] = az;");
+        if (o.prefetch)                                       // the atom's map cell on its way into L2 while the rest of phase 1 runs
+            S("            prefetch_l2(maps + ((long long)(r.w >> 8) * a.map_stride + cell_index(a, ax + tx, ay + ty, az + tz)));");
         S("        }");
         S("    }");
         if (d.N & 1) S("    xyf[%d] = 0.0f; xyf[%d] = 0.0f; zf[%d] = 0.0f;", (d.D - 1) * 128 + 1, (d.D - 1) * 128 + 3, (d.D - 1) * 64 + 1);
@@ -474,7 +487,7 @@ struct Gen {
         t += "struct __align__(16) JitF3I { float x, y, z; int w; };\n__constant__ JitF3I jit_ref[" + std::to_string(d.N) + "] = {\n";
         for (int s = 0; s < d.N; ++s) {
             snprintf(b, sizeof b, "    {%s, %s, %s, %d}%s\n", FS(d.ref[3 * s]), FS(d.ref[3 * s + 1]), FS(d.ref[3 * s + 2]),
-                     2 * duo_of[s] + half_of[s], s + 1 < d.N ? "," : "};");
+                     (2 * duo_of[s] + half_of[s]) | (d.map[s] << 8), s + 1 < d.N ? "," : "};");
             t += b;
         }
         if (d.T > 0) {
@@ -502,9 +515,10 @@ struct Gen {
         // duo are clamped and their results masked.
         const int U = o.grid_unroll;
         const int D2 = d.N / 2;                              // full duos
-        const int n_it = (D2 + 2 * U - 1) / (2 * U);
-        const bool ragged = D2 % (2 * U) != 0;
-        S("    // ---- phase 2a: A3 (map lookups), 2 x %d atoms per iteration ----", 2 * U);
+        const int NS = o.grid_sets;                          // register sets: NS - 1 of them are in flight
+        const int n_it = (D2 + NS * U - 1) / (NS * U);
+        const bool ragged = D2 % (NS * U) != 0;
+        S("    // ---- phase 2a: A3 (map lookups), %d x %d atoms per iteration ----", NS, 2 * U);
         S("    float e_grid = 0.0f, e_wall = 0.0f;");
         auto issue = [&](char set, const std::string &dd, int u) {           // locate + gather of duo dd into the set's registers
             S("        { const int di = min(%s, %d); const float4 c = xyq[di * 32]; const float2 w = zq[di * 32];", dd.c_str(), std::max(D2 - 1, 0));
@@ -534,16 +548,21 @@ struct Gen {
         };
         if (D2 > 0) {
             S("    {");
-            for (int u = 0; u < U; ++u)
-                S("    CellRef rA%da, rA%db, rB%da, rB%db; float4 pA%da0, pA%da1, pA%db0, pA%db1, pB%da0, pB%da1, pB%db0, pB%db1;", u, u, u, u, u, u, u, u, u, u, u, u);
-            for (int u = 0; u < U; ++u) issue('A', std::to_string(u), u);
+            for (int j = 0; j < NS; ++j)
+                for (int u = 0; u < U; ++u) {
+                    const char c = (char)('A' + j);
+                    S("    CellRef r%c%da, r%c%db; float4 p%c%da0, p%c%da1, p%c%db0, p%c%db1;", c, u, c, u, c, u, c, u, c, u, c, u);
+                }
+            for (int j = 0; j + 1 < NS; ++j)
+                for (int u = 0; u < U; ++u) issue((char)('A' + j), std::to_string(j * U + u), u);
             S("    #pragma unroll 1");
             S("    for (int it = 0; it < %d; ++it) {", n_it);
-            S("        const int base = it * %d;", 2 * U);
-            for (int u = 0; u < U; ++u) issue('B', "base + " + std::to_string(U + u), u);
-            for (int u = 0; u < U; ++u) consume('A', "base + " + std::to_string(u), u);
-            for (int u = 0; u < U; ++u) issue('A', "base + " + std::to_string(2 * U + u), u);
-            for (int u = 0; u < U; ++u) consume('B', "base + " + std::to_string(U + u), u);
+            S("        const int base = it * %d;", NS * U);
+            for (int j = 0; j < NS; ++j) {
+                const int jn = (j + NS - 1) % NS;          // the set consumed longest ago is refilled, NS - 1 sets ahead
+                for (int u = 0; u < U; ++u) issue((char)('A' + jn), "base + " + std::to_string((j + NS - 1) * U + u), u);
+                for (int u = 0; u < U; ++u) consume((char)('A' + j), "base + " + std::to_string(j * U + u), u);
+            }
             S("    }");
             S("    }");
         }
@@ -986,6 +1005,8 @@ JitOpts jit_default_opts()
     o.sync_every = 0;
     o.reuse = 1;
     o.grid_unroll = 1;
+    o.grid_sets = 2;
+    o.prefetch = 0;          // measured: 0.853-0.873 ms with it, 0.841 ms without (configs[1])
     o.atom_unroll = 2;
     if (const char *e = getenv("DOCK_JIT_TUNE")) {        // tuning aid, e.g. "group=6,warps=8,minb=1,gu=2,reuse=2"
         int v;
@@ -995,6 +1016,8 @@ JitOpts jit_default_opts()
         if ((q = strstr(e, "minb=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 1 && v <= 16) o.min_blocks = v;
         if ((q = strstr(e, "maxrreg=")) && sscanf(q + 8, "%d", &v) == 1 && v >= 0 && v <= 255) o.maxrreg = v;
         if ((q = strstr(e, "sync=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 0 && v <= 1024) o.sync_every = v;
+        if ((q = strstr(e, "pf=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 0 && v <= 1) o.prefetch = v;
+        if ((q = strstr(e, "gs=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 2 && v <= 6) o.grid_sets = v;
         if ((q = strstr(e, "au=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 1 && v <= 8) o.atom_unroll = v;
         if ((q = strstr(e, "gu=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 1 && v <= 8) o.grid_unroll = v;
         if ((q = strstr(e, "reuse=")) && sscanf(q + 6, "%d", &v) == 1 && v >= 0 && v <= 1000) o.reuse = v;

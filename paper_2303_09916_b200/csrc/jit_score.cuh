@@ -15,6 +15,8 @@ struct JitOpts {          // all ints: hashed as raw bytes (no padding)
     int maxrreg;        // --maxrregcount (0 = none)
     int reuse;          // a duo's coordinates loaded for group g are reused by groups g+1 .. g+reuse before being reloaded
     int grid_unroll;    // duos per iteration of the map-lookup loop
+    int grid_sets;      // register sets of the map-lookup loop (grid_sets - 1 gathers-in-flight sets ahead of the interpolation)
+    int prefetch;       // 1: the kinematics loop prefetches every atom's map cell into L2
     int atom_unroll;    // unroll factor of the atom loop of the kinematics
     int sync_every;     // __syncthreads() every this many groups (0 = never): the warps of a CTA share the i-cache window
 };
