@@ -164,6 +164,23 @@ __device__ __forceinline__ void ldg_cell(const Cell8 *p, float4 &lo, float4 &hi)
 // stays behind the volatile loads issued before it (without it the compiler sinks the next iteration's gathers below the
 // interpolation of the current one and their latency is exposed: 16 % of all stall samples, profiles/r2b.md)
 __device__ __forceinline__ void pin4(float4 &v) { asm volatile("" : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)); }
+// quad image (JIT_QUAD): entry (ix,iy,iz) = the four (x,y) corners of the cell in plane iz; planes iz and iz+1 are adjacent
+__device__ __forceinline__ void ldg_quad(const float4 *p, float4 &lo, float4 &hi)
+{
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w) : "l"(p));
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4+16];" : "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w) : "l"(p));
+}
+// the same gather with an L2 cache hint (policy from createpolicy: evict_last keeps the map image in L2 against the
+// streaming poses and outputs)
+__device__ __forceinline__ void ldg_cell_hint(const Cell8 *p, float4 &lo, float4 &hi, unsigned long long pol)
+{
+    unsigned long long a, b, c, d;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.b64 {%0,%1,%2,%3}, [%4], %5;" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p), "l"(pol));
+    lo.x = __uint_as_float((unsigned)a); lo.y = __uint_as_float((unsigned)(a >> 32));
+    lo.z = __uint_as_float((unsigned)b); lo.w = __uint_as_float((unsigned)(b >> 32));
+    hi.x = __uint_as_float((unsigned)c); hi.y = __uint_as_float((unsigned)(c >> 32));
+    hi.z = __uint_as_float((unsigned)d); hi.w = __uint_as_float((unsigned)(d >> 32));
+}
 // volatile: the loads stay where the generator put them (one group ahead of their use) and are not forwarded from
 // the phase-1 stores, which would pin every coordinate in a register
 __device__ __forceinline__ float4 lds4(const float4 *p)
@@ -215,7 +232,7 @@ __device__ __forceinline__ CellRef locate_cell(const JitArgs &G, float x, float 
     const float fz = fminf(floorf(cz), G.hi_z - 1.0f);
     c.px = cx - fx; c.py = cy - fy; c.pz = cz - fz;
     const int ix = (int)fx + G.icx, iy = (int)fy + G.icy, iz = (int)fz + G.icz;
-    c.idx = (iz * G.ny + iy) * G.nx + ix;
+    c.idx = JIT_QUAD ? (iy * G.nx + ix) * G.nz + iz : (iz * G.ny + iy) * G.nx + ix;
     return c;
 }
 // the index part of locate_cell alone, and an L2 prefetch of the cell
@@ -225,7 +242,8 @@ __device__ __forceinline__ int cell_index(const JitArgs &G, float x, float y, fl
     const float fx = fminf(floorf(fminf(fmaxf(ux, G.lo_x), G.hi_x)), G.hi_x - 1.0f);
     const float fy = fminf(floorf(fminf(fmaxf(uy, G.lo_y), G.hi_y)), G.hi_y - 1.0f);
     const float fz = fminf(floorf(fminf(fmaxf(uz, G.lo_z), G.hi_z)), G.hi_z - 1.0f);
-    return (((int)fz + G.icz) * G.ny + (int)fy + G.icy) * G.nx + (int)fx + G.icx;
+    const int ix = (int)fx + G.icx, iy = (int)fy + G.icy, iz = (int)fz + G.icz;
+    return JIT_QUAD ? (iy * G.nx + ix) * G.nz + iz : (iz * G.ny + iy) * G.nx + ix;
 }
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 // eq. 2 + eq. 3 + wall (reading S7), same arithmetic as mathx.cuh::trilinear
@@ -523,8 +541,8 @@ struct Gen {
         auto issue = [&](char set, const std::string &dd, int u) {           // locate + gather of duo dd into the set's registers
             S("        { const int di = min(%s, %d); const float4 c = xyq[di * 32]; const float2 w = zq[di * 32];", dd.c_str(), std::max(D2 - 1, 0));
             S("          r%c%da = locate_cell(a, c.x + tx, c.z + ty, w.x + tz); r%c%db = locate_cell(a, c.y + tx, c.w + ty, w.y + tz);", set, u, set, u);
-            S("          ldg_cell(maps + ((long long)jit_maps[2 * di] * a.map_stride + r%c%da.idx), p%c%da0, p%c%da1);", set, u, set, u, set, u);
-            S("          ldg_cell(maps + ((long long)jit_maps[2 * di + 1] * a.map_stride + r%c%db.idx), p%c%db0, p%c%db1); }", set, u, set, u, set, u);
+            S("          LDG_CELL(maps + ((long long)jit_maps[2 * di] * a.map_stride + r%c%da.idx), p%c%da0, p%c%da1);", set, u, set, u, set, u);
+            S("          LDG_CELL(maps + ((long long)jit_maps[2 * di + 1] * a.map_stride + r%c%db.idx), p%c%db0, p%c%db1); }", set, u, set, u, set, u);
         };
         auto consume = [&](char set, const std::string &dd, int u) {
             S("        { float g0x, g0y, g0z, g1x, g1y, g1z, ew = 0.0f;");
@@ -571,7 +589,7 @@ struct Gen {
             S("    {");
             S("        const float4 c = xyq[%d]; const float2 w = zq[%d];", dd * 32, dd * 32);
             S("        const CellRef r0 = locate_cell(a, c.x + tx, c.z + ty, w.x + tz);");
-            S("        float4 p0, p1; ldg_cell(maps + (%dLL * a.map_stride + r0.idx), p0, p1);", d.map[mem[2 * dd]]);
+            S("        float4 p0, p1; LDG_CELL(maps + (%dLL * a.map_stride + r0.idx), p0, p1);", d.map[mem[2 * dd]]);
             S("        float g0x, g0y, g0z; e_grid += trilinear(a, r0, p0, p1, e_wall, g0x, g0y, g0z);");
             if (o.want_grad) {
                 S("        gq4[%d] = make_float4(K_sigma * g0x, 0.0f, K_sigma * g0y, 0.0f);", dd * 32);
@@ -844,6 +862,7 @@ struct Gen {
         choose_duos();
         S("// generated by libdock_b200 (jit_score.cu): N = %d, T = %d, P = %zu, grad = %d", d.N, d.T, d.pairs.size(), (int)o.want_grad);
         S("struct JitArgs { %s };", DOCK_JIT_STR(DOCK_JIT_ARGS_BODY));
+        S("#define JIT_QUAD %d", o.quad ? 1 : 0);
         S.s += k_prelude;
         S.s += tables();
         S("extern \"C\" __global__ void __launch_bounds__(%d, %d) dock_score_jit(const JitArgs a)", 32 * o.warps, o.min_blocks);
@@ -864,7 +883,17 @@ struct Gen {
         S("    if (p > a.n_poses - 1) p = a.n_poses - 1;   // idle lanes of the last warp redo the last pose (same bits, same stores)");
         S("    const float *__restrict__ pose = a.poses + p * %d;", 7 + d.T);
         if (o.want_grad) S("    float *__restrict__ grad = a.grad + p * %d;", 6 + d.T);
-        S("    const Cell8 *__restrict__ maps = reinterpret_cast<const Cell8 *>(a.packed);");
+        if (o.quad) {
+            S("    const float4 *__restrict__ maps = reinterpret_cast<const float4 *>(a.packed);");
+            S("#define LDG_CELL(ptr, lo, hi) ldg_quad(ptr, lo, hi)");
+        } else
+            S("    const Cell8 *__restrict__ maps = reinterpret_cast<const Cell8 *>(a.packed);");
+        if (o.quad) {
+        } else if (o.l2_hint) {
+            S("    unsigned long long l2_keep; asm volatile(\"createpolicy.fractional.L2::evict_last.b64 %%0, 1.0;\" : \"=l\"(l2_keep));");
+            S("#define LDG_CELL(ptr, lo, hi) ldg_cell_hint(ptr, lo, hi, l2_keep)");
+        } else
+            S("#define LDG_CELL(ptr, lo, hi) ldg_cell(ptr, lo, hi)");
         S("    constexpr float K_cutoff2 = %s, K_lw2b = %s, K_q = %s, K_m3q = %s, K_c4 = %s, K_sigma = %s, K_eA = %s, K_eB = %s;",
           k_cutoff2.c_str(), k_lw2b.c_str(), k_q.c_str(), k_m3q.c_str(), k_c4.c_str(), k_sigma.c_str(), k_eA.c_str(), k_eB.c_str());
         S("    const float K_lw1 = %s, K_whp = %s, K_whbp = %s;", k_lw1.c_str(), k_whp.c_str(), k_whbp.c_str());
@@ -994,6 +1023,34 @@ std::pair<uint64_t, uint64_t> jit_key(const dock_params *p, const dock_grid *g, 
 
 }  // namespace
 
+// Quad image for the specialised kernel: float4 [n_maps][ny][nx][nz], entry (ix,iy,iz) = {G(ix,iy), G(ix+1,iy), G(ix,iy+1),
+// G(ix+1,iy+1)} of plane iz (indices clamped to the last node).  4x the map bytes instead of the 8x of the Cell8 image:
+// 68 MB for 81^3 x 8, which an L2 half (63 MB per die; the 136 MB Cell8 image hits 46 %) nearly holds; a lookup is two
+// adjacent 16-byte loads.  Rebuilt from the plain maps into the caller's workspace by every call (tens of microseconds).
+namespace {
+__global__ void __launch_bounds__(256) quad_pack_kernel(const float *__restrict__ data, float4 *__restrict__ quad, int nx, int ny, int nz, int zt)
+{
+    __shared__ float4 tile[32][9];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;              // read phase: ix = tile + tx, iz = tile + ty
+    const int iy = blockIdx.y, m = blockIdx.z / zt, iz0 = (blockIdx.z % zt) * 8, ix0 = blockIdx.x * 32;
+    {
+        const int ix = min(ix0 + tx, nx - 1), iz = min(iz0 + ty, nz - 1);
+        const int ix1 = min(ix + 1, nx - 1), iy1 = min(iy + 1, ny - 1);
+        const float *pl = data + ((size_t)m * nz + iz) * ny * nx;
+        tile[tx][ty] = make_float4(pl[(size_t)iy * nx + ix], pl[(size_t)iy * nx + ix1], pl[(size_t)iy1 * nx + ix], pl[(size_t)iy1 * nx + ix1]);
+    }
+    __syncthreads();
+    const int wx = threadIdx.x >> 3, wz = threadIdx.x & 7;               // write phase: 8 consecutive iz per ix
+    if (ix0 + wx < nx && iz0 + wz < nz) quad[(((size_t)m * ny + iy) * nx + ix0 + wx) * nz + iz0 + wz] = tile[wx][wz];
+}
+}  // namespace
+
+size_t jit_score_ws_bytes(const dock_grid *g)
+{
+    if (!g || !jit_default_opts().quad) return 0;
+    return align_up((size_t)g->n_maps * g->dims[0] * g->dims[1] * g->dims[2] * sizeof(float4), 256);
+}
+
 JitOpts jit_default_opts()
 {
     JitOpts o;
@@ -1006,6 +1063,8 @@ JitOpts jit_default_opts()
     o.reuse = 1;
     o.grid_unroll = 1;
     o.grid_sets = 2;
+    o.quad = 1;
+    o.l2_hint = 0;           // measured: 0.925 ms with evict_last on the gathers, 0.838 ms without; the L2 hit rate stays 46 %
     o.prefetch = 0;          // measured: 0.853-0.873 ms with it, 0.841 ms without (configs[1])
     o.atom_unroll = 2;
     if (const char *e = getenv("DOCK_JIT_TUNE")) {        // tuning aid, e.g. "group=6,warps=8,minb=1,gu=2,reuse=2"
@@ -1016,6 +1075,8 @@ JitOpts jit_default_opts()
         if ((q = strstr(e, "minb=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 1 && v <= 16) o.min_blocks = v;
         if ((q = strstr(e, "maxrreg=")) && sscanf(q + 8, "%d", &v) == 1 && v >= 0 && v <= 255) o.maxrreg = v;
         if ((q = strstr(e, "sync=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 0 && v <= 1024) o.sync_every = v;
+        if ((q = strstr(e, "quad=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 0 && v <= 1) o.quad = v;
+        if ((q = strstr(e, "l2=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 0 && v <= 1) o.l2_hint = v;
         if ((q = strstr(e, "pf=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 0 && v <= 1) o.prefetch = v;
         if ((q = strstr(e, "gs=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 2 && v <= 6) o.grid_sets = v;
         if ((q = strstr(e, "au=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 1 && v <= 8) o.atom_unroll = v;
@@ -1041,7 +1102,7 @@ int jit_score_source(const dock_params *p, const dock_grid *g, const dock_ligand
 
 int jit_score_launch(const dock_params *p, const dock_grid *g, const dock_ligand *L, const DevParams &P, const DevGrid &G,
                      long long n_poses, const float *poses_dev, float *energy_dev, float *grad_dev, float *terms_dev,
-                     cudaStream_t stream)
+                     void *quad_ws, bool pack, cudaStream_t stream)
 {
     if (!p || !g || !L || L->N < 1 || L->N > DOCK_JIT_MAX_ATOMS || L->T < 0 || L->P < 0 || g->n_channels == 4) return DOCK_EINVAL;
     if (!L->ref_xyz || !L->type || !L->atom_fragment || (L->T > 0 && (!L->tors_parent || !L->tors_a || !L->tors_b)) || (L->P > 0 && !L->pairs))
@@ -1075,13 +1136,21 @@ int jit_score_launch(const dock_params *p, const dock_grid *g, const dock_ligand
         k = it->second;
     }
     if (k.status != DOCK_OK) return k.status;
+    if (o.quad) {
+        if (!quad_ws) return DOCK_EWORKSPACE;
+        if (pack) {
+            const int zt = (G.nz + 7) / 8;
+            quad_pack_kernel<<<dim3((G.nx + 31) / 32, G.ny, g->n_maps * zt), 256, 0, stream>>>(G.data, (float4 *)quad_ws, G.nx, G.ny, G.nz, zt);
+            DOCK_LAUNCH_CHECK();
+        }
+    }
     JitArgs a;
-    a.nx = G.nx; a.ny = G.ny; a.icx = G.icx; a.icy = G.icy; a.icz = G.icz;
+    a.nx = G.nx; a.ny = G.ny; a.nz = G.nz; a.icx = G.icx; a.icy = G.icy; a.icz = G.icz;
     a.rx = G.rx; a.ry = G.ry; a.rz = G.rz; a.rdx = G.rdx; a.rdy = G.rdy; a.rdz = G.rdz;
     a.lo_x = G.lo_x; a.lo_y = G.lo_y; a.lo_z = G.lo_z; a.hi_x = G.hi_x; a.hi_y = G.hi_y; a.hi_z = G.hi_z;
     a.inv_h = G.inv_h; a.inv_h_lo = G.inv_h_lo; a.kw_g = G.kw_g; a.kw_e = G.kw_e;
     a.map_stride = (long long)G.chan_stride * G.channels;
-    a.packed = G.packed;
+    a.packed = o.quad ? quad_ws : (const void *)G.packed;
     a.n_poses = n_poses; a.poses = poses_dev; a.energy = energy_dev; a.grad = grad_dev; a.terms = terms_dev;
     const long long per_cta = 32LL * k.warps;
     const long long blocks = (n_poses + per_cta - 1) / per_cta;
