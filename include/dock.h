@@ -80,7 +80,8 @@ typedef struct dock_params {
     int32_t score_kernel;                     /* dock_score_batch[_host]: 0 or 1 = the generic thread-per-pose kernel; 2 = a kernel specialised
                                                * for this ligand, generated and compiled at run time (NVRTC, 0.4-6 s per ligand, cached per
                                                * device / ligand / parameters): DOCK_ECUDA if the compiler is missing, DOCK_EINVAL above 40
-                                               * atoms or with eq. 4 maps.  Same arithmetic per pair / atom / torsion; sums are taken in a
+                                               * atoms or with eq. 4 maps.  It keeps its own 4-corner map image in the workspace (rebuilt by
+                                               * every call), so *needed grows by 16 bytes per map node.  Same arithmetic per pair / atom / torsion; sums are taken in a
                                                * different order */
 } dock_params;
 
