@@ -246,21 +246,25 @@ __device__ __forceinline__ int cell_index(const JitArgs &G, float x, float y, fl
     return JIT_QUAD ? (iy * G.nx + ix) * G.nz + iz : (iz * G.ny + iy) * G.nx + ix;
 }
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
-// eq. 2 + eq. 3 + wall (reading S7), same arithmetic as mathx.cuh::trilinear
+// eq. 2 + eq. 3 + wall (reading S7).  Same interpolant as mathx.cuh::trilinear, evaluated z first, then y, then x so that
+// the four (x,y) corners of a plane run two per fp32x2 instruction: 8 packed + 6 scalar instructions instead of 22.
 __device__ __forceinline__ float trilinear(const JitArgs &G, const CellRef &c, const float4 q0, const float4 q1,
                                            float &e_wall, float &gx, float &gy, float &gz)
 {
-    const float d00 = q0.y - q0.x, d10 = q0.w - q0.z, d01 = q1.y - q1.x, d11 = q1.w - q1.z;
-    const float c00 = fmaf(c.px, d00, q0.x), c10 = fmaf(c.px, d10, q0.z);
-    const float c01 = fmaf(c.px, d01, q1.x), c11 = fmaf(c.px, d11, q1.z);
-    const float dy0 = c10 - c00, dy1 = c11 - c01;
-    const float c0 = fmaf(c.py, dy0, c00), c1 = fmaf(c.py, dy1, c01);
-    const float dz = c1 - c0;
-    const float e = fmaf(c.pz, dz, c0);
-    const float dx0 = fmaf(c.py, d10 - d00, d00), dx1 = fmaf(c.py, d11 - d01, d01);
-    float ggx = fmaf(c.pz, dx1 - dx0, dx0) * G.inv_h;
-    float ggy = fmaf(c.pz, dy1 - dy0, dy0) * G.inv_h;
-    float ggz = dz * G.inv_h;
+    const f32x2 lo0 = pk2(q0.x, q0.y), hi0 = pk2(q0.z, q0.w);             // plane iz: (x0,x1) at y0, (x0,x1) at y1
+    const f32x2 dzl = sub2(pk2(q1.x, q1.y), lo0), dzh = sub2(pk2(q1.z, q1.w), hi0);
+    const f32x2 pz2 = bc2(c.pz), py2 = bc2(c.py);
+    const f32x2 cl = fma2(pz2, dzl, lo0), ch = fma2(pz2, dzh, hi0);        // interpolated along z
+    const f32x2 dy = sub2(ch, cl);
+    const f32x2 cy = fma2(py2, dy, cl);                                    // ... along y: (value at x0, value at x1)
+    const f32x2 dzy = fma2(py2, sub2(dzh, dzl), dzl);                      // d/dz interpolated along y
+    float c0, c1, dy0, dy1, dz0, dz1;
+    up2(cy, c0, c1); up2(dy, dy0, dy1); up2(dzy, dz0, dz1);
+    const float ex = c1 - c0;
+    const float e = fmaf(c.px, ex, c0);                                    // eq. 2
+    float ggx = ex * G.inv_h;                                              // eq. 3
+    float ggy = fmaf(c.px, dy1 - dy0, dy0) * G.inv_h;
+    float ggz = fmaf(c.px, dz1 - dz0, dz0) * G.inv_h;
     if (c.ox != 0.0f) ggx = 0.0f;
     if (c.oy != 0.0f) ggy = 0.0f;
     if (c.oz != 0.0f) ggz = 0.0f;
