@@ -80,8 +80,7 @@ typedef struct dock_params {
     int32_t score_kernel;                     /* dock_score_batch[_host]: 0 or 1 = the generic thread-per-pose kernel; 2 = a kernel specialised
                                                * for this ligand, generated and compiled at run time (NVRTC, 0.4-6 s per ligand, cached per
                                                * device / ligand / parameters): DOCK_ECUDA if the compiler is missing, DOCK_EINVAL above 40
-                                               * atoms or with eq. 4 maps.  It keeps its own 4-corner map image in the workspace (rebuilt by
-                                               * every call), so *needed grows by 16 bytes per map node.  Same arithmetic per pair / atom / torsion; sums are taken in a
+                                               * atoms or with eq. 4 maps (it reads dock_grid.quad_dev).  Same arithmetic per pair / atom / torsion; sums are taken in a
                                                * different order */
 } dock_params;
 
@@ -122,7 +121,8 @@ typedef struct dock_ligand {
  *              (ix,iy,iz) = the 8 corners of the cell whose low corner is that node, in the order
  *              {G(ix,iy,iz), G(ix+1,iy,iz), G(ix,iy+1,iz), G(ix+1,iy+1,iz)} then the same four at
  *              iz+1 (indices clamped to the last node), so a cell is ONE aligned 32-byte load
- *              (DESIGN.md "Data layout").  Values are bit-identical copies of data_dev. */
+ *              (DESIGN.md "Data layout").  Values are bit-identical copies of data_dev.
+ *   quad_dev   the 4-corner image described at the field (single-channel maps only). */
 typedef struct dock_grid {
     int32_t      dims[3];                          /* nx, ny, nz */
     float        origin[3];
@@ -133,6 +133,10 @@ typedef struct dock_grid {
     const float *packed_dev;                       /* DEVICE pointer into the same buffer */
     int32_t      n_channels;                       /* 1: data_dev [n_maps][nz][ny][nx]; 4 (eq. 4): [n_maps][4][nz][ny][nx] with channels
                                                     * (score, d/dx, d/dy, d/dz) -- packed_dev likewise; 0 is read as 1 */
+    const float *quad_dev;                         /* DEVICE pointer into the same buffer, or NULL (eq. 4 maps): the 4-corner image
+                                                    * [n_maps][ny][nx][nz][4] = {G(ix,iy,iz), G(ix+1,iy,iz), G(ix,iy+1,iz), G(ix+1,iy+1,iz)},
+                                                    * z fastest, so the planes iz and iz+1 of a cell are two adjacent 16-byte loads; half
+                                                    * the bytes of packed_dev (it fits an L2 half); read by the specialised score kernel */
 } dock_grid;
 
 /* Optional per-(system, copy, step) trace of the search; with the stateless Philox counter it

@@ -73,7 +73,7 @@ class dock_grid(C.Structure):
     _fields_ = [
         ("dims", C.c_int32 * 3), ("origin", C.c_float * 3), ("spacing", C.c_float),
         ("n_maps", C.c_int32), ("type_to_map", C.c_int32 * DOCK_MAX_XS_TYPES), ("data_dev", C.c_void_p),
-        ("packed_dev", C.c_void_p), ("n_channels", C.c_int32),
+        ("packed_dev", C.c_void_p), ("n_channels", C.c_int32), ("quad_dev", C.c_void_p),
     ]
 
 

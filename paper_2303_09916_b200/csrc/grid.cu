@@ -34,6 +34,7 @@ struct GridSysArgs {
     int   pad_;
     float *out;            // [n_maps][channels][nz][ny][nx]
     Cell8 *packed;         // gather image of the same maps
+    float4 *quad;          // 4-corner image (single-channel maps), or NULL
 };
 
 struct GridBuildArgs {
@@ -233,6 +234,27 @@ __global__ void __launch_bounds__(256) grid_pack_kernel(const GridSysArgs *__res
     }
 }
 
+// 4-corner image (dock.h: dock_grid.quad_dev): float4 [n_maps][ny][nx][nz].  A 32 (x) by 8 (z) tile goes through shared
+// memory: rows of the plain maps are read along x, entries are written along z.  blockIdx.z = (system, map, z tile).
+__global__ void __launch_bounds__(256) grid_quad_kernel(const GridSysArgs *__restrict__ sys, int n_maps, int zt_max)
+{
+    __shared__ float4 tile[32][9];
+    const GridSysArgs S = sys[blockIdx.z / (n_maps * zt_max)];
+    const int rem = blockIdx.z % (n_maps * zt_max), m = rem / zt_max, iz0 = (rem % zt_max) * 8, ix0 = blockIdx.x * 32, iy = blockIdx.y;
+    const int nx = S.nx, ny = S.ny, nz = S.nz;
+    if (!S.quad || iy >= ny || ix0 >= nx || iz0 >= nz) return;        // uniform per block
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    {
+        const int ix = min(ix0 + tx, nx - 1), iz = min(iz0 + ty, nz - 1);
+        const int ix1 = min(ix + 1, nx - 1), iy1 = min(iy + 1, ny - 1);
+        const float *pl = S.out + ((size_t)m * nz + iz) * ny * nx;
+        tile[tx][ty] = make_float4(pl[(size_t)iy * nx + ix], pl[(size_t)iy * nx + ix1], pl[(size_t)iy1 * nx + ix], pl[(size_t)iy1 * nx + ix1]);
+    }
+    __syncthreads();
+    const int wx = threadIdx.x >> 3, wz = threadIdx.x & 7;
+    if (ix0 + wx < nx && iz0 + wz < nz) S.quad[(((size_t)m * ny + iy) * nx + ix0 + wx) * nz + iz0 + wz] = tile[wx][wz];
+}
+
 struct GridPlan {
     int dims[3];
     float origin[3];
@@ -333,7 +355,7 @@ extern "C" size_t dock_grid_bytes(const dock_params *params, const dock_box *box
     if (!params || n_lig_types < 1 || n_lig_types > DOCK_MAX_XS_TYPES || dock_grid_dims(box, dims) != DOCK_OK) return 0;
     const size_t ch = params->grad_mode == 1 ? 4 : 1;
     const size_t nodes = (size_t)dims[0] * dims[1] * dims[2] * (size_t)n_lig_types * ch;
-    return align_up(nodes * sizeof(float), 256) + nodes * sizeof(Cell8);
+    return align_up(nodes * sizeof(float), 256) + align_up(nodes * sizeof(Cell8), 256) + (ch == 1 ? nodes * sizeof(float4) : 0);
 }
 
 // All systems in ONE upload and two launches (build, pack): the per-system lattice descriptions, cell lists and sorted
@@ -390,6 +412,7 @@ extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_syste
         const size_t nodes = (size_t)sys[s].nx * sys[s].ny * sys[s].nz * (size_t)n_lig_types * channels;
         sys[s].out = grid_dev[s];
         sys[s].packed = reinterpret_cast<Cell8 *>(reinterpret_cast<unsigned char *>(grid_dev[s]) + align_up(nodes * sizeof(float), 256));
+        sys[s].quad = channels == 1 ? reinterpret_cast<float4 *>(reinterpret_cast<unsigned char *>(sys[s].packed) + align_up(nodes * sizeof(Cell8), 256)) : nullptr;
     }
     // one host image, one copy
     std::vector<unsigned char> image(need, 0);
@@ -424,6 +447,15 @@ extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_syste
     const unsigned pack_x = (unsigned)std::max(1, std::min(148 * 16, 148 * 16 * 4 / n_systems + 1));
     grid_pack_kernel<<<dim3(pack_x, (unsigned)n_systems), 256, 0, stream>>>(A.sys, n_lig_types * channels);
     DOCK_LAUNCH_CHECK();
+    if (channels == 1) {
+        int mx = 0, my = 0, mz = 0;
+        for (int s = 0; s < n_systems; ++s) { mx = std::max(mx, sys[s].nx); my = std::max(my, sys[s].ny); mz = std::max(mz, sys[s].nz); }
+        const int zt = (mz + 7) / 8;
+        const long long gz = (long long)n_systems * n_lig_types * zt;
+        if (gz > 65535 || my > 65535) return DOCK_EINVAL;
+        grid_quad_kernel<<<dim3((unsigned)((mx + 31) / 32), (unsigned)my, (unsigned)gz), 256, 0, stream>>>(A.sys, n_lig_types, zt);
+        DOCK_LAUNCH_CHECK();
+    }
 
     for (int s = 0; s < n_systems; ++s) {
         dock_grid *d = &out_descs[s];
@@ -436,6 +468,7 @@ extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_syste
         d->data_dev = grid_dev[s];
         d->packed_dev = reinterpret_cast<const float *>(sys[s].packed);
         d->n_channels = channels;
+        d->quad_dev = reinterpret_cast<const float *>(sys[s].quad);
     }
     return DOCK_OK;
 }

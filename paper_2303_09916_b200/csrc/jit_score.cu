@@ -14,6 +14,8 @@
 //   phase 1   A2: loop over fragments and atoms, tables in the constant bank, frames in shared memory.  Coordinates
 //             go to shared memory packed by DUO (two atoms that share fp32x2 register pairs): float4 (x0,x1,y0,y1)
 //             + float2 (z0,z1).
+//   (map image) the gathers read dock_grid.quad_dev, the 4-corner image (68 MB for 81^3 x 8: it fits an L2 half, which the
+//             136 MB 8-corner image of the other evaluators does not -- L2 hit rate 78 % against 46 %).
 //   phase 2a  A3: loop over duos, 2U atoms per iteration, software-pipelined by one iteration (the 32-byte map
 //             gathers of the next atoms are in flight while the current ones are interpolated); sigma-scaled grid
 //             forces go to shared memory and seed the force registers.
@@ -1027,34 +1029,6 @@ std::pair<uint64_t, uint64_t> jit_key(const dock_params *p, const dock_grid *g, 
 
 }  // namespace
 
-// Quad image for the specialised kernel: float4 [n_maps][ny][nx][nz], entry (ix,iy,iz) = {G(ix,iy), G(ix+1,iy), G(ix,iy+1),
-// G(ix+1,iy+1)} of plane iz (indices clamped to the last node).  4x the map bytes instead of the 8x of the Cell8 image:
-// 68 MB for 81^3 x 8, which an L2 half (63 MB per die; the 136 MB Cell8 image hits 46 %) nearly holds; a lookup is two
-// adjacent 16-byte loads.  Rebuilt from the plain maps into the caller's workspace by every call (tens of microseconds).
-namespace {
-__global__ void __launch_bounds__(256) quad_pack_kernel(const float *__restrict__ data, float4 *__restrict__ quad, int nx, int ny, int nz, int zt)
-{
-    __shared__ float4 tile[32][9];
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;              // read phase: ix = tile + tx, iz = tile + ty
-    const int iy = blockIdx.y, m = blockIdx.z / zt, iz0 = (blockIdx.z % zt) * 8, ix0 = blockIdx.x * 32;
-    {
-        const int ix = min(ix0 + tx, nx - 1), iz = min(iz0 + ty, nz - 1);
-        const int ix1 = min(ix + 1, nx - 1), iy1 = min(iy + 1, ny - 1);
-        const float *pl = data + ((size_t)m * nz + iz) * ny * nx;
-        tile[tx][ty] = make_float4(pl[(size_t)iy * nx + ix], pl[(size_t)iy * nx + ix1], pl[(size_t)iy1 * nx + ix], pl[(size_t)iy1 * nx + ix1]);
-    }
-    __syncthreads();
-    const int wx = threadIdx.x >> 3, wz = threadIdx.x & 7;               // write phase: 8 consecutive iz per ix
-    if (ix0 + wx < nx && iz0 + wz < nz) quad[(((size_t)m * ny + iy) * nx + ix0 + wx) * nz + iz0 + wz] = tile[wx][wz];
-}
-}  // namespace
-
-size_t jit_score_ws_bytes(const dock_grid *g)
-{
-    if (!g || !jit_default_opts().quad) return 0;
-    return align_up((size_t)g->n_maps * g->dims[0] * g->dims[1] * g->dims[2] * sizeof(float4), 256);
-}
-
 JitOpts jit_default_opts()
 {
     JitOpts o;
@@ -1106,7 +1080,7 @@ int jit_score_source(const dock_params *p, const dock_grid *g, const dock_ligand
 
 int jit_score_launch(const dock_params *p, const dock_grid *g, const dock_ligand *L, const DevParams &P, const DevGrid &G,
                      long long n_poses, const float *poses_dev, float *energy_dev, float *grad_dev, float *terms_dev,
-                     void *quad_ws, bool pack, cudaStream_t stream)
+                     cudaStream_t stream)
 {
     if (!p || !g || !L || L->N < 1 || L->N > DOCK_JIT_MAX_ATOMS || L->T < 0 || L->P < 0 || g->n_channels == 4) return DOCK_EINVAL;
     if (!L->ref_xyz || !L->type || !L->atom_fragment || (L->T > 0 && (!L->tors_parent || !L->tors_a || !L->tors_b)) || (L->P > 0 && !L->pairs))
@@ -1140,21 +1114,14 @@ int jit_score_launch(const dock_params *p, const dock_grid *g, const dock_ligand
         k = it->second;
     }
     if (k.status != DOCK_OK) return k.status;
-    if (o.quad) {
-        if (!quad_ws) return DOCK_EWORKSPACE;
-        if (pack) {
-            const int zt = (G.nz + 7) / 8;
-            quad_pack_kernel<<<dim3((G.nx + 31) / 32, G.ny, g->n_maps * zt), 256, 0, stream>>>(G.data, (float4 *)quad_ws, G.nx, G.ny, G.nz, zt);
-            DOCK_LAUNCH_CHECK();
-        }
-    }
+    if (o.quad && !g->quad_dev) return DOCK_EINVAL;        // descriptor without the 4-corner image (dock.h: dock_grid.quad_dev)
     JitArgs a;
     a.nx = G.nx; a.ny = G.ny; a.nz = G.nz; a.icx = G.icx; a.icy = G.icy; a.icz = G.icz;
     a.rx = G.rx; a.ry = G.ry; a.rz = G.rz; a.rdx = G.rdx; a.rdy = G.rdy; a.rdz = G.rdz;
     a.lo_x = G.lo_x; a.lo_y = G.lo_y; a.lo_z = G.lo_z; a.hi_x = G.hi_x; a.hi_y = G.hi_y; a.hi_z = G.hi_z;
     a.inv_h = G.inv_h; a.inv_h_lo = G.inv_h_lo; a.kw_g = G.kw_g; a.kw_e = G.kw_e;
     a.map_stride = (long long)G.chan_stride * G.channels;
-    a.packed = o.quad ? quad_ws : (const void *)G.packed;
+    a.packed = o.quad ? (const void *)g->quad_dev : (const void *)G.packed;
     a.n_poses = n_poses; a.poses = poses_dev; a.energy = energy_dev; a.grad = grad_dev; a.terms = terms_dev;
     const long long per_cta = 32LL * k.warps;
     const long long blocks = (n_poses + per_cta - 1) / per_cta;

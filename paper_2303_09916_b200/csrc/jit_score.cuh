@@ -16,7 +16,7 @@ struct JitOpts {          // all ints: hashed as raw bytes (no padding)
     int reuse;          // a duo's coordinates loaded for group g are reused by groups g+1 .. g+reuse before being reloaded
     int grid_unroll;    // duos per iteration of the map-lookup loop
     int grid_sets;      // register sets of the map-lookup loop (grid_sets - 1 gathers-in-flight sets ahead of the interpolation)
-    int quad;           // 1: gathers read the quad image (float4 per (x,y) cell and plane, rebuilt in the workspace per call)
+    int quad;           // 1: gathers read the 4-corner image dock_grid.quad_dev (two adjacent 16-byte loads); 0: the Cell8 image
     int l2_hint;        // 1: the map gathers carry an L2 evict_last policy
     int prefetch;       // 1: the kinematics loop prefetches every atom's map cell into L2
     int atom_unroll;    // unroll factor of the atom loop of the kinematics
@@ -29,6 +29,4 @@ bool jit_available();
 int jit_score_source(const dock_params *p, const dock_grid *g, const dock_ligand *L, const JitOpts &o, std::string &out);
 int jit_score_launch(const dock_params *p, const dock_grid *g, const dock_ligand *L, const DevParams &P, const DevGrid &G,
                      long long n_poses, const float *poses_dev, float *energy_dev, float *grad_dev, float *terms_dev,
-                     void *quad_ws, bool pack, cudaStream_t stream);
-// bytes of workspace the specialised kernel wants for its own map image (0 if it reads the Cell8 image)
-size_t jit_score_ws_bytes(const dock_grid *g);
+                     cudaStream_t stream);

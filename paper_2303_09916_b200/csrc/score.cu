@@ -149,13 +149,12 @@ extern "C" int dock_score_batch(const dock_params *params, const dock_grid *grid
     const int rc = plan_score(params, grid, ligand, pl);
     if (rc != DOCK_OK) return rc;
     if (n_poses < 0) return DOCK_EINVAL;
-    const size_t b_quad = params->score_kernel == 2 ? jit_score_ws_bytes(grid) : 0;      // the specialised kernel's map image
-    if (needed) *needed = pl.need + b_quad;
-    if (!ws_dev || ws_bytes < pl.need + b_quad) return DOCK_EWORKSPACE;
+    if (needed) *needed = pl.need;
+    if (!ws_dev || ws_bytes < pl.need) return DOCK_EWORKSPACE;
     if (n_poses > 0 && (!poses_dev || !energy_dev)) return DOCK_EINVAL;
     if (use_jit(params, grid, ligand, n_poses)) {
         const int rj = jit_score_launch(params, grid, ligand, pl.P, pl.G, n_poses, poses_dev, energy_dev, grad_dev, terms_dev,
-                                        (unsigned char *)ws_dev + pl.need, true, (cudaStream_t)stream_);
+                                        (cudaStream_t)stream_);
         if (rj == DOCK_OK || params->score_kernel == 2) return rj;      // forced: report the failure; auto: generic kernel
     }
     return score_launch(pl, n_poses, poses_dev, energy_dev, grad_dev, terms_dev, ws_dev, (cudaStream_t)stream_);
@@ -176,8 +175,7 @@ extern "C" int dock_score_batch_host(const dock_params *params, const dock_grid 
     const size_t b_e = align_up((size_t)n_poses * sizeof(float), 256);
     const size_t b_g = grad_host ? align_up((size_t)n_poses * ng * sizeof(float), 256) : 0;
     const size_t b_t = terms_host ? align_up((size_t)n_poses * 3 * sizeof(float), 256) : 0;
-    const size_t b_quad = params->score_kernel == 2 ? jit_score_ws_bytes(grid) : 0;
-    const size_t need = b_blob + b_pose + b_e + b_g + b_t + b_quad;
+    const size_t need = b_blob + b_pose + b_e + b_g + b_t;
     if (needed) *needed = need;
     if (!ws_dev || ws_bytes < need) return DOCK_EWORKSPACE;
     if (n_poses > 0 && (!poses_host || !energy_host)) return DOCK_EINVAL;
@@ -214,7 +212,7 @@ extern "C" int dock_score_batch_host(const dock_params *params, const dock_grid 
             DOCK_CUDA_CHECK(cudaStreamWaitEvent(stream, hp.ev_in[c], 0));
             int rc2 = DOCK_EINVAL;
             if (jit) rc2 = jit_score_launch(params, grid, ligand, pl.P, pl.G, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr,
-                                            d_t ? d_t + o * 3 : nullptr, ws + b_blob + b_pose + b_e + b_g + b_t, c == 0, stream);
+                                            d_t ? d_t + o * 3 : nullptr, stream);
             if (rc2 != DOCK_OK && !(jit && params->score_kernel == 2))
                 rc2 = score_launch(pl, m, d_pose + o * np_, d_e + o, d_g ? d_g + o * ng : nullptr, d_t ? d_t + o * 3 : nullptr,
                                    ws, stream, !uploaded), uploaded = true;

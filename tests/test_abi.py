@@ -88,7 +88,11 @@ def test_build_grids_size_query_and_validation(lib):
     one = dk.dock_grid_bytes(p, box, len(lt))
     p4 = dk.dock_default_params()
     p4.grad_mode = 1
-    assert dk.dock_grid_bytes(p4, box, len(lt)) == 4 * (one - one % 256) + (256 if one % 256 else 0) or dk.dock_grid_bytes(p4, box, len(lt)) > 3 * one
+    nodes = int(np.prod(dk.dock_grid_dims(box))) * len(lt)
+    up = lambda b: (b + 255) // 256 * 256
+    assert one == up(4 * nodes) + up(32 * nodes) + 16 * nodes              # maps + 8-corner image + 4-corner image (dock.h)
+    four = dk.dock_grid_bytes(p4, box, len(lt))
+    assert four == up(16 * nodes) + up(128 * nodes) and four > one         # eq. 4: four channels, no 4-corner image
     desc = B.dock_grid()
     rc = lib.dock_build_grids(C.byref(p4), C.byref(prot), C.byref(box), len(lt), lt.ctypes.data_as(C.c_void_p),
                               C.c_void_p(1 << 20), C.c_size_t(one), C.byref(desc), C.c_void_p(1 << 21), C.c_size_t(need.value),

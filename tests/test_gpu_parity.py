@@ -950,3 +950,21 @@ def test_specialised_score_kernel_limits(dk, torch, micro):
         dk.dock_score_batch(_jit_params(dk), grid, lig, poses)
     e, _, _ = dk.dock_score_batch(dk.dock_default_params(), grid, lig, poses)      # default: generic kernel
     assert bool(torch.isfinite(e).all())
+
+
+def test_quad_image_is_a_copy_of_the_maps(dk, torch, tiny):
+    """dock_grid.quad_dev (read by the specialised score kernel): entry (m, iy, ix, iz) = the four (x, y) corners of the
+    cell at plane iz, bit-identical copies of data_dev, indices clamped at the last node."""
+    import ctypes as C
+    s, (p, box, grid, lig), _ = tiny
+    nx, ny, nz = grid.dims
+    nm = grid.data.shape[0]
+    assert grid.desc.quad_dev
+    off = grid.desc.quad_dev - grid.buf.data_ptr()
+    quad = grid.buf[off: off + nm * ny * nx * nz * 16].view(torch.float32).view(nm, ny, nx, nz, 4).cpu().numpy()
+    g = grid.data.cpu().numpy()                                            # [m][z][y][x]
+    ix1 = np.minimum(np.arange(nx) + 1, nx - 1)
+    iy1 = np.minimum(np.arange(ny) + 1, ny - 1)
+    gt = g.transpose(0, 2, 3, 1)                                           # [m][y][x][z]
+    want = np.stack([gt, gt[:, :, ix1, :], gt[:, iy1, :, :], gt[:, iy1][:, :, ix1]], axis=-1)
+    assert np.array_equal(quad, want)
