@@ -494,7 +494,7 @@ def run_ours(args) -> dict:
 # per-launch DRAM traffic of the score kernels from the committed `ncu --set full` captures
 TRAFFIC_BYTES_PER_LAUNCH = {
     "score_thread_kernel": 821.8e6,   # profiles/r2c_score_thread_kernel_details.txt: dram read 755.6 MB + write 66.2 MB
-    "dock_score_jit": 232.8e6,        # profiles/r2b_dock_score_jit_details.txt: dram read 173.5 MB + write 59.3 MB (quad map image)
+    "dock_score_jit": 237.4e6,        # profiles/r2b_dock_score_jit_details.txt: dram read 177.0 MB + write 60.4 MB (4-corner map image)
 }
 
 
