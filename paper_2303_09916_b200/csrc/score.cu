@@ -132,7 +132,7 @@ int pipe_init(HostPipe &hp)
 }
 
 // The ligand-specialised kernel (jit_score.cu) is opt-in: it costs a run-time compilation per ligand (0.4-6 s, cached) and
-// gains 1.10x on BASELINE configs[1] (profiles/r2b.md), so score_kernel = 0 keeps the generic kernel.
+// gains 1.15x on BASELINE configs[1] (profiles/r2b.md), so score_kernel = 0 keeps the generic kernel.
 bool use_jit(const dock_params *params, const dock_grid *grid, const dock_ligand *lig, int64_t n_poses)
 {
     return params->score_kernel == 2 && n_poses >= 1 && lig && grid;
