@@ -438,7 +438,7 @@ struct Gen {
         S("    float2 *const fr = reinterpret_cast<float2 *>(reg2) + lane;     // [T][6], stride 32");
         S("    float m00, m01, m02, m10, m11, m12, m20, m21, m22, c0 = 0.0f, c1 = 0.0f, c2 = 0.0f;");
         S("    {");
-        S("        float w = pose[3], x = pose[4], y = pose[5], z = pose[6];");
+        S("        float w = POSE(3), x = POSE(4), y = POSE(5), z = POSE(6);");
         S("        const float n2 = fmaf(w, w, fmaf(x, x, fmaf(y, y, z * z)));");
         S("        if (n2 > 0.0f) { const float inv = 1.0f / sqrtf(n2); w *= inv; x *= inv; y *= inv; z *= inv; } else { w = 1.0f; x = y = z = 0.0f; }");
         S("        const float x2 = x + x, y2 = y + y, z2 = z + z;");
@@ -450,7 +450,7 @@ struct Gen {
         if (T > 0) {                                          // all torsion angles in one burst (one exposed load latency)
             S("    float *const thf = reinterpret_cast<float *>(reg2) + %d + lane;", 12 * T * 32);
             S("    #pragma unroll");
-            S("    for (int k = 0; k < %d; ++k) thf[k * 32] = pose[7 + k];", T);
+            S("    for (int k = 0; k < %d; ++k) thf[k * 32] = POSE(7 + k);", T);
         }
         S("    int s = 0;");
         S("    #pragma unroll 1");
@@ -844,7 +844,7 @@ struct Gen {
             S("        const float xbx = %s, xby = %s, xbz = %s;", sx(t.b_slot).c_str(), sy(t.b_slot).c_str(), sz(t.b_slot).c_str());
             S("        const float w = %s * K_sigma;", FS(t.inv_len));
             S("        const float ux = (xbx - %s) * w, uy = (xby - %s) * w, uz = (xbz - %s) * w;", sx(t.a_slot).c_str(), sy(t.a_slot).c_str(), sz(t.a_slot).c_str());
-            S("        grad[%d] = fmaf(ux, M%d_x, fmaf(uy, M%d_y, uz * M%d_z));", 6 + f - 1, f, f, f);
+            S("        OUT(grad + %d, fmaf(ux, M%d_x, fmaf(uy, M%d_y, uz * M%d_z)));", 6 + f - 1, f, f, f);
             const int p = t.parent;
             if (p > 0) {
                 S("        const float lx = xbx - o%d_x, ly = xby - o%d_y, lz = xbz - o%d_z;", p, p, p);
@@ -859,8 +859,8 @@ struct Gen {
             S("        F%d_x += F%d_x; F%d_y += F%d_y; F%d_z += F%d_z;", p, f, p, f, p, f);
             S("    }");
         }
-        S("    grad[0] = K_sigma * F0_x; grad[1] = K_sigma * F0_y; grad[2] = K_sigma * F0_z;");
-        S("    grad[3] = K_sigma * M0_x; grad[4] = K_sigma * M0_y; grad[5] = K_sigma * M0_z;");
+        S("    OUT(grad + 0, K_sigma * F0_x); OUT(grad + 1, K_sigma * F0_y); OUT(grad + 2, K_sigma * F0_z);");
+        S("    OUT(grad + 3, K_sigma * M0_x); OUT(grad + 4, K_sigma * M0_y); OUT(grad + 5, K_sigma * M0_z);");
     }
 
     std::string run()
@@ -869,6 +869,13 @@ struct Gen {
         S("// generated by libdock_b200 (jit_score.cu): N = %d, T = %d, P = %zu, grad = %d", d.N, d.T, d.pairs.size(), (int)o.want_grad);
         S("struct JitArgs { %s };", DOCK_JIT_STR(DOCK_JIT_ARGS_BODY));
         S("#define JIT_QUAD %d", o.quad ? 1 : 0);
+        if (o.stream) {                                   // poses and outputs pass through L2 once: streaming hints keep the maps in
+            S("#define POSE(k) __ldcs(pose + (k))");
+            S("#define OUT(ptr, v) __stcs(ptr, v)");
+        } else {
+            S("#define POSE(k) pose[k]");
+            S("#define OUT(ptr, v) (*(ptr) = (v))");
+        }
         S.s += k_prelude;
         S.s += tables();
         S("extern \"C\" __global__ void __launch_bounds__(%d, %d) dock_score_jit(const JitArgs a)", 32 * o.warps, o.min_blocks);
@@ -903,13 +910,13 @@ struct Gen {
         S("    constexpr float K_cutoff2 = %s, K_lw2b = %s, K_q = %s, K_m3q = %s, K_c4 = %s, K_sigma = %s, K_eA = %s, K_eB = %s;",
           k_cutoff2.c_str(), k_lw2b.c_str(), k_q.c_str(), k_m3q.c_str(), k_c4.c_str(), k_sigma.c_str(), k_eA.c_str(), k_eB.c_str());
         S("    const float K_lw1 = %s, K_whp = %s, K_whbp = %s;", k_lw1.c_str(), k_whp.c_str(), k_whbp.c_str());
-        S("    const float tx = (pose[0] - a.rx) - a.rdx, ty = (pose[1] - a.ry) - a.rdy, tz = (pose[2] - a.rz) - a.rdz;");
+        S("    const float tx = (POSE(0) - a.rx) - a.rdx, ty = (POSE(1) - a.ry) - a.rdy, tz = (POSE(2) - a.rz) - a.rdz;");
         kinematics();
         grid_loop();
         pair_phase();
         if (o.want_grad) chain_rule();
-        S("    a.energy[p] = e_grid + e_wall + e_intra;");
-        S("    if (a.terms) { a.terms[3 * p] = e_grid; a.terms[3 * p + 1] = e_wall; a.terms[3 * p + 2] = e_intra; }");
+        S("    OUT(a.energy + p, e_grid + e_wall + e_intra);");
+        S("    if (a.terms) { OUT(a.terms + 3 * p, e_grid); OUT(a.terms + 3 * p + 1, e_wall); OUT(a.terms + 3 * p + 2, e_intra); }");
         S("}");
         return S.s;
     }
@@ -1041,6 +1048,7 @@ JitOpts jit_default_opts()
     o.reuse = 1;
     o.grid_unroll = 1;
     o.grid_sets = 2;
+    o.stream = 1;
     o.quad = 1;
     o.l2_hint = 0;           // measured: 0.925 ms with evict_last on the gathers, 0.838 ms without; the L2 hit rate stays 46 %
     o.prefetch = 0;          // measured: 0.853-0.873 ms with it, 0.841 ms without (configs[1])
@@ -1053,6 +1061,7 @@ JitOpts jit_default_opts()
         if ((q = strstr(e, "minb=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 1 && v <= 16) o.min_blocks = v;
         if ((q = strstr(e, "maxrreg=")) && sscanf(q + 8, "%d", &v) == 1 && v >= 0 && v <= 255) o.maxrreg = v;
         if ((q = strstr(e, "sync=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 0 && v <= 1024) o.sync_every = v;
+        if ((q = strstr(e, "st=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 0 && v <= 1) o.stream = v;
         if ((q = strstr(e, "quad=")) && sscanf(q + 5, "%d", &v) == 1 && v >= 0 && v <= 1) o.quad = v;
         if ((q = strstr(e, "l2=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 0 && v <= 1) o.l2_hint = v;
         if ((q = strstr(e, "pf=")) && sscanf(q + 3, "%d", &v) == 1 && v >= 0 && v <= 1) o.prefetch = v;

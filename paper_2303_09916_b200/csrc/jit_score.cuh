@@ -16,6 +16,7 @@ struct JitOpts {          // all ints: hashed as raw bytes (no padding)
     int reuse;          // a duo's coordinates loaded for group g are reused by groups g+1 .. g+reuse before being reloaded
     int grid_unroll;    // duos per iteration of the map-lookup loop
     int grid_sets;      // register sets of the map-lookup loop (grid_sets - 1 gathers-in-flight sets ahead of the interpolation)
+    int stream;         // 1: pose loads / output stores carry streaming (evict-first) cache hints
     int quad;           // 1: gathers read the 4-corner image dock_grid.quad_dev (two adjacent 16-byte loads); 0: the Cell8 image
     int l2_hint;        // 1: the map gathers carry an L2 evict_last policy
     int prefetch;       // 1: the kinematics loop prefetches every atom's map cell into L2
