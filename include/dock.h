@@ -73,10 +73,11 @@ typedef struct dock_params {
                                                * per-vertex gradients (eq. 4; NEXT-2).  Read by dock_build_grids,
                                                * which then writes 4 channels per map; the evaluators follow dock_grid.n_channels */
     int32_t search_kernel;                    /* decomposition of dock_search / dock_local_opt_*: 1 = one warp per copy; 2 = one CTA of
-                                               * 4 warps per copy whose warps evaluate 4 consecutive backtracking trials of the line
-                                               * search at once (the latency form for a few hundred copies);
-                                               * 0 = chosen by the library from n_systems x copies.  Both give bit-identical results;
-                                               * only evaluations the sequential line search would make are counted */
+                                               * 4 warps per copy -- with BFGS the warps evaluate 4 consecutive backtracking trials of the
+                                               * line search at once (bit-identical to 1; only evaluations the sequential line search would
+                                               * make are counted), with Barzilai-Borwein (no line search) they share each evaluation (atoms
+                                               * over the threads, pair rounds over the warps: results agree with 1 to round-off);
+                                               * 0 = chosen by the library: 2 for n_systems x copies <= 512, else 1 */
     int32_t score_kernel;                     /* dock_score_batch[_host]: 0 or 1 = the generic thread-per-pose kernel; 2 = a kernel specialised
                                                * for this ligand, generated and compiled at run time (NVRTC, 0.4-6 s per ligand, cached per
                                                * device / ligand / parameters): DOCK_ECUDA if the compiler is missing, DOCK_EINVAL above 40

@@ -717,7 +717,7 @@ bool use_cta_kernel(const dock_params *p, long long total_copies)
 {
     if (p->search_kernel == 2) return true;
     if (p->search_kernel == 1) return false;
-    return p->optimizer == 0 && total_copies <= CTA_AUTO_MAX;       // Barzilai-Borwein has no line search to speculate on
+    return total_copies <= CTA_AUTO_MAX;       // BFGS: speculative line search; Barzilai-Borwein: the four warps share each evaluation
 }
 
 int local_opt_launch(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,

@@ -9,11 +9,15 @@
 // the extra, mostly discarded, work.  Every evaluation is the warp evaluator of eval_warp.cuh and warp 0 carries out the
 // optimizer's vector arithmetic exactly as local_opt_warp does, so the results are BIT-IDENTICAL to the warp-per-copy
 // kernel (tests/test_gpu_parity.py::test_search_kernels_agree_bitwise); only evaluations the sequential algorithm would
-// have made are counted.  Barzilai-Borwein has no line search: there the four warps evaluate the same pose.
+// have made are counted.  Barzilai-Borwein has no line search: there the four warps SHARE each evaluation (eval_cta.cuh:
+// atoms over the 128 threads, pair rounds over the warps), which changes the order of the force sums -- BB results of
+// the two kernels agree to round-off, not bit for bit.
 //
 // Selected by dock_params.search_kernel (0 = auto: this kernel when n_systems x copies is small, see search.cu).
 // (included by search.cu inside its anonymous namespace, after local_opt_warp's helpers)
 #pragma once
+
+#include "eval_cta.cuh"
 
 constexpr int CTA_WARPS = 4;
 constexpr int CTA_THREADS = CTA_WARPS * 32;
@@ -87,7 +91,10 @@ __device__ __forceinline__ float local_opt_spec(const DevParams &P, const DevGri
             if (init) for (int k = lane; k < np_; k += 32) xt_mine[k] = b.x[k];
             else pose_add_warp(T, b.x, b.d, alpha, xt_mine);
             __syncwarp();
-            ft = eval_pose_warp<true, EQ4, VEC4>(P, G, L, xt_mine, gt_mine, sc_mine, nullptr);
+            if (bb)                                // one evaluation shared by the four warps (eval_cta.cuh); gradient -> slot 0
+                ft = eval_pose_cta<EQ4, VEC4>(P, G, L, xt_mine, b.gt, b.scratch, b.sc_stride, reinterpret_cast<double *>(b.f));
+            else
+                ft = eval_pose_warp<true, EQ4, VEC4>(P, G, L, xt_mine, gt_mine, sc_mine, nullptr);
             __syncthreads();                       // every warp has read x and d before warp 0 moves them
         } else {
             slot = trial & (CTA_WARPS - 1);
