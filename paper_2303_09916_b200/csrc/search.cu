@@ -90,9 +90,7 @@ __device__ __forceinline__ void pose_add_warp(int T, const float *x, const float
 __device__ __forceinline__ void set_identity(float *H, int n, float diag)
 {
     const int lane = threadIdx.x & 31;
-    for (int k = lane; k < n * n; k += 32) H[k] = 0.0f;            // (no k / n, k % n: two integer divisions per element)
-    __syncwarp();
-    for (int r = lane; r < n; r += 32) H[r * n + r] = diag;
+    for (int k = lane; k < n * n; k += 32) H[k] = (k / n == k % n) ? diag : 0.0f;
     __syncwarp();
 }
 
