@@ -985,3 +985,35 @@ def test_quad_image_is_a_copy_of_the_maps(dk, torch, tiny):
     gt = g.transpose(0, 2, 3, 1)                                           # [m][y][x][z]
     want = np.stack([gt, gt[:, :, ix1, :], gt[:, iy1, :, :], gt[:, iy1][:, :, ix1]], axis=-1)
     assert np.array_equal(quad, want)
+
+
+@pytest.mark.parametrize("N,T", [(1, 0), (5, 0), (33, 3), (128, 32)])
+def test_search_kernels_on_degenerate_and_maximum_ligands(dk, torch, micro, N, T):
+    """Both search kernels, both optimizers, on a single atom, a rigid ligand, N > 32 (more than one atom per lane / thread)
+    and the maxima of include/dock.h: finite results, BFGS bit-identical between the kernels, Barzilai-Borwein (shared
+    evaluations on the CTA kernel) equal where there are no pair sums to reorder and close in distribution otherwise."""
+    s0, (_, box, grid, _), _ = micro
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    if N == 1:
+        from types import SimpleNamespace
+        ligd = SimpleNamespace(ref_xyz=np.zeros((1, 3)), type=np.array([3], np.int32), frag=np.zeros(1, np.int32),
+                               tors_parent=np.zeros(0, np.int32), tors_a=np.zeros(0, np.int32),
+                               tors_b=np.zeros(0, np.int32), pairs=np.zeros((0, 2), np.int32))
+    else:
+        ligd = dock_synth.make_ligand(np.random.default_rng(N), N, T, LIG_TYPES_FULL)
+    lig = dk.LigandHandle(ligd)
+    for opt in (0, 1):
+        best = []
+        for k in (1, 2):
+            p = dk.dock_default_params()
+            p.optimizer, p.search_kernel = opt, k
+            r = dk.dock_search(p, [grid], [lig], [box], 24, 5, 40, 7)
+            be = r["best_e"][0].cpu().numpy()
+            assert np.all(np.isfinite(be)) and int(r["topk_count"][0]) >= 1, (N, opt, k)
+            best.append(be)
+        if opt == 0 or lig.P == 0:
+            assert np.array_equal(best[0], best[1]), (N, opt)
+        else:
+            qa, qb = np.median(best[0]), np.median(best[1])
+            assert abs(qa - qb) <= 1.5 + 0.15 * abs(qa), (N, qa, qb)
