@@ -43,6 +43,7 @@ extern "C" {
 #define DOCK_EINVAL     (-1)   /* null pointer, bad size, malformed torsion tree, type without a map ... */
 #define DOCK_EWORKSPACE (-2)   /* workspace too small; *needed holds the requirement */
 #define DOCK_ECUDA      (-3)   /* a CUDA call failed; see dock_last_cuda_error() */
+#define DOCK_ECAPACITY  (-4)   /* dock_topk_fixed only: the ligand needs more than the library's built-in scratch array */
 
 /* Scoring + search parameters.  The paper prints none of them ("the same scoring
  * function" as Vina); dock_default_params() fills the readings S1, S2, S3, S7, S12, S14, S15, S19
@@ -272,6 +273,30 @@ int dock_topk(const dock_params *params, const dock_ligand *ligand, int32_t n,
               const float *poses_dev, const float *e_dev,
               int32_t *out_idx_dev, int32_t *out_count_dev,
               void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
+
+/* ---- A8 without any device allocation ---------------------------------------
+ * dock_topk for callers that cannot allocate device memory, and therefore have no workspace to hand over: a
+ * plug-in given raw pointers but no allocator, code inside a region where cudaMalloc / cudaFree are forbidden or
+ * would synchronise the device, a loop with a hard latency budget.  Inputs, outputs and results are exactly
+ * dock_topk's (same kernel, same tables); only the workspace arguments are gone.  The ligand tables and the system
+ * descriptor the kernel reads go into an array of DOCK_TOPK_FIXED_BYTES that is part of the library's device image.
+ * What that implies:
+ *  - Cost: every GPU that loads libdock_b200.so carries those DOCK_TOPK_FIXED_BYTES until the process exits, used or not.
+ *  - Limit: the ligand's tables must fit (*needed, if non-NULL, receives their size; a 60-atom / 15-torsion ligand
+ *    with 1483 scoring pairs takes 26 368 bytes).  A larger ligand is refused with DOCK_ECAPACITY before anything is
+ *    enqueued or written; use dock_topk with your own workspace for it.  The other limits are dock_topk's.
+ *  - The call makes no cudaMalloc, cudaFree or other allocating library call, at any time.
+ *  - Set-up: the FIRST call on each device (with that device current) asks the runtime for the array's device
+ *    address and keeps it; make that first call outside any stream capture.  Later calls only read the cached address.
+ *  - One array per device, shared by every call: calls on the same stream are ordered and safe; calls whose GPU work
+ *    can overlap (different streams, different host threads on one device) overwrite each other's tables -- a data race
+ *    with undefined results.  Serialise them yourself.  The array keeps the last call's contents between calls;
+ *    nothing relies on that: each call rewrites everything its kernel will read.
+ * Errors: DOCK_EINVAL as dock_topk; DOCK_ECAPACITY as above; DOCK_ECUDA if the address query or an enqueue fails. */
+#define DOCK_TOPK_FIXED_BYTES 65536
+int dock_topk_fixed(const dock_params *params, const dock_ligand *ligand, int32_t n,
+                    const float *poses_dev, const float *e_dev,
+                    int32_t *out_idx_dev, int32_t *out_count_dev, size_t *needed, void *stream);
 
 /* ---- end-to-end convenience with HOST buffers: build grids + search + top-k for one system ----
  * out_topk_pose_host [k][7+T], out_topk_e_host [k], out_count_host [1]; copies H<->D inside. */

@@ -31,6 +31,7 @@ from .binding import (  # noqa: F401
     dock_search,
     dock_system_host,
     dock_topk,
+    dock_topk_fixed,
     launch_count,
     load_library,
     make_box,

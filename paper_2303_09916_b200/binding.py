@@ -21,12 +21,13 @@ DOCK_MAX_ATOMS = 128
 DOCK_TRACE_HEADER = 8
 DOCK_ITER_HEADER = 12
 DOCK_EXIT_GTOL, DOCK_EXIT_CAP, DOCK_EXIT_LINESEARCH = 1, 2, 3
-DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA = 0, -1, -2, -3
+DOCK_OK, DOCK_EINVAL, DOCK_EWORKSPACE, DOCK_ECUDA, DOCK_ECAPACITY = 0, -1, -2, -3, -4
+DOCK_TOPK_FIXED_BYTES = 65536
 
 EXPORTS = [
     "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_build_grids_batch", "dock_score_batch",
     "dock_score_batch_host", "dock_local_opt_batch", "dock_local_opt_trace", "dock_init_poses", "dock_init_poses_site",
-    "dock_search", "dock_topk", "dock_system_host", "dock_probe_peaks", "dock_last_cuda_error", "dock_version",
+    "dock_search", "dock_topk", "dock_topk_fixed", "dock_system_host", "dock_probe_peaks", "dock_last_cuda_error", "dock_version",
     "dock_launch_count", "dock_score_jit_source", "dock_score_jit_compile", "dock_score_jit_log",
 ]
 
@@ -99,7 +100,8 @@ def load_library(path: Optional[str] = None):
 def _check(rc: int, what: str):
     if rc == DOCK_OK:
         return
-    names = {DOCK_EINVAL: "DOCK_EINVAL", DOCK_EWORKSPACE: "DOCK_EWORKSPACE", DOCK_ECUDA: "DOCK_ECUDA"}
+    names = {DOCK_EINVAL: "DOCK_EINVAL", DOCK_EWORKSPACE: "DOCK_EWORKSPACE", DOCK_ECUDA: "DOCK_ECUDA",
+             DOCK_ECAPACITY: "DOCK_ECAPACITY"}
     extra = ""
     if rc == DOCK_ECUDA:
         extra = f" (cudaError {load_library().dock_last_cuda_error()})"
@@ -444,6 +446,25 @@ def dock_topk(params: dock_params, ligand: LigandHandle, poses, e, stream=None):
     ws = _ws.get(need.value, stream)
     _check(lib.dock_topk(C.byref(params), C.byref(ligand.c), n, _ptr(poses), _ptr(e), _ptr(out_idx), _ptr(out_cnt),
                          _ptr(ws), C.c_size_t(ws.numel()), C.byref(need), _stream(stream)), "dock_topk")
+    return out_idx, out_cnt
+
+
+def dock_topk_fixed(params: dock_params, ligand: LigandHandle, poses, e, out_idx, out_cnt, stream=None):
+    """dock_topk for callers that cannot allocate on the device (dock.h: dock_topk_fixed).
+
+    Nothing is allocated here either: `out_idx` (int32 [params.topk]) and `out_cnt` (int32 [1]) are the caller's
+    device tensors, and the kernel's tables live in the library's built-in scratch array, DOCK_TOPK_FIXED_BYTES per
+    GPU, shared by all calls on that GPU (so overlapping calls race).  Raises DockError("... DOCK_ECAPACITY ...") when
+    the ligand's tables do not fit.  Make the first call on a device outside stream capture."""
+    _torch()
+    lib = load_library()
+    need = C.c_size_t(0)
+    rc = lib.dock_topk_fixed(C.byref(params), C.byref(ligand.c), int(poses.shape[0]), _ptr(poses), _ptr(e), _ptr(out_idx),
+                             _ptr(out_cnt), C.byref(need), _stream(stream))
+    if rc == DOCK_ECAPACITY:
+        raise DockError(f"dock_topk_fixed failed: DOCK_ECAPACITY (ligand tables need {need.value} bytes, the built-in "
+                        f"scratch holds {DOCK_TOPK_FIXED_BYTES}; use dock_topk with a workspace)")
+    _check(rc, "dock_topk_fixed")
     return out_idx, out_cnt
 
 

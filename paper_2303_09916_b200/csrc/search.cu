@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
@@ -995,4 +996,70 @@ extern "C" int dock_system_host(const dock_params *params, const dock_protein *p
     if (out_evals_host) DOCK_CUDA_CHECK(cudaMemcpyAsync(out_evals_host, d_ev, sizeof(uint64_t), cudaMemcpyDeviceToHost, stream));
     DOCK_CUDA_CHECK(cudaStreamSynchronize(stream));
     return DOCK_OK;
+}
+
+// ---- dock_topk_fixed: A8 for callers that cannot allocate device memory ------------------------
+// dock_topk keeps the compiled ligand tables and the system descriptor its kernel reads in a workspace the caller
+// allocates.  Some callers have no way to do that: code running where a cudaMalloc is illegal or would stall (inside
+// another framework's stream-ordered region, a plug-in that was handed pointers but no allocator, a real-time loop
+// that must not touch the driver's heap).  For them the same scratch lives in the array below, which is part of the
+// loaded library image: DOCK_TOPK_FIXED_BYTES on EVERY device that loads libdock_b200.so, from load until exit.
+//
+// The array's name is only meaningful to device code.  On the host it is a shadow symbol, not a device address, so the
+// launch path never passes it along: each device's real address is looked up once with cudaGetSymbolAddress (with that
+// device current) and cached in g_topk_fixed_addr.
+namespace {
+
+static __device__ __align__(256) unsigned char g_topk_fixed_scratch[DOCK_TOPK_FIXED_BYTES];
+
+constexpr int TOPK_FIXED_MAX_DEVICES = 64;
+std::mutex g_topk_fixed_mu;
+unsigned char *g_topk_fixed_addr[TOPK_FIXED_MAX_DEVICES];   // per device, nullptr until the first call on it
+
+// Device address of the scratch array on the CURRENT device (looked up on the first call there, then cached).
+int topk_fixed_scratch(unsigned char **out)
+{
+    int dev = -1;
+    DOCK_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= TOPK_FIXED_MAX_DEVICES) return DOCK_EINVAL;
+    std::lock_guard<std::mutex> lock(g_topk_fixed_mu);
+    if (!g_topk_fixed_addr[dev]) {
+        void *p = nullptr;
+        DOCK_CUDA_CHECK(cudaGetSymbolAddress(&p, g_topk_fixed_scratch));
+        if (!p) return DOCK_ECUDA;
+        g_topk_fixed_addr[dev] = (unsigned char *)p;
+    }
+    *out = g_topk_fixed_addr[dev];
+    return DOCK_OK;
+}
+
+}  // namespace
+
+extern "C" int dock_topk_fixed(const dock_params *params, const dock_ligand *ligand, int32_t n,
+                               const float *poses_dev, const float *e_dev,
+                               int32_t *out_idx_dev, int32_t *out_count_dev, size_t *needed, void *stream_)
+{
+    if (dock_validate_params(params) != DOCK_OK || !ligand || n < 0) return DOCK_EINVAL;
+    LigandBlob blob;
+    if (dock_compile_ligand(params, nullptr, ligand, blob) != DOCK_OK) return DOCK_EINVAL;
+    const size_t need = blob.bytes.size() + align_up(sizeof(DevSystem), 256);      // same layout as dock_topk's workspace
+    if (needed) *needed = need;
+    if (need > (size_t)DOCK_TOPK_FIXED_BYTES) return DOCK_ECAPACITY;                // nothing enqueued, nothing written
+    if (!out_idx_dev || !out_count_dev || (n > 0 && (!poses_dev || !e_dev))) return DOCK_EINVAL;
+    DevSystem sys;
+    std::memset(&sys, 0, sizeof(sys));
+    sys.lig = blob.rel;                                                             // sizes only, for the shared-memory check
+    if (topk_smem_bytes(1, &sys.lig, n, 7 + ligand->T, params->topk, nullptr) > 200 * 1024) return DOCK_EINVAL;
+    unsigned char *scratch = nullptr;
+    const int rc = topk_fixed_scratch(&scratch);
+    if (rc != DOCK_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    // Nothing in the scratch has to start at zero: both regions the kernel reads are overwritten in full here, in stream
+    // order, so whatever the previous call (any ligand) left behind is never seen.
+    DOCK_CUDA_CHECK(cudaMemcpyAsync(scratch, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, stream));
+    sys.lig = dock_relocate_ligand(blob, scratch);
+    DevSystem *sys_dev = (DevSystem *)(scratch + blob.bytes.size());
+    DOCK_CUDA_CHECK(cudaMemcpyAsync(sys_dev, &sys, sizeof(sys), cudaMemcpyHostToDevice, stream));
+    return launch_topk(sys_dev, 1, &sys.lig, n, 7 + ligand->T, params->topk, params->cluster_rmsd, poses_dev, e_dev,
+                       out_idx_dev, out_count_dev, nullptr, nullptr, stream);
 }
