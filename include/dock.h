@@ -248,7 +248,9 @@ int dock_init_poses_site(const dock_box *box, int32_t T, uint64_t seed, uint32_t
  * descriptors.  T_max = max over systems of T; pose rows are 7+T_max floats wide (unused tail 0).
  * system_base / copy_base: system s, copy c of this call draw the Philox streams of (system_base + s,
  * copy_base + c) -- a multi-GPU run that shards systems or copies passes the index of its
- * first unit and reproduces the unsharded run bit for bit; 0, 0 otherwise.
+ * first unit and reproduces the unsharded run bit for bit; 0, 0 otherwise.  (One condition: with search_kernel = 0 the
+ * kernel is chosen from the size of EACH call.  BFGS gives the same bits on both kernels; Barzilai-Borwein only agrees to
+ * round-off between them, so a BB run that must reproduce across shardings sets search_kernel to 1 or 2.)
  * Everything that can be rejected (sizes, shared-memory needs, mixed gradient modes) is rejected before any work is
  * enqueued.
  * init_poses_dev [n_systems][copies][7+T_max] or NULL (then generated by dock_init_poses' rule).

@@ -69,7 +69,7 @@ def merge_shards(mode: str, parts, topk_fn, n_systems: int):
     return dict(best_pose=pose, best_e=en, topk_idx=torch.stack(idx), topk_e=torch.stack(te), topk_count=torch.cat(cnt))
 
 
-def dock_search_sharded(search_fn, topk_fn, n_systems: int, copies: int, mode: str, rank: int, world: int):
+def dock_search_sharded(search_fn, topk_fn, n_systems: int, copies: int, mode: str, rank: int, world: int, device=None):
     """NEXT-4 ("independently and asynchronously"): one many-copy search split over `world`
     ranks with NO exchange during the search and ONE all-gather at the end.
 
@@ -86,38 +86,56 @@ def dock_search_sharded(search_fn, topk_fn, n_systems: int, copies: int, mode: s
     search_fn(sys_begin, sys_end, copy_begin, copy_end, want_topk) -> dict with best_pose [ns, nc, row], best_e [ns, nc]
         and, if want_topk, topk_idx [ns, k], topk_e [ns, k], topk_count [ns];
     topk_fn(system, poses [copies, row], e [copies]) -> (idx [k], count).
+    Pose rows: a rank's best_pose is 7 + T_max of its OWN systems wide; the gather pads every rank's rows with zeros to
+    the widest, which is the unsharded run's row.  A rank that owns no unit (world > units) calls neither function and
+    only takes part in the gather; `device` is where it builds its empty contribution (default: the current CUDA device
+    under nccl, else the CPU).
+    Kernel choice: with params.search_kernel = 0 the library picks the search kernel from the size of EACH call, so a
+    shard may run the CTA kernel where the unsharded run took the warp kernel.  For BFGS the two are bit-identical; for
+    Barzilai-Borwein they agree to round-off only, so pin search_kernel (1 or 2) when a BB run must reproduce across
+    shardings.
     Returns a dict with best_pose [n_systems, copies, row], best_e, topk_idx, topk_e, topk_count -- the same on every rank."""
     import torch
     import torch.distributed as dist
     multi = dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1
+    if device is None:
+        device = torch.device("cuda", torch.cuda.current_device()) if multi and dist.get_backend() == "nccl" else torch.device("cpu")
 
     def gather(t):
-        """all-gather of per-rank tensors whose leading size differs by at most one -> list in rank order"""
+        """all-gather of per-rank tensors -> list in rank order.  The leading size may differ from rank to rank (also 0:
+        `t` is None on a rank that owns no unit), and so may the trailing ones: a rank's pose rows are 7 + T_max of ITS
+        systems wide.  Every rank pads with zeros to the element-wise MAX shape (the unsharded run's "unused tail 0",
+        dock.h), sends that, and the leading padding is cut off again on arrival."""
         if not multi:
-            return [t]
-        n = torch.tensor([t.shape[0]], dtype=torch.int64, device=t.device)
-        ns = [torch.zeros_like(n) for _ in range(world)]
-        dist.all_gather(ns, n)
-        m = int(max(int(x) for x in ns))
-        pad = torch.zeros((m,) + tuple(t.shape[1:]), dtype=t.dtype, device=t.device)
-        pad[: t.shape[0]] = t
+            return [t] if t is not None else []
+        metas = [None] * world
+        dist.all_gather_object(metas, None if t is None else (tuple(t.shape), str(t.dtype).split(".")[-1]))
+        ref = next((m for m in metas if m is not None), None)
+        if ref is None:
+            raise ValueError("no rank holds any unit")
+        shapes = [m[0] if m is not None else (0,) + tuple(ref[0][1:]) for m in metas]
+        full = tuple(max(sh[d] for sh in shapes) for d in range(len(ref[0])))
+        dev = t.device if t is not None else device
+        pad = torch.zeros(full, dtype=getattr(torch, ref[1]), device=dev)
+        if t is not None:
+            pad[tuple(slice(0, n) for n in t.shape)] = t
         out = [torch.empty_like(pad) for _ in range(world)]
         dist.all_gather(out, pad)
-        return [o[: int(k)] for o, k in zip(out, ns)]
+        return [o[: sh[0]] for o, sh in zip(out, shapes) if sh[0] > 0]
 
     if mode == "systems":
         b, e = shard_range(n_systems, rank, world)
-        r = search_fn(b, e, 0, copies, True)
+        r = search_fn(b, e, 0, copies, True) if e > b else None         # world > n_systems: this rank only takes part in the gather
         keys = ("best_pose", "best_e", "topk_idx", "topk_e", "topk_count")
-        cols = {k: gather(r[k].contiguous()) for k in keys}
+        cols = {k: gather(r[k].contiguous() if r is not None else None) for k in keys}
         parts = [{k: cols[k][q] for k in keys} for q in range(len(cols["best_e"]))]
         return merge_shards(mode, parts, topk_fn, n_systems)
     if mode != "copies":
         raise ValueError("mode must be 'systems' or 'copies'")
     b, e = shard_range(copies, rank, world)
-    r = search_fn(0, n_systems, b, e, False)
+    r = search_fn(0, n_systems, b, e, False) if e > b else None
     # the copy axis is the one that is split: move it to the front for the variable-length all-gather
-    gp = gather(r["best_pose"].transpose(0, 1).contiguous())
-    ge = gather(r["best_e"].transpose(0, 1).contiguous())
+    gp = gather(r["best_pose"].transpose(0, 1).contiguous() if r is not None else None)
+    ge = gather(r["best_e"].transpose(0, 1).contiguous() if r is not None else None)
     parts = [dict(best_pose=a.transpose(0, 1), best_e=c.transpose(0, 1)) for a, c in zip(gp, ge)]
     return merge_shards(mode, parts, topk_fn, n_systems)

@@ -75,6 +75,20 @@ def test_merge_of_shards_equals_the_unsharded_run():
                 assert torch.equal(m[k], whole[k]), (world, mode, k)
 
 
+_T = [2, 4, 3, 0, 1]                       # torsions per system: the pose rows a rank returns are 7 + max(T of ITS systems) wide
+
+
+def _ragged_search(sb, se, cb, ce, want_topk):
+    """_fake_search with the row convention of dock_search: 7 + T_max of the systems of THIS call, unused tail 0."""
+    r = _fake_search(sb, se, cb, ce, want_topk)
+    row = 7 + max(_T[sb:se])
+    pose = torch.zeros(se - sb, ce - cb, row, dtype=torch.float64)
+    for s in range(sb, se):
+        pose[s - sb, :, : 7 + _T[s]] = r["best_pose"][s - sb, :, : 7 + _T[s]]
+    r["best_pose"] = pose
+    return r
+
+
 def _worker(rank, world, port, out_dir):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -89,6 +103,7 @@ def _worker(rank, world, port, out_dir):
         ge, gp = gather_candidates(energy_all[loc], poses_all[loc])
         t = max_over_ranks(1.0 + rank)
         sh = {m: dock_search_sharded(_fake_search, _fake_topk, _NS, _NC, m, rank, world) for m in ("systems", "copies")}
+        sh["ragged"] = dock_search_sharded(_ragged_search, _fake_topk, _NS, _NC, "systems", rank, world)
         torch.save({"e": ge, "p": gp, "t": t, "span": (b, e), "sharded": sh}, os.path.join(out_dir, f"r{rank}.pt"))
     finally:
         dist.destroy_process_group()
@@ -113,3 +128,45 @@ def test_two_ranks_gloo(tmp_path):
         for mode in ("systems", "copies"):
             for k in ("best_pose", "best_e", "topk_idx", "topk_e", "topk_count"):
                 assert torch.equal(r[rank]["sharded"][mode][k], whole[k]), (rank, mode, k)
+    # ranks whose systems have different T_max return pose rows of different widths (7 + 4 and 7 + 1 here): the driver
+    # pads them to the unsharded row instead of handing mismatched shapes to all_gather
+    ragged = _ragged_search(0, _NS, 0, _NC, True)
+    assert _ragged_search(0, 3, 0, _NC, True)["best_pose"].shape[-1] != _ragged_search(3, _NS, 0, _NC, True)["best_pose"].shape[-1]
+    for rank in range(world):
+        for k in ("best_pose", "best_e", "topk_idx", "topk_e", "topk_count"):
+            assert torch.equal(r[rank]["sharded"]["ragged"][k], ragged[k]), (rank, k)
+
+
+def _worker_more_ranks_than_units(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        calls = []
+
+        def search(sb, se, cb, ce, want_topk):
+            assert se > sb and ce > cb, "an empty shard must not reach the search call (dock_search rejects n_systems = 0)"
+            calls.append((sb, se, cb, ce))
+            return _ragged_search(sb, se, cb, ce, want_topk)
+
+        sh = {m: dock_search_sharded(search, _fake_topk, 2, 2, m, rank, world) for m in ("systems", "copies")}
+        torch.save({"sharded": sh, "calls": calls}, os.path.join(out_dir, f"r{rank}.pt"))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_more_ranks_than_units_gloo(tmp_path):
+    """world 3, two systems x two copies: the third rank owns nothing in either mode, skips the search and still
+    ends up with the full result."""
+    world = 3
+    mp.spawn(_worker_more_ranks_than_units, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    r = [torch.load(os.path.join(tmp_path, f"r{i}.pt")) for i in range(world)]
+    whole = _ragged_search(0, 2, 0, 2, True)
+    assert r[2]["calls"] == [] and len(r[0]["calls"]) == len(r[1]["calls"]) == 2
+    used = whole["topk_idx"] >= 0                            # two copies, k = 4: the unused slots' energies are unspecified
+    for rank in range(world):
+        for mode in ("systems", "copies"):
+            got = r[rank]["sharded"][mode]
+            for k in ("best_pose", "best_e", "topk_idx", "topk_count"):
+                assert torch.equal(got[k], whole[k]), (rank, mode, k)
+            assert torch.equal(got["topk_e"][used], whole["topk_e"][used]), (rank, mode)
