@@ -117,8 +117,13 @@ __global__ void __launch_bounds__(128) grid_build_kernel(GridBuildArgs A)
     const int cy_lo = max((int)floorf((cyw - reach - S.clo[1]) * S.inv_cell), 0), cy_hi = min((int)floorf((cyw + reach - S.clo[1]) * S.inv_cell), S.ncy - 1);
     const int cz_lo = max((int)floorf((czw - reach - S.clo[2]) * S.inv_cell), 0), cz_hi = min((int)floorf((czw + reach - S.clo[2]) * S.inv_cell), S.ncz - 1);
 
-    // |r2_fp32 - r2_exact| <= ~2 r (ulp of a 60 A coordinate) + 3 ulp(r2): well inside 1e-3 A^2 for boxes up to a few hundred A
-    const float cut_window = 1e-3f;
+    // |r2_fp32 - r2_exact| <= 2 sqrt(3) r (ulp(node coordinate) / 2 + ulp(8) / 2) + 3 ulp(r2) < 14 r_cut/8 2^-23 c_max + 2e-5, c_max the
+    // largest |node coordinate| of this lattice: well inside 1e-3 A^2 up to c_max ~ 260 A; beyond, the window grows with c_max
+    // (32 x 2^-23 c_max, a factor 2 of margin) so that a box far from the origin keeps the exact decision too
+    const float cmax = fmaxf(fmaxf(fmaxf(fabsf(S.ox), fabsf(fmaf((float)(S.nx - 1), S.h, S.ox))),
+                                   fmaxf(fabsf(S.oy), fabsf(fmaf((float)(S.ny - 1), S.h, S.oy)))),
+                             fmaxf(fabsf(S.oz), fabsf(fmaf((float)(S.nz - 1), S.h, S.oz))));
+    const float cut_window = fmaxf(1e-3f, 3.8e-6f * cmax);
     float acc[MAPS_PER_PASS], agx[MAPS_PER_PASS], agy[MAPS_PER_PASS], agz[MAPS_PER_PASS];
 #pragma unroll
     for (int m = 0; m < MAPS_PER_PASS; ++m) acc[m] = agx[m] = agy[m] = agz[m] = 0.0f;
@@ -451,10 +456,14 @@ extern "C" int dock_build_grids_batch(const dock_params *params, int32_t n_syste
         int mx = 0, my = 0, mz = 0;
         for (int s = 0; s < n_systems; ++s) { mx = std::max(mx, sys[s].nx); my = std::max(my, sys[s].ny); mz = std::max(mz, sys[s].nz); }
         const int zt = (mz + 7) / 8;
-        const long long gz = (long long)n_systems * n_lig_types * zt;
-        if (gz > 65535 || my > 65535) return DOCK_EINVAL;
-        grid_quad_kernel<<<dim3((unsigned)((mx + 31) / 32), (unsigned)my, (unsigned)gz), 256, 0, stream>>>(A.sys, n_lig_types, zt);
-        DOCK_LAUNCH_CHECK();
+        // blockIdx.z = (system, map, z tile) is limited to 65535: as many systems per launch as fit (n_maps <= 32 and
+        // zt <= 512, so one system always does; my <= 4096 by dock_grid_dims) -- nothing to reject here, after the enqueues
+        const int per_launch = std::max(1, 65535 / (n_lig_types * zt));
+        for (int s0 = 0; s0 < n_systems; s0 += per_launch) {
+            const unsigned gz = (unsigned)(std::min(per_launch, n_systems - s0) * n_lig_types * zt);
+            grid_quad_kernel<<<dim3((unsigned)((mx + 31) / 32), (unsigned)my, gz), 256, 0, stream>>>(A.sys + s0, n_lig_types, zt);
+            DOCK_LAUNCH_CHECK();
+        }
     }
 
     for (int s = 0; s < n_systems; ++s) {

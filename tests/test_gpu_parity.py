@@ -77,6 +77,14 @@ def test_grid_edge_cases(dk, orc, torch):
     g = dk.dock_build_grids(p, xyz, typ, box, all_types)
     og = orc.build_grid(op, xyz, typ, [0, 0, 0], [6.0, 4.5, 3.0], 0.375, all_types)
     compare_grid(orc, op, xyz, g.data.cpu().numpy(), og, "17 types")
+    # the same protein and box 2000 A from the origin: the fp32 error of r^2 (~2e-3 A^2) is above the 1e-3 A^2 window that is
+    # enough near the origin, so the window of the exact cutoff re-decision has to follow the coordinates (grid.cu: cut_window)
+    off = np.array([1500.0, -1200.0, 900.0], np.float32)
+    xyz_far = (xyz + off).astype(np.float32)
+    box_far = dk.make_box(off.tolist(), [6.0, 4.5, 3.0], 0.375)
+    g = dk.dock_build_grids(p, xyz_far, typ, box_far, all_types)
+    og = orc.build_grid(op, xyz_far, typ, off.tolist(), [6.0, 4.5, 3.0], 0.375, all_types)
+    compare_grid(orc, op, xyz_far, g.data.cpu().numpy(), og, "far from the origin")
 
 
 # ----------------------------------------------------------------------------------- A2-A5 per pose
@@ -797,6 +805,18 @@ def test_batched_grid_build_equals_single_builds(dk, torch):
         off = (g.data.numel() * 4 + 255) // 256 * 256                        # ... and the packed gather image behind them
         assert torch.equal(g.buf[off:], one.buf[off:])
     assert dk.dock_build_grids_batch(p, [], [], lt) == []
+    # a batch whose (system, map, z tile) count exceeds one launch's blockIdx.z range (80 x 17 x 51 = 69 360 > 65 535): the
+    # 4-corner image is written by several launches, each over a range of systems -- accepted, and equal to single builds
+    rng = np.random.default_rng(4)
+    all_types = list(range(17))
+    prots = [((rng.random((40, 3)) * [3, 3, 150] - [1.5, 1.5, 75]).astype(np.float32), rng.integers(0, 17, 40).astype(np.int32))
+             for _ in range(80)]
+    boxes = [dk.make_box([0, 0, 0], [0.75, 0.75, 150.0], 0.375)] * 80
+    batch = dk.dock_build_grids_batch(p, prots, boxes, all_types)
+    assert tuple(batch[0].dims) == (3, 3, 401)
+    for i in (0, 37, 75, 76, 79):                                            # 75 systems fit the first launch
+        one = dk.dock_build_grids(p, prots[i][0], prots[i][1], boxes[i], all_types)
+        assert torch.equal(batch[i].buf, one.buf), i
 
 
 # ----------------------------------------------------------------------------------- NEXT-4: sharded search, streams
