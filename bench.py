@@ -202,9 +202,10 @@ def run_ours(args) -> dict:
     s, poses_h = _workload(rank)
     p = dk.dock_default_params()
     box = dk.make_box(s.box_center, s.box_size, s.spacing)
-    # which score kernel the headline times: 2 = specialised for the ligand at run time (NVRTC; the faster one on
-    # configs[1], compiled during the warm-up), 0 / 1 = the generic kernel (the library's default).  -1 (default here) =
-    # 2 if the compiler is there, else generic.  The other kernel is timed beside it (extra.*_score_kernel).
+    # which score kernel the headline times: 0 / 1 (default here) = the generic kernel, which is what dock_score_batch runs
+    # unless the caller opts in; 2 = the kernel specialised for the ligand at run time (NVRTC; compiled during the
+    # warm-up, i.e. its 0.4-6 s per ligand are NOT in the number); -1 = 2 if the compiler is there, else generic.
+    # The other kernel is timed beside it (extra.*_score_kernel, with its first-call cost and break-even batch size).
     args.score_kernel_note = ""
     if args.score_kernel < 0:
         args.score_kernel = 2
@@ -308,10 +309,18 @@ def run_ours(args) -> dict:
             to = _time_events(torch, lambda: dk.dock_score_batch(po, grid, lig, poses, out=oo), min(args.steps, 20), flush)
             de = float((oo[0] - out[0]).abs().max())
             dg = float(((oo[1] - out[1]).abs() / (1e-3 + 1e-4 * out[1].abs())).max())
+            t_other, t_head = float(np.mean(to)) / 1e3, float(np.mean(ts)) / 1e3
+            t_spec, t_gen = (t_other, t_head) if name.startswith("spec") else (t_head, t_other)
             extra[name] = {"ms_per_step": float(np.mean(to)), "evals_per_s": n / (float(np.mean(to)) / 1e3),
+                           "specialised_over_generic": t_gen / t_spec,
                            "first_call_s": t_first, "max_abs_dE_vs_headline_kernel": de, "max_dgrad_tol_units_vs_headline_kernel": dg,
                            "note": "dock_params.score_kernel = 2 (jit_score.cu): first_call_s includes the NVRTC compilation for this ligand"
                                    if name.startswith("spec") else "dock_params.score_kernel = 1"}
+            if name.startswith("spec"):
+                gain = (t_gen - t_spec) / n                     # seconds saved per pose once the kernel is compiled
+                extra[name]["break_even_poses"] = (t_first - t_spec) / gain if gain > 0 else None
+                extra[name]["break_even_note"] = ("poses of ONE ligand after which first_call_s (compilation) is paid back by the faster "
+                                                  "kernel; null = never (the generic kernel is at least as fast for this ligand)")
             del oo
         except dk.DockError as e:
             extra[name] = {"unavailable": str(e)}
@@ -347,6 +356,8 @@ def run_ours(args) -> dict:
             dist.all_reduce(tot)
             ev3 = int(tot.item())
         best3 = r3["topk_e"][:, 0].cpu().numpy()
+        best3_pose = [r3["best_pose"][i].cpu().numpy() for i in range(min(2, len(sy)))]
+        ev3_rank0, t_3_rank0 = int(r3["evals"].sum()), t_3
         extra["screening"] = {"workload": f"configs[3]: {n3} systems x 128 copies x 40 steps, BFGS<=300, ONE dock_build_grids_batch + ONE "
                                           f"dock_search launch per rank ({world} rank(s), systems sharded, no exchange)",
                               "systems": n3, "search_s": t_3, "grid_build_s": t_g3, "evals": ev3, "evals_per_s": ev3 / t_3,
@@ -375,11 +386,20 @@ def run_ours(args) -> dict:
     counted = O.count_eval_ops(op, og, oL, p64[:2048])                    # the oracle's own statements, operation by operation
     t_kernel = float(np.mean(ts)) / 1e3
     achieved = flops * n / t_kernel / 1e12
+    counters = kernel_counters()
+    head_kernel = "dock_score_jit" if args.score_kernel == 2 else "score_thread_kernel"
+    kc_head = counters.get(head_kernel, {})
+    for name in ("generic_score_kernel", "specialised_score_kernel"):
+        if name in extra and "ms_per_step" in extra[name]:
+            extra[name]["roofline_frac"] = flops * n / (extra[name]["ms_per_step"] / 1e3) / 1e12 / ALU_PEAK_TFLOPS
     peak_meas = max(peaks["ffma_tflops"], peaks["ffma2_tflops"])
     line["roofline"] = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                         "frac": achieved / ALU_PEAK_TFLOPS,
-                        "traffic": TRAFFIC_BYTES_PER_LAUNCH["dock_score_jit" if args.score_kernel == 2 else "score_thread_kernel"],
-                        "kernel": "dock_score_jit" if args.score_kernel == 2 else "score_thread_kernel", "flops_per_eval": flops, "pairs_in_range_mean": p_in,
+                        "traffic": kc_head.get("dram_bytes_per_launch"),
+                        "traffic_source": (f"{kc_head['source']} at commit {kc_head['commit']} (profiles/kernel_counters.json; ncu, not "
+                                           "measured by this run)") if kc_head else None,
+                        "achieved_occupancy_pct_ncu": kc_head.get("achieved_occupancy_pct"),
+                        "kernel": head_kernel, "flops_per_eval": flops, "pairs_in_range_mean": p_in,
                         "peak_source": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                         "peak_measured": peak_meas, "frac_of_measured": achieved / peak_meas,
                         "peak_measured_source": "dock_probe_peaks: FFMA / FFMA2 loops, 8 independent chains per thread, this run",
@@ -400,16 +420,35 @@ def run_ours(args) -> dict:
     err = np.abs(ge - oe) / (1e-3 + 1e-4 * np.abs(oe))
     line["parity_in_bench"] = {"poses": int(safe.sum()), "max_err_tol_units": float(err[safe].max())}
 
-    def oracle_search_rate(q, n_copies, steps, cap, system=0):
-        """The oracle's own search on the first n_copies copies (copies are independent): evaluations/s on the host cores."""
+    pairs_in_range = {}
+
+    def oracle_search_rate(q, n_copies, steps, cap, system=0, gpu_best=None, tag=None):
+        """The oracle's own search on the first n_copies copies (copies are independent): evaluations/s on the host cores.
+        gpu_best: poses the GPU search ended at; their mean number of in-range intra pairs (an oracle diagnostic) is kept
+        under `tag` for the flop figure of search_roofline()."""
         qp = O.params_as_fp32(O.default_params())
         qg = O.build_grid(qp, q.protein_xyz, q.protein_type, q.box_center, q.box_size, q.spacing, q.lig_types)
         qL = O.Ligand(q.ligand)
+        if gpu_best is not None:
+            dg = O.score_batch(qp, qg, qL, np.asarray(gpu_best, np.float64)[:, :7 + qL.T], want_grad=False)[3]
+            pairs_in_range[tag] = float(dg["pairs_in_range"].mean())
         init = O.init_poses(q.box_center, q.box_size, qL.T, 2023, system, n_copies)
         t0 = time.perf_counter()
         r = O.search(qp, qg, qL, init, steps, cap, 2023, system)
         dt = time.perf_counter() - t0
         return r["evals"], dt
+
+    def search_roofline(parts, seconds, kernel):
+        """SURVEY.md 8(d) "Search configs": the roofline fraction of a search, for information.  parts = [(evaluations,
+        ligand, mean in-range pairs)]; flops = evaluations x 8(d)'s per-evaluation formula, so the optimizer's own
+        vector algebra (BFGS update, line-search bookkeeping, Philox) counts as overhead, not as work."""
+        fl = sum(ev * algorithmic_flops(L.N, L.T, pin, L.P - pin) for ev, L, pin in parts)
+        kc = counters.get(kernel, {})
+        return {"roofline_frac": fl / seconds / 1e12 / ALU_PEAK_TFLOPS, "achieved_tflops": fl / seconds / 1e12, "kernel": kernel,
+                "pairs_in_range_mean": float(np.mean([pin for _, _, pin in parts])),
+                "pairs_in_range_source": "oracle diagnostic on the poses the GPU search ended at",
+                "achieved_occupancy_pct_ncu": kc.get("achieved_occupancy_pct"),
+                "occupancy_source": f"{kc['source']} at commit {kc['commit']}" if kc else None}
 
     # extras: A1 and A6-A8 next to the headline
     extra.update({"grid_build_ms": float(np.median(t_grid)), "grid_nodes": int(np.prod(grid.dims)) * len(s.lig_types)})
@@ -429,7 +468,7 @@ def run_ours(args) -> dict:
         r_h = dk.dock_system_host(p, s2.protein_xyz, s2.protein_type, box2, lig2, s2.lig_types, s2.copies, s2.steps,
                                   s2.bfgs_cap, 2023)
         t_h = time.perf_counter() - t0
-        oev, odt = oracle_search_rate(s2, s2.copies, s2.steps, s2.bfgs_cap)
+        oev, odt = oracle_search_rate(s2, s2.copies, s2.steps, s2.bfgs_cap, gpu_best=res["best_pose"][0].cpu().numpy(), tag="cfg2")
         extra["site_docking"] = {"workload": "configs[2]: 384 copies x 40 steps, BFGS<=300", "search_s": t_s,
                                  "evals": int(res["evals"][0]), "evals_per_s": int(res["evals"][0]) / t_s,
                                  "systems_per_s_search_only": 1.0 / t_s, "end_to_end_host_s": t_h,
@@ -437,6 +476,7 @@ def run_ours(args) -> dict:
                                  "cpu_baseline": {"kind": "oracle", "cores": O.num_threads(), "sample": "all 384 copies x 40 steps (grid build not included)",
                                                   "search_s": odt, "evals": oev, "evals_per_s": oev / odt, "systems_per_s": 1.0 / odt},
                                  "paper_context": "DSDP 384x40 redocking 0.55 s/system on RTX 2080 SUPER (PAPER.md:108)"}
+        extra["site_docking"].update(search_roofline([(int(res["evals"][0]), lig2, pairs_in_range["cfg2"])], t_s, "search_cta_kernel"))
         # the same site docking driven by the paper's Barzilai-Borwein optimizer (NEXT-1), 150 iterations
         pb = dk.dock_default_params()
         pb.optimizer = 1
@@ -450,12 +490,19 @@ def run_ours(args) -> dict:
         extra["site_docking_bb"] = {"workload": "configs[2] with the Barzilai-Borwein optimizer, <=150 iterations", "search_s": t_b,
                                     "evals": int(rb["evals"][0]), "evals_per_s": int(rb["evals"][0]) / t_b,
                                     "systems_per_s_search_only": 1.0 / t_b, "best_e": float(rb["topk_e"][0, 0])}
+        extra["site_docking_bb"].update(search_roofline([(int(rb["evals"][0]), lig2, pairs_in_range["cfg2"])], t_b, "search_cta_kernel"))
         # configs[3] oracle baseline: the first two systems of the batch, 32 copies x 40 steps each
         oev = odt = 0.0
         for i, q in enumerate(sys3_keep):
-            a, b_ = oracle_search_rate(q, 32, 40, 300, system=i)
+            a, b_ = oracle_search_rate(q, 32, 40, 300, system=i, gpu_best=best3_pose[i], tag=f"cfg3_{i}")
             oev += a
             odt += b_
+        # flop figure of the batch: the launch has ONE evaluation counter, so the evaluations are spread evenly over the
+        # systems' ligands; the in-range pair FRACTION of the systems the oracle looked at stands in for the others
+        frac3 = float(np.mean([pairs_in_range[f"cfg3_{i}"] / max(1, lg[i].P) for i in range(len(sys3_keep))]))
+        extra["screening"].update(search_roofline([(ev3_rank0 / len(lg), L_, frac3 * L_.P) for L_ in lg], t_3_rank0, "search_kernel"))
+        extra["screening"]["roofline_note"] = (f"rank 0's {len(lg)} systems, evaluations spread evenly over them; in-range pair "
+                                               f"fraction {frac3:.3f} from the first {len(sys3_keep)}")
         extra["screening"]["cpu_baseline"] = {"kind": "oracle", "cores": O.num_threads(),
                                               "sample": f"first {len(sys3_keep)} systems, 32 of 128 copies x 40 steps each (grid build not included)",
                                               "search_s": odt, "evals": int(oev), "evals_per_s": oev / odt,
@@ -477,7 +524,7 @@ def run_ours(args) -> dict:
         r4 = run4()
         torch.cuda.synchronize()
         t_4 = time.perf_counter() - t0
-        oev, odt = oracle_search_rate(s4, 32, s4.steps, s4.bfgs_cap)
+        oev, odt = oracle_search_rate(s4, 32, s4.steps, s4.bfgs_cap, gpu_best=r4["best_pose"][0].cpu().numpy(), tag="cfg4")
         extra["large_blind_box"] = {"workload": "configs[4]: 8000 atoms, 161^3 x 8 maps, 2048 copies x 80 steps, BFGS<=300",
                                     "search_s": t_4, "grid_build_s": t_g4, "evals": int(r4["evals"][0]),
                                     "evals_per_s": int(r4["evals"][0]) / t_4, "systems_per_s_with_grid": 1.0 / (t_4 + t_g4),
@@ -486,16 +533,21 @@ def run_ours(args) -> dict:
                                                      "sample": "first 32 of 2048 copies x 80 steps (grid build not included)",
                                                      "search_s": odt, "evals": oev, "evals_per_s": oev / odt,
                                                      "systems_per_s_scaled": 1.0 / (odt * 2048 / 32)}}
+        extra["large_blind_box"].update(search_roofline([(int(r4["evals"][0]), lig4, pairs_in_range["cfg4"])], t_4, "search_kernel"))
         del grid4
     line["extra"] = extra
     return line
 
 
-# per-launch DRAM traffic of the score kernels from the committed `ncu --set full` captures
-TRAFFIC_BYTES_PER_LAUNCH = {
-    "score_thread_kernel": 821.8e6,   # profiles/r2c_score_thread_kernel_details.txt: dram read 755.6 MB + write 66.2 MB
-    "dock_score_jit": 237.4e6,        # profiles/r2b_dock_score_jit_details.txt: dram read 177.0 MB + write 60.4 MB (4-corner map image)
-}
+def kernel_counters() -> dict:
+    """ncu-only counters (DRAM bytes per launch, achieved occupancy) of the committed captures: profiles/kernel_counters.json,
+    each entry with the capture file and the commit it was taken at.  {} if the file is missing (the fields print as null)."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "kernel_counters.json")
+    try:
+        with open(path) as f:
+            return {k: v for k, v in json.load(f).items() if isinstance(v, dict)}
+    except (OSError, ValueError):
+        return {}
 
 
 def main():
@@ -507,9 +559,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=1048576, help="poses the CPU oracle scores per step")
     ap.add_argument("--no-flush", action="store_true")
     ap.add_argument("--no-search", action="store_true")
-    ap.add_argument("--score-kernel", type=int, default=-1, choices=[-1, 0, 1, 2],
-                    help="dock_params.score_kernel for the headline step: 0/1 generic (the library default), 2 specialised at run "
-                         "time, -1 (default) = 2 if NVRTC is available, else generic")
+    ap.add_argument("--score-kernel", type=int, default=0, choices=[-1, 0, 1, 2],
+                    help="dock_params.score_kernel for the headline step: 0/1 generic (the library default, and the default here), "
+                         "2 specialised at run time (compilation outside the timed region), -1 = 2 if NVRTC is available, else generic")
     ap.add_argument("--screen-systems", type=int, default=256, help="systems of the configs[3] screening batch (256 = the config)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -317,7 +317,8 @@ int dock_system_host(const dock_params *params, const dock_protein *protein, con
  * peaks MEASURED_PEAKS.json holds).  ws_dev: 32-byte aligned, *needed bytes (about 16 MB). */
 int dock_probe_peaks(float *out_host, void *ws_dev, size_t ws_bytes, size_t *needed, void *stream);
 
-/* ---- diagnostics ------------------------------------------------------------------------------ */
+/* ---- diagnostics and measurement: NOT part of the hot-path boundary of SURVEY.md 8(b) ---------
+ * (dock_probe_peaks above belongs here too: bench.py divides by its output.) */
 /* CUDA source of the ligand-specialised score kernel dock_score_batch would compile for (params, grid, ligand)
  * (score_kernel = 2; A2-A5).  buf: HOST, cap bytes; *needed = length + 1; DOCK_EWORKSPACE if cap is short,
  * DOCK_EINVAL if the ligand is outside what the generator covers.  No device work. */
@@ -327,6 +328,12 @@ int dock_score_jit_source(const dock_params *params, const dock_grid *grid, cons
  * of the run-time kernel.  DOCK_ECUDA if NVRTC (libnvrtc.so.12 of CUDA >= 12.9) is missing or the compilation fails. */
 int dock_score_jit_compile(const dock_params *params, const dock_grid *grid, const dock_ligand *ligand,
                            int32_t want_grad, size_t *cubin_bytes);
+/* The specialised kernels are cached per (device, ligand, parameters, want_grad), at most `limit` per device (default 64):
+ * when a device's cache is full the least recently used kernel is unloaded (after a cudaDeviceSynchronize on that device:
+ * it may still be running) before the new one is compiled.  new_limit in [1, 65536] sets the limit for later insertions,
+ * new_limit < 0 only queries; *old_limit / *entries (nullable) receive the limit before the call and the number of cached
+ * kernels over all devices.  DOCK_EINVAL for new_limit = 0 or > 65536. */
+int dock_score_jit_cache(int32_t new_limit, int32_t *old_limit, int32_t *entries);
 const char *dock_score_jit_log(void);            /* compiler log of the last failed run-time compilation ("" = none) */
 int         dock_last_cuda_error(void);          /* cudaError_t of the last failing CUDA call (0 = none) */
 const char *dock_version(void);

@@ -774,21 +774,6 @@ typedef struct {
  * implementation difference.  drop_bits < 0 switches it off. */
 static int g_eval_drop_bits = -1;
 void orc_diag_round_eval_fp32(int drop_bits) { g_eval_drop_bits = drop_bits; }
-/* Second noise model of the same diagnostic: every value the optimizer sees carries ONE fp32 rounding error of its
- * CONDITIONING SCALE -- E of |E_grid| + |E_wall| + |E_intra|, gradient component k of A_k (orc_grad_cond: the sum of
- * the absolute values of its terms) -- times `c`, with a deterministic pseudo-random sign and size in [-1, 1], and is
- * then rounded to fp32.  This is how an fp32 sum behaves (error ~ eps x sum of |terms|, not eps x |result|); the
- * level-1 tests allow the kernel 8 such units per gradient component (reading S20').  c <= 0 switches it off. */
-static double g_eval_noise_c = 0.0;
-void orc_diag_eval_noise(double c) { g_eval_noise_c = c; }
-static double hash_unit(uint64_t x)                    /* splitmix64 -> [-1, 1) */
-{
-    x += 0x9E3779B97F4A7C15ull;
-    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
-    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
-    x ^= x >> 31;
-    return (double)(int64_t)x / 9223372036854775808.0;
-}
 static double round_sig(double x, int bits)
 {
     if (x == 0.0 || !isfinite(x)) return x;
@@ -872,18 +857,6 @@ static double dock_fn(void *c, const double *x, double *grad)
     if (g_eval_drop_bits >= 0) {
         e = round_sig(e, 24 - g_eval_drop_bits);
         for (int i = 0; i < 6 + k->L->T; ++i) grad[i] = round_sig(grad[i], 24 - g_eval_drop_bits);
-    }
-    if (g_eval_noise_c > 0.0) {
-        const int n = 6 + k->L->T;
-        double tr[3], *A = (double *)malloc(sizeof(double) * n);
-        orc_eval(k->p, k->g, k->L, x, tr, NULL, NULL);
-        orc_grad_cond(k->p, k->g, k->L, x, A);
-        uint64_t seed;
-        memcpy(&seed, &e, sizeof(seed));
-        const double u = g_eval_noise_c * 5.9604644775390625e-08;   /* c 2^-24 */
-        e = (double)(float)(e + hash_unit(seed) * u * (fabs(tr[0]) + fabs(tr[1]) + fabs(tr[2])));
-        for (int i = 0; i < n; ++i) grad[i] = (double)(float)(grad[i] + hash_unit(seed + 1 + (uint64_t)i) * u * A[i]);
-        free(A);
     }
     return e;
 }

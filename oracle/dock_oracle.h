@@ -270,9 +270,6 @@ int    orc_num_threads(void);
 /* diagnostic switch (default off = negative): the objective seen by the optimizers is rounded to a (24 - drop_bits)-bit
  * significand -- see dock_oracle.c */
 void   orc_diag_round_eval_fp32(int drop_bits);
-/* second noise model (default off = 0): one fp32 rounding error of the conditioning scale of E and of every gradient
- * component, times c -- see dock_oracle.c */
-void   orc_diag_eval_noise(double c);
 
 #ifdef __cplusplus
 }

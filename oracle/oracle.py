@@ -215,21 +215,6 @@ class round_eval_fp32:
         return False
 
 
-class eval_noise:
-    """Context manager for the second chaos-ceiling model (dock_oracle.c: orc_diag_eval_noise): inside, every energy /
-    gradient component the optimizers see carries c fp32 rounding errors of its conditioning scale."""
-
-    def __init__(self, c: float = 1.0):
-        self.c = float(c)
-
-    def __enter__(self):
-        lib().orc_diag_eval_noise(C.c_double(self.c))
-
-    def __exit__(self, *exc):
-        lib().orc_diag_eval_noise(C.c_double(0.0))
-        return False
-
-
 def num_threads() -> int:
     return int(lib().orc_num_threads())
 

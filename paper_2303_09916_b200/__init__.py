@@ -35,4 +35,5 @@ from .binding import (  # noqa: F401
     launch_count,
     load_library,
     make_box,
+    score_jit_cache,
 )

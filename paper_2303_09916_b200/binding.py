@@ -28,7 +28,7 @@ EXPORTS = [
     "dock_default_params", "dock_grid_dims", "dock_grid_bytes", "dock_build_grids", "dock_build_grids_batch", "dock_score_batch",
     "dock_score_batch_host", "dock_local_opt_batch", "dock_local_opt_trace", "dock_init_poses", "dock_init_poses_site",
     "dock_search", "dock_topk", "dock_topk_fixed", "dock_system_host", "dock_probe_peaks", "dock_last_cuda_error", "dock_version",
-    "dock_launch_count", "dock_score_jit_source", "dock_score_jit_compile", "dock_score_jit_log",
+    "dock_launch_count", "dock_score_jit_source", "dock_score_jit_compile", "dock_score_jit_log", "dock_score_jit_cache",
 ]
 
 
@@ -157,6 +157,13 @@ class _Workspace:
 
 
 _ws = _Workspace()
+
+
+def score_jit_cache(new_limit: int = -1):
+    """(limit before the call, cached specialised kernels); new_limit >= 1 sets the per-device limit (dock.h)."""
+    old, n = C.c_int32(0), C.c_int32(0)
+    _check(load_library().dock_score_jit_cache(int(new_limit), C.byref(old), C.byref(n)), "dock_score_jit_cache")
+    return int(old.value), int(n.value)
 
 
 def launch_count() -> int:

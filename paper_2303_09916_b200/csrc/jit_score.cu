@@ -1003,9 +1003,34 @@ struct JitKernel {
     int warps = 0;
     size_t smem = 0;
     int status = DOCK_OK;                 // a failed compilation is remembered: no retry storm
+    uint64_t last_use = 0;                // g_cache_tick at the last launch: the least recently used entry is evicted
 };
-// (device, digest of everything the generated text depends on) -> kernel
+// (device, digest of everything the generated text depends on) -> kernel.  Bounded per device (a screening run sees
+// thousands of ligands): at g_cache_limit entries the least recently used one of that device is unloaded first.
 std::map<std::pair<int, std::pair<uint64_t, uint64_t>>, JitKernel> g_cache;
+uint64_t g_cache_tick = 0;
+int g_cache_limit = 64;
+
+// Called under g_jit_mu before an entry for `dev` is added.  The victim's kernel may still be running on some stream of the
+// device, so the device is synchronised before cudaLibraryUnload; this happens only next to a compilation (0.4-6 s).
+void jit_cache_make_room(int dev)
+{
+    for (;;) {
+        int n = 0;
+        auto victim = g_cache.end();
+        for (auto it = g_cache.begin(); it != g_cache.end(); ++it) {
+            if (it->first.first != dev) continue;
+            ++n;
+            if (victim == g_cache.end() || it->second.last_use < victim->second.last_use) victim = it;
+        }
+        if (n < g_cache_limit || victim == g_cache.end()) return;
+        if (victim->second.lib) {
+            cudaDeviceSynchronize();
+            cudaLibraryUnload(victim->second.lib);
+        }
+        g_cache.erase(victim);
+    }
+}
 
 struct Digest {                                            // two independent 64-bit FNV-1a style streams
     uint64_t a = 1469598103934665603ull, b = 0x9e3779b97f4a7c15ull;
@@ -1118,8 +1143,10 @@ int jit_score_launch(const dock_params *p, const dock_grid *g, const dock_ligand
                     e = cudaFuncSetAttribute((const void *)nk.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nk.smem);
                 if (e != cudaSuccess) { g_dock_last_cuda_error.store((int)e); nk.status = DOCK_ECUDA; }
             }
+            jit_cache_make_room(dev);
             it = g_cache.emplace(key, nk).first;
         }
+        it->second.last_use = ++g_cache_tick;
         k = it->second;
     }
     if (k.status != DOCK_OK) return k.status;
@@ -1170,6 +1197,17 @@ extern "C" int dock_score_jit_compile(const dock_params *params, const dock_grid
     const int rc2 = compile_cubin(src, o, cubin);
     if (cubin_bytes) *cubin_bytes = cubin.size();
     return rc2;
+}
+
+extern "C" int dock_score_jit_cache(int32_t new_limit, int32_t *old_limit, int32_t *entries)
+{
+    std::lock_guard<std::mutex> lock(g_jit_mu);
+    if (old_limit) *old_limit = g_cache_limit;
+    if (entries) *entries = (int32_t)g_cache.size();
+    if (new_limit < 0) return DOCK_OK;
+    if (new_limit < 1 || new_limit > 65536) return DOCK_EINVAL;
+    g_cache_limit = new_limit;
+    return DOCK_OK;
 }
 
 extern "C" const char *dock_score_jit_log(void)

@@ -275,3 +275,15 @@ def test_specialised_score_kernel_source_and_compilation(lib):
     assert lib.dock_score_jit_source(C.byref(p), C.byref(g), C.byref(big.c), 1, None, C.c_size_t(0), C.byref(need)) == B.DOCK_EINVAL
     g.n_channels = 4
     assert lib.dock_score_jit_source(C.byref(p), C.byref(g), C.byref(lig.c), 1, None, C.c_size_t(0), C.byref(need)) == B.DOCK_EINVAL
+
+
+def test_specialised_kernel_cache_limit_arguments():
+    """dock_score_jit_cache: query, set, and the rejected limits (host only)."""
+    import paper_2303_09916_b200 as dk
+    from paper_2303_09916_b200 import binding as B
+    old, n = dk.score_jit_cache()
+    assert old >= 1 and n >= 0
+    assert dk.score_jit_cache(5) == (old, n) and dk.score_jit_cache()[0] == 5
+    lib = dk.load_library()
+    assert lib.dock_score_jit_cache(0, None, None) == B.DOCK_EINVAL and lib.dock_score_jit_cache(1 << 20, None, None) == B.DOCK_EINVAL
+    assert dk.score_jit_cache(old)[0] == 5 and dk.score_jit_cache()[0] == old

@@ -816,7 +816,12 @@ def test_batched_grid_build_equals_single_builds(dk, torch):
     assert tuple(batch[0].dims) == (3, 3, 401)
     for i in (0, 37, 75, 76, 79):                                            # 75 systems fit the first launch
         one = dk.dock_build_grids(p, prots[i][0], prots[i][1], boxes[i], all_types)
-        assert torch.equal(batch[i].buf, one.buf), i
+        nodes = one.data.numel()
+        o1 = (nodes * 4 + 255) // 256 * 256                                   # the three images, without the alignment gaps
+        o2 = o1 + (nodes * 32 + 255) // 256 * 256
+        for lo, hi in ((0, nodes * 4), (o1, o1 + nodes * 32), (o2, o2 + nodes * 16)):
+            assert torch.equal(batch[i].buf[lo:hi], one.buf[lo:hi]), (i, lo)
+        assert batch[i].buf.numel() == o2 + nodes * 16
 
 
 # ----------------------------------------------------------------------------------- NEXT-4: sharded search, streams
@@ -991,6 +996,31 @@ def test_specialised_score_kernel_limits(dk, torch, micro):
         dk.dock_score_batch(_jit_params(dk), grid, lig, poses)
     e, _, _ = dk.dock_score_batch(dk.dock_default_params(), grid, lig, poses)      # default: generic kernel
     assert bool(torch.isfinite(e).all())
+
+
+def test_specialised_kernel_cache_is_bounded(dk, torch, micro):
+    """The per-device cache of compiled kernels evicts its least recently used entry at the limit (dock.h:
+    dock_score_jit_cache); an evicted ligand is compiled again on its next call and gives the same bits."""
+    s0, (_, box, grid, _), _ = micro
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    p = _jit_params(dk)
+    ligs = [dk.LigandHandle(dock_synth.make_ligand(np.random.default_rng(900 + i), 4 + i, 0, LIG_TYPES_FULL)) for i in range(3)]
+    poses = torch.from_numpy(random_poses(np.random.default_rng(7), 257, s0.box_center, s0.box_size, 0)).cuda()
+    old, _ = dk.score_jit_cache(2)
+    try:
+        first = [tuple(x.clone() for x in dk.dock_score_batch(p, grid, ligs[0], poses))]
+        assert dk.score_jit_cache()[1] <= 2                      # whatever earlier tests left was cut down to the limit
+        first.append(tuple(x.clone() for x in dk.dock_score_batch(p, grid, ligs[1], poses)))
+        dk.dock_score_batch(p, grid, ligs[0], poses)             # ligand 0 is now the more recently used of the two
+        first.append(tuple(x.clone() for x in dk.dock_score_batch(p, grid, ligs[2], poses)))   # evicts ligand 1
+        assert dk.score_jit_cache()[1] == 2
+        for i in (1, 0, 2):                                       # 1 is compiled again (evicting 0), then 0 (evicting 2), ...
+            again = dk.dock_score_batch(p, grid, ligs[i], poses)
+            assert all(torch.equal(a, b) for a, b in zip(again, first[i])), i
+            assert dk.score_jit_cache()[1] == 2
+    finally:
+        dk.score_jit_cache(old)
 
 
 def test_quad_image_is_a_copy_of_the_maps(dk, torch, tiny):
