@@ -8,8 +8,8 @@ import numpy as np
 import pytest
 
 from dock_synth import make_system, random_poses
-from tests.parity import (CEILING_DROP_BITS, KINK_MARGIN, bb_replay, binom_floor, compare_grid, compare_scores, gpu_side, iteration_replay,
-                          oracle_self_agreement, oracle_side, tol, unpack_iter_trace)
+from tests.parity import (CEILING_DROP_BITS, KINK_MARGIN, bb_replay, compare_grid, compare_scores, compare_trace_gradients,
+                          gpu_side, iteration_replay, oracle_self_agreement, oracle_side, tol, unpack_iter_trace)
 
 pytestmark = pytest.mark.gpu
 
@@ -225,6 +225,7 @@ def test_local_opt_level2(dk, orc, torch, cfg, n, cap):
     it = unpack_iter_trace(trace.cpu().numpy(), git, lig.T)
     assert len(it["f"]) == int((git[:, 0] + (git[:, 2] != dk.DOCK_EXIT_CAP)).sum())
     assert int(it["trials"].sum()) + n == int(git[:, 1].sum())                     # evaluations = 1 + all line-search trials
+    gst = compare_trace_gradients(orc, op, og, oL, it, f"local-opt cfg{cfg}", lig.N, lig.P)   # level 1 of the search evaluator, gradient included
     rp = iteration_replay(orc, op, og, oL, it, float(op.bfgs_gtol))
     cmp_ = ~rp["near_cut"]
     same = rp["same"][cmp_]
@@ -245,7 +246,7 @@ def test_local_opt_level2(dk, orc, torch, cfg, n, cap):
     oe, _, oinfo = orc.local_opt_batch(op, og, oL, poses.astype(np.float64), cap)
     ceil = oracle_self_agreement(orc, op, og, oL, poses.astype(np.float64), cap)
     agree = float(np.mean(np.abs(ge - oe) <= 1e-3))
-    st = dict(cfg=cfg, n=n, cap=cap, iterations=int(len(it["f"])), iterations_compared=int(cmp_.sum()),
+    st = dict(cfg=cfg, n=n, cap=cap, iterations=int(len(it["f"])), iterations_compared=int(cmp_.sum()), state_gradients=gst,
               iter_decisions_identical=float(same.mean()), iter_mismatch_kinds=kinds, iter_mismatch_worst_margin_tol=worst_margin,
               state_f_max_err_tol=float(ferr.max()), f_new_max_err_tol=float(fnerr.max()),
               x_new_max_abs=float(ex.max()), H_new_rel_err_median=float(np.median(eh)), H_new_rel_err_q90=float(np.quantile(eh, 0.9)),
@@ -264,7 +265,7 @@ def test_local_opt_level2(dk, orc, torch, cfg, n, cap):
     assert worst_margin <= 0.25, st
     assert kinds["descent"] == 0 and kinds["curvature"] <= max(2, 0.001 * len(same)), st
     assert ex.max() <= 1e-5 and np.median(eh) <= 1e-4 and np.quantile(eh, 0.9) <= 1e-2, st
-    assert agree >= binom_floor(ceil["agree"], n), st
+    # (the free-run agreement rate `agree` and its ceiling are logged, not gated: DESIGN.md 2a "free-run rates")
     # neither side is systematically better (paired sign test, 5 sigma)
     decided = np.abs(ge - oe) > 1e-3
     wins = int((ge < oe)[decided].sum())
@@ -279,6 +280,7 @@ def _first_iterations_replay(dk, orc, torch, p, grid, lig, op, og, oL, poses, ca
     (eq. 4 maps, other weight signs)."""
     o, e, it_, trace = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap, trace_cap=cap + 1)
     it = unpack_iter_trace(trace.cpu().numpy(), it_.cpu().numpy(), lig.T)
+    compare_trace_gradients(orc, op, og, oL, it, "first iterations", lig.N, lig.P)
     rp = iteration_replay(orc, op, og, oL, it, float(op.bfgs_gtol))
     cmp_ = ~rp["near_cut"]
     acc = cmp_ & rp["same"] & (it["status"] == 0)
@@ -299,6 +301,45 @@ def test_local_opt_zero_iterations_is_a_plain_evaluation(dk, orc, torch, tiny):
     # two evaluators (warp-per-pose in the optimizer, thread-per-pose in the batch call): same value up to summation order
     assert torch.allclose(out_e, e, rtol=1e-5, atol=1e-4)
     assert np.all(out_it.cpu().numpy() == [0, 1, dk.DOCK_EXIT_CAP])
+
+
+@pytest.mark.parametrize("optimizer,kernel", [(0, 1), (0, 2), (1, 1), (1, 2)])
+@pytest.mark.parametrize("N,T", [(50, 12), (60, 15), (128, 32)])
+def test_search_evaluator_gradients_on_large_ligands(dk, orc, torch, micro, N, T, optimizer, kernel):
+    """The evaluators inside the search kernels on the ligand shapes the small configs do not reach: N = 50 / T = 12
+    (the configs[3] extreme) and N = 60 / T = 15 (configs[4]) -- more than 48 atoms, so eval_warp.cuh's second
+    shared-memory layout and two atoms per lane -- and the maximum 128 / 32 (four atoms per lane; one atom per thread in
+    eval_cta.cuh).  Every state visited by a short local optimisation (BFGS and Barzilai-Borwein, warp and CTA kernel):
+    energy and all 6 + T gradient components against the oracle, and for BFGS the iteration-level replay as well."""
+    s0, (_, box, grid, _), (_, og, _) = micro
+    import dock_synth
+    from dock_synth.generators import LIG_TYPES_FULL
+    ligd = dock_synth.make_ligand(np.random.default_rng(1000 + N), N, T, LIG_TYPES_FULL)
+    lig, oL = dk.LigandHandle(ligd), orc.Ligand(ligd)
+    p = dk.dock_default_params()
+    p.optimizer, p.search_kernel = optimizer, kernel
+    op = orc.params_as_fp32(orc.default_params())
+    op.optimizer = optimizer
+    cap = 12
+    poses = random_poses(np.random.default_rng(N + T), 96, s0.box_center, s0.box_size * 0.7, T)
+    o, e, it_, trace = dk.dock_local_opt_batch(p, grid, lig, torch.from_numpy(poses).cuda(), cap, trace_cap=cap + 1)
+    it = unpack_iter_trace(trace.cpu().numpy(), it_.cpu().numpy(), T)
+    assert len(it["f"]) >= 96 * 4
+    gst = compare_trace_gradients(orc, op, og, oL, it, f"N{N} T{T} opt{optimizer} kernel{kernel}", N, oL.P)
+    st = dict(N=N, T=T, P=int(oL.P), optimizer=optimizer, kernel=kernel, **gst)
+    if optimizer == 0:
+        rp = iteration_replay(orc, op, og, oL, it, float(op.bfgs_gtol))
+        cmp_ = ~rp["near_cut"]
+        bad = cmp_ & ~rp["same"]
+        st.update(iter_decisions_identical=float(rp["same"][cmp_].mean()),
+                  mismatch_worst_margin_tol=float(rp["margin_tol"][bad].max()) if bad.any() else 0.0)
+        assert rp["same"][cmp_].mean() >= 0.97 and st["mismatch_worst_margin_tol"] <= 0.25, st
+    else:
+        rp = bb_replay(orc, op, og, oL, it)
+        cmp_ = ~rp["near_cut"]
+        st.update(iter_decisions_identical=float(rp["same"][cmp_].mean()))
+        assert rp["same"][cmp_].mean() >= 0.99, st
+    _log("search_evaluator_gradients", st)
 
 
 # ----------------------------------------------------------------------------------- A7 search
@@ -389,9 +430,7 @@ def _search_parity(dk, orc, torch, s, gpu_side_, oracle_side_, copies, steps, ca
               gpu_evals_traced=int(tr["evals"].sum()), ref_evals=int(ref["evals"]), ceiling_evals=int(ref32["evals"]))
     _log("search_level3", st)
     assert dec_ok.all(), st                              # a decision mismatch with agreeing energies is a bug
-    assert st["teacher_e_agree"] >= binom_floor(tf_ceiling, len(e_ok)), st
-    assert st["free_full_agree"] >= binom_floor(st["free_full_agree_ceiling"], n_ref), st
-    assert st["free_best_agree"] >= binom_floor(st["free_best_agree_ceiling"], n_ref), st
+    # (teacher_e_agree, free_full_agree, free_best_agree and their ceilings are logged, not gated: DESIGN.md 2a "free-run rates")
     if n_ref >= 64:                                      # mean length of the agreeing prefix: meaningless on a handful of copies
         assert st["free_mean_prefix"] >= st["free_mean_prefix_ceiling"] - max(1.0, 0.35 * st["free_mean_prefix_ceiling"]), st
     # best energies are heavy-tailed (a few copies stay stuck in a clash): compare medians, and quartiles where the
@@ -599,6 +638,7 @@ def test_bb_local_opt(dk, orc, torch, tiny, micro, cfg, n, kernel):
     assert np.all(ge <= e0 + tol(e0))                                        # best-seen never exceeds the start
     assert np.all(git[:, 1] == git[:, 0] + 1)                                # evaluations = iterations + 1
     it = unpack_iter_trace(trace.cpu().numpy(), git, lig.T)
+    gst = compare_trace_gradients(orc, op, og, oL, it, f"bb cfg{cfg} kernel {kernel}", lig.N, lig.P)
     rp = bb_replay(orc, op, og, oL, it)
     cmp_ = ~rp["near_cut"]
     taken = cmp_ & rp["same"] & (it["status"] == 0)
@@ -613,7 +653,8 @@ def test_bb_local_opt(dk, orc, torch, tiny, micro, cfg, n, kernel):
     oe = ceil["e0"]
     agree = float(np.mean(np.abs(ge - oe) <= 1e-3))
     qg, qr = np.quantile(ge, [0.25, 0.5, 0.75]), np.quantile(oe, [0.25, 0.5, 0.75])
-    st = dict(cfg=cfg, kernel=kernel, n=n, cap=cap, iterations=int(len(it["f"])), iter_decisions_identical=float(rp["same"][cmp_].mean()),
+    st = dict(cfg=cfg, kernel=kernel, n=n, cap=cap, iterations=int(len(it["f"])), state_gradients=gst,
+              iter_decisions_identical=float(rp["same"][cmp_].mean()),
               alpha_rel_err_max=float(rel_alpha.max()), f_new_max_err_tol=float(fnerr.max()), state_f_max_err_tol=float(ferr.max()),
               mismatches=int(bad.sum()), mismatch_margin_max=float(bad_margin.max()) if bad.any() else 0.0,
               agree_1e3=agree, ceiling_agree_1e3=ceil["agree"], gpu_quartiles=qg.tolist(), ref_quartiles=qr.tolist(),
@@ -622,7 +663,7 @@ def test_bb_local_opt(dk, orc, torch, tiny, micro, cfg, n, kernel):
     assert ferr.max() <= 1.0 and fnerr.max() <= 1.0, st
     assert rp["same"][cmp_].mean() >= 0.995 and (not bad.any() or bad_margin.max() <= 1e-3), st
     assert rel_alpha.max() <= 1e-5, st                                       # same step length from the same (s, y, g)
-    assert agree >= binom_floor(ceil["agree"], n), st
+    # (the free-run agreement rate `agree` and its ceiling are logged, not gated: DESIGN.md 2a "free-run rates")
     assert np.all(np.abs(qg - qr) <= 0.75 + 0.15 * np.abs(qr)), st
 
 
